@@ -116,7 +116,7 @@ def _uniform_state(G, C, N0, nH, T, x, y):
 
 def config0(n=32):
     """Isothermal single-source ionisation (octant of a Stroemgren sphere)."""
-    box = 6.6 * KPC * n / 32.0 if n < 32 else 6.6 * KPC
+    box = 6.6 * KPC
     mesh = M.cartesian(n, box, periodic=False,
                        bc=(M.BC_REFLECT, M.BC_OUTFLOW, M.BC_REFLECT, M.BC_OUTFLOW, M.BC_REFLECT, M.BC_OUTFLOW))
     ct = 0.01 * C_LIGHT

@@ -1,0 +1,159 @@
+/* librt.so — C ABI of the B200-native AREPO-RT subcycle (arXiv 2404.17630).
+ *
+ * The calls follow the paper's problem statement: the mesh is static during the subcycles, so
+ * "most of the data can be transferred to the GPU once before the first subcycle and only copied
+ * back after the completion of the full RT step":
+ *
+ *     rt_create -> rt_mesh_upload -> rt_state_init -> rt_step (many) -> rt_download -> rt_destroy
+ *
+ * One subcycle (Fig. 1) = thermochemistry, then two
+ * Heun stages of [gradients + limiter (eqs 13-15) -> face fluxes
+ * (eqs 6-10) -> apply fluxes and sources per cell].  Every step
+ * runs in the library's sm_100a kernels; there is no CPU fallback.
+ *
+ * Conventions
+ *  - fp64 everywhere; int32 cell/face ids; SoA arrays; a (k, n) array is k contiguous rows of n.
+ *  - A pointer is a HOST or a DEVICE pointer as the struct's mem_kind says (all pointers of one
+ *    struct alike, except where stated).  Every input pointer is borrowed for the duration of
+ *    the call only; outputs are caller-allocated.  The library allocates nothing on the device
+ *    except inside the caller's workspace, and never frees caller memory.
+ *  - Cell order is the caller's, both ways; the library reorders cells along a Peano-Hilbert
+ *    curve and faces by owner and keeps the permutation private.
+ *  - Return value: 0 (RT_OK) or a negative RT_E* code; the message is in rt_last_error().
+ *    No exception or abort crosses the ABI.
+ *  - Calls on one context are asynchronous on the context's stream unless stated; they must be
+ *    issued from one host thread at a time.
+ */
+#ifndef RT_H_
+#define RT_H_
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RT_MAXG 8 /* maximum number of frequency groups */
+
+enum { RT_OK = 0, RT_EINVAL = -1, RT_ENOMEM = -2, RT_ECUDA = -3, RT_ESTATE = -4, RT_EMESH = -5 };
+enum { RT_MEM_HOST = 0, RT_MEM_DEVICE = 1 };
+/* rt_mesh.right codes for boundary faces (reading S13) */
+enum { RT_BC_OUTFLOW = -1, RT_BC_REFLECT = -2, RT_BC_DIRICHLET0 = -3 /* -3-k: ghost state k */ };
+enum { RT_CHEM_NONE = 0, RT_CHEM_FIXED_OPACITY = 1, RT_CHEM_H_ISOTHERMAL = 2, RT_CHEM_HHE_THERMAL = 3 };
+
+typedef struct rt_ctx rt_ctx; /* opaque, owned by the library */
+
+/* Static unstructured mesh (per-interface left/right cell index).
+ * Each face is stored once; `normal` is the unit normal pointing from `left` to `right`;
+ * `fcentroid` is given in the left cell's frame (it may lie outside the box when periodic). */
+typedef struct {
+  int64_t ncell, nface;
+  double box[3];
+  int32_t periodic[3];
+  int32_t mem_kind;        /* of the seven array pointers below */
+  const double *volume;    /* (C)    > 0 */
+  const double *centroid;  /* (3, C) geometric centroid s_i (reading S7) */
+  const double *area;      /* (F)    > 0 */
+  const double *normal;    /* (3, F) */
+  const double *fcentroid; /* (3, F) */
+  const int32_t *left;     /* (F)    in [0, C) */
+  const int32_t *right;    /* (F)    in [0, C), or an RT_BC_* code */
+  int32_t nghost;          /* number of Dirichlet ghost states */
+  int32_t ngroup;          /* G, fixed for the life of the mesh (sizes the workspace) */
+  const double *ghost_state; /* HOST (nghost, 4G): N, Fx, Fy, Fz per group */
+} rt_mesh;
+
+/* Radiation + gas state, caller's cell order. N (G, C) photon number density; F (G, 3, C) photon
+ * flux; ionised fractions x_HII, x_HeII, x_HeIII (C); thermal energy density eth (C) [erg cm^-3];
+ * hydrogen number density nH (C) [cm^-3] (input only; rt_download does not write it). */
+typedef struct {
+  int32_t mem_kind;
+  int32_t pad;
+  double *N, *F, *xHII, *xHeII, *xHeIII, *eth, *nH;
+} rt_state;
+
+/* Point sources S of eq (6): photons/s per group injected into `cell`. HOST. */
+typedef struct {
+  int32_t nsrc;
+  int32_t pad;
+  const int32_t *cell; /* (nsrc), caller's numbering, distinct */
+  const double *rate;  /* (G, nsrc) */
+} rt_sources;
+
+typedef struct {
+  int32_t ngroup;
+  int32_t chem_mode;        /* RT_CHEM_* */
+  int32_t order;            /* 1: piecewise constant, 2: limited linear reconstruction */
+  int32_t heun;             /* 1: two-stage Heun, 0: one forward-Euler stage */
+  double ctilde;            /* reduced speed of light */
+  double sigma[RT_MAXG][3];    /* grey cross-sections per group for HI, HeI, HeII [cm^2] */
+  double eps_heat[RT_MAXG][3]; /* photo-heating energy per absorption [erg] */
+  double T_fixed;           /* H_ISOTHERMAL: temperature [K] */
+  double alphaB_override;   /* > 0 replaces alpha_B(HII) */
+  double y_he;              /* n_He / n_H */
+  double f_accept;          /* 0.1 */
+  double f_target;          /* 0.05 */
+  double x_floor_rel;       /* denominator floor of relative abundance changes (S18) */
+  double n_floor;           /* floor on N, ledgered as floor_added (S11) */
+  int64_t max_substeps;     /* cap on chemistry attempts per cell and subcycle */
+  int32_t kappa_mem_kind;
+  int32_t pad;
+  const double *kappa;      /* (C) FIXED_OPACITY only: absorption coefficient [1/length], caller's order */
+} rt_params;
+
+/* Photon budget since rt_state_init, per group, photons:
+ * stored + absorbed + outflow = stored(0) + injected + inflow_bc + floor_added. */
+typedef struct {
+  double stored[RT_MAXG], injected[RT_MAXG], absorbed[RT_MAXG], outflow[RT_MAXG], inflow_bc[RT_MAXG],
+      floor_added[RT_MAXG];
+  int64_t substeps_total, substeps_max, cells_hit_cap;
+  int64_t nsub_done;
+} rt_ledger;
+
+/* Creates a context on CUDA device `device` issuing all work on `cuda_stream` (a cudaStream_t;
+ * NULL = the legacy default stream).  The stream is borrowed and must outlive the context. */
+int rt_create(rt_ctx **out, int device, void *cuda_stream);
+
+/* Bytes of device workspace rt_mesh_upload needs for this problem size (0 on invalid sizes).
+ * flags: reserved, pass 0. */
+size_t rt_workspace_bytes(int64_t ncell, int64_t nface, int ngroup, int flags);
+
+/* Validates the mesh (index ranges, positive volumes and areas, unit normals, closed cells:
+ * |sum_f s_if A_f n_f| <= 1e-10 sum_f A_f), reorders it (Peano-Hilbert on centroids, faces by
+ * owner, cell -> face lists: PAPER.md:272) and precomputes the mesh-only parts of eq (15): the
+ * inverse 3x3 matrix per cell and the per-face prefactors.
+ * `dev_workspace` (256-byte aligned DEVICE memory of >= rt_workspace_bytes, e.g. a torch tensor's
+ * data_ptr) is borrowed until rt_destroy or the next rt_mesh_upload.  Synchronises the stream.
+ * Errors: RT_EINVAL (null/sizes/alignment), RT_ENOMEM (workspace too small), RT_EMESH (validation
+ * failed; message says which check), RT_ECUDA. */
+int rt_mesh_upload(rt_ctx *ctx, const rt_mesh *mesh, void *dev_workspace, size_t bytes);
+
+/* Sets parameters, sources and the initial state; resets the ledger.  `src` may be NULL.
+ * Needs a mesh (else RT_ESTATE).  Synchronises the stream (inputs are free on return). */
+int rt_state_init(rt_ctx *ctx, const rt_params *p, const rt_state *s0, const rt_sources *src);
+
+/* Advances `nsub` subcycles of length dt [same time unit as 1/ctilde * length].  Asynchronous:
+ * only enqueues kernels on the context's stream.  Needs rt_state_init (else RT_ESTATE). */
+int rt_step(rt_ctx *ctx, double dt, int nsub);
+
+/* Copies the state (any pointer of `out` may be NULL to skip it; nH is never written) and the
+ * ledger (may be NULL) out, in the caller's cell order.  Synchronises the stream. */
+int rt_download(rt_ctx *ctx, rt_state *out, rt_ledger *ledger);
+
+/* Number of kernels the context has launched since rt_create (for bench.py's gpu_launches). */
+int64_t rt_kernel_launches(const rt_ctx *ctx);
+
+/* Slope-limited gradients of the current state in the caller's order, DEVICE or HOST as
+ * mem_kind says: gN (G, 3, C), gF (G, 3 components, 3 directions, C).  For tests. Synchronises. */
+int rt_debug_gradients(rt_ctx *ctx, int mem_kind, double *gN, double *gF);
+
+/* Last error message of this context ("" if none); valid until the next call on it. */
+const char *rt_last_error(const rt_ctx *ctx);
+
+/* Frees the context (not the workspace, which is the caller's).  NULL is allowed. */
+void rt_destroy(rt_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RT_H_ */

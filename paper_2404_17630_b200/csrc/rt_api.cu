@@ -1,0 +1,257 @@
+// The C ABI of include/rt.h: argument checking, marshalling and stream-ordered copies.
+// All arithmetic of the method lives in rt_chem.cu / rt_transport.cu (per subcycle) and
+// rt_setup.cu (per mesh).
+#include <stdarg.h>
+#include <string.h>
+#include <new>
+#include <vector>
+#include "rt_internal.cuh"
+
+int rt_fail(rt_ctx *c, int code, const char *fmt, ...) {
+  if (c) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(c->err, sizeof(c->err), fmt, ap);
+    va_end(ap);
+  }
+  return code;
+}
+
+extern "C" {
+
+int rt_create(rt_ctx **out, int device, void *cuda_stream) {
+  if (!out) return RT_EINVAL;
+  *out = nullptr;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return RT_ECUDA;
+  rt_ctx *c = new (std::nothrow) rt_ctx();
+  if (!c) return RT_ENOMEM;
+  memset(c, 0, sizeof(*c));
+  c->device = device;
+  c->stream = (cudaStream_t)cuda_stream;
+  if (cudaSetDevice(device) != cudaSuccess) { delete c; return RT_ECUDA; }
+  *out = c;
+  return RT_OK;
+}
+
+void rt_destroy(rt_ctx *c) { delete c; }
+
+const char *rt_last_error(const rt_ctx *c) { return c ? c->err : "null context"; }
+
+int64_t rt_kernel_launches(const rt_ctx *c) { return c ? c->launches : 0; }
+
+size_t rt_workspace_bytes(int64_t ncell, int64_t nface, int ngroup, int flags) {
+  (void)flags;
+  if (ncell < 1 || nface < 1 || ngroup < 1 || ngroup > RT_MAXG || ncell > 0x7fffffffLL || nface > 0x7fffffffLL) return 0;
+  return rt_make_layout(ncell, nface, ngroup).total;
+}
+
+int rt_mesh_upload(rt_ctx *c, const rt_mesh *m, void *ws, size_t bytes) {
+  if (!c) return RT_EINVAL;
+  c->err[0] = 0;
+  c->have_mesh = c->have_state = false;
+  if (!m || !ws) return rt_fail(c, RT_EINVAL, "null mesh or workspace");
+  if (m->ncell < 1 || m->nface < 1 || m->ncell > 0x7fffffffLL || m->nface > 0x7fffffffLL)
+    return rt_fail(c, RT_EINVAL, "ncell/nface out of range");
+  if (m->ngroup < 1 || m->ngroup > RT_MAXG) return rt_fail(c, RT_EINVAL, "ngroup must be in [1, %d]", RT_MAXG);
+  if (!m->volume || !m->centroid || !m->area || !m->normal || !m->fcentroid || !m->left || !m->right)
+    return rt_fail(c, RT_EINVAL, "null mesh array");
+  if (m->nghost < 0 || m->nghost > 64 || (m->nghost > 0 && !m->ghost_state))
+    return rt_fail(c, RT_EINVAL, "nghost must be in [0, 64] with ghost_state set");
+  if (((uintptr_t)ws & 255) != 0) return rt_fail(c, RT_EINVAL, "workspace must be 256-byte aligned");
+  for (int a = 0; a < 3; a++)
+    if (!(m->box[a] > 0.0)) return rt_fail(c, RT_EINVAL, "box side must be positive");
+  RT_CUDA(c, cudaSetDevice(c->device));
+  c->C = m->ncell; c->F = m->nface; c->G = m->ngroup; c->nghost = m->nghost;
+  for (int a = 0; a < 3; a++) { c->box[a] = m->box[a]; c->per[a] = m->periodic[a] != 0; }
+  c->lay = rt_make_layout(c->C, c->F, c->G);
+  if (bytes < c->lay.total)
+    return rt_fail(c, RT_ENOMEM, "workspace has %zu bytes, rt_workspace_bytes says %zu", bytes, c->lay.total);
+  c->ws = (char *)ws;
+  c->ws_bytes = bytes;
+  int rc = rt_setup_mesh(c, m);
+  if (rc != RT_OK) return rc;
+  c->have_mesh = true;
+  return RT_OK;
+}
+
+// copy `rows` rows of C doubles (caller's order, host or device) into dst in the internal order
+static int put_rows(rt_ctx *c, const double *src, int mem_kind, double *dst, int rows, double *stage) {
+  const size_t n = (size_t)rows * c->C;
+  if (mem_kind == RT_MEM_HOST) {
+    RT_CUDA(c, cudaMemcpyAsync(stage, src, n * 8, cudaMemcpyHostToDevice, c->stream));
+    src = stage;
+  }
+  return rt_launch_permute_in(c, src, dst, rows);
+}
+
+int rt_state_init(rt_ctx *c, const rt_params *p, const rt_state *s0, const rt_sources *src) {
+  if (!c) return RT_EINVAL;
+  c->err[0] = 0;
+  if (!c->have_mesh) return rt_fail(c, RT_ESTATE, "rt_state_init needs rt_mesh_upload first");
+  if (!p || !s0) return rt_fail(c, RT_EINVAL, "null params or state");
+  if (p->ngroup != c->G) return rt_fail(c, RT_EINVAL, "params.ngroup %d != mesh.ngroup %d", p->ngroup, c->G);
+  if (p->chem_mode < RT_CHEM_NONE || p->chem_mode > RT_CHEM_HHE_THERMAL) return rt_fail(c, RT_EINVAL, "bad chem_mode");
+  if (!(p->ctilde > 0.0)) return rt_fail(c, RT_EINVAL, "ctilde must be positive");
+  if (p->order < 1 || p->order > 2) return rt_fail(c, RT_EINVAL, "order must be 1 or 2");
+  if (!s0->N || !s0->F) return rt_fail(c, RT_EINVAL, "state needs N and F");
+  const bool chem = p->chem_mode >= RT_CHEM_H_ISOTHERMAL;
+  if (chem && (!s0->xHII || !s0->xHeII || !s0->xHeIII || !s0->eth || !s0->nH))
+    return rt_fail(c, RT_EINVAL, "chemistry needs xHII, xHeII, xHeIII, eth, nH");
+  if (chem && (!(p->f_accept > 0.0) || !(p->f_target > 0.0) || p->max_substeps < 1))
+    return rt_fail(c, RT_EINVAL, "chemistry needs f_accept, f_target > 0 and max_substeps >= 1");
+  if (p->chem_mode == RT_CHEM_FIXED_OPACITY && !p->kappa) return rt_fail(c, RT_EINVAL, "FIXED_OPACITY needs kappa");
+  const int nsrc = src ? src->nsrc : 0;
+  if (nsrc < 0 || nsrc > 65536 || (nsrc > 0 && (!src->cell || !src->rate)))
+    return rt_fail(c, RT_EINVAL, "nsrc must be in [0, 65536] with cell and rate set");
+  for (int k = 0; k < nsrc; k++)
+    if (src->cell[k] < 0 || src->cell[k] >= c->C) return rt_fail(c, RT_EINVAL, "source cell out of range");
+  RT_CUDA(c, cudaSetDevice(c->device));
+  c->par = *p;
+  c->par.kappa = nullptr;
+  const rt_layout &l = c->lay;
+  const int G = c->G;
+  const int64_t C = c->C;
+  double *stage = rt_ptr<double>(c, l.grad);  // 12 G C doubles: free between steps
+  double *Ua = rt_ptr<double>(c, l.Ua);
+  int rc;
+  // N (G,C) and F (G,3,C) -> U[g][4][C]
+  for (int g = 0; g < G; g++) {
+    if ((rc = put_rows(c, s0->N + (size_t)g * C, s0->mem_kind, Ua + (size_t)4 * g * C, 1, stage))) return rc;
+    if ((rc = put_rows(c, s0->F + (size_t)3 * g * C, s0->mem_kind, Ua + (size_t)(4 * g + 1) * C, 3, stage + C))) return rc;
+    stage += 4 * C;
+  }
+  stage = rt_ptr<double>(c, l.grad) + (size_t)4 * G * C;
+  const double *xs[5] = {s0->xHII, s0->xHeII, s0->xHeIII, s0->eth, s0->nH};
+  const size_t xo[5] = {l.xHII, l.xHeII, l.xHeIII, l.eth, l.nH};
+  for (int k = 0; k < 5; k++) {
+    if (xs[k]) { if ((rc = put_rows(c, xs[k], s0->mem_kind, rt_ptr<double>(c, xo[k]), 1, stage + (size_t)k * C))) return rc; }
+    else RT_CUDA(c, cudaMemsetAsync(rt_ptr<double>(c, xo[k]), 0, 8 * C, c->stream));
+  }
+  if (p->chem_mode == RT_CHEM_FIXED_OPACITY) {
+    if ((rc = put_rows(c, p->kappa, p->kappa_mem_kind, rt_ptr<double>(c, l.kappa), 1, stage + (size_t)5 * C))) return rc;
+  }
+  // sources
+  c->nsrc = nsrc;
+  for (int g = 0; g < RT_MAXG; g++) { c->src_total[g] = 0.0; c->injected[g][0] = c->injected[g][1] = 0.0; }
+  int32_t *cell_dev = rt_ptr<int32_t>(c, l.Ub);  // free until the first step
+  if (nsrc > 0) {
+    RT_CUDA(c, cudaMemcpyAsync(cell_dev, src->cell, 4 * (size_t)nsrc, cudaMemcpyHostToDevice, c->stream));
+    RT_CUDA(c, cudaMemcpyAsync(rt_ptr<double>(c, l.srcrate), src->rate, 8 * (size_t)nsrc * G, cudaMemcpyHostToDevice, c->stream));
+    for (int g = 0; g < G; g++) {
+      double s = 0.0, cc = 0.0;
+      for (int k = 0; k < nsrc; k++) {
+        const double x = src->rate[(size_t)g * nsrc + k], t = s + x;
+        cc += fabs(s) >= fabs(x) ? (s - t) + x : (x - t) + s;
+        s = t;
+      }
+      c->src_total[g] = s + cc;
+    }
+  }
+  rt_launch_init_sources(c, cell_dev, nsrc);
+  RT_CUDA(c, cudaMemsetAsync(rt_ptr<rt_dev_ledger>(c, l.led), 0, sizeof(rt_dev_ledger), c->stream));
+  c->nsub_done = 0;
+  RT_CUDA(c, cudaStreamSynchronize(c->stream));
+  RT_CUDA(c, cudaGetLastError());
+  c->have_state = true;
+  return RT_OK;
+}
+
+int rt_step(rt_ctx *c, double dt, int nsub) {
+  if (!c) return RT_EINVAL;
+  c->err[0] = 0;
+  if (!c->have_state) return rt_fail(c, RT_ESTATE, "rt_step needs rt_state_init first");
+  if (!(dt > 0.0) || nsub < 0) return rt_fail(c, RT_EINVAL, "dt must be positive and nsub >= 0");
+  RT_CUDA(c, cudaSetDevice(c->device));
+  for (int s = 0; s < nsub; s++) {
+    int rc = rt_launch_step(c, dt);
+    if (rc != RT_OK) return rc;
+  }
+  return RT_OK;
+}
+
+static int get_rows(rt_ctx *c, const double *src, double *dst, int mem_kind, int rows, double *stage) {
+  const size_t n = (size_t)rows * c->C;
+  if (mem_kind == RT_MEM_HOST) {
+    rt_launch_permute_out(c, src, stage, rows);
+    RT_CUDA(c, cudaMemcpyAsync(dst, stage, n * 8, cudaMemcpyDeviceToHost, c->stream));
+    return RT_OK;
+  }
+  return rt_launch_permute_out(c, src, dst, rows);
+}
+
+int rt_download(rt_ctx *c, rt_state *out, rt_ledger *led) {
+  if (!c) return RT_EINVAL;
+  c->err[0] = 0;
+  if (!c->have_state) return rt_fail(c, RT_ESTATE, "rt_download needs rt_state_init first");
+  RT_CUDA(c, cudaSetDevice(c->device));
+  const rt_layout &l = c->lay;
+  const int G = c->G;
+  const int64_t C = c->C;
+  int rc;
+  if (out) {
+    double *stage = rt_ptr<double>(c, l.grad);
+    const double *Ua = rt_ptr<double>(c, l.Ua);
+    for (int g = 0; g < G; g++) {
+      if (out->N && (rc = get_rows(c, Ua + (size_t)4 * g * C, out->N + (size_t)g * C, out->mem_kind, 1, stage))) return rc;
+      if (out->F && (rc = get_rows(c, Ua + (size_t)(4 * g + 1) * C, out->F + (size_t)3 * g * C, out->mem_kind, 3, stage + C)))
+        return rc;
+      stage += 4 * C;
+    }
+    double *xs[4] = {out->xHII, out->xHeII, out->xHeIII, out->eth};
+    const size_t xo[4] = {l.xHII, l.xHeII, l.xHeIII, l.eth};
+    for (int k = 0; k < 4; k++)
+      if (xs[k] && (rc = get_rows(c, rt_ptr<double>(c, xo[k]), xs[k], out->mem_kind, 1, stage + (size_t)k * C))) return rc;
+  }
+  rt_dev_ledger h;
+  if (led) {
+    rt_launch_stored(c);
+    RT_CUDA(c, cudaMemcpyAsync(&h, rt_ptr<rt_dev_ledger>(c, l.led), sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+  }
+  RT_CUDA(c, cudaStreamSynchronize(c->stream));
+  RT_CUDA(c, cudaGetLastError());
+  if (led) {
+    memset(led, 0, sizeof(*led));
+    for (int g = 0; g < G; g++) {
+      led->absorbed[g] = h.acc[0][g][0] + h.acc[0][g][1];
+      led->outflow[g] = h.acc[1][g][0] + h.acc[1][g][1];
+      led->inflow_bc[g] = h.acc[2][g][0] + h.acc[2][g][1];
+      led->floor_added[g] = h.acc[3][g][0] + h.acc[3][g][1];
+      led->stored[g] = h.acc[4][g][0];
+      led->injected[g] = c->injected[g][0] + c->injected[g][1];
+    }
+    led->substeps_total = (int64_t)h.substeps_total;
+    led->substeps_max = (int64_t)h.substeps_max;
+    led->cells_hit_cap = (int64_t)h.cells_hit_cap;
+    led->nsub_done = c->nsub_done;
+  }
+  return RT_OK;
+}
+
+int rt_debug_gradients(rt_ctx *c, int mem_kind, double *gN, double *gF) {
+  if (!c) return RT_EINVAL;
+  c->err[0] = 0;
+  if (!c->have_state) return rt_fail(c, RT_ESTATE, "rt_debug_gradients needs rt_state_init first");
+  if (!gN || !gF) return rt_fail(c, RT_EINVAL, "null output");
+  RT_CUDA(c, cudaSetDevice(c->device));
+  const rt_layout &l = c->lay;
+  const int64_t C = c->C;
+  rt_launch_gradients(c, rt_ptr<double>(c, l.Ua));
+  double *grad = rt_ptr<double>(c, l.grad);
+  double *stage = rt_ptr<double>(c, l.Ub);  // 4 G C doubles, free between steps; used 3 and 9 rows at a time
+  int rc;
+  for (int g = 0; g < c->G; g++) {
+    if ((rc = get_rows(c, grad + (size_t)12 * g * C, gN + (size_t)3 * g * C, mem_kind, 3, stage))) return rc;
+    RT_CUDA(c, cudaStreamSynchronize(c->stream));
+    // 9 rows do not fit a 4-row stage when G == 1: go 3 rows at a time
+    for (int q = 0; q < 3; q++) {
+      if ((rc = get_rows(c, grad + (size_t)(12 * g + 3 + 3 * q) * C, gF + (size_t)(9 * g + 3 * q) * C, mem_kind, 3, stage)))
+        return rc;
+      RT_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+  }
+  RT_CUDA(c, cudaGetLastError());
+  return RT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,250 @@
+// a1: per-cell thermochemistry over one subcycle (PAPER.md:125-127 semi-implicit scheme,
+// PAPER.md:236-238 adaptive sub-stepping on the GPU).  One thread per cell; the whole sub-step
+// loop runs in registers with no main-memory access inside the iterations.
+// Formulas: readings S17-S24 of DESIGN.md (the paper defers them to Kannan+19); rate fits:
+// DESIGN.md appendix A.
+#include "rt_internal.cuh"
+#include "rt_kernels.cuh"
+
+#define KB_CGS 1.380649e-16
+#define T_FLOOR 10.0
+
+struct rate_set {
+  double aHII, aHeII, aHeIII;      // case-B recombination
+  double bHI, bHeI, bHeII;         // collisional ionisation
+  double cool_ion[3];              // cooling per n_e n_X for X = HII, HeII, HeIII (recombination + brems)
+  double cool_neu[3];              // cooling per n_e n_X for X = HI, HeI, HeII (coll. ionisation + excitation)
+};
+
+__device__ inline double recomb_fit(double lam) {
+  return 2.753e-14 * lam * sqrt(lam) / pow(1.0 + pow(lam * (1.0 / 2.74), 0.407), 2.242);
+}
+__device__ inline double recomb_cool_fit(double T, double lam) {
+  return 3.435e-30 * T * pow(lam, 1.970) / pow(1.0 + pow(lam * (1.0 / 2.250), 0.376), 3.720);
+}
+
+template <bool THERMAL>
+__device__ inline void eval_rates(double T, double aB_override, rate_set &r) {
+  const double iT = 1.0 / T;
+  const double lHI = 2.0 * 157807.0 * iT, lHeI = 2.0 * 285335.0 * iT, lHeII = 2.0 * 631515.0 * iT;
+  const double sq = sqrt(T), q = 1.0 / (1.0 + sqrt(T * 1.0e-5));
+  const double eHI = exp(-157809.1 * iT), eHeI = exp(-285335.4 * iT), eHeII = exp(-631515.0 * iT);
+  const double sqq = sq * q;
+  r.aHII = aB_override > 0.0 ? aB_override : recomb_fit(lHI);
+  r.aHeII = 1.26e-14 * pow(lHeI, 0.75);
+  r.aHeIII = 2.0 * recomb_fit(lHeII);
+  r.bHI = 5.85e-11 * sqq * eHI;
+  r.bHeI = 2.38e-11 * sqq * eHeI;
+  r.bHeII = 5.68e-12 * sqq * eHeII;
+  if (THERMAL) {
+    const double lt = log10(T);
+    const double brem = 1.42e-27 * (1.1 + 0.34 * exp(-(5.5 - lt) * (5.5 - lt) * (1.0 / 3.0))) * sq;
+    r.cool_ion[0] = recomb_cool_fit(T, lHI) + brem;
+    r.cool_ion[1] = KB_CGS * T * r.aHeII + brem;
+    r.cool_ion[2] = 8.0 * recomb_cool_fit(T, lHeII) + 4.0 * brem;
+    r.cool_neu[0] = 1.27e-21 * sqq * eHI + 7.50e-19 * exp(-118348.0 * iT) * q;
+    r.cool_neu[1] = 9.38e-22 * sqq * eHeI;
+    r.cool_neu[2] = 4.95e-22 * sqq * eHeII + 5.54e-17 * pow(T, -0.397) * exp(-473638.0 * iT) * q;
+  }
+}
+
+template <int G>
+struct cell_state {
+  double N[G], Fx[G], Fy[G], Fz[G], xHII, xHeII, xHeIII, e;
+};
+
+// one trial sub-step of size h from s into o; returns the controller's f (C1-C7)
+template <int G, bool THERMAL>
+__device__ inline double trial(const rt_chem_par &P, const cell_state<G> &s, double nH, double h, const rate_set &r,
+                               cell_state<G> &o) {
+  const double y = P.y_he, nHe = y * nH;
+  const double xe = s.xHII + y * (s.xHeII + 2.0 * s.xHeIII);
+  const double ne = nH * xe;
+  const double nHI = nH * (1.0 - s.xHII), nHeI = nHe * (1.0 - s.xHeII - s.xHeIII), nHeII = nHe * s.xHeII;
+  double pHI = 0.0, pHeI = 0.0, pHeII = 0.0, heat = 0.0;
+#pragma unroll
+  for (int g = 0; g < G; g++) {
+    const double k0 = P.sigma[g][0] * nHI, k1 = P.sigma[g][1] * nHeI, k2 = P.sigma[g][2] * nHeII;
+    const double k = k0 + k1 + k2;
+    const double inv = 1.0 / (1.0 + h * P.ctilde * k);
+    o.N[g] = s.N[g] * inv; o.Fx[g] = s.Fx[g] * inv; o.Fy[g] = s.Fy[g] * inv; o.Fz[g] = s.Fz[g] * inv;
+    if (k > 0.0) {
+      const double dNk = (s.N[g] - o.N[g]) / k;
+      const double a0 = dNk * k0, a1 = dNk * k1, a2 = dNk * k2;
+      pHI += a0; pHeI += a1; pHeII += a2;
+      if (THERMAL) heat += a0 * P.eps[g][0] + a1 * P.eps[g][1] + a2 * P.eps[g][2];
+    }
+  }
+  // hydrogen: backward Euler, n_e frozen
+  double nHIIn = (nH * s.xHII + pHI + h * r.bHI * ne * nH) / (1.0 + h * ne * (r.bHI + r.aHII));
+  nHIIn = fmin(fmax(nHIIn, 0.0), nH);
+  o.xHII = nHIIn / nH;
+  double nHeIn = 0.0, nHeIIn = 0.0, nHeIIIn = 0.0;
+  if (nHe > 0.0) {
+    const double hn = h * ne;
+    const double a11 = 1.0 + hn * (r.bHeI + r.aHeII), a12 = hn * r.aHeII;
+    const double a21 = hn * r.bHeII, a22 = 1.0 + hn * (r.aHeIII + r.bHeII);
+    const double b1 = nHeI - pHeI + hn * r.aHeII * nHe;
+    const double b2 = nHe * s.xHeIII + pHeII + hn * r.bHeII * nHe;
+    const double idet = 1.0 / (a11 * a22 - a12 * a21);
+    double a = (b1 * a22 - a12 * b2) * idet, c = (a11 * b2 - a21 * b1) * idet;
+    a = fmin(fmax(a, 0.0), nHe);
+    c = fmin(fmax(c, 0.0), nHe - a);
+    nHeIn = a; nHeIIIn = c; nHeIIn = nHe - a - c;
+    o.xHeII = nHeIIn / nHe; o.xHeIII = nHeIIIn / nHe;
+  } else { o.xHeII = s.xHeII; o.xHeIII = s.xHeIII; }
+  double f = 0.0;
+  if (THERMAL) {
+    const double xen = o.xHII + y * (o.xHeII + 2.0 * o.xHeIII);
+    const double nen = nH * xen;
+    const double lam = nen * (r.cool_ion[0] * nHIIn + r.cool_ion[1] * nHeIIn + r.cool_ion[2] * nHeIIIn +
+                              r.cool_neu[0] * (nH - nHIIn) + r.cool_neu[1] * nHeIn + r.cool_neu[2] * nHeIIn);
+    double en = s.e + heat - h * lam;
+    en = fmax(en, 1.5 * nH * (1.0 + y + xen) * KB_CGS * T_FLOOR);
+    o.e = en;
+    f = fabs(en - s.e) / s.e;
+  } else o.e = s.e;
+  const double fl = P.x_floor_rel;
+  f = fmax(f, fabs(o.xHII - s.xHII) / fmax(s.xHII, fl));
+  f = fmax(f, fabs((1.0 - o.xHII) - (1.0 - s.xHII)) / fmax(1.0 - s.xHII, fl));
+  if (nHe > 0.0) {
+    f = fmax(f, fabs(o.xHeII - s.xHeII) / fmax(s.xHeII, fl));
+    f = fmax(f, fabs(o.xHeIII - s.xHeIII) / fmax(s.xHeIII, fl));
+    f = fmax(f, fabs((1.0 - o.xHeII - o.xHeIII) - (1.0 - s.xHeII - s.xHeIII)) / fmax(1.0 - s.xHeII - s.xHeIII, fl));
+  }
+  return f;
+}
+
+// deterministic block sum over RT_BLOCK threads (fixed tree), result valid in thread 0
+__device__ inline double block_sum(double v, double *sm) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  const int w = threadIdx.x >> 5;
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) sm[w] = v;
+  __syncthreads();
+  double t = 0.0;
+  if (threadIdx.x == 0)
+    for (int k = 0; k < RT_BLOCK / 32; k++) t += sm[k];
+  return t;
+}
+
+template <int G, int MODE>
+__global__ void __launch_bounds__(RT_BLOCK) k_chem(rt_chem_par P, int64_t C, double dt, double *__restrict__ U,
+                                                   double *__restrict__ xHII, double *__restrict__ xHeII,
+                                                   double *__restrict__ xHeIII, double *__restrict__ eth,
+                                                   const double *__restrict__ nHv, const double *__restrict__ vol,
+                                                   const double *__restrict__ kappa, double *__restrict__ part_abs,
+                                                   rt_dev_ledger *led) {
+  constexpr bool THERMAL = (MODE == RT_CHEM_HHE_THERMAL);
+  __shared__ double sm[RT_BLOCK / 32];
+  const int64_t i = (int64_t)blockIdx.x * RT_BLOCK + threadIdx.x;
+  const bool live = i < C;
+  double absd[G];
+#pragma unroll
+  for (int g = 0; g < G; g++) absd[g] = 0.0;
+  unsigned long long attempts = 0;
+  int capped = 0;
+  if (live) {
+    cell_state<G> s;
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+      s.N[g] = U[(size_t)(4 * g) * C + i]; s.Fx[g] = U[(size_t)(4 * g + 1) * C + i];
+      s.Fy[g] = U[(size_t)(4 * g + 2) * C + i]; s.Fz[g] = U[(size_t)(4 * g + 3) * C + i];
+      absd[g] = s.N[g];
+    }
+    if (MODE == RT_CHEM_FIXED_OPACITY) {
+      // one implicit step of the absorption terms of eqs (6)-(7): N' = N/(1 + dt c kappa)
+      const double den = 1.0 + dt * P.ctilde * kappa[i];
+#pragma unroll
+      for (int g = 0; g < G; g++) { s.N[g] /= den; s.Fx[g] /= den; s.Fy[g] /= den; s.Fz[g] /= den; }
+    } else {
+      const double nH = nHv[i];
+      s.xHII = xHII[i]; s.xHeII = xHeII[i]; s.xHeIII = xHeIII[i]; s.e = eth[i];
+      rate_set r;
+      if (!THERMAL) eval_rates<false>(P.T_fixed, P.alphaB_override, r);
+      // controller of PAPER.md:238: start with h = dt; reject if f > 0.1 and shrink by f_s/f; on
+      // accept scale by f_s/f but at most double; the last step is clipped to end at dt
+      double t = 0.0, h = dt;
+      bool last = true;
+      while (true) {
+        if ((long long)attempts >= P.max_substeps) { capped = 1; break; }
+        if (THERMAL) {
+          const double xe = s.xHII + P.y_he * (s.xHeII + 2.0 * s.xHeIII);
+          const double T = (2.0 / 3.0) * s.e / (KB_CGS * (nH * (1.0 + P.y_he + xe)));
+          eval_rates<true>(T, P.alphaB_override, r);
+        }
+        cell_state<G> o;
+        const double f = trial<G, THERMAL>(P, s, nH, h, r, o);
+        attempts++;
+        if (f > P.f_accept) { h = h * P.f_target / f; last = false; continue; }
+        s = o;
+        if (last) break;
+        t += h;
+        h = h * fmin(2.0, P.f_target / fmax(f, 1e-300));
+        if (h >= dt - t) { h = dt - t; last = true; }
+      }
+      xHII[i] = s.xHII; xHeII[i] = s.xHeII; xHeIII[i] = s.xHeIII;
+      if (THERMAL) eth[i] = s.e;
+    }
+    const double V = vol[i];
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+      U[(size_t)(4 * g) * C + i] = s.N[g]; U[(size_t)(4 * g + 1) * C + i] = s.Fx[g];
+      U[(size_t)(4 * g + 2) * C + i] = s.Fy[g]; U[(size_t)(4 * g + 3) * C + i] = s.Fz[g];
+      absd[g] = V * (absd[g] - s.N[g]);
+    }
+  }
+#pragma unroll
+  for (int g = 0; g < G; g++) {
+    const double t = block_sum(absd[g], sm);
+    if (threadIdx.x == 0) part_abs[(size_t)blockIdx.x * G + g] = t;
+  }
+  if (MODE != RT_CHEM_FIXED_OPACITY) {
+    // integer counters: order-independent, so atomics keep the result deterministic
+    unsigned long long wsum = attempts, wmax = attempts;
+    int wcap = capped;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      wsum += __shfl_down_sync(0xffffffffu, wsum, o);
+      unsigned long long m = __shfl_down_sync(0xffffffffu, wmax, o);
+      wmax = m > wmax ? m : wmax;
+      wcap += __shfl_down_sync(0xffffffffu, wcap, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+      atomicAdd(&led->substeps_total, wsum);
+      atomicMax(&led->substeps_max, wmax);
+      if (wcap) atomicAdd(&led->cells_hit_cap, (unsigned long long)wcap);
+    }
+  }
+}
+
+template <int G>
+static void launch_chem_g(rt_ctx *c, const rt_chem_par &P, double dt, double *U) {
+  const rt_layout &l = c->lay;
+  dim3 grid((unsigned)l.nbc), block(RT_BLOCK);
+  double *part = rt_ptr<double>(c, l.part);
+#define CHEM_ARGS P, c->C, dt, U, rt_ptr<double>(c, l.xHII), rt_ptr<double>(c, l.xHeII), rt_ptr<double>(c, l.xHeIII), \
+      rt_ptr<double>(c, l.eth), rt_ptr<double>(c, l.nH), rt_ptr<double>(c, l.vol), rt_ptr<double>(c, l.kappa), part, \
+      rt_ptr<rt_dev_ledger>(c, l.led)
+  switch (c->par.chem_mode) {
+    case RT_CHEM_FIXED_OPACITY: k_chem<G, RT_CHEM_FIXED_OPACITY><<<grid, block, 0, c->stream>>>(CHEM_ARGS); break;
+    case RT_CHEM_H_ISOTHERMAL: k_chem<G, RT_CHEM_H_ISOTHERMAL><<<grid, block, 0, c->stream>>>(CHEM_ARGS); break;
+    default: k_chem<G, RT_CHEM_HHE_THERMAL><<<grid, block, 0, c->stream>>>(CHEM_ARGS); break;
+  }
+#undef CHEM_ARGS
+}
+
+void rt_launch_chem(rt_ctx *c, const rt_chem_par &P, double dt, double *U) {
+  switch (c->G) {
+    case 1: launch_chem_g<1>(c, P, dt, U); break;
+    case 2: launch_chem_g<2>(c, P, dt, U); break;
+    case 3: launch_chem_g<3>(c, P, dt, U); break;
+    case 4: launch_chem_g<4>(c, P, dt, U); break;
+    case 5: launch_chem_g<5>(c, P, dt, U); break;
+    case 6: launch_chem_g<6>(c, P, dt, U); break;
+    case 7: launch_chem_g<7>(c, P, dt, U); break;
+    default: launch_chem_g<8>(c, P, dt, U); break;
+  }
+  c->launches++;
+}

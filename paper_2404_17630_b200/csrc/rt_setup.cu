@@ -1,0 +1,342 @@
+// rt_mesh_upload's device-side setup: validation, Peano-Hilbert reordering, faces by owner,
+// cell -> face lists, and the mesh-only parts of eq (15).
+// Runs once per mesh, outside the timed subcycles.  CUB is used for the two radix sorts.
+#include <cub/cub.cuh>
+#include "rt_internal.cuh"
+
+#define SETUP_BLOCK 256
+static inline unsigned nblk(int64_t n) { return (unsigned)((n + SETUP_BLOCK - 1) / SETUP_BLOCK); }
+
+struct geom_in {
+  const double *volume, *centroid, *area, *normal, *fcentroid;
+  const int32_t *left, *right;
+};
+
+// error flag bits
+enum { E_LEFT = 1, E_RIGHT = 2, E_VOL = 4, E_AREA = 8, E_NORMAL = 16, E_CLOSURE = 32, E_MATRIX = 64, E_GHOST = 128 };
+
+__global__ void k_validate(geom_in g, int64_t C, int64_t F, int nghost, int *flags) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int e = 0;
+  if (i < C && !(g.volume[i] > 0.0)) e |= E_VOL;
+  if (i < F) {
+    if (g.left[i] < 0 || g.left[i] >= C) e |= E_LEFT;
+    int32_t r = g.right[i];
+    if (r >= C || r == g.left[i]) e |= E_RIGHT;
+    if (r <= RT_BC_DIRICHLET0 && (RT_BC_DIRICHLET0 - r) >= nghost) e |= E_GHOST;
+    if (!(g.area[i] > 0.0)) e |= E_AREA;
+    double nx = g.normal[i], ny = g.normal[F + i], nz = g.normal[2 * F + i];
+    if (!(fabs(nx * nx + ny * ny + nz * nz - 1.0) < 1e-10)) e |= E_NORMAL;
+  }
+  if (e) atomicOr(flags, e);
+}
+
+// Hilbert index of a 3-D point with 21 bits per axis (Skilling's transpose algorithm).
+__device__ inline uint64_t hilbert3(uint32_t x, uint32_t y, uint32_t z) {
+  const int b = 21;
+  uint32_t X[3] = {x, y, z};
+  uint32_t M = 1u << (b - 1);
+  for (uint32_t Q = M; Q > 1; Q >>= 1) {
+    uint32_t P = Q - 1;
+    for (int i = 0; i < 3; i++) {
+      if (X[i] & Q) X[0] ^= P;
+      else { uint32_t t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
+    }
+  }
+  X[1] ^= X[0]; X[2] ^= X[1];
+  uint32_t t = 0;
+  for (uint32_t Q = M; Q > 1; Q >>= 1) if (X[2] & Q) t ^= Q - 1;
+  X[0] ^= t; X[1] ^= t; X[2] ^= t;
+  uint64_t key = 0;
+  for (int k = b - 1; k >= 0; k--)
+    for (int i = 0; i < 3; i++) key = (key << 1) | ((X[i] >> k) & 1u);
+  return key;
+}
+
+__global__ void k_cell_keys(const double *centroid, int64_t C, double bx, double by, double bz, uint64_t *keys,
+                            int32_t *idx) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= C) return;
+  double b[3] = {bx, by, bz};
+  uint32_t q[3];
+  for (int a = 0; a < 3; a++) {
+    double u = centroid[a * C + i] / b[a];
+    u -= floor(u);  // wrap into [0,1)
+    double v = u * 2097152.0;
+    q[a] = v >= 2097151.0 ? 2097151u : (uint32_t)v;
+  }
+  keys[i] = hilbert3(q[0], q[1], q[2]);
+  idx[i] = (int32_t)i;
+}
+
+__global__ void k_permute_cells(geom_in g, int64_t C, const int32_t *perm, int32_t *iperm, double *vol, double *s) {
+  int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= C) return;
+  int32_t o = perm[p];
+  iperm[o] = (int32_t)p;
+  vol[p] = g.volume[o];
+  for (int a = 0; a < 3; a++) s[a * C + p] = g.centroid[a * C + o];
+}
+
+__device__ inline uint64_t face_key(int32_t l, int32_t r) {
+  uint32_t sub = r >= 0 ? (uint32_t)r : 0x80000000u + (uint32_t)(-r);
+  return ((uint64_t)(uint32_t)l << 32) | sub;
+}
+
+__global__ void k_face_keys(geom_in g, int64_t F, const int32_t *iperm, uint64_t *keys, int32_t *idx) {
+  int64_t f = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (f >= F) return;
+  int32_t l = iperm[g.left[f]], r = g.right[f];
+  if (r >= 0) { r = iperm[r]; if (r < l) { int32_t t = l; l = r; r = t; } }
+  keys[f] = face_key(l, r);
+  idx[f] = (int32_t)f;
+}
+
+__global__ void k_gather_faces(geom_in g, int64_t C, int64_t F, const int32_t *order, const uint64_t *keys,
+                               const int32_t *iperm, const double *s, double bx, double by, double bz, int p0, int p1,
+                               int p2, double *A, double *nrm, double *cf, int32_t *L, int32_t *R) {
+  int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= F) return;
+  int32_t f = order[q];
+  int32_t l = (int32_t)(keys[q] >> 32);
+  int32_t ro = g.right[f];
+  int32_t r = ro >= 0 ? iperm[ro] : ro;
+  bool flip = (iperm[g.left[f]] != l);
+  if (flip) r = iperm[g.left[f]];
+  L[q] = l; R[q] = r;
+  A[q] = g.area[f];
+  double sg = flip ? -1.0 : 1.0;
+  double b[3] = {bx, by, bz};
+  int per[3] = {p0, p1, p2};
+  for (int a = 0; a < 3; a++) {
+    nrm[a * F + q] = sg * g.normal[a * F + f];
+    double sl = s[a * C + l];
+    cf[a * F + q] = sl + rt_wrap(g.fcentroid[a * F + f] - sl, b[a], per[a]);  // left cell's frame
+  }
+}
+
+// first index q in sorted keys with keys[q] >= (i << 32), for i = 0..C
+__global__ void k_lower_bounds(const uint64_t *keys, int64_t n, int64_t C, int64_t *out) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i > C) return;
+  uint64_t target = (uint64_t)i << 32;
+  int64_t lo = 0, hi = n;
+  while (lo < hi) {
+    int64_t mid = (lo + hi) >> 1;
+    if (keys[mid] < target) lo = mid + 1; else hi = mid;
+  }
+  out[i] = lo;
+}
+
+__global__ void k_rkeys(const int32_t *R, int64_t F, uint64_t *keys) {
+  int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= F) return;
+  keys[q] = R[q] >= 0 ? (((uint64_t)(uint32_t)R[q] << 32) | (uint32_t)q) : ~0ull;
+}
+
+__global__ void k_rlist(const uint64_t *keys, int64_t NR, int32_t *rl) {
+  int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < NR) rl[k] = (int32_t)(keys[k] & 0xffffffffu);
+}
+
+// per-face prefactor of eq (15)'s second term, seen from the left cell: w = A d/|d|^2,
+// d = s_R - s_L measured through the face; boundary faces use the mirror point (S13)
+__global__ void k_face_geom(int64_t C, int64_t F, const double *s, const double *A, const double *nrm, const double *cf,
+                            const int32_t *L, const int32_t *R, double bx, double by, double bz, int p0, int p1, int p2,
+                            double *w) {
+  int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= F) return;
+  double b[3] = {bx, by, bz};
+  int per[3] = {p0, p1, p2};
+  int32_t l = L[q], r = R[q];
+  double d[3];
+  if (r >= 0) {
+    for (int a = 0; a < 3; a++) {
+      double c = cf[a * F + q];
+      d[a] = (c - s[a * C + l]) - rt_wrap(c - s[a * C + r], b[a], per[a]);
+    }
+  } else {
+    double n[3] = {nrm[q], nrm[F + q], nrm[2 * F + q]};
+    double p = 0.0;
+    for (int a = 0; a < 3; a++) p += (cf[a * F + q] - s[a * C + l]) * n[a];
+    for (int a = 0; a < 3; a++) d[a] = 2.0 * p * n[a];
+  }
+  double d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+  double k = A[q] / d2;
+  for (int a = 0; a < 3; a++) w[a * F + q] = k * d[a];
+}
+
+// per cell: M = sum_f A n n^T (n = d/|d| = w/|w|), its inverse, and the closure check
+__global__ void k_cell_geom(int64_t C, int64_t F, const double *A, const double *nrm, const double *w,
+                            const int64_t *fo, const int64_t *ro, const int32_t *rl, double *Minv, int *flags) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= C) return;
+  double m[6] = {0, 0, 0, 0, 0, 0}, cl[3] = {0, 0, 0}, sa = 0.0;
+  int64_t n_own = fo[i + 1] - fo[i], n_r = ro[i + 1] - ro[i];
+  for (int64_t k = 0; k < n_own + n_r; k++) {
+    int64_t q = k < n_own ? fo[i] + k : rl[ro[i] + (k - n_own)];
+    double sg = k < n_own ? 1.0 : -1.0;
+    double a = A[q];
+    double wx = w[q], wy = w[F + q], wz = w[2 * F + q];
+    double w2 = wx * wx + wy * wy + wz * wz;
+    double f = a / w2;  // A n n^T = A w w^T / |w|^2
+    m[0] += f * wx * wx; m[1] += f * wx * wy; m[2] += f * wx * wz;
+    m[3] += f * wy * wy; m[4] += f * wy * wz; m[5] += f * wz * wz;
+    cl[0] += sg * a * nrm[q]; cl[1] += sg * a * nrm[F + q]; cl[2] += sg * a * nrm[2 * F + q];
+    sa += a;
+  }
+  int e = 0;
+  if (!(sqrt(cl[0] * cl[0] + cl[1] * cl[1] + cl[2] * cl[2]) <= 1e-10 * sa)) e |= E_CLOSURE;
+  double c00 = m[3] * m[5] - m[4] * m[4], c01 = m[4] * m[2] - m[1] * m[5], c02 = m[1] * m[4] - m[3] * m[2];
+  double det = m[0] * c00 + m[1] * c01 + m[2] * c02;
+  if (!(fabs(det) > 0.0)) { e |= E_MATRIX; det = 1.0; }
+  double id = 1.0 / det;
+  Minv[0 * C + i] = c00 * id;
+  Minv[1 * C + i] = c01 * id;
+  Minv[2 * C + i] = c02 * id;
+  Minv[3 * C + i] = (m[0] * m[5] - m[2] * m[2]) * id;
+  Minv[4 * C + i] = (m[1] * m[2] - m[0] * m[4]) * id;
+  Minv[5 * C + i] = (m[0] * m[3] - m[1] * m[1]) * id;
+  if (e) atomicOr(flags, e);
+}
+
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
+  const int64_t C = c->C, F = c->F;
+  const rt_layout &lay = c->lay;
+  cudaStream_t st = c->stream;
+  // carve the scratch region
+  size_t o = lay.temp;
+  auto take = [&](size_t bytes) { size_t r = o; o = align256(o + bytes); return r; };
+  const int64_t NM = C > F ? C : F;
+  uint64_t *k0 = rt_ptr<uint64_t>(c, take(8 * NM)), *k1 = rt_ptr<uint64_t>(c, take(8 * NM));
+  int32_t *v0 = rt_ptr<int32_t>(c, take(4 * NM)), *v1 = rt_ptr<int32_t>(c, take(4 * NM));
+  int *flags = rt_ptr<int>(c, take(256));
+  size_t cub_bytes = 0;
+  {
+    cub::DoubleBuffer<uint64_t> dk(k0, k1);
+    cub::DoubleBuffer<int32_t> dv(v0, v1);
+    size_t b1 = 0, b2 = 0;
+    cub::DeviceRadixSort::SortPairs(nullptr, b1, dk, dv, NM, 0, 64, st);
+    cub::DeviceRadixSort::SortKeys(nullptr, b2, dk, NM, 0, 64, st);
+    cub_bytes = b1 > b2 ? b1 : b2;
+  }
+  void *cub_tmp = rt_ptr<void>(c, take(cub_bytes));
+  geom_in g;
+  if (m->mem_kind == RT_MEM_HOST) {
+    double *dv = rt_ptr<double>(c, take(8 * C)), *dc = rt_ptr<double>(c, take(24 * C));
+    double *da = rt_ptr<double>(c, take(8 * F)), *dn = rt_ptr<double>(c, take(24 * F)), *df = rt_ptr<double>(c, take(24 * F));
+    int32_t *dl = rt_ptr<int32_t>(c, take(4 * F)), *dr = rt_ptr<int32_t>(c, take(4 * F));
+    if (o > c->ws_bytes) return rt_fail(c, RT_ENOMEM, "workspace too small for host-mesh staging");
+    RT_CUDA(c, cudaMemcpyAsync(dv, m->volume, 8 * C, cudaMemcpyHostToDevice, st));
+    RT_CUDA(c, cudaMemcpyAsync(dc, m->centroid, 24 * C, cudaMemcpyHostToDevice, st));
+    RT_CUDA(c, cudaMemcpyAsync(da, m->area, 8 * F, cudaMemcpyHostToDevice, st));
+    RT_CUDA(c, cudaMemcpyAsync(dn, m->normal, 24 * F, cudaMemcpyHostToDevice, st));
+    RT_CUDA(c, cudaMemcpyAsync(df, m->fcentroid, 24 * F, cudaMemcpyHostToDevice, st));
+    RT_CUDA(c, cudaMemcpyAsync(dl, m->left, 4 * F, cudaMemcpyHostToDevice, st));
+    RT_CUDA(c, cudaMemcpyAsync(dr, m->right, 4 * F, cudaMemcpyHostToDevice, st));
+    g = {dv, dc, da, dn, df, dl, dr};
+  } else {
+    g = {m->volume, m->centroid, m->area, m->normal, m->fcentroid, m->left, m->right};
+  }
+  if (o > c->ws_bytes) return rt_fail(c, RT_ENOMEM, "workspace too small for setup scratch");
+  RT_CUDA(c, cudaMemsetAsync(flags, 0, sizeof(int), st));
+  k_validate<<<nblk(NM), SETUP_BLOCK, 0, st>>>(g, C, F, m->nghost, flags);
+  int hflags = 0;
+  RT_CUDA(c, cudaMemcpyAsync(&hflags, flags, sizeof(int), cudaMemcpyDeviceToHost, st));
+  RT_CUDA(c, cudaStreamSynchronize(st));
+  if (hflags)
+    return rt_fail(c, RT_EMESH, "mesh validation failed:%s%s%s%s%s%s", hflags & E_LEFT ? " left index out of range;" : "",
+                   hflags & E_RIGHT ? " right index out of range or equal to left;" : "",
+                   hflags & E_GHOST ? " Dirichlet ghost index >= nghost;" : "", hflags & E_VOL ? " volume <= 0;" : "",
+                   hflags & E_AREA ? " area <= 0;" : "", hflags & E_NORMAL ? " normal not unit;" : "");
+  int32_t *perm = rt_ptr<int32_t>(c, lay.perm), *iperm = rt_ptr<int32_t>(c, lay.iperm);
+  double *vol = rt_ptr<double>(c, lay.vol), *s = rt_ptr<double>(c, lay.s);
+  // 1. cells along the Peano-Hilbert curve
+  {
+    k_cell_keys<<<nblk(C), SETUP_BLOCK, 0, st>>>(g.centroid, C, c->box[0], c->box[1], c->box[2], k0, v0);
+    cub::DoubleBuffer<uint64_t> dk(k0, k1);
+    cub::DoubleBuffer<int32_t> dv(v0, v1);
+    size_t b = cub_bytes;
+    RT_CUDA(c, cub::DeviceRadixSort::SortPairs(cub_tmp, b, dk, dv, C, 0, 63, st));
+    RT_CUDA(c, cudaMemcpyAsync(perm, dv.Current(), 4 * C, cudaMemcpyDeviceToDevice, st));
+    k_permute_cells<<<nblk(C), SETUP_BLOCK, 0, st>>>(g, C, perm, iperm, vol, s);
+  }
+  // 2. faces by owner
+  double *A = rt_ptr<double>(c, lay.A), *nrm = rt_ptr<double>(c, lay.nrm), *cf = rt_ptr<double>(c, lay.cf);
+  double *w = rt_ptr<double>(c, lay.w);
+  int32_t *L = rt_ptr<int32_t>(c, lay.L), *R = rt_ptr<int32_t>(c, lay.R);
+  int64_t *fo = rt_ptr<int64_t>(c, lay.fo), *ro = rt_ptr<int64_t>(c, lay.ro);
+  int32_t *rl = rt_ptr<int32_t>(c, lay.rl);
+  {
+    k_face_keys<<<nblk(F), SETUP_BLOCK, 0, st>>>(g, F, iperm, k0, v0);
+    cub::DoubleBuffer<uint64_t> dk(k0, k1);
+    cub::DoubleBuffer<int32_t> dv(v0, v1);
+    size_t b = cub_bytes;
+    RT_CUDA(c, cub::DeviceRadixSort::SortPairs(cub_tmp, b, dk, dv, F, 0, 64, st));
+    k_gather_faces<<<nblk(F), SETUP_BLOCK, 0, st>>>(g, C, F, dv.Current(), dk.Current(), iperm, s, c->box[0], c->box[1],
+                                                    c->box[2], c->per[0], c->per[1], c->per[2], A, nrm, cf, L, R);
+    k_lower_bounds<<<nblk(C + 1), SETUP_BLOCK, 0, st>>>(dk.Current(), F, C, fo);
+  }
+  // 3. right lists
+  {
+    k_rkeys<<<nblk(F), SETUP_BLOCK, 0, st>>>(R, F, k0);
+    cub::DoubleBuffer<uint64_t> dk(k0, k1);
+    size_t b = cub_bytes;
+    RT_CUDA(c, cub::DeviceRadixSort::SortKeys(cub_tmp, b, dk, F, 0, 64, st));
+    k_lower_bounds<<<nblk(C + 1), SETUP_BLOCK, 0, st>>>(dk.Current(), F, C, ro);
+    int64_t NR = 0;
+    RT_CUDA(c, cudaMemcpyAsync(&NR, ro + C, 8, cudaMemcpyDeviceToHost, st));
+    RT_CUDA(c, cudaStreamSynchronize(st));
+    c->NR = NR;
+    if (NR > 0) k_rlist<<<nblk(NR), SETUP_BLOCK, 0, st>>>(dk.Current(), NR, rl);
+  }
+  // 4. geometry of eq (15)
+  k_face_geom<<<nblk(F), SETUP_BLOCK, 0, st>>>(C, F, s, A, nrm, cf, L, R, c->box[0], c->box[1], c->box[2], c->per[0],
+                                               c->per[1], c->per[2], w);
+  k_cell_geom<<<nblk(C), SETUP_BLOCK, 0, st>>>(C, F, A, nrm, w, fo, ro, rl, rt_ptr<double>(c, lay.Minv), flags);
+  RT_CUDA(c, cudaMemcpyAsync(&hflags, flags, sizeof(int), cudaMemcpyDeviceToHost, st));
+  if (m->nghost > 0)
+    RT_CUDA(c, cudaMemcpyAsync(rt_ptr<double>(c, lay.ghost), m->ghost_state, sizeof(double) * m->nghost * 4 * c->G,
+                               cudaMemcpyHostToDevice, st));
+  RT_CUDA(c, cudaStreamSynchronize(st));
+  RT_CUDA(c, cudaGetLastError());
+  if (hflags)
+    return rt_fail(c, RT_EMESH, "mesh validation failed:%s%s",
+                   hflags & E_CLOSURE ? " a cell is not closed (|sum s A n| > 1e-10 sum A);" : "",
+                   hflags & E_MATRIX ? " singular gradient matrix;" : "");
+  return RT_OK;
+}
+
+rt_layout rt_make_layout(int64_t C, int64_t F, int G) {
+  rt_layout l;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o = align256(o + bytes); return r; };
+  l.nbc = (C + RT_BLOCK - 1) / RT_BLOCK;
+  l.nbf = (F + RT_BLOCK - 1) / RT_BLOCK;
+  l.perm = take(4 * C); l.iperm = take(4 * C);
+  l.vol = take(8 * C); l.s = take(24 * C); l.Minv = take(48 * C);
+  l.A = take(8 * F); l.nrm = take(24 * F); l.cf = take(24 * F); l.w = take(24 * F);
+  l.L = take(4 * F); l.R = take(4 * F);
+  l.fo = take(8 * (C + 1)); l.ro = take(8 * (C + 1)); l.rl = take(4 * F);
+  l.ghost = take(8 * 4 * RT_MAXG * 64);
+  l.led = take(sizeof(rt_dev_ledger));
+  l.temp = o;
+  l.Ua = take(32 * (size_t)G * C); l.Ub = take(32 * (size_t)G * C);
+  l.grad = take(96 * (size_t)G * C);
+  l.phi = take(32 * (size_t)G * F);
+  l.xHII = take(8 * C); l.xHeII = take(8 * C); l.xHeIII = take(8 * C); l.eth = take(8 * C); l.nH = take(8 * C);
+  l.kappa = take(8 * C);
+  l.srcidx = take(4 * C);
+  l.srcrate = take(8 * (size_t)G * 65536);
+  // partial sums: chem absorbed [nbc][G], update floor + stored [nbc][2G], flux outflow + inflow [nbf][2G]
+  l.part = take(8 * (size_t)G * (3 * l.nbc + 2 * l.nbf));
+  l.scratch_end = o;
+  // setup scratch aliases the state region; make sure it fits (incl. staging of a host mesh)
+  int64_t NM = C > F ? C : F;
+  size_t need = 24 * (size_t)NM + 4096 + (size_t)(64 << 20) + 88 * (size_t)F + 32 * (size_t)C + 16 * 256;
+  if (l.temp + need > o) o = align256(l.temp + need);
+  l.total = o;
+  return l;
+}

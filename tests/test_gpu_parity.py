@@ -1,0 +1,165 @@
+"""GPU <-> oracle parity through the C ABI (run with -m gpu on the B200 box)."""
+import numpy as np
+import pytest
+
+from paper_2404_17630_b200.inputs import configs as cfg
+from paper_2404_17630_b200.inputs import mesh as M
+import parity as P
+
+pytestmark = pytest.mark.gpu
+
+
+def _pair(oracle_mod, w):
+    from paper_2404_17630_b200 import rt
+    o = oracle_mod.Oracle(w.mesh, w.params); o.set_sources(w.sources); o.set_state(w.state)
+    s = rt.Solver(w.mesh, w.params); s.init(w.state, w.sources)
+    return o, s
+
+
+CASES = [(0, 12), (1, 24), (2, 10), (3, 10), (4, 9)]
+
+
+@pytest.mark.parametrize("c,n", CASES)
+def test_first_subcycle(oracle_mod, c, n):
+    w = cfg.get(c, n)
+    o, s = _pair(oracle_mod, w)
+    prev = o.get_state()
+    o.step(w.dt, 1); s.step(w.dt, 1)
+    got, lg = s.download()
+    e = P.step_errors(w.mesh, w.params.ctilde, prev, o.get_state(), got)
+    assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
+    assert max(e["xHII"], e["xHeII"], e["xHeIII"]) <= 1e-10 and e["eth"] <= 1e-9, e
+    assert P.ledger_errors(o.ledger(), lg) <= P.TOL_LEDGER
+
+
+@pytest.mark.parametrize("c,n,k", [(0, 12, 40), (1, 24, 40), (2, 10, 30), (3, 10, 20), (4, 9, 20)])
+def test_step_from_developed_state(oracle_mod, c, n, k):
+    """GPU runs k subcycles and downloads; the oracle advances that state by one subcycle and is
+    compared with the GPU's k+1 (SURVEY.md 8(c) parity metric)."""
+    from paper_2404_17630_b200 import rt
+    w = cfg.get(c, n)
+    s = rt.Solver(w.mesh, w.params); s.init(w.state, w.sources)
+    s.step(w.dt, k)
+    dev, _ = s.download()
+    dev["nH"] = w.state.nH
+    s.step(w.dt, 1)
+    got, _ = s.download()
+    o = oracle_mod.Oracle(w.mesh, w.params); o.set_sources(w.sources); o.set_state(P.as_state(dev))
+    o.step(w.dt, 1)
+    e = P.step_errors(w.mesh, w.params.ctilde, dev, o.get_state(), got)
+    assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
+    assert max(e["xHII"], e["xHeII"], e["xHeIII"]) <= 1e-9 and e["eth"] <= 1e-8, e
+
+
+@pytest.mark.parametrize("c,n", [(0, 12), (2, 10), (3, 10)])
+def test_100_subcycles_fractions_and_ledger(oracle_mod, c, n):
+    w = cfg.get(c, n)
+    o, s = _pair(oracle_mod, w)
+    stored0 = (w.state.N * w.mesh.volume).sum(1)
+    o.step(w.dt, 100); s.step(w.dt, 100)
+    got, lg = s.download()
+    ref = o.get_state()
+    for k in ("xHII", "xHeII", "xHeIII"):
+        assert np.max(np.abs(got[k] - ref[k])) <= P.TOL_X, k
+    lo = o.ledger()
+    assert P.ledger_errors(lo, lg) <= 1e-11
+    assert P.budget_residual(lg, stored0).max() <= P.TOL_LEDGER
+    assert lg["substeps_total"] == lo["substeps_total"] and lg["substeps_max"] == lo["substeps_max"]
+    assert got["N"].min() >= w.params.n_floor
+    for g in range(w.params.ngroup):
+        fn = np.sqrt((got["F"][g] ** 2).sum(0))
+        assert np.all(fn <= w.params.ctilde * got["N"][g] * (1 + 1e-14))
+
+
+def test_gradients_match_oracle(oracle_mod):
+    w = cfg.get(2, 8)
+    rs = np.random.RandomState(0)
+    C = w.mesh.ncell
+    w.state.N[:] = rs.uniform(0.5, 2, (3, C))
+    w.state.F[:] = rs.randn(3, 3, C) * 0.1
+    o, s = _pair(oracle_mod, w)
+    gN, gF = o.gradients()
+    hN, hF = s.gradients()
+    sc = np.abs(gN).max()
+    assert np.max(np.abs(gN - hN)) <= 1e-12 * sc
+    assert np.max(np.abs(gF - hF)) <= 1e-12 * np.abs(gF).max()
+
+
+@pytest.mark.parametrize("kind", ["open2", "periodic2", "mixed_bc3"])
+def test_tiny_meshes_and_boundaries(oracle_mod, kind):
+    ct = 0.8
+    ghost = np.array([[1.3, 0.5, 0.1, -0.2]])
+    mesh = {"open2": lambda: M.cartesian(2, 1.0, periodic=False), "periodic2": lambda: M.cartesian(2, 1.0, periodic=True),
+            "mixed_bc3": lambda: M.cartesian(3, 1.5, periodic=False, bc=(-2, -1, -3, -2, -1, -3))}[kind]()
+    rs = np.random.RandomState(3)
+    C = mesh.ncell
+    N = rs.uniform(0.5, 2.0, (1, C)); F = rs.randn(1, 3, C) * 0.2
+    st = cfg.State(N, F, np.zeros(C), np.zeros(C), np.zeros(C), np.ones(C), np.ones(C))
+    p = cfg.Params(ngroup=1, ctilde=ct, ghost_state=ghost)
+    w = cfg.Workload(kind, mesh, p, st, cfg.Sources(np.zeros(0, np.int32), np.zeros((1, 0))), cfg.cfl_dt(mesh, ct))
+    o, s = _pair(oracle_mod, w)
+    prev = o.get_state()
+    o.step(w.dt, 3); s.step(w.dt, 3)
+    got, lg = s.download()
+    e = P.step_errors(mesh, ct, prev, o.get_state(), got)
+    assert e["N"] <= 1e-12 and e["F"] <= 1e-12, e
+    assert P.ledger_errors(o.ledger(), lg) <= P.TOL_LEDGER
+
+
+def test_restart_bit_exact_and_first_order_euler(oracle_mod):
+    from paper_2404_17630_b200 import rt
+    w = cfg.get(2, 8)
+    a = rt.Solver(w.mesh, w.params); a.init(w.state, w.sources); a.step(w.dt, 6)
+    b = rt.Solver(w.mesh, w.params); b.init(w.state, w.sources); b.step(w.dt, 3)
+    mid, _ = b.download(); mid["nH"] = w.state.nH
+    c = rt.Solver(w.mesh, w.params); c.init(mid, w.sources); c.step(w.dt, 3)
+    sa, _ = a.download(); sc, _ = c.download()
+    for k in sa:
+        assert np.array_equal(sa[k], sc[k]), k                       # P13
+    w.params.order, w.params.heun = 1, 0
+    o, s = _pair(oracle_mod, w)
+    prev = o.get_state()
+    o.step(w.dt, 5); s.step(w.dt, 5)
+    got, lg = s.download()
+    e = P.step_errors(w.mesh, w.params.ctilde, prev, o.get_state(), got)
+    assert e["N"] <= 1e-9 and e["F"] <= 1e-9, e
+
+
+def test_device_resident_inputs_and_outputs(oracle_mod):
+    import torch
+    from paper_2404_17630_b200 import rt
+    w = cfg.get(3, 8)
+    h = rt.Solver(w.mesh, w.params); h.init(w.state, w.sources); h.step(w.dt, 4)
+    ref, _ = h.download()
+    dm = M.Mesh(w.mesh.ncell, w.mesh.nface, w.mesh.box, w.mesh.periodic,
+                *[torch.as_tensor(getattr(w.mesh, k)).cuda() for k in
+                  ("volume", "centroid", "area", "normal", "fcentroid", "left", "right")])
+    ds = {k: torch.as_tensor(getattr(w.state, k)).cuda() for k in ("N", "F", "xHII", "xHeII", "xHeIII", "eth", "nH")}
+    d = rt.Solver(dm, w.params); d.init(ds, w.sources); d.step(w.dt, 4)
+    got, _ = d.download(device=True)
+    for k in ref:
+        assert np.array_equal(ref[k], got[k].cpu().numpy()), k
+
+
+def test_errors_are_reported_not_thrown_across_the_abi():
+    import torch
+    from paper_2404_17630_b200 import rt
+    mesh = M.cartesian(3, 1.0)
+    p = cfg.Params(ngroup=1)
+    bad = M.cartesian(3, 1.0)
+    bad.right[0] = 10 ** 6
+    with pytest.raises(rt.RTError, match="right index"):
+        rt.Solver(bad, p)
+    bad = M.cartesian(3, 1.0)
+    bad.area[5] *= 1.5
+    with pytest.raises(rt.RTError, match="not closed"):
+        rt.Solver(bad, p)
+    h = rt.rt_create(0, None)
+    with pytest.raises(rt.RTError, match="rt_mesh_upload first"):
+        rt.rt_state_init(h, p, cfg._uniform_state(1, 27, 1.0, 1.0, 1.0, (0, 0, 0), 0.0))
+    with pytest.raises(rt.RTError, match="rt_state_init first"):
+        rt.rt_step(h, 0.1, 1)
+    ws = torch.empty(16, dtype=torch.float64, device="cuda")
+    with pytest.raises(rt.RTError, match="workspace has"):
+        rt.rt_mesh_upload(h, mesh, 1, None, ws)
+    rt.rt_destroy(h)

@@ -589,11 +589,14 @@ static void fluxes(oracle_ctx *c, double dt) {
       double ph[4];
       oracle_riemann(UL, UR, n, c->ctilde, ph);
       /* "a further limiter is applied to prevent negative photon densities" PAPER.md:155 (S11):
-       * the donor cell cannot lose more than it holds through this face in dt */
+       * the donor cell cannot lose more photons than it holds through this face in dt, so the
+       * magnitude of the number flux is clamped; the momentum flux Phi_F is left alone (scaling
+       * it by the same factor is discontinuous where Phi_N changes sign next to an empty cell:
+       * tests/test_oracle_conditioning.py) */
       int64_t d = ph[0] > 0.0 ? L : (ph[0] < 0.0 ? R : -1);
       if (d >= 0) {
-        double cap = c->N[(size_t)g * c->C + d] * c->volume[d] / (dt * c->area[f] * fabs(ph[0]));
-        if (cap < 1.0) for (int q = 0; q < 4; q++) ph[q] *= cap;
+        double lim = c->N[(size_t)g * c->C + d] * c->volume[d] / (dt * c->area[f]);
+        if (fabs(ph[0]) > lim) ph[0] = ph[0] > 0.0 ? lim : -lim;
       }
       for (int q = 0; q < 4; q++) c->phi[((size_t)f * G + g) * 4 + q] = ph[q];
     }

@@ -154,11 +154,12 @@ __global__ void __launch_bounds__(RT_BLOCK * GG) k_flux(rt_geom m, const double 
     const double hc2 = 0.5 * ct * ct, hc = 0.5 * ct;
 #pragma unroll
     for (int a = 0; a < 3; a++) ph[1 + a] = hc2 * (PL[a] + PR[a]) - hc * (UR[1 + a] - UL[1 + a]);
-    // donor cap (S11): the donor cannot lose more than it holds through this face in dt
+    // donor cap (S11): the donor cannot lose more photons than it holds through this face in dt;
+    // only the number flux is clamped (continuous in the state; Phi_F is left alone)
     const int32_t d = ph[0] > 0.0 ? l : (ph[0] < 0.0 ? r : -1);
     if (d >= 0) {
-      const double cap = Ug[d] * m.vol[d] / (dt * A * fabs(ph[0]));
-      if (cap < 1.0) { ph[0] *= cap; ph[1] *= cap; ph[2] *= cap; ph[3] *= cap; }
+      const double lim = Ug[d] * m.vol[d] / (dt * A);
+      if (fabs(ph[0]) > lim) ph[0] = ph[0] > 0.0 ? lim : -lim;
     }
     double *po = phi + (size_t)4 * g * F;
     po[q] = ph[0]; po[F + q] = ph[1]; po[2 * F + q] = ph[2]; po[3 * F + q] = ph[3];

@@ -102,9 +102,9 @@ def rhs(mesh, U, ct, dt, ghost, order):
         ph = _glf(UL, UR, n, ct)
         d = L if ph[0] > 0 else (Rr if ph[0] < 0 else -1)
         if d >= 0:
-            cap = U[d, 0] * mesh.volume[d] / (dt * mesh.area[f] * abs(ph[0]))
-            if cap < 1:
-                ph = ph * cap
+            lim = U[d, 0] * mesh.volume[d] / (dt * mesh.area[f])
+            if abs(ph[0]) > lim:
+                ph[0] = np.sign(ph[0]) * lim
         R[L] -= mesh.area[f] * ph / mesh.volume[L]
         if Rr >= 0:
             R[Rr] += mesh.area[f] * ph / mesh.volume[Rr]

@@ -1,0 +1,322 @@
+#!/usr/bin/env python
+"""Benchmark of the RT subcycle (BASELINE.json metric: RT cell-group-updates/s per subcycle on
+one B200, and % of the HBM roofline).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--n 384] [--impl reference]
+
+A "step" is one subcycle = one pass of the whole hot path (chemistry, then two Heun stages of
+gradient -> face flux -> update) over the synthetic workload of BASELINE.json configs[4] (384^3
+jittered-lattice Voronoi cells, periodic, 3 groups, H+He chemistry; recipe in DESIGN.md 4),
+built on the device.  One process per GPU; N > 1 runs N independent replicas (DESIGN.md 8:
+"replicas only", no data-path collective) and reports the aggregate.  Prints ONE JSON line.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
+recipe on the host cores; the ratio to it is context, not the headline (parity and the roofline
+fraction are).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "rt_cell_group_updates_per_s"
+UNIT = "cell-group-updates/s"
+FULL_N = {0: 32, 1: 128, 2: 64, 3: 256, 4: 384}
+SAMPLE_N = {0: 24, 1: 32, 2: 24, 3: 28, 4: 28}
+
+
+def workload_name(c, n):
+    return "config%d_%s_n%d" % (c, ("stromgren", "beam", "hhe_voronoi", "reion_voronoi", "reion_voronoi")[c], n)
+
+
+# ------------------------------------------------------------------ CPU oracle legs
+def oracle_sample(c, budget_s, steps=None):
+    """Times the oracle on the config-c recipe at a reduced lattice.  Returns (value, info)."""
+    import oracle
+    from paper_2404_17630_b200.inputs import configs as cfg
+    n = SAMPLE_N[c]
+    w = cfg.get(c, n)
+    o = oracle.Oracle(w.mesh, w.params)
+    o.set_sources(w.sources)
+    o.set_state(w.state)
+    C, G = w.mesh.ncell, w.params.ngroup
+    t0 = time.perf_counter()
+    o.step(w.dt, 1)
+    t1 = time.perf_counter() - t0
+    if steps is None:
+        steps = int(max(1, min(200, budget_s / max(t1, 1e-6) - 1)))
+    t0 = time.perf_counter()
+    o.step(w.dt, steps)
+    el = time.perf_counter() - t0
+    val = C * G * steps / el
+    info = {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "%s recipe on a %d^3 lattice (%d cells, %d groups), %d subcycles after 1 untimed, %.1f s"
+                      % (workload_name(c, FULL_N[c]), n, C, G, steps, el)}
+    return val, info, el / steps * 1e3
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    c = args.config
+    import oracle
+    from paper_2404_17630_b200.inputs import configs as cfg
+    n = SAMPLE_N[c]
+    w = cfg.get(c, n)
+    o = oracle.Oracle(w.mesh, w.params)
+    o.set_sources(w.sources)
+    o.set_state(w.state)
+    C, G = w.mesh.ncell, w.params.ngroup
+    o.step(w.dt, args.warmup)
+    t0 = time.perf_counter()
+    o.step(w.dt, args.steps)
+    el = time.perf_counter() - t0
+    val = C * G * args.steps / el
+    sample = "%s recipe on a %d^3 lattice (%d cells, %d groups), one subcycle per step" % (
+        workload_name(c, FULL_N[c]), n, C, G)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": el / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(c, args.n or FULL_N[c]), "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------ clocks
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.rows = []
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.p = None
+
+    def _read(self):
+        for line in self.p.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        sm, mx, reasons = [], None, set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for t, l in self.rows:
+            if t < t0 or t > t1 + 0.2:
+                continue
+            f = [x.strip() for x in l.split(",")]
+            try:
+                sm.append(float(f[0])); mx = float(f[1])
+            except Exception:
+                continue
+            for k, nm in enumerate(names):
+                if len(f) > 3 + k and f[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ------------------------------------------------------------------ algorithmic bytes
+def algorithmic_bytes(C, F, NR, G, heun=True, chem=True):
+    """Bytes each kernel must move per launch if every array is read or written once."""
+    grad = 32 * G * C + (24 + 24 + 8) * F + 4 * NR + 16 * C + 24 * C + 48 * C + 96 * G * C
+    flux = 32 * G * C + 96 * G * C + (8 + 24 + 24 + 8) * F + 24 * C + 8 * C + 32 * G * F
+    update = 32 * G * F + 8 * F + 4 * NR + 16 * C + 64 * G * C + 8 * C + 4 * C + 32 * G * C
+    chemb = 64 * G * C + 64 * C + 16 * C
+    per_sub = (2 if heun else 1) * (grad + flux + update) + (chemb if chem else 0)
+    return {"grad": grad, "flux": flux, "update": update, "chem": chemb, "subcycle": per_sub}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--n", type=int, default=None, help="lattice cells per dimension (default: the config's full size)")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.warmup < 3:
+        args.warmup = 3
+
+    import torch
+    from paper_2404_17630_b200 import rt
+    from paper_2404_17630_b200.inputs import configs as cfg
+    from paper_2404_17630_b200.inputs import device as devin
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the RT path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    c = args.config
+    n = args.n or FULL_N[c]
+    t_build = time.perf_counter()
+    if c >= 3:
+        w = devin.config34_device(n, c, "cuda:%d" % local)
+    else:
+        w = cfg.get(c, n)
+    C, F, G = int(w.mesh.ncell), int(w.mesh.nface), int(w.params.ngroup)
+    NR = int((w.mesh.right >= 0).sum())
+    s = rt.Solver(w.mesh, w.params, device=local)
+    w.mesh = None
+    torch.cuda.empty_cache()
+    s.init(w.state, w.sources)
+    t_build = time.perf_counter() - t_build
+    stored0 = None
+    s.step(w.dt, args.warmup)
+    torch.cuda.synchronize()
+
+    # ---- timed region: K subcycles, state (>= 20 GB at full size) far larger than the 126 MB L2
+    sampler = ClockSampler(local)
+    time.sleep(0.3)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = s.launches()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    s.profile(True)
+    tw0 = time.perf_counter()
+    e0.record()
+    s.step(w.dt, args.steps)
+    e1.record()
+    torch.cuda.synchronize()
+    tw1 = time.perf_counter()
+    if dist is not None:
+        dist.barrier()
+    ms = e0.elapsed_time(e1)
+    prof = s.profile_read()
+    s.profile(False)
+    launches = s.launches() - l0
+    clocks = sampler.stop(tw0, tw1)
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * C * G * args.steps / (ms * 1e-3)
+
+    # ---- ledger sanity after the timed region (photon budget closes)
+    led = s.ledger()
+
+    # ---- end to end through the C ABI with HOST buffers: H2D state, one subcycle, D2H state
+    e2e = None
+    if args.e2e_steps > 0:
+        shapes = {"N": (G, C), "F": (G, 3, C), "xHII": (C,), "xHeII": (C,), "xHeIII": (C,), "eth": (C,)}
+        host = {k: torch.empty(sh, dtype=torch.float64).pin_memory() for k, sh in shapes.items()}
+        nH = w.state.nH
+        host_in = dict(host)
+        host_in["nH"] = (nH.cpu() if hasattr(nH, "cpu") else torch.as_tensor(nH)).pin_memory()
+        rt.rt_download(s.h, host, False, G)
+        for _ in range(1):  # warm-up of the copy path
+            rt.rt_state_init(s.h, w.params, host_in, w.sources); rt.rt_step(s.h, w.dt, 1); rt.rt_download(s.h, host, False, G)
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            rt.rt_state_init(s.h, w.params, host_in, w.sources)
+            rt.rt_step(s.h, w.dt, 1)
+            rt.rt_download(s.h, host, False, G)
+        torch.cuda.synchronize()
+        el = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([el], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            el = float(t.item())
+        e2e = {"value": world * C * G * args.e2e_steps / el, "unit": UNIT, "h2d_bytes_per_step": (4 * G + 5) * 8 * C,
+               "d2h_bytes_per_step": (4 * G + 4) * 8 * C, "steps": args.e2e_steps, "ms_per_step": el / args.e2e_steps * 1e3}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel
+    peaks_file = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_file):
+        peak, peak_src = float(json.load(open(peaks_file))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    else:
+        peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
+    ab = algorithmic_bytes(C, F, NR, G, bool(w.params.heun), w.params.chem_mode != 0)
+    kern = {}
+    for k in ("chem", "grad", "flux", "update", "reduce"):
+        tms, cnt = prof[k]
+        if cnt == 0:
+            continue
+        avg = tms / cnt
+        d = {"launches": cnt, "avg_ms": avg, "share": tms / ms}
+        if k in ab:
+            d["algorithmic_bytes"] = ab[k]
+            d["GBps"] = ab[k] / (avg * 1e-3) / 1e9
+            d["frac_of_hbm_peak"] = d["GBps"] / peak
+        kern[k] = d
+    dom = max((k for k in kern if k in ab), key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"])
+    traffic = None
+    tf = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tf):
+        traffic = json.load(open(tf)).get(workload_name(c, n), {}).get(dom)
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["GBps"], "peak": peak, "unit": "GB/s",
+                "frac": kern[dom]["GBps"] / peak, "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": ab[dom],
+                "subcycle": {"algorithmic_bytes": ab["subcycle"], "GBps": ab["subcycle"] * args.steps / (ms * 1e-3) / 1e9,
+                             "frac": ab["subcycle"] * args.steps / (ms * 1e-3) / 1e9 / peak,
+                             "bytes_per_cell_group_update": ab["subcycle"] / (C * G)}}
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        _, cpu, _ = oracle_sample(c, args.cpu_seconds)
+
+    stored_scale = float(np.max(np.abs(led["injected"]) + np.abs(led["stored"])) + 1e-300)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(c, n), "cells": C, "faces": F, "groups": G,
+                       "chem_mode": int(w.params.chem_mode), "dt": w.dt, "parallelism": "replicas x%d" % world,
+                       "l2": "inputs larger than L2 (%.1f GB of state and geometry per subcycle)" % (ab["subcycle"] / 1e9),
+                       "build_s": t_build},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "kernels": kern,
+            "cpu_baseline": cpu,
+            "ledger": {"substeps_total": int(led["substeps_total"]), "substeps_max": int(led["substeps_max"]),
+                       "cells_hit_cap": int(led["cells_hit_cap"]),
+                       "budget_residual": float(np.max(np.abs(led["stored"] + led["absorbed"] + led["outflow"]
+                                                              - led["injected"] - led["inflow_bc"] - led["floor_added"]))
+                                                / stored_scale)}}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -143,6 +143,14 @@ int rt_download(rt_ctx *ctx, rt_state *out, rt_ledger *ledger);
 /* Number of kernels the context has launched since rt_create (for bench.py's gpu_launches). */
 int64_t rt_kernel_launches(const rt_ctx *ctx);
 
+/* Per-kernel timing with CUDA events recorded on the context's stream around every launch of
+ * rt_step.  rt_profile(ctx, 1) starts recording, rt_profile(ctx, 0) stops.  rt_profile_read
+ * synchronises and returns, per kernel class (0 chemistry, 1 gradient, 2 face flux, 3 update,
+ * 4 ledger reduction, 5 other), the summed milliseconds and the number of launches since the last
+ * read; ms and count are HOST arrays of 6. */
+int rt_profile(rt_ctx *ctx, int enable);
+int rt_profile_read(rt_ctx *ctx, double *ms, int64_t *count);
+
 /* Slope-limited gradients of the current state in the caller's order, DEVICE or HOST as
  * mem_kind says: gN (G, 3, C), gF (G, 3 components, 3 directions, C).  For tests. Synchronises. */
 int rt_debug_gradients(rt_ctx *ctx, int mem_kind, double *gN, double *gF);

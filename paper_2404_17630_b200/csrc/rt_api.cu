@@ -7,6 +7,23 @@
 #include <vector>
 #include "rt_internal.cuh"
 
+void rt_prof_begin(rt_ctx *c, int cls) {
+  if (!c->prof_on) return;
+  if (c->prof_used * 2 >= c->prof_ev.size()) {
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    c->prof_ev.push_back(a); c->prof_ev.push_back(b);
+    c->prof_cls.push_back(cls);
+  }
+  c->prof_cls[c->prof_used] = cls;
+  cudaEventRecord(c->prof_ev[2 * c->prof_used], c->stream);
+}
+void rt_prof_end(rt_ctx *c) {
+  if (!c->prof_on) return;
+  cudaEventRecord(c->prof_ev[2 * c->prof_used + 1], c->stream);
+  c->prof_used++;
+}
+
 int rt_fail(rt_ctx *c, int code, const char *fmt, ...) {
   if (c) {
     va_list ap;
@@ -26,7 +43,10 @@ int rt_create(rt_ctx **out, int device, void *cuda_stream) {
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return RT_ECUDA;
   rt_ctx *c = new (std::nothrow) rt_ctx();
   if (!c) return RT_ENOMEM;
-  memset(c, 0, sizeof(*c));
+  c->device = 0; c->stream = 0; c->err[0] = 0; c->C = c->F = c->NR = 0; c->G = 0; c->nghost = 0; c->ws = nullptr;
+  c->ws_bytes = 0; c->have_mesh = c->have_state = false; c->nsrc = 0; c->nsub_done = 0; c->launches = 0;
+  c->prof_on = false; c->prof_used = 0;
+  memset(&c->par, 0, sizeof(c->par)); memset(&c->lay, 0, sizeof(c->lay));
   c->device = device;
   c->stream = (cudaStream_t)cuda_stream;
   if (cudaSetDevice(device) != cudaSuccess) { delete c; return RT_ECUDA; }
@@ -34,7 +54,32 @@ int rt_create(rt_ctx **out, int device, void *cuda_stream) {
   return RT_OK;
 }
 
-void rt_destroy(rt_ctx *c) { delete c; }
+void rt_destroy(rt_ctx *c) {
+  if (!c) return;
+  for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
+  delete c;
+}
+
+int rt_profile(rt_ctx *c, int enable) {
+  if (!c) return RT_EINVAL;
+  c->prof_on = enable != 0;
+  if (enable) c->prof_used = 0;
+  return RT_OK;
+}
+
+int rt_profile_read(rt_ctx *c, double *ms, int64_t *count) {
+  if (!c || !ms || !count) return RT_EINVAL;
+  RT_CUDA(c, cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < RT_K_NCLS; k++) { ms[k] = 0.0; count[k] = 0; }
+  for (size_t i = 0; i < c->prof_used; i++) {
+    float t = 0.f;
+    RT_CUDA(c, cudaEventElapsedTime(&t, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]));
+    ms[c->prof_cls[i]] += t;
+    count[c->prof_cls[i]]++;
+  }
+  c->prof_used = 0;
+  return RT_OK;
+}
 
 const char *rt_last_error(const rt_ctx *c) { return c ? c->err : "null context"; }
 

@@ -236,6 +236,7 @@ static void launch_chem_g(rt_ctx *c, const rt_chem_par &P, double dt, double *U)
 }
 
 void rt_launch_chem(rt_ctx *c, const rt_chem_par &P, double dt, double *U) {
+  rt_prof_begin(c, RT_K_CHEM);
   switch (c->G) {
     case 1: launch_chem_g<1>(c, P, dt, U); break;
     case 2: launch_chem_g<2>(c, P, dt, U); break;
@@ -246,5 +247,6 @@ void rt_launch_chem(rt_ctx *c, const rt_chem_par &P, double dt, double *U) {
     case 7: launch_chem_g<7>(c, P, dt, U); break;
     default: launch_chem_g<8>(c, P, dt, U); break;
   }
+  rt_prof_end(c);
   c->launches++;
 }

@@ -13,6 +13,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <vector>
 #include "rt.h"
 
 #define RT_BLOCK 128
@@ -49,7 +50,16 @@ struct rt_ctx {
   double injected[RT_MAXG][2];  // host-side compensated sum
   int64_t nsub_done;
   int64_t launches;
+  // optional per-kernel timing with CUDA events on the context's stream (rt_profile)
+  bool prof_on;
+  std::vector<cudaEvent_t> prof_ev;   // pairs (start, stop)
+  std::vector<int> prof_cls;
+  size_t prof_used;
 };
+
+enum { RT_K_CHEM = 0, RT_K_GRAD = 1, RT_K_FLUX = 2, RT_K_UPDATE = 3, RT_K_REDUCE = 4, RT_K_OTHER = 5, RT_K_NCLS = 6 };
+void rt_prof_begin(rt_ctx *c, int cls);
+void rt_prof_end(rt_ctx *c);
 
 template <class T>
 static inline T *rt_ptr(const rt_ctx *c, size_t off) { return (T *)(c->ws + off); }

@@ -339,7 +339,9 @@ int rt_launch_gradients(rt_ctx *c, const double *U) {
 }
 
 static void reduce2(rt_ctx *c, reduce_job a, reduce_job b, int njobs) {
+  rt_prof_begin(c, RT_K_REDUCE);
   k_reduce<<<dim3(c->G, njobs), 1024, 0, c->stream>>>(a, b, c->G, rt_ptr<rt_dev_ledger>(c, c->lay.led));
+  rt_prof_end(c);
   c->launches++;
 }
 
@@ -353,14 +355,23 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
   double *part = rt_ptr<double>(c, l.part);
   double *p_floor = part + (size_t)G * l.nbc, *p_out = part + (size_t)G * 3 * l.nbc, *p_in = p_out + (size_t)G * l.nbf;
   const int second = c->par.order >= 2;
-  if (second) { DISPATCH_G(G, k_grad, (unsigned)l.nbc, dim3(RT_BLOCK, G), c->stream, m, Uin, grad); c->launches++; }
+  if (second) {
+    rt_prof_begin(c, RT_K_GRAD);
+    DISPATCH_G(G, k_grad, (unsigned)l.nbc, dim3(RT_BLOCK, G), c->stream, m, Uin, grad);
+    rt_prof_end(c);
+    c->launches++;
+  }
+  rt_prof_begin(c, RT_K_FLUX);
   DISPATCH_G(G, k_flux, (unsigned)l.nbf, dim3(RT_BLOCK, G), c->stream, m, Uin, grad, phi, c->par.ctilde, dt, second, p_out,
              p_in);
+  rt_prof_end(c);
   c->launches++;
   reduce2(c, {p_out, l.nbf, wl * dt, 1}, {p_in, l.nbf, wl * dt, 2}, 2);
+  rt_prof_begin(c, RT_K_UPDATE);
   DISPATCH_G(G, k_update, (unsigned)l.nbc, dim3(RT_BLOCK, G), c->stream, m, Uin, U0, phi, Uout,
              rt_ptr<int32_t>(c, l.srcidx), rt_ptr<double>(c, l.srcrate), c->nsrc, ca, cb, dt, c->par.ctilde,
              c->par.n_floor, p_floor);
+  rt_prof_end(c);
   c->launches++;
   reduce2(c, {p_floor, l.nbc, wf, 3}, {p_floor, l.nbc, wf, 3}, 1);
 }

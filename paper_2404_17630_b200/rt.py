@@ -74,6 +74,10 @@ def lib():
         L.rt_kernel_launches.argtypes = [_vp]
         L.rt_debug_gradients.restype = ctypes.c_int
         L.rt_debug_gradients.argtypes = [_vp, ctypes.c_int, _vp, _vp]
+        L.rt_profile.restype = ctypes.c_int
+        L.rt_profile.argtypes = [_vp, ctypes.c_int]
+        L.rt_profile_read.restype = ctypes.c_int
+        L.rt_profile_read.argtypes = [_vp, _vp, _vp]
         L.rt_last_error.restype = ctypes.c_char_p
         L.rt_last_error.argtypes = [_vp]
         L.rt_destroy.restype = None
@@ -278,6 +282,16 @@ class Solver:
         _check(self.h, lib().rt_debug_gradients(self.h, RT_MEM_HOST, _vp(gN.ctypes.data), _vp(gF.ctypes.data)),
                "rt_debug_gradients")
         return gN, gF
+
+    def profile(self, enable):
+        _check(self.h, lib().rt_profile(self.h, int(bool(enable))), "rt_profile")
+
+    def profile_read(self):
+        ms = np.zeros(6)
+        cnt = np.zeros(6, dtype=np.int64)
+        _check(self.h, lib().rt_profile_read(self.h, _vp(ms.ctypes.data), _vp(cnt.ctypes.data)), "rt_profile_read")
+        names = ("chem", "grad", "flux", "update", "reduce", "other")
+        return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(names)}
 
     def launches(self):
         return int(lib().rt_kernel_launches(self.h))

@@ -121,13 +121,14 @@ int rt_mesh_upload(rt_ctx *c, const rt_mesh *m, void *ws, size_t bytes) {
 }
 
 // copy `rows` rows of C doubles (caller's order, host or device) into dst in the internal order
-static int put_rows(rt_ctx *c, const double *src, int mem_kind, double *dst, int rows, double *stage) {
+// dst[p*stride + r] = src[r][perm[p]]
+static int put_rows(rt_ctx *c, const double *src, int mem_kind, double *dst, int rows, int stride, double *stage) {
   const size_t n = (size_t)rows * c->C;
   if (mem_kind == RT_MEM_HOST) {
     RT_CUDA(c, cudaMemcpyAsync(stage, src, n * 8, cudaMemcpyHostToDevice, c->stream));
     src = stage;
   }
-  return rt_launch_permute_in(c, src, dst, rows);
+  return rt_launch_permute_in(c, src, dst, rows, stride);
 }
 
 int rt_state_init(rt_ctx *c, const rt_params *p, const rt_state *s0, const rt_sources *src) {
@@ -160,21 +161,21 @@ int rt_state_init(rt_ctx *c, const rt_params *p, const rt_state *s0, const rt_so
   double *stage = rt_ptr<double>(c, l.grad);  // 12 G C doubles: free between steps
   double *Ua = rt_ptr<double>(c, l.Ua);
   int rc;
-  // N (G,C) and F (G,3,C) -> U[g][4][C]
+  // N (G,C) and F (G,3,C) -> U[g][C][4]
   for (int g = 0; g < G; g++) {
-    if ((rc = put_rows(c, s0->N + (size_t)g * C, s0->mem_kind, Ua + (size_t)4 * g * C, 1, stage))) return rc;
-    if ((rc = put_rows(c, s0->F + (size_t)3 * g * C, s0->mem_kind, Ua + (size_t)(4 * g + 1) * C, 3, stage + C))) return rc;
+    if ((rc = put_rows(c, s0->N + (size_t)g * C, s0->mem_kind, Ua + (size_t)4 * g * C, 1, 4, stage))) return rc;
+    if ((rc = put_rows(c, s0->F + (size_t)3 * g * C, s0->mem_kind, Ua + (size_t)4 * g * C + 1, 3, 4, stage + C))) return rc;
     stage += 4 * C;
   }
   stage = rt_ptr<double>(c, l.grad) + (size_t)4 * G * C;
   const double *xs[5] = {s0->xHII, s0->xHeII, s0->xHeIII, s0->eth, s0->nH};
   const size_t xo[5] = {l.xHII, l.xHeII, l.xHeIII, l.eth, l.nH};
   for (int k = 0; k < 5; k++) {
-    if (xs[k]) { if ((rc = put_rows(c, xs[k], s0->mem_kind, rt_ptr<double>(c, xo[k]), 1, stage + (size_t)k * C))) return rc; }
+    if (xs[k]) { if ((rc = put_rows(c, xs[k], s0->mem_kind, rt_ptr<double>(c, xo[k]), 1, 1, stage + (size_t)k * C))) return rc; }
     else RT_CUDA(c, cudaMemsetAsync(rt_ptr<double>(c, xo[k]), 0, 8 * C, c->stream));
   }
   if (p->chem_mode == RT_CHEM_FIXED_OPACITY) {
-    if ((rc = put_rows(c, p->kappa, p->kappa_mem_kind, rt_ptr<double>(c, l.kappa), 1, stage + (size_t)5 * C))) return rc;
+    if ((rc = put_rows(c, p->kappa, p->kappa_mem_kind, rt_ptr<double>(c, l.kappa), 1, 1, stage + (size_t)5 * C))) return rc;
   }
   // sources
   c->nsrc = nsrc;
@@ -215,14 +216,15 @@ int rt_step(rt_ctx *c, double dt, int nsub) {
   return RT_OK;
 }
 
-static int get_rows(rt_ctx *c, const double *src, double *dst, int mem_kind, int rows, double *stage) {
+// dst[r][perm[p]] = src[p*stride + r]
+static int get_rows(rt_ctx *c, const double *src, double *dst, int mem_kind, int rows, int stride, double *stage) {
   const size_t n = (size_t)rows * c->C;
   if (mem_kind == RT_MEM_HOST) {
-    rt_launch_permute_out(c, src, stage, rows);
+    rt_launch_permute_out(c, src, stage, rows, stride);
     RT_CUDA(c, cudaMemcpyAsync(dst, stage, n * 8, cudaMemcpyDeviceToHost, c->stream));
     return RT_OK;
   }
-  return rt_launch_permute_out(c, src, dst, rows);
+  return rt_launch_permute_out(c, src, dst, rows, stride);
 }
 
 int rt_download(rt_ctx *c, rt_state *out, rt_ledger *led) {
@@ -238,15 +240,15 @@ int rt_download(rt_ctx *c, rt_state *out, rt_ledger *led) {
     double *stage = rt_ptr<double>(c, l.grad);
     const double *Ua = rt_ptr<double>(c, l.Ua);
     for (int g = 0; g < G; g++) {
-      if (out->N && (rc = get_rows(c, Ua + (size_t)4 * g * C, out->N + (size_t)g * C, out->mem_kind, 1, stage))) return rc;
-      if (out->F && (rc = get_rows(c, Ua + (size_t)(4 * g + 1) * C, out->F + (size_t)3 * g * C, out->mem_kind, 3, stage + C)))
+      if (out->N && (rc = get_rows(c, Ua + (size_t)4 * g * C, out->N + (size_t)g * C, out->mem_kind, 1, 4, stage))) return rc;
+      if (out->F && (rc = get_rows(c, Ua + (size_t)4 * g * C + 1, out->F + (size_t)3 * g * C, out->mem_kind, 3, 4, stage + C)))
         return rc;
       stage += 4 * C;
     }
     double *xs[4] = {out->xHII, out->xHeII, out->xHeIII, out->eth};
     const size_t xo[4] = {l.xHII, l.xHeII, l.xHeIII, l.eth};
     for (int k = 0; k < 4; k++)
-      if (xs[k] && (rc = get_rows(c, rt_ptr<double>(c, xo[k]), xs[k], out->mem_kind, 1, stage + (size_t)k * C))) return rc;
+      if (xs[k] && (rc = get_rows(c, rt_ptr<double>(c, xo[k]), xs[k], out->mem_kind, 1, 1, stage + (size_t)k * C))) return rc;
   }
   rt_dev_ledger h;
   if (led) {
@@ -286,11 +288,11 @@ int rt_debug_gradients(rt_ctx *c, int mem_kind, double *gN, double *gF) {
   double *stage = rt_ptr<double>(c, l.Ub);  // 4 G C doubles, free between steps; used 3 and 9 rows at a time
   int rc;
   for (int g = 0; g < c->G; g++) {
-    if ((rc = get_rows(c, grad + (size_t)12 * g * C, gN + (size_t)3 * g * C, mem_kind, 3, stage))) return rc;
+    if ((rc = get_rows(c, grad + (size_t)12 * g * C, gN + (size_t)3 * g * C, mem_kind, 3, 12, stage))) return rc;
     RT_CUDA(c, cudaStreamSynchronize(c->stream));
     // 9 rows do not fit a 4-row stage when G == 1: go 3 rows at a time
     for (int q = 0; q < 3; q++) {
-      if ((rc = get_rows(c, grad + (size_t)(12 * g + 3 + 3 * q) * C, gF + (size_t)(9 * g + 3 * q) * C, mem_kind, 3, stage)))
+      if ((rc = get_rows(c, grad + (size_t)12 * g * C + 3 + 3 * q, gF + (size_t)(9 * g + 3 * q) * C, mem_kind, 3, 12, stage)))
         return rc;
       RT_CUDA(c, cudaStreamSynchronize(c->stream));
     }

@@ -115,30 +115,23 @@ __device__ inline double trial(const rt_chem_par &P, const cell_state<G> &s, dou
   return f;
 }
 
-// deterministic block sum over RT_BLOCK threads (fixed tree), result valid in thread 0
-__device__ inline double block_sum(double v, double *sm) {
+// deterministic sum over the block's single warp (fixed tree), result valid in thread 0
+__device__ inline double block_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-  const int w = threadIdx.x >> 5;
-  __syncthreads();
-  if ((threadIdx.x & 31) == 0) sm[w] = v;
-  __syncthreads();
-  double t = 0.0;
-  if (threadIdx.x == 0)
-    for (int k = 0; k < RT_BLOCK / 32; k++) t += sm[k];
-  return t;
+  return v;
 }
 
 template <int G, int MODE>
-__global__ void __launch_bounds__(RT_BLOCK) k_chem(rt_chem_par P, int64_t C, double dt, double *__restrict__ U,
+__global__ void __launch_bounds__(RT_CHEM_BLOCK) k_chem(rt_chem_par P, int64_t C, double dt, double *__restrict__ U,
                                                    double *__restrict__ xHII, double *__restrict__ xHeII,
                                                    double *__restrict__ xHeIII, double *__restrict__ eth,
-                                                   const double *__restrict__ nHv, const double *__restrict__ vol,
+                                                   const double *__restrict__ nHv, const double *__restrict__ cellS,
                                                    const double *__restrict__ kappa, double *__restrict__ part_abs,
                                                    rt_dev_ledger *led) {
   constexpr bool THERMAL = (MODE == RT_CHEM_HHE_THERMAL);
-  __shared__ double sm[RT_BLOCK / 32];
-  const int64_t i = (int64_t)blockIdx.x * RT_BLOCK + threadIdx.x;
+  static_assert(RT_CHEM_BLOCK == 32, "block_sum assumes one warp");
+  const int64_t i = (int64_t)blockIdx.x * RT_CHEM_BLOCK + threadIdx.x;
   const bool live = i < C;
   double absd[G];
 #pragma unroll
@@ -149,8 +142,8 @@ __global__ void __launch_bounds__(RT_BLOCK) k_chem(rt_chem_par P, int64_t C, dou
     cell_state<G> s;
 #pragma unroll
     for (int g = 0; g < G; g++) {
-      s.N[g] = U[(size_t)(4 * g) * C + i]; s.Fx[g] = U[(size_t)(4 * g + 1) * C + i];
-      s.Fy[g] = U[(size_t)(4 * g + 2) * C + i]; s.Fz[g] = U[(size_t)(4 * g + 3) * C + i];
+      const double4 u = *reinterpret_cast<const double4 *>(U + ((size_t)g * C + i) * 4);
+      s.N[g] = u.x; s.Fx[g] = u.y; s.Fy[g] = u.z; s.Fz[g] = u.w;
       absd[g] = s.N[g];
     }
     if (MODE == RT_CHEM_FIXED_OPACITY) {
@@ -166,10 +159,11 @@ __global__ void __launch_bounds__(RT_BLOCK) k_chem(rt_chem_par P, int64_t C, dou
       // controller of PAPER.md:238: start with h = dt; reject if f > 0.1 and shrink by f_s/f; on
       // accept scale by f_s/f but at most double; the last step is clipped to end at dt
       double t = 0.0, h = dt;
-      bool last = true;
+      bool last = true, stale = true;  // rates depend on the state only: a retry reuses them
       while (true) {
         if ((long long)attempts >= P.max_substeps) { capped = 1; break; }
-        if (THERMAL) {
+        if (THERMAL && stale) {
+          stale = false;
           const double xe = s.xHII + P.y_he * (s.xHeII + 2.0 * s.xHeIII);
           const double T = (2.0 / 3.0) * s.e / (KB_CGS * (nH * (1.0 + P.y_he + xe)));
           eval_rates<true>(T, P.alphaB_override, r);
@@ -179,6 +173,7 @@ __global__ void __launch_bounds__(RT_BLOCK) k_chem(rt_chem_par P, int64_t C, dou
         attempts++;
         if (f > P.f_accept) { h = h * P.f_target / f; last = false; continue; }
         s = o;
+        stale = true;
         if (last) break;
         t += h;
         h = h * fmin(2.0, P.f_target / fmax(f, 1e-300));
@@ -187,17 +182,16 @@ __global__ void __launch_bounds__(RT_BLOCK) k_chem(rt_chem_par P, int64_t C, dou
       xHII[i] = s.xHII; xHeII[i] = s.xHeII; xHeIII[i] = s.xHeIII;
       if (THERMAL) eth[i] = s.e;
     }
-    const double V = vol[i];
+    const double V = cellS[4 * i + 3];
 #pragma unroll
     for (int g = 0; g < G; g++) {
-      U[(size_t)(4 * g) * C + i] = s.N[g]; U[(size_t)(4 * g + 1) * C + i] = s.Fx[g];
-      U[(size_t)(4 * g + 2) * C + i] = s.Fy[g]; U[(size_t)(4 * g + 3) * C + i] = s.Fz[g];
+      *reinterpret_cast<double4 *>(U + ((size_t)g * C + i) * 4) = make_double4(s.N[g], s.Fx[g], s.Fy[g], s.Fz[g]);
       absd[g] = V * (absd[g] - s.N[g]);
     }
   }
 #pragma unroll
   for (int g = 0; g < G; g++) {
-    const double t = block_sum(absd[g], sm);
+    const double t = block_sum(absd[g]);
     if (threadIdx.x == 0) part_abs[(size_t)blockIdx.x * G + g] = t;
   }
   if (MODE != RT_CHEM_FIXED_OPACITY) {
@@ -222,10 +216,10 @@ __global__ void __launch_bounds__(RT_BLOCK) k_chem(rt_chem_par P, int64_t C, dou
 template <int G>
 static void launch_chem_g(rt_ctx *c, const rt_chem_par &P, double dt, double *U) {
   const rt_layout &l = c->lay;
-  dim3 grid((unsigned)l.nbc), block(RT_BLOCK);
+  dim3 grid((unsigned)((c->C + RT_CHEM_BLOCK - 1) / RT_CHEM_BLOCK)), block(RT_CHEM_BLOCK);
   double *part = rt_ptr<double>(c, l.part);
 #define CHEM_ARGS P, c->C, dt, U, rt_ptr<double>(c, l.xHII), rt_ptr<double>(c, l.xHeII), rt_ptr<double>(c, l.xHeIII), \
-      rt_ptr<double>(c, l.eth), rt_ptr<double>(c, l.nH), rt_ptr<double>(c, l.vol), rt_ptr<double>(c, l.kappa), part, \
+      rt_ptr<double>(c, l.eth), rt_ptr<double>(c, l.nH), rt_ptr<double>(c, l.cellS), rt_ptr<double>(c, l.kappa), part, \
       rt_ptr<rt_dev_ledger>(c, l.led)
   switch (c->par.chem_mode) {
     case RT_CHEM_FIXED_OPACITY: k_chem<G, RT_CHEM_FIXED_OPACITY><<<grid, block, 0, c->stream>>>(CHEM_ARGS); break;

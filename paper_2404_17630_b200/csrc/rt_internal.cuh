@@ -1,14 +1,21 @@
 // Internal declarations of librt.so (not part of the ABI; see include/rt.h).
 //
-// Device data layout (all inside the caller's workspace, SoA, fp64, 256-byte aligned blocks):
+// Device data layout (all inside the caller's workspace, fp64, 256-byte aligned blocks).  Arrays
+// that are gathered through an index (neighbour states, gradients, face fluxes, cell geometry) are
+// packed so that one gather is one or a few 32-byte sectors ("array of small structs"); arrays
+// that are only streamed are plain.
 //   cells in Peano-Hilbert order p = 0..C-1:   perm[p] = caller's id, iperm = inverse
-//     vol[C], s[3][C], Minv[6][C] (symmetric inverse of sum_f A n n^T, eq (15))
+//     cellS[C][4] = (sx, sy, sz, V); Minv[C][6] (symmetric inverse of sum_f A n n^T, eq (15))
 //   faces sorted by owner (= left cell, the lower new id), then by right id, boundary faces last:
-//     A[F], nrm[3][F], cf[3][F] (left frame), w[3][F] = A d/|d|^2 with d = s_R - s_L,
+//     faceC[F][4] = (cx, cy, cz, A)  centroid in the left cell's frame and area
+//     faceN[F][3] = unit normal L -> R
+//     faceW[F][3] = A d/|d|^2, d = s_R - s_L: prefactor of eq (15)'s second term
 //     L[F], R[F]
 //   cell -> faces: owned faces are the contiguous range fo[i]..fo[i+1]; faces where
-//     the cell is the right one are listed in rl[ro[i]..ro[i+1]] (ascending face id)
-//   state: Ua, Ub [G][4][C] (N, Fx, Fy, Fz), grad [G][12][C], phi [G][4][F], x*, eth, nH, kappa
+//     the cell is the right one are listed in rl[ro[i]..ro[i+1]] (ascending face id), with the
+//     cell across each of them (= L[rl[k]]) in rn[k]
+//   state: Ua, Ub [G][C][4] = (N, Fx, Fy, Fz); grad [G][C][12] (field-major, then direction);
+//     phi [G][F][4] = A * (Phi_N, Phi_F); xHII, xHeII, xHeIII, eth, nH, kappa [C]
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -16,7 +23,10 @@
 #include <vector>
 #include "rt.h"
 
+#ifndef RT_BLOCK
 #define RT_BLOCK 128
+#endif
+#define RT_CHEM_BLOCK 32  // one warp per block: a slow cell holds back 31 others, not 127
 
 struct rt_dev_ledger {  // accumulators on the device (value + compensation)
   double acc[5][RT_MAXG][2];  // 0 absorbed, 1 outflow, 2 inflow_bc, 3 floor_added, 4 stored (value only)
@@ -24,7 +34,7 @@ struct rt_dev_ledger {  // accumulators on the device (value + compensation)
 };
 
 struct rt_layout {
-  size_t perm, iperm, vol, s, Minv, A, nrm, cf, w, L, R, fo, ro, rl, ghost, led;
+  size_t perm, iperm, cellS, Minv, faceC, faceN, faceW, L, R, fo, ro, rl, rn, ghost, led;
   size_t Ua, Ub, grad, phi, xHII, xHeII, xHeIII, eth, nH, kappa, srcidx, srcrate, part, scratch_end;
   size_t temp;        // start of the setup-time scratch (aliases the state region)
   size_t total;
@@ -78,8 +88,9 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m);
 // rt_kernels.cu
 int rt_launch_step(rt_ctx *c, double dt);
 int rt_launch_gradients(rt_ctx *c, const double *U);
-int rt_launch_permute_in(rt_ctx *c, const double *src, double *dst, int rows);   // dst[r][p] = src[r][perm[p]]
-int rt_launch_permute_out(rt_ctx *c, const double *src, double *dst, int rows);  // dst[r][perm[p]] = src[r][p]
+// dst[p*stride + r] = src[r*C + perm[p]]  /  dst[r*C + perm[p]] = src[p*stride + r], r < rows
+int rt_launch_permute_in(rt_ctx *c, const double *src, double *dst, int rows, int stride);
+int rt_launch_permute_out(rt_ctx *c, const double *src, double *dst, int rows, int stride);
 int rt_launch_init_sources(rt_ctx *c, const int32_t *cell_dev, int nsrc);
 int rt_launch_stored(rt_ctx *c);
 

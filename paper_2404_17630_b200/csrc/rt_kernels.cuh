@@ -11,8 +11,8 @@ struct rt_chem_par {
 // geometry + box block passed by value to the transport kernels
 struct rt_geom {
   int64_t C, F;
-  const double *vol, *s, *Minv, *A, *nrm, *cf, *w;
-  const int32_t *L, *R, *rl;
+  const double *cellS, *Minv, *faceC, *faceN, *faceW;
+  const int32_t *L, *R, *rl, *rn;
   const int64_t *fo, *ro;
   const double *ghost;
   double box[3];

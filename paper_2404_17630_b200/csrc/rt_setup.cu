@@ -69,13 +69,13 @@ __global__ void k_cell_keys(const double *centroid, int64_t C, double bx, double
   idx[i] = (int32_t)i;
 }
 
-__global__ void k_permute_cells(geom_in g, int64_t C, const int32_t *perm, int32_t *iperm, double *vol, double *s) {
+__global__ void k_permute_cells(geom_in g, int64_t C, const int32_t *perm, int32_t *iperm, double *cellS) {
   int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= C) return;
   int32_t o = perm[p];
   iperm[o] = (int32_t)p;
-  vol[p] = g.volume[o];
-  for (int a = 0; a < 3; a++) s[a * C + p] = g.centroid[a * C + o];
+  for (int a = 0; a < 3; a++) cellS[4 * p + a] = g.centroid[a * C + o];
+  cellS[4 * p + 3] = g.volume[o];
 }
 
 __device__ inline uint64_t face_key(int32_t l, int32_t r) {
@@ -93,8 +93,8 @@ __global__ void k_face_keys(geom_in g, int64_t F, const int32_t *iperm, uint64_t
 }
 
 __global__ void k_gather_faces(geom_in g, int64_t C, int64_t F, const int32_t *order, const uint64_t *keys,
-                               const int32_t *iperm, const double *s, double bx, double by, double bz, int p0, int p1,
-                               int p2, double *A, double *nrm, double *cf, int32_t *L, int32_t *R) {
+                               const int32_t *iperm, const double *cellS, double bx, double by, double bz, int p0,
+                               int p1, int p2, double *faceC, double *faceN, int32_t *L, int32_t *R) {
   int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (q >= F) return;
   int32_t f = order[q];
@@ -104,14 +104,14 @@ __global__ void k_gather_faces(geom_in g, int64_t C, int64_t F, const int32_t *o
   bool flip = (iperm[g.left[f]] != l);
   if (flip) r = iperm[g.left[f]];
   L[q] = l; R[q] = r;
-  A[q] = g.area[f];
+  faceC[4 * q + 3] = g.area[f];
   double sg = flip ? -1.0 : 1.0;
   double b[3] = {bx, by, bz};
   int per[3] = {p0, p1, p2};
   for (int a = 0; a < 3; a++) {
-    nrm[a * F + q] = sg * g.normal[a * F + f];
-    double sl = s[a * C + l];
-    cf[a * F + q] = sl + rt_wrap(g.fcentroid[a * F + f] - sl, b[a], per[a]);  // left cell's frame
+    faceN[3 * q + a] = sg * g.normal[a * F + f];
+    double sl = cellS[4 * (int64_t)l + a];
+    faceC[4 * q + a] = sl + rt_wrap(g.fcentroid[a * F + f] - sl, b[a], per[a]);  // left cell's frame
   }
 }
 
@@ -134,16 +134,19 @@ __global__ void k_rkeys(const int32_t *R, int64_t F, uint64_t *keys) {
   keys[q] = R[q] >= 0 ? (((uint64_t)(uint32_t)R[q] << 32) | (uint32_t)q) : ~0ull;
 }
 
-__global__ void k_rlist(const uint64_t *keys, int64_t NR, int32_t *rl) {
+__global__ void k_rlist(const uint64_t *keys, int64_t NR, const int32_t *L, int32_t *rl, int32_t *rn) {
   int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k < NR) rl[k] = (int32_t)(keys[k] & 0xffffffffu);
+  if (k >= NR) return;
+  int32_t q = (int32_t)(keys[k] & 0xffffffffu);
+  rl[k] = q;
+  rn[k] = L[q];
 }
 
 // per-face prefactor of eq (15)'s second term, seen from the left cell: w = A d/|d|^2,
 // d = s_R - s_L measured through the face; boundary faces use the mirror point (S13)
-__global__ void k_face_geom(int64_t C, int64_t F, const double *s, const double *A, const double *nrm, const double *cf,
+__global__ void k_face_geom(int64_t C, int64_t F, const double *cellS, const double *faceC, const double *faceN,
                             const int32_t *L, const int32_t *R, double bx, double by, double bz, int p0, int p1, int p2,
-                            double *w) {
+                            double *faceW) {
   int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (q >= F) return;
   double b[3] = {bx, by, bz};
@@ -152,22 +155,22 @@ __global__ void k_face_geom(int64_t C, int64_t F, const double *s, const double 
   double d[3];
   if (r >= 0) {
     for (int a = 0; a < 3; a++) {
-      double c = cf[a * F + q];
-      d[a] = (c - s[a * C + l]) - rt_wrap(c - s[a * C + r], b[a], per[a]);
+      double c = faceC[4 * q + a];
+      d[a] = (c - cellS[4 * (int64_t)l + a]) - rt_wrap(c - cellS[4 * (int64_t)r + a], b[a], per[a]);
     }
   } else {
-    double n[3] = {nrm[q], nrm[F + q], nrm[2 * F + q]};
+    double n[3] = {faceN[3 * q], faceN[3 * q + 1], faceN[3 * q + 2]};
     double p = 0.0;
-    for (int a = 0; a < 3; a++) p += (cf[a * F + q] - s[a * C + l]) * n[a];
+    for (int a = 0; a < 3; a++) p += (faceC[4 * q + a] - cellS[4 * (int64_t)l + a]) * n[a];
     for (int a = 0; a < 3; a++) d[a] = 2.0 * p * n[a];
   }
   double d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
-  double k = A[q] / d2;
-  for (int a = 0; a < 3; a++) w[a * F + q] = k * d[a];
+  double k = faceC[4 * q + 3] / d2;
+  for (int a = 0; a < 3; a++) faceW[3 * q + a] = k * d[a];
 }
 
 // per cell: M = sum_f A n n^T (n = d/|d| = w/|w|), its inverse, and the closure check
-__global__ void k_cell_geom(int64_t C, int64_t F, const double *A, const double *nrm, const double *w,
+__global__ void k_cell_geom(int64_t C, int64_t F, const double *faceC, const double *faceN, const double *faceW,
                             const int64_t *fo, const int64_t *ro, const int32_t *rl, double *Minv, int *flags) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= C) return;
@@ -176,13 +179,13 @@ __global__ void k_cell_geom(int64_t C, int64_t F, const double *A, const double 
   for (int64_t k = 0; k < n_own + n_r; k++) {
     int64_t q = k < n_own ? fo[i] + k : rl[ro[i] + (k - n_own)];
     double sg = k < n_own ? 1.0 : -1.0;
-    double a = A[q];
-    double wx = w[q], wy = w[F + q], wz = w[2 * F + q];
+    double a = faceC[4 * q + 3];
+    double wx = faceW[3 * q], wy = faceW[3 * q + 1], wz = faceW[3 * q + 2];
     double w2 = wx * wx + wy * wy + wz * wz;
     double f = a / w2;  // A n n^T = A w w^T / |w|^2
     m[0] += f * wx * wx; m[1] += f * wx * wy; m[2] += f * wx * wz;
     m[3] += f * wy * wy; m[4] += f * wy * wz; m[5] += f * wz * wz;
-    cl[0] += sg * a * nrm[q]; cl[1] += sg * a * nrm[F + q]; cl[2] += sg * a * nrm[2 * F + q];
+    cl[0] += sg * a * faceN[3 * q]; cl[1] += sg * a * faceN[3 * q + 1]; cl[2] += sg * a * faceN[3 * q + 2];
     sa += a;
   }
   int e = 0;
@@ -191,12 +194,12 @@ __global__ void k_cell_geom(int64_t C, int64_t F, const double *A, const double 
   double det = m[0] * c00 + m[1] * c01 + m[2] * c02;
   if (!(fabs(det) > 0.0)) { e |= E_MATRIX; det = 1.0; }
   double id = 1.0 / det;
-  Minv[0 * C + i] = c00 * id;
-  Minv[1 * C + i] = c01 * id;
-  Minv[2 * C + i] = c02 * id;
-  Minv[3 * C + i] = (m[0] * m[5] - m[2] * m[2]) * id;
-  Minv[4 * C + i] = (m[1] * m[2] - m[0] * m[4]) * id;
-  Minv[5 * C + i] = (m[0] * m[3] - m[1] * m[1]) * id;
+  Minv[6 * i + 0] = c00 * id;
+  Minv[6 * i + 1] = c01 * id;
+  Minv[6 * i + 2] = c02 * id;
+  Minv[6 * i + 3] = (m[0] * m[5] - m[2] * m[2]) * id;
+  Minv[6 * i + 4] = (m[1] * m[2] - m[0] * m[4]) * id;
+  Minv[6 * i + 5] = (m[0] * m[3] - m[1] * m[1]) * id;
   if (e) atomicOr(flags, e);
 }
 
@@ -252,7 +255,7 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
                    hflags & E_GHOST ? " Dirichlet ghost index >= nghost;" : "", hflags & E_VOL ? " volume <= 0;" : "",
                    hflags & E_AREA ? " area <= 0;" : "", hflags & E_NORMAL ? " normal not unit;" : "");
   int32_t *perm = rt_ptr<int32_t>(c, lay.perm), *iperm = rt_ptr<int32_t>(c, lay.iperm);
-  double *vol = rt_ptr<double>(c, lay.vol), *s = rt_ptr<double>(c, lay.s);
+  double *cellS = rt_ptr<double>(c, lay.cellS);
   // 1. cells along the Peano-Hilbert curve
   {
     k_cell_keys<<<nblk(C), SETUP_BLOCK, 0, st>>>(g.centroid, C, c->box[0], c->box[1], c->box[2], k0, v0);
@@ -261,11 +264,11 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
     size_t b = cub_bytes;
     RT_CUDA(c, cub::DeviceRadixSort::SortPairs(cub_tmp, b, dk, dv, C, 0, 63, st));
     RT_CUDA(c, cudaMemcpyAsync(perm, dv.Current(), 4 * C, cudaMemcpyDeviceToDevice, st));
-    k_permute_cells<<<nblk(C), SETUP_BLOCK, 0, st>>>(g, C, perm, iperm, vol, s);
+    k_permute_cells<<<nblk(C), SETUP_BLOCK, 0, st>>>(g, C, perm, iperm, cellS);
   }
   // 2. faces by owner
-  double *A = rt_ptr<double>(c, lay.A), *nrm = rt_ptr<double>(c, lay.nrm), *cf = rt_ptr<double>(c, lay.cf);
-  double *w = rt_ptr<double>(c, lay.w);
+  double *faceC = rt_ptr<double>(c, lay.faceC), *faceN = rt_ptr<double>(c, lay.faceN);
+  double *faceW = rt_ptr<double>(c, lay.faceW);
   int32_t *L = rt_ptr<int32_t>(c, lay.L), *R = rt_ptr<int32_t>(c, lay.R);
   int64_t *fo = rt_ptr<int64_t>(c, lay.fo), *ro = rt_ptr<int64_t>(c, lay.ro);
   int32_t *rl = rt_ptr<int32_t>(c, lay.rl);
@@ -275,8 +278,8 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
     cub::DoubleBuffer<int32_t> dv(v0, v1);
     size_t b = cub_bytes;
     RT_CUDA(c, cub::DeviceRadixSort::SortPairs(cub_tmp, b, dk, dv, F, 0, 64, st));
-    k_gather_faces<<<nblk(F), SETUP_BLOCK, 0, st>>>(g, C, F, dv.Current(), dk.Current(), iperm, s, c->box[0], c->box[1],
-                                                    c->box[2], c->per[0], c->per[1], c->per[2], A, nrm, cf, L, R);
+    k_gather_faces<<<nblk(F), SETUP_BLOCK, 0, st>>>(g, C, F, dv.Current(), dk.Current(), iperm, cellS, c->box[0], c->box[1],
+                                                    c->box[2], c->per[0], c->per[1], c->per[2], faceC, faceN, L, R);
     k_lower_bounds<<<nblk(C + 1), SETUP_BLOCK, 0, st>>>(dk.Current(), F, C, fo);
   }
   // 3. right lists
@@ -290,12 +293,12 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
     RT_CUDA(c, cudaMemcpyAsync(&NR, ro + C, 8, cudaMemcpyDeviceToHost, st));
     RT_CUDA(c, cudaStreamSynchronize(st));
     c->NR = NR;
-    if (NR > 0) k_rlist<<<nblk(NR), SETUP_BLOCK, 0, st>>>(dk.Current(), NR, rl);
+    if (NR > 0) k_rlist<<<nblk(NR), SETUP_BLOCK, 0, st>>>(dk.Current(), NR, L, rl, rt_ptr<int32_t>(c, lay.rn));
   }
   // 4. geometry of eq (15)
-  k_face_geom<<<nblk(F), SETUP_BLOCK, 0, st>>>(C, F, s, A, nrm, cf, L, R, c->box[0], c->box[1], c->box[2], c->per[0],
-                                               c->per[1], c->per[2], w);
-  k_cell_geom<<<nblk(C), SETUP_BLOCK, 0, st>>>(C, F, A, nrm, w, fo, ro, rl, rt_ptr<double>(c, lay.Minv), flags);
+  k_face_geom<<<nblk(F), SETUP_BLOCK, 0, st>>>(C, F, cellS, faceC, faceN, L, R, c->box[0], c->box[1], c->box[2],
+                                               c->per[0], c->per[1], c->per[2], faceW);
+  k_cell_geom<<<nblk(C), SETUP_BLOCK, 0, st>>>(C, F, faceC, faceN, faceW, fo, ro, rl, rt_ptr<double>(c, lay.Minv), flags);
   RT_CUDA(c, cudaMemcpyAsync(&hflags, flags, sizeof(int), cudaMemcpyDeviceToHost, st));
   if (m->nghost > 0)
     RT_CUDA(c, cudaMemcpyAsync(rt_ptr<double>(c, lay.ghost), m->ghost_state, sizeof(double) * m->nghost * 4 * c->G,
@@ -316,10 +319,10 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G) {
   l.nbc = (C + RT_BLOCK - 1) / RT_BLOCK;
   l.nbf = (F + RT_BLOCK - 1) / RT_BLOCK;
   l.perm = take(4 * C); l.iperm = take(4 * C);
-  l.vol = take(8 * C); l.s = take(24 * C); l.Minv = take(48 * C);
-  l.A = take(8 * F); l.nrm = take(24 * F); l.cf = take(24 * F); l.w = take(24 * F);
+  l.cellS = take(32 * C); l.Minv = take(48 * C);
+  l.faceC = take(32 * F); l.faceN = take(24 * F); l.faceW = take(24 * F);
   l.L = take(4 * F); l.R = take(4 * F);
-  l.fo = take(8 * (C + 1)); l.ro = take(8 * (C + 1)); l.rl = take(4 * F);
+  l.fo = take(8 * (C + 1)); l.ro = take(8 * (C + 1)); l.rl = take(4 * F); l.rn = take(4 * F);
   l.ghost = take(8 * 4 * RT_MAXG * 64);
   l.led = take(sizeof(rt_dev_ledger));
   l.temp = o;
@@ -330,8 +333,8 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G) {
   l.kappa = take(8 * C);
   l.srcidx = take(4 * C);
   l.srcrate = take(8 * (size_t)G * 65536);
-  // partial sums: chem absorbed [nbc][G], update floor + stored [nbc][2G], flux outflow + inflow [nbf][2G]
-  l.part = take(8 * (size_t)G * (3 * l.nbc + 2 * l.nbf));
+  // partial sums: chem absorbed [<= 4 nbc + 1][G], update floor [<= 8 nbc + 1][G], flux outflow + inflow [nbf][2G]
+  l.part = take(8 * (size_t)G * (13 * l.nbc + 2 * l.nbf + 16));
   l.scratch_end = o;
   // setup scratch aliases the state region; make sure it fits (incl. staging of a host mesh)
   int64_t NM = C > F ? C : F;

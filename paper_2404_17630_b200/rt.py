@@ -56,7 +56,7 @@ def lib():
     global _lib
     if _lib is None:
         from .build import build_rt
-        so = build_rt()
+        so = os.environ.get("RT_LIB") or build_rt()   # RT_LIB: an alternative build, for experiments
         L = ctypes.CDLL(so)
         L.rt_create.restype = ctypes.c_int
         L.rt_create.argtypes = [ctypes.POINTER(_vp), ctypes.c_int, _vp]

@@ -116,6 +116,7 @@ int rt_mesh_upload(rt_ctx *c, const rt_mesh *m, void *ws, size_t bytes) {
   c->ws_bytes = bytes;
   int rc = rt_setup_mesh(c, m);
   if (rc != RT_OK) return rc;
+  if ((rc = rt_transport_configure(c)) != RT_OK) return rc;
   c->have_mesh = true;
   return RT_OK;
 }
@@ -161,10 +162,10 @@ int rt_state_init(rt_ctx *c, const rt_params *p, const rt_state *s0, const rt_so
   double *stage = rt_ptr<double>(c, l.grad);  // 12 G C doubles: free between steps
   double *Ua = rt_ptr<double>(c, l.Ua);
   int rc;
-  // N (G,C) and F (G,3,C) -> U[g][C][4]
+  // N (G,C) and F (G,3,C) -> U[C][G][4]
   for (int g = 0; g < G; g++) {
-    if ((rc = put_rows(c, s0->N + (size_t)g * C, s0->mem_kind, Ua + (size_t)4 * g * C, 1, 4, stage))) return rc;
-    if ((rc = put_rows(c, s0->F + (size_t)3 * g * C, s0->mem_kind, Ua + (size_t)4 * g * C + 1, 3, 4, stage + C))) return rc;
+    if ((rc = put_rows(c, s0->N + (size_t)g * C, s0->mem_kind, Ua + 4 * g, 1, 4 * G, stage))) return rc;
+    if ((rc = put_rows(c, s0->F + (size_t)3 * g * C, s0->mem_kind, Ua + 4 * g + 1, 3, 4 * G, stage + C))) return rc;
     stage += 4 * C;
   }
   stage = rt_ptr<double>(c, l.grad) + (size_t)4 * G * C;
@@ -240,8 +241,8 @@ int rt_download(rt_ctx *c, rt_state *out, rt_ledger *led) {
     double *stage = rt_ptr<double>(c, l.grad);
     const double *Ua = rt_ptr<double>(c, l.Ua);
     for (int g = 0; g < G; g++) {
-      if (out->N && (rc = get_rows(c, Ua + (size_t)4 * g * C, out->N + (size_t)g * C, out->mem_kind, 1, 4, stage))) return rc;
-      if (out->F && (rc = get_rows(c, Ua + (size_t)4 * g * C + 1, out->F + (size_t)3 * g * C, out->mem_kind, 3, 4, stage + C)))
+      if (out->N && (rc = get_rows(c, Ua + 4 * g, out->N + (size_t)g * C, out->mem_kind, 1, 4 * G, stage))) return rc;
+      if (out->F && (rc = get_rows(c, Ua + 4 * g + 1, out->F + (size_t)3 * g * C, out->mem_kind, 3, 4 * G, stage + C)))
         return rc;
       stage += 4 * C;
     }
@@ -288,11 +289,11 @@ int rt_debug_gradients(rt_ctx *c, int mem_kind, double *gN, double *gF) {
   double *stage = rt_ptr<double>(c, l.Ub);  // 4 G C doubles, free between steps; used 3 and 9 rows at a time
   int rc;
   for (int g = 0; g < c->G; g++) {
-    if ((rc = get_rows(c, grad + (size_t)12 * g * C, gN + (size_t)3 * g * C, mem_kind, 3, 12, stage))) return rc;
+    if ((rc = get_rows(c, grad + 12 * g, gN + (size_t)3 * g * C, mem_kind, 3, 12 * c->G, stage))) return rc;
     RT_CUDA(c, cudaStreamSynchronize(c->stream));
     // 9 rows do not fit a 4-row stage when G == 1: go 3 rows at a time
     for (int q = 0; q < 3; q++) {
-      if ((rc = get_rows(c, grad + (size_t)12 * g * C + 3 + 3 * q, gF + (size_t)(9 * g + 3 * q) * C, mem_kind, 3, 12, stage)))
+      if ((rc = get_rows(c, grad + 12 * g + 3 + 3 * q, gF + (size_t)(9 * g + 3 * q) * C, mem_kind, 3, 12 * c->G, stage)))
         return rc;
       RT_CUDA(c, cudaStreamSynchronize(c->stream));
     }

@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(RT_CHEM_BLOCK) k_chem(rt_chem_par P, int64_t C
     cell_state<G> s;
 #pragma unroll
     for (int g = 0; g < G; g++) {
-      const double4 u = *reinterpret_cast<const double4 *>(U + ((size_t)g * C + i) * 4);
+      const double4 u = *reinterpret_cast<const double4 *>(U + ((size_t)i * G + g) * 4);
       s.N[g] = u.x; s.Fx[g] = u.y; s.Fy[g] = u.z; s.Fz[g] = u.w;
       absd[g] = s.N[g];
     }
@@ -185,7 +185,7 @@ __global__ void __launch_bounds__(RT_CHEM_BLOCK) k_chem(rt_chem_par P, int64_t C
     const double V = cellS[4 * i + 3];
 #pragma unroll
     for (int g = 0; g < G; g++) {
-      *reinterpret_cast<double4 *>(U + ((size_t)g * C + i) * 4) = make_double4(s.N[g], s.Fx[g], s.Fy[g], s.Fz[g]);
+      *reinterpret_cast<double4 *>(U + ((size_t)i * G + g) * 4) = make_double4(s.N[g], s.Fx[g], s.Fy[g], s.Fz[g]);
       absd[g] = V * (absd[g] - s.N[g]);
     }
   }

@@ -1,21 +1,24 @@
 // Internal declarations of librt.so (not part of the ABI; see include/rt.h).
 //
-// Device data layout (all inside the caller's workspace, fp64, 256-byte aligned blocks).  Arrays
-// that are gathered through an index (neighbour states, gradients, face fluxes, cell geometry) are
-// packed so that one gather is one or a few 32-byte sectors ("array of small structs"); arrays
-// that are only streamed are plain.
+// Device data layout (all inside the caller's workspace, fp64, 256-byte aligned blocks).
 //   cells in Peano-Hilbert order p = 0..C-1:   perm[p] = caller's id, iperm = inverse
 //     cellS[C][4] = (sx, sy, sz, V); Minv[C][6] (symmetric inverse of sum_f A n n^T, eq (15))
-//   faces sorted by owner (= left cell, the lower new id), then by right id, boundary faces last:
-//     faceC[F][4] = (cx, cy, cz, A)  centroid in the left cell's frame and area
-//     faceN[F][3] = unit normal L -> R
-//     faceW[F][3] = A d/|d|^2, d = s_R - s_L: prefactor of eq (15)'s second term
-//     L[F], R[F]
-//   cell -> faces: owned faces are the contiguous range fo[i]..fo[i+1]; faces where
-//     the cell is the right one are listed in rl[ro[i]..ro[i+1]] (ascending face id), with the
-//     cell across each of them (= L[rl[k]]) in rn[k]
-//   state: Ua, Ub [G][C][4] = (N, Fx, Fy, Fz); grad [G][C][12] (field-major, then direction);
-//     phi [G][F][4] = A * (Phi_N, Phi_F); xHII, xHeII, xHeIII, eth, nH, kappa [C]
+//   faces sorted by owner (= left cell, the lower new id), then by right id, boundary faces last;
+//   every face array is [F][4] doubles = one aligned 32-byte sector per face:
+//     faceC = (cx, cy, cz, A)     centroid in the left cell's frame and area
+//     faceN = (nx, ny, nz, L|R)   unit normal L -> R; the fourth slot holds the two int32 ids
+//     faceW = (wx, wy, wz, L|R)   w = A d/|d|^2, d = s_R - s_L: prefactor of eq (15)'s second
+//                                 term
+//   cell -> faces: owned faces are the contiguous range fo[i]..fo[i+1]; the faces
+//     where the cell is the right one are r-list entries ro[i]..ro[i+1] (ascending face id)
+//   tiles: TC consecutive cells (a compact blob of the Hilbert curve) are one thread block's
+//     work.  A tile's "slots" are its owned faces (slot s = face - fo[c0]) followed by its
+//     incoming faces (right cell in the tile, owner in an earlier tile), listed in
+//     incf[inco[t]..inco[t+1]].  rslot[k] is the slot of r-list entry k inside its cell's tile,
+//     so a cell finds every one of its faces in the tile's shared-memory slot arrays.
+//   state, cell-major so that a tile is one contiguous run:
+//     Ua, Ub [C][G][4] = (N, Fx, Fy, Fz); grad [C][G][12] (field-major, then direction);
+//     xHII, xHeII, xHeIII, eth, nH, kappa [C]
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -27,6 +30,8 @@
 #define RT_BLOCK 128
 #endif
 #define RT_CHEM_BLOCK 32  // one warp per block: a slow cell holds back 31 others, not 127
+#define RT_REC 18        // doubles per (cell, group) row of U + gradients in shared memory (16 + 2 pad: bank spread)
+#define RT_MIN_TILE 8     // smallest tile size rt_mesh_upload will fall back to
 
 struct rt_dev_ledger {  // accumulators on the device (value + compensation)
   double acc[5][RT_MAXG][2];  // 0 absorbed, 1 outflow, 2 inflow_bc, 3 floor_added, 4 stored (value only)
@@ -34,11 +39,12 @@ struct rt_dev_ledger {  // accumulators on the device (value + compensation)
 };
 
 struct rt_layout {
-  size_t perm, iperm, cellS, Minv, faceC, faceN, faceW, L, R, fo, ro, rl, rn, ghost, led;
-  size_t Ua, Ub, grad, phi, xHII, xHeII, xHeIII, eth, nH, kappa, srcidx, srcrate, part, scratch_end;
+  size_t perm, iperm, cellS, Minv, faceC, faceN, faceW, L, R, fo, ro, rl, rn, rslot, incf, inco, ghost, led;
+  size_t Ua, Ub, grad, xHII, xHeII, xHeIII, eth, nH, kappa, srcidx, srcrate, part, scratch_end;
   size_t temp;        // start of the setup-time scratch (aliases the state region)
   size_t total;
-  int64_t nbc, nbf;   // blocks over cells / faces (partial-sum rows)
+  int64_t nbc;        // blocks of RT_BLOCK cells (partial-sum rows of k_stored)
+  int64_t max_tiles;  // tiles at the smallest tile size (sizes inco and the partial sums)
 };
 
 struct rt_ctx {
@@ -47,6 +53,10 @@ struct rt_ctx {
   char err[512];
   int64_t C, F, NR;
   int G;
+  int TC;             // cells per tile
+  int64_t T;          // number of tiles
+  int smax;           // largest slot count of any tile
+  int64_t ninc;       // total incoming faces over all tiles
   double box[3];
   int per[3];
   int nghost;
@@ -71,6 +81,15 @@ enum { RT_K_CHEM = 0, RT_K_GRAD = 1, RT_K_FLUX = 2, RT_K_UPDATE = 3, RT_K_REDUCE
 void rt_prof_begin(rt_ctx *c, int cls);
 void rt_prof_end(rt_ctx *c);
 
+// dynamic shared memory of the two tile kernels (rt_transport.cu) for a tile of TC cells whose
+// slot count is at most smax
+static inline size_t rt_smem_grad(int TC, int G, int smax) { return (size_t)64 * smax + (size_t)32 * TC * G; }
+static inline size_t rt_smem_stage(int TC, int G, int smax) {
+  return (size_t)32 * G * smax + (size_t)RT_REC * 8 * TC * G + (size_t)32 * TC;
+}
+#define RT_SMEM_MAX 232448     // 227 KB: the most one block may have on sm_100
+#define RT_SMEM_TARGET 110000  // two blocks per SM
+
 template <class T>
 static inline T *rt_ptr(const rt_ctx *c, size_t off) { return (T *)(c->ws + off); }
 
@@ -86,6 +105,7 @@ int rt_fail(rt_ctx *c, int code, const char *fmt, ...);
 // rt_setup.cu
 int rt_setup_mesh(rt_ctx *c, const rt_mesh *m);
 // rt_kernels.cu
+int rt_transport_configure(rt_ctx *c);  // after rt_setup_mesh: shared-memory opt-in of the tile kernels
 int rt_launch_step(rt_ctx *c, double dt);
 int rt_launch_gradients(rt_ctx *c, const double *U);
 // dst[p*stride + r] = src[r*C + perm[p]]  /  dst[r*C + perm[p]] = src[p*stride + r], r < rows

@@ -1,5 +1,6 @@
 // Kernel-side parameter blocks and launch wrappers shared by the .cu files of librt.so.
 #pragma once
+#include <string.h>
 #include "rt_internal.cuh"
 
 struct rt_chem_par {
@@ -8,17 +9,33 @@ struct rt_chem_par {
   double sigma[RT_MAXG][3], eps[RT_MAXG][3];
 };
 
-// geometry + box block passed by value to the transport kernels
+// geometry + tile tables passed by value to the transport kernels (layout: rt_internal.cuh)
 struct rt_geom {
   int64_t C, F;
   const double *cellS, *Minv, *faceC, *faceN, *faceW;
-  const int32_t *L, *R, *rl, *rn;
-  const int64_t *fo, *ro;
+  const int64_t *fo, *ro, *inco;
+  const int32_t *incf;
+  const uint16_t *rslot;
   const double *ghost;
   double box[3];
   int per[3];
-  int G;
+  int G, TC, smax;
 };
+
+// the two int32 ids packed in the fourth slot of a faceN / faceW record
+__host__ __device__ inline double rt_pack_lr(int32_t l, int32_t r) {
+  const unsigned long long u = (unsigned long long)(uint32_t)l | ((unsigned long long)(uint32_t)r << 32);
+#ifdef __CUDA_ARCH__
+  return __longlong_as_double((long long)u);
+#else
+  double d; memcpy(&d, &u, 8); return d;
+#endif
+}
+__device__ __forceinline__ void rt_unpack_lr(double d, int32_t &l, int32_t &r) {
+  const unsigned long long u = (unsigned long long)__double_as_longlong(d);
+  l = (int32_t)(uint32_t)(u & 0xffffffffull);
+  r = (int32_t)(uint32_t)(u >> 32);
+}
 
 void rt_launch_chem(rt_ctx *c, const rt_chem_par &P, double dt, double *U);
 rt_geom rt_geom_of(const rt_ctx *c);

@@ -2,7 +2,10 @@
 // cell -> face lists, and the mesh-only parts of eq (15).
 // Runs once per mesh, outside the timed subcycles.  CUB is used for the two radix sorts.
 #include <cub/cub.cuh>
+#include <string.h>
+#include <stdlib.h>
 #include "rt_internal.cuh"
+#include "rt_kernels.cuh"
 
 #define SETUP_BLOCK 256
 static inline unsigned nblk(int64_t n) { return (unsigned)((n + SETUP_BLOCK - 1) / SETUP_BLOCK); }
@@ -104,12 +107,13 @@ __global__ void k_gather_faces(geom_in g, int64_t C, int64_t F, const int32_t *o
   bool flip = (iperm[g.left[f]] != l);
   if (flip) r = iperm[g.left[f]];
   L[q] = l; R[q] = r;
+  faceN[4 * q + 3] = rt_pack_lr(l, r);
   faceC[4 * q + 3] = g.area[f];
   double sg = flip ? -1.0 : 1.0;
   double b[3] = {bx, by, bz};
   int per[3] = {p0, p1, p2};
   for (int a = 0; a < 3; a++) {
-    faceN[3 * q + a] = sg * g.normal[a * F + f];
+    faceN[4 * q + a] = sg * g.normal[a * F + f];
     double sl = cellS[4 * (int64_t)l + a];
     faceC[4 * q + a] = sl + rt_wrap(g.fcentroid[a * F + f] - sl, b[a], per[a]);  // left cell's frame
   }
@@ -159,14 +163,15 @@ __global__ void k_face_geom(int64_t C, int64_t F, const double *cellS, const dou
       d[a] = (c - cellS[4 * (int64_t)l + a]) - rt_wrap(c - cellS[4 * (int64_t)r + a], b[a], per[a]);
     }
   } else {
-    double n[3] = {faceN[3 * q], faceN[3 * q + 1], faceN[3 * q + 2]};
+    double n[3] = {faceN[4 * q], faceN[4 * q + 1], faceN[4 * q + 2]};
     double p = 0.0;
     for (int a = 0; a < 3; a++) p += (faceC[4 * q + a] - cellS[4 * (int64_t)l + a]) * n[a];
     for (int a = 0; a < 3; a++) d[a] = 2.0 * p * n[a];
   }
   double d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
   double k = faceC[4 * q + 3] / d2;
-  for (int a = 0; a < 3; a++) faceW[3 * q + a] = k * d[a];
+  for (int a = 0; a < 3; a++) faceW[4 * q + a] = k * d[a];
+  faceW[4 * q + 3] = rt_pack_lr(l, r);
 }
 
 // per cell: M = sum_f A n n^T (n = d/|d| = w/|w|), its inverse, and the closure check
@@ -180,12 +185,12 @@ __global__ void k_cell_geom(int64_t C, int64_t F, const double *faceC, const dou
     int64_t q = k < n_own ? fo[i] + k : rl[ro[i] + (k - n_own)];
     double sg = k < n_own ? 1.0 : -1.0;
     double a = faceC[4 * q + 3];
-    double wx = faceW[3 * q], wy = faceW[3 * q + 1], wz = faceW[3 * q + 2];
+    double wx = faceW[4 * q], wy = faceW[4 * q + 1], wz = faceW[4 * q + 2];
     double w2 = wx * wx + wy * wy + wz * wz;
     double f = a / w2;  // A n n^T = A w w^T / |w|^2
     m[0] += f * wx * wx; m[1] += f * wx * wy; m[2] += f * wx * wz;
     m[3] += f * wy * wy; m[4] += f * wy * wz; m[5] += f * wz * wz;
-    cl[0] += sg * a * faceN[3 * q]; cl[1] += sg * a * faceN[3 * q + 1]; cl[2] += sg * a * faceN[3 * q + 2];
+    cl[0] += sg * a * faceN[4 * q]; cl[1] += sg * a * faceN[4 * q + 1]; cl[2] += sg * a * faceN[4 * q + 2];
     sa += a;
   }
   int e = 0;
@@ -201,6 +206,46 @@ __global__ void k_cell_geom(int64_t C, int64_t F, const double *faceC, const dou
   Minv[6 * i + 4] = (m[1] * m[2] - m[0] * m[4]) * id;
   Minv[6 * i + 5] = (m[0] * m[3] - m[1] * m[1]) * id;
   if (e) atomicOr(flags, e);
+}
+
+
+// ---- tiles: incoming-face lists and per-cell slot numbers (layout: rt_internal.cuh)
+// number of r-list entries of cell i whose owner lies in an earlier tile (they come first: the
+// r-list is sorted by face id = by owner)
+__global__ void k_tile_count(int64_t C, int TC, const int64_t *ro, const int32_t *rn, int32_t *cellInc) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= C) return;
+  const int32_t c0 = (int32_t)((i / TC) * TC);
+  int n = 0;
+  for (int64_t k = ro[i]; k < ro[i + 1]; k++) n += rn[k] < c0;
+  cellInc[i] = n;
+}
+// per tile: exclusive prefix of cellInc over its cells (in place), the tile's total, max slots
+__global__ void k_tile_scan(int64_t C, int TC, int64_t T, const int64_t *fo, int32_t *cellInc, int64_t *tileInc,
+                            int *maxSlots) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= T) return;
+  const int64_t c0 = t * TC, c1 = c0 + TC < C ? c0 + TC : C;
+  int run = 0;
+  for (int64_t i = c0; i < c1; i++) { int n = cellInc[i]; cellInc[i] = run; run += n; }
+  tileInc[t] = run;
+  const int64_t slots = fo[c1] - fo[c0] + run;
+  atomicMax(maxSlots, slots > 0x7fffffff ? 0x7fffffff : (int)slots);
+}
+__global__ void k_tile_fill(int64_t C, int TC, const int64_t *fo, const int64_t *ro, const int32_t *rl, const int32_t *rn,
+                            const int32_t *cellInc, const int64_t *inco, int32_t *incf, uint16_t *rslot) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= C) return;
+  const int64_t t = i / TC, c0 = t * TC, c1 = c0 + TC < C ? c0 + TC : C;
+  const int64_t fbase = fo[c0], nown = fo[c1] - fbase;
+  int j = cellInc[i];
+  for (int64_t k = ro[i]; k < ro[i + 1]; k++) {
+    if (rn[k] < c0) {
+      incf[inco[t] + j] = rl[k];
+      rslot[k] = (uint16_t)(nown + j);
+      j++;
+    } else rslot[k] = (uint16_t)(rl[k] - fbase);
+  }
 }
 
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -223,7 +268,10 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
     size_t b1 = 0, b2 = 0;
     cub::DeviceRadixSort::SortPairs(nullptr, b1, dk, dv, NM, 0, 64, st);
     cub::DeviceRadixSort::SortKeys(nullptr, b2, dk, NM, 0, 64, st);
+    size_t b3 = 0;
+    cub::DeviceScan::ExclusiveSum(nullptr, b3, (int64_t *)nullptr, (int64_t *)nullptr, NM + 1, st);
     cub_bytes = b1 > b2 ? b1 : b2;
+    if (b3 > cub_bytes) cub_bytes = b3;
   }
   void *cub_tmp = rt_ptr<void>(c, take(cub_bytes));
   geom_in g;
@@ -300,6 +348,43 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
                                                c->per[0], c->per[1], c->per[2], faceW);
   k_cell_geom<<<nblk(C), SETUP_BLOCK, 0, st>>>(C, F, faceC, faceN, faceW, fo, ro, rl, rt_ptr<double>(c, lay.Minv), flags);
   RT_CUDA(c, cudaMemcpyAsync(&hflags, flags, sizeof(int), cudaMemcpyDeviceToHost, st));
+  // 5. tiles: the largest tile size (halving from RT_TILE_CELLS, default 64) whose shared memory fits
+  {
+    int32_t *cellInc = v0;
+    int64_t *tileInc = (int64_t *)k0;
+    int *maxSlots = flags + 1;
+    const int32_t *rn = rt_ptr<int32_t>(c, lay.rn);
+    int64_t *inco = rt_ptr<int64_t>(c, lay.inco);
+    const char *env = getenv("RT_TILE_CELLS");
+    int tc0 = env ? atoi(env) : 64;
+    if (tc0 < RT_MIN_TILE || tc0 > 1024) tc0 = 64;
+    int best = 0, best_smax = 0;
+    for (int pass = 0; pass < 2 && !best; pass++) {
+      const size_t limit = pass == 0 ? RT_SMEM_TARGET : RT_SMEM_MAX;
+      for (int TC = tc0; TC >= RT_MIN_TILE; TC /= 2) {
+        const int64_t T = (C + TC - 1) / TC;
+        RT_CUDA(c, cudaMemsetAsync(maxSlots, 0, sizeof(int), st));
+        k_tile_count<<<nblk(C), SETUP_BLOCK, 0, st>>>(C, TC, ro, rn, cellInc);
+        k_tile_scan<<<nblk(T), SETUP_BLOCK, 0, st>>>(C, TC, T, fo, cellInc, tileInc, maxSlots);
+        int smax = 0;
+        RT_CUDA(c, cudaMemcpyAsync(&smax, maxSlots, sizeof(int), cudaMemcpyDeviceToHost, st));
+        RT_CUDA(c, cudaStreamSynchronize(st));
+        if (smax < 65536 && rt_smem_stage(TC, c->G, smax) <= limit && rt_smem_grad(TC, c->G, smax) <= limit) {
+          best = TC; best_smax = smax;
+          break;
+        }
+      }
+    }
+    if (!best) return rt_fail(c, RT_EMESH, "a cell has too many faces for one thread block's shared memory");
+    c->TC = best; c->smax = best_smax; c->T = (C + best - 1) / best;
+    // tileInc / cellInc hold the accepted tile size's counts (the loop stops at the first fit)
+    size_t b = cub_bytes;
+    RT_CUDA(c, cudaMemsetAsync(tileInc + c->T, 0, 8, st));
+    RT_CUDA(c, cub::DeviceScan::ExclusiveSum(cub_tmp, b, tileInc, inco, c->T + 1, st));
+    k_tile_fill<<<nblk(C), SETUP_BLOCK, 0, st>>>(C, best, fo, ro, rl, rn, cellInc, inco, rt_ptr<int32_t>(c, lay.incf),
+                                                 rt_ptr<uint16_t>(c, lay.rslot));
+    RT_CUDA(c, cudaMemcpyAsync(&c->ninc, inco + c->T, 8, cudaMemcpyDeviceToHost, st));
+  }
   if (m->nghost > 0)
     RT_CUDA(c, cudaMemcpyAsync(rt_ptr<double>(c, lay.ghost), m->ghost_state, sizeof(double) * m->nghost * 4 * c->G,
                                cudaMemcpyHostToDevice, st));
@@ -317,24 +402,24 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G) {
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t r = o; o = align256(o + bytes); return r; };
   l.nbc = (C + RT_BLOCK - 1) / RT_BLOCK;
-  l.nbf = (F + RT_BLOCK - 1) / RT_BLOCK;
+  l.max_tiles = (C + RT_MIN_TILE - 1) / RT_MIN_TILE;
   l.perm = take(4 * C); l.iperm = take(4 * C);
   l.cellS = take(32 * C); l.Minv = take(48 * C);
-  l.faceC = take(32 * F); l.faceN = take(24 * F); l.faceW = take(24 * F);
+  l.faceC = take(32 * F); l.faceN = take(32 * F); l.faceW = take(32 * F);
   l.L = take(4 * F); l.R = take(4 * F);
   l.fo = take(8 * (C + 1)); l.ro = take(8 * (C + 1)); l.rl = take(4 * F); l.rn = take(4 * F);
+  l.rslot = take(2 * F); l.incf = take(4 * F); l.inco = take(8 * (l.max_tiles + 2));
   l.ghost = take(8 * 4 * RT_MAXG * 64);
   l.led = take(sizeof(rt_dev_ledger));
   l.temp = o;
   l.Ua = take(32 * (size_t)G * C); l.Ub = take(32 * (size_t)G * C);
   l.grad = take(96 * (size_t)G * C);
-  l.phi = take(32 * (size_t)G * F);
   l.xHII = take(8 * C); l.xHeII = take(8 * C); l.xHeIII = take(8 * C); l.eth = take(8 * C); l.nH = take(8 * C);
   l.kappa = take(8 * C);
   l.srcidx = take(4 * C);
   l.srcrate = take(8 * (size_t)G * 65536);
-  // partial sums: chem absorbed [<= 4 nbc + 1][G], update floor [<= 8 nbc + 1][G], flux outflow + inflow [nbf][2G]
-  l.part = take(8 * (size_t)G * (13 * l.nbc + 2 * l.nbf + 16));
+  // partial sums: chem absorbed [<= 4 nbc + 1][G]; per tile: floor, outflow, inflow [max_tiles][G] each
+  l.part = take(8 * (size_t)G * (5 * l.nbc + 3 * l.max_tiles + 16));
   l.scratch_end = o;
   // setup scratch aliases the state region; make sure it fits (incl. staging of a host mesh)
   int64_t NM = C > F ? C : F;

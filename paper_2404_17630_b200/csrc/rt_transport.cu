@@ -1,162 +1,165 @@
-// a2-a4: the transport kernels of one Heun stage.
-//   k_grad    LPC lanes per (cell, group): second term of eq (15) over the cell's faces with the
-//             stored per-face prefactors, lane-reduced by warp shuffles, multiplied by the stored
-//             inverse matrix; second pass over the faces for the slope limiter
-//
-//   k_flux    one thread per (face, group): extrapolate both cells to the face centre, M1 closure,
-//             global Lax-Friedrichs flux with signal speed c~, donor cap; the flux (times the face
-//             area) is saved to memory, not scattered
-//   k_update  LPC lanes per (cell, group): sum the saved fluxes over the cell's face list, add the
-//             source, Heun combine, floor and |F| <= c~ N (S3, S11, S12)
-// Packed layouts (rt_internal.cuh): U[g][C][4], grad[g][C][12], phi[g][F][4], cellS[C][4],
-// faceC[F][4], faceN[F][3], faceW[F][3]: one gather = one or a few whole 32-byte sectors.
+// a2-a4: the transport kernels of one Heun stage, one thread block per tile of TC consecutive
+// cells of the Peano-Hilbert order (layout and tile tables: rt_internal.cuh).
+//   k_grad   stages the tile's face records (eq (15) prefactors, face centres, neighbour ids) and
+//            its cells' U in shared memory with coalesced loads; then one thread per (cell, group)
+//            sums the second term of eq (15) over the cell's faces, multiplies by the stored
+//            inverse matrix and runs the slope limiter
+//   k_stage  stages the tile's U and gradients in shared memory; one thread per face slot
+//            extrapolates both cells to the face centre, evaluates the M1 closure and the global
+//            Lax-Friedrichs flux with signal speed c~ and the donor cap for every group, and
+//            leaves A*Phi in shared memory; after a barrier one thread per
+//            (cell, group) sums the cell's face list in fixed order, adds the source, does the Heun
+//            combine, the floor and |F| <= c~ N (S3, S11, S12).  The fluxes
+//            never go to HBM; a face shared by two tiles is evaluated by both.
 #include "rt_internal.cuh"
 #include "rt_kernels.cuh"
 
-#include <stdlib.h>
-// lanes per (cell, group) in k_grad / k_update: tuned on config 3/4 (profiles/); RT_LPC_GRAD and
-// RT_LPC_UPD in the environment override them for experiments
-static int lpc_of(const char *name, int dflt) {
-  const char *e = getenv(name);
-  int v = e ? atoi(e) : dflt;
-  return (v == 1 || v == 2 || v == 4 || v == 8) ? v : dflt;
-}
-static int lpc_grad() { static int v = lpc_of("RT_LPC_GRAD", 1); return v; }
-static int lpc_upd() { static int v = lpc_of("RT_LPC_UPD", 1); return v; }
+typedef unsigned long long u64;
 
 __device__ __forceinline__ double4 ld4(const double *p) { return *reinterpret_cast<const double4 *>(p); }
 __device__ __forceinline__ void st4(double *p, double a, double b, double c, double d) {
   *reinterpret_cast<double4 *>(p) = make_double4(a, b, c, d);
 }
 
-template <int W>
-__device__ __forceinline__ double lanes_sum(double v) {
-#pragma unroll
-  for (int o = W / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o, W);
-  return v;
-}
-template <int W>
-__device__ __forceinline__ double lanes_max(double v) {
-#pragma unroll
-  for (int o = W / 2; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o, W));
-  return v;
-}
-template <int W>
-__device__ __forceinline__ double lanes_min(double v) {
-#pragma unroll
-  for (int o = W / 2; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o, W));
-  return v;
-}
-
 // neighbour or ghost state seen across a boundary face with right code `code` (S13)
-__device__ __forceinline__ double4 ghost_for_gradient(int code, const double4 Ui, const double *n3,
+__device__ __forceinline__ double4 ghost_for_gradient(int code, const double4 Ui, const double *faceN, int64_t q,
                                                       const double *ghost, int G, int g) {
   if (code == RT_BC_OUTFLOW) return Ui;
   if (code == RT_BC_REFLECT) {
-    const double p = 2.0 * (Ui.y * n3[0] + Ui.z * n3[1] + Ui.w * n3[2]);
-    return make_double4(Ui.x, Ui.y - p * n3[0], Ui.z - p * n3[1], Ui.w - p * n3[2]);
+    const double4 n = ld4(faceN + 4 * q);
+    const double p = 2.0 * (Ui.y * n.x + Ui.z * n.y + Ui.w * n.z);
+    return make_double4(Ui.x, Ui.y - p * n.x, Ui.z - p * n.y, Ui.w - p * n.z);
   }
   return ld4(ghost + ((size_t)(RT_BC_DIRICHLET0 - code) * G + g) * 4);
 }
 
-template <int GG, int LPC>
-__global__ void __launch_bounds__(RT_BLOCK *GG) k_grad(rt_geom m, const double *__restrict__ U,
-                                                        double *__restrict__ grad) {
-  constexpr int CPB = RT_BLOCK / LPC;  // cells per block
-  const int64_t C = m.C;
-  const int lane = threadIdx.x % LPC;
-  const int64_t i = (int64_t)blockIdx.x * CPB + threadIdx.x / LPC;
-  const int g = threadIdx.y;
-  const bool live = i < C;
-  const int64_t ic = live ? i : C - 1;  // dead lanes shadow the last cell (keeps shuffles uniform)
-  const double *Ug = U + (size_t)4 * g * C;
-  const double4 Ui = ld4(Ug + 4 * ic);
-  double b[4][3], hi[4] = {Ui.x, Ui.y, Ui.z, Ui.w}, lo[4] = {Ui.x, Ui.y, Ui.z, Ui.w};
+// fixed-order block sum of v over the block's threads; result valid in thread 0.
+// red: shared scratch of >= 32 doubles.
+__device__ __forceinline__ double block_sum(double v, double *red) {
 #pragma unroll
-  for (int v = 0; v < 4; v++) b[v][0] = b[v][1] = b[v][2] = 0.0;
-  const int64_t f0 = m.fo[ic], r0 = m.ro[ic];
-  const int nown = (int)(m.fo[ic + 1] - f0), nr = (int)(m.ro[ic + 1] - r0);
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  const int w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) red[w] = v;
+  __syncthreads();
+  double t = 0.0;
+  if (threadIdx.x == 0)
+    for (int k = 0; k < nw; k++) t += red[k];
+  return t;
+}
 
-  auto accumulate = [&](const double4 Uj, double wx, double wy, double wz) {
-    const double d0 = Uj.x - Ui.x, d1 = Uj.y - Ui.y, d2 = Uj.z - Ui.z, d3 = Uj.w - Ui.w;
-    b[0][0] += wx * d0; b[0][1] += wy * d0; b[0][2] += wz * d0;
-    b[1][0] += wx * d1; b[1][1] += wy * d1; b[1][2] += wz * d1;
-    b[2][0] += wx * d2; b[2][1] += wy * d2; b[2][2] += wz * d2;
-    b[3][0] += wx * d3; b[3][1] += wy * d3; b[3][2] += wz * d3;
-    hi[0] = fmax(hi[0], Uj.x); hi[1] = fmax(hi[1], Uj.y); hi[2] = fmax(hi[2], Uj.z); hi[3] = fmax(hi[3], Uj.w);
-    lo[0] = fmin(lo[0], Uj.x); lo[1] = fmin(lo[1], Uj.y); lo[2] = fmin(lo[2], Uj.z); lo[3] = fmin(lo[3], Uj.w);
-  };
-  // first pass: sum_f w_f (phi_j - phi_i), min/max.  Owned faces: the cell is the left one.
-#pragma unroll 2
-  for (int k = lane; k < nown; k += LPC) {
-    const int64_t q = f0 + k;
-    const int32_t j = m.R[q];
-    const double *w = m.faceW + 3 * q;
-    const double wx = w[0], wy = w[1], wz = w[2];
-    const double4 Uj = j >= 0 ? ld4(Ug + 4 * (int64_t)j) : ghost_for_gradient(j, Ui, m.faceN + 3 * q, m.ghost, m.G, g);
-    accumulate(Uj, wx, wy, wz);
+// ------------------------------------------------------------------ a2: gradients + limiter
+template <int G>
+__global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restrict__ U, double *__restrict__ grad) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double *sW = reinterpret_cast<double *>(smem_raw);  // [smax][4]  (w, L|R)
+  double *sC = sW + (size_t)4 * m.smax;               // [smax][4]  (c, A)
+  double *sU = sC + (size_t)4 * m.smax;               // [TC][G][4]
+  const int64_t C = m.C;
+  const int64_t c0 = (int64_t)blockIdx.x * m.TC;
+  const int ncell = (int)(c0 + m.TC < C ? m.TC : C - c0);
+  const int64_t fbase = m.fo[c0];
+  const int nown = (int)(m.fo[c0 + ncell] - fbase);
+  const int64_t ib = m.inco[blockIdx.x];
+  const int ns = nown + (int)(m.inco[blockIdx.x + 1] - ib);
+  // stage the slot records and the tile's U
+  for (int s = threadIdx.x; s < ns; s += blockDim.x) {
+    const int64_t q = s < nown ? fbase + s : (int64_t)m.incf[ib + (s - nown)];
+    *reinterpret_cast<double4 *>(sW + 4 * s) = ld4(m.faceW + 4 * q);
+    *reinterpret_cast<double4 *>(sC + 4 * s) = ld4(m.faceC + 4 * q);
   }
-  // faces where the cell is the right one: d = s_L - s_R, so the prefactor changes sign
-#pragma unroll 2
-  for (int k = lane; k < nr; k += LPC) {
-    const int64_t q = m.rl[r0 + k];
-    const int32_t j = m.rn[r0 + k];
-    const double *w = m.faceW + 3 * q;
-    const double wx = -w[0], wy = -w[1], wz = -w[2];
-    accumulate(ld4(Ug + 4 * (int64_t)j), wx, wy, wz);
-  }
+  for (int x = threadIdx.x; x < ncell * G; x += blockDim.x)
+    *reinterpret_cast<double4 *>(sU + 4 * x) = ld4(U + 4 * (c0 * G + x));
+  __syncthreads();
+
+  for (int item = threadIdx.x; item < ncell * G; item += blockDim.x) {
+    const int il = item / G, g = item - il * G;
+    const int64_t i = c0 + il;
+    const double4 Ui = ld4(sU + 4 * item);
+    double b[4][3], hi[4] = {Ui.x, Ui.y, Ui.z, Ui.w}, lo[4] = {Ui.x, Ui.y, Ui.z, Ui.w};
 #pragma unroll
-  for (int v = 0; v < 4; v++) {
-    b[v][0] = lanes_sum<LPC>(b[v][0]); b[v][1] = lanes_sum<LPC>(b[v][1]); b[v][2] = lanes_sum<LPC>(b[v][2]);
-    hi[v] = lanes_max<LPC>(hi[v]); lo[v] = lanes_min<LPC>(lo[v]);
-  }
-  const double *Mi = m.Minv + 6 * ic;
-  const double m00 = Mi[0], m01 = Mi[1], m02 = Mi[2], m11 = Mi[3], m12 = Mi[4], m22 = Mi[5];
-  double gr[4][3];
-#pragma unroll
-  for (int v = 0; v < 4; v++) {
-    gr[v][0] = m00 * b[v][0] + m01 * b[v][1] + m02 * b[v][2];
-    gr[v][1] = m01 * b[v][0] + m11 * b[v][1] + m12 * b[v][2];
-    gr[v][2] = m02 * b[v][0] + m12 * b[v][1] + m22 * b[v][2];
-  }
-  // second pass: extreme extrapolated increments at the face centres.  min_f (hi-phi)/D_f is
-  // attained at the largest D_f (division is monotone), so only the extremes are kept.
-  const double4 si = ld4(m.cellS + 4 * ic);
-  double dmax[4] = {0, 0, 0, 0}, dmin[4] = {0, 0, 0, 0};
-  auto extremes = [&](double rx, double ry, double rz) {
+    for (int v = 0; v < 4; v++) b[v][0] = b[v][1] = b[v][2] = 0.0;
+    const int s0 = (int)(m.fo[i] - fbase), no = (int)(m.fo[i + 1] - m.fo[i]);
+    const int64_t r0 = m.ro[i];
+    const int nr = (int)(m.ro[i + 1] - r0);
+    const uint16_t *rs = m.rslot + r0;
+
+    auto neighbour = [&](int32_t j) -> double4 {
+      const unsigned jl = (unsigned)(j - (int32_t)c0);
+      return jl < (unsigned)ncell ? ld4(sU + 4 * ((int)jl * G + g)) : ld4(U + 4 * ((int64_t)j * G + g));
+    };
+    auto accumulate = [&](const double4 Uj, double wx, double wy, double wz) {
+      const double d0 = Uj.x - Ui.x, d1 = Uj.y - Ui.y, d2 = Uj.z - Ui.z, d3 = Uj.w - Ui.w;
+      b[0][0] += wx * d0; b[0][1] += wy * d0; b[0][2] += wz * d0;
+      b[1][0] += wx * d1; b[1][1] += wy * d1; b[1][2] += wz * d1;
+      b[2][0] += wx * d2; b[2][1] += wy * d2; b[2][2] += wz * d2;
+      b[3][0] += wx * d3; b[3][1] += wy * d3; b[3][2] += wz * d3;
+      hi[0] = fmax(hi[0], Uj.x); hi[1] = fmax(hi[1], Uj.y); hi[2] = fmax(hi[2], Uj.z); hi[3] = fmax(hi[3], Uj.w);
+      lo[0] = fmin(lo[0], Uj.x); lo[1] = fmin(lo[1], Uj.y); lo[2] = fmin(lo[2], Uj.z); lo[3] = fmin(lo[3], Uj.w);
+    };
+    // first pass: sum_f w_f (phi_j - phi_i), min/max.  Owned faces: the cell is the left one.
+#pragma unroll 2
+    for (int k = 0; k < no; k++) {
+      const double4 w = ld4(sW + 4 * (s0 + k));
+      int32_t l, j;
+      rt_unpack_lr(w.w, l, j);
+      const double4 Uj = j >= 0 ? neighbour(j) : ghost_for_gradient(j, Ui, m.faceN, fbase + s0 + k, m.ghost, G, g);
+      accumulate(Uj, w.x, w.y, w.z);
+    }
+    // faces where the cell is the right one: d = s_L - s_R, so the prefactor changes sign
+#pragma unroll 2
+    for (int k = 0; k < nr; k++) {
+      const double4 w = ld4(sW + 4 * (int)rs[k]);
+      int32_t j, r;
+      rt_unpack_lr(w.w, j, r);
+      accumulate(neighbour(j), -w.x, -w.y, -w.z);
+    }
+    const double *Mi = m.Minv + 6 * i;
+    const double m00 = Mi[0], m01 = Mi[1], m02 = Mi[2], m11 = Mi[3], m12 = Mi[4], m22 = Mi[5];
+    double gr[4][3];
 #pragma unroll
     for (int v = 0; v < 4; v++) {
-      const double d = gr[v][0] * rx + gr[v][1] * ry + gr[v][2] * rz;
-      dmax[v] = fmax(dmax[v], d); dmin[v] = fmin(dmin[v], d);
+      gr[v][0] = m00 * b[v][0] + m01 * b[v][1] + m02 * b[v][2];
+      gr[v][1] = m01 * b[v][0] + m11 * b[v][1] + m12 * b[v][2];
+      gr[v][2] = m02 * b[v][0] + m12 * b[v][1] + m22 * b[v][2];
     }
-  };
-#pragma unroll 2
-  for (int k = lane; k < nown; k += LPC) {
-    const double4 c = ld4(m.faceC + 4 * (f0 + k));  // already in this cell's frame
-    extremes(c.x - si.x, c.y - si.y, c.z - si.z);
-  }
-#pragma unroll 2
-  for (int k = lane; k < nr; k += LPC) {
-    const double4 c = ld4(m.faceC + 4 * (int64_t)m.rl[r0 + k]);
-    extremes(rt_wrap(c.x - si.x, m.box[0], m.per[0]), rt_wrap(c.y - si.y, m.box[1], m.per[1]),
-             rt_wrap(c.z - si.z, m.box[2], m.per[2]));
-  }
+    // second pass: extreme extrapolated increments at the face centres.  min_f (hi-phi)/D_f is
+    // attained at the largest D_f (division is monotone), so only the extremes are kept.
+    const double4 si = ld4(m.cellS + 4 * i);
+    double dmax[4] = {0, 0, 0, 0}, dmin[4] = {0, 0, 0, 0};
+    auto extremes = [&](double rx, double ry, double rz) {
 #pragma unroll
-  for (int v = 0; v < 4; v++) { dmax[v] = lanes_max<LPC>(dmax[v]); dmin[v] = lanes_min<LPC>(dmin[v]); }
-  if (!live) return;
-  // lane v scales and writes field v (3 doubles each: the cell's 96 bytes leave as one run)
-  double *out = grad + ((size_t)g * C + i) * 12;
-  const double Uiv[4] = {Ui.x, Ui.y, Ui.z, Ui.w};
+      for (int v = 0; v < 4; v++) {
+        const double d = gr[v][0] * rx + gr[v][1] * ry + gr[v][2] * rz;
+        dmax[v] = fmax(dmax[v], d); dmin[v] = fmin(dmin[v], d);
+      }
+    };
+#pragma unroll 2
+    for (int k = 0; k < no; k++) {
+      const double4 c = ld4(sC + 4 * (s0 + k));  // already in this cell's frame
+      extremes(c.x - si.x, c.y - si.y, c.z - si.z);
+    }
+#pragma unroll 2
+    for (int k = 0; k < nr; k++) {
+      const double4 c = ld4(sC + 4 * (int)rs[k]);
+      extremes(rt_wrap(c.x - si.x, m.box[0], m.per[0]), rt_wrap(c.y - si.y, m.box[1], m.per[1]),
+               rt_wrap(c.z - si.z, m.box[2], m.per[2]));
+    }
+    double *out = grad + (size_t)12 * (i * G + g);
+    const double Uiv[4] = {Ui.x, Ui.y, Ui.z, Ui.w};
+    double o[12];
 #pragma unroll
-  for (int v = 0; v < 4; v++) {
-    if (v % LPC != lane) continue;
-    double a = 1.0;
-    if (dmax[v] > 0.0) a = fmin(a, (hi[v] - Uiv[v]) / dmax[v]);
-    if (dmin[v] < 0.0) a = fmin(a, (lo[v] - Uiv[v]) / dmin[v]);
-    out[3 * v] = a * gr[v][0]; out[3 * v + 1] = a * gr[v][1]; out[3 * v + 2] = a * gr[v][2];
+    for (int v = 0; v < 4; v++) {
+      double a = 1.0;
+      if (dmax[v] > 0.0) a = fmin(a, (hi[v] - Uiv[v]) / dmax[v]);
+      if (dmin[v] < 0.0) a = fmin(a, (lo[v] - Uiv[v]) / dmin[v]);
+      o[3 * v] = a * gr[v][0]; o[3 * v + 1] = a * gr[v][1]; o[3 * v + 2] = a * gr[v][2];
+    }
+    st4(out, o[0], o[1], o[2], o[3]); st4(out + 4, o[4], o[5], o[6], o[7]); st4(out + 8, o[8], o[9], o[10], o[11]);
   }
 }
 
+// ------------------------------------------------------------------ a3 + a4: fluxes and update
 // N D.n for the M1 closure (S1), lab frame: D = (1-chi)/2 I + (3 chi - 1)/2 nF nF^T
 __device__ __forceinline__ void pressure_dot_n(const double U[4], const double n[3], double ct, double out[3]) {
   const double f2n = U[1] * U[1] + U[2] * U[2] + U[3] * U[3];
@@ -170,13 +173,15 @@ __device__ __forceinline__ void pressure_dot_n(const double U[4], const double n
 }
 
 // U_face = U_i + grad U_i . r  (linear extrapolation to the centre of the interface)
-__device__ __forceinline__ void extrapolate(const double *__restrict__ Ug, const double *__restrict__ gg, int64_t i,
-                                            double rx, double ry, double rz, bool second_order, double Uo[4]) {
-  const double4 u = ld4(Ug + 4 * i);
+// pu: the cell's (N, Fx, Fy, Fz); pg: its 12 gradient components (field-major); shared or global
+template <bool SECOND>
+__device__ __forceinline__ void extrapolate(const double *pu, const double *pg, double rx, double ry, double rz,
+                                            double Uo[4], double &Ncentre) {
+  const double4 u = ld4(pu);
+  Ncentre = u.x;
   Uo[0] = u.x; Uo[1] = u.y; Uo[2] = u.z; Uo[3] = u.w;
-  if (second_order) {
-    const double *p = gg + 12 * i;
-    const double4 a = ld4(p), b = ld4(p + 4), c = ld4(p + 8);
+  if (SECOND) {
+    const double4 a = ld4(pg), b = ld4(pg + 4), c = ld4(pg + 8);
     Uo[0] += a.x * rx + a.y * ry + a.z * rz;
     Uo[1] += a.w * rx + b.x * ry + b.y * rz;
     Uo[2] += b.z * rx + b.w * ry + c.x * rz;
@@ -184,133 +189,161 @@ __device__ __forceinline__ void extrapolate(const double *__restrict__ Ug, const
   }
 }
 
-template <int GG>
-__global__ void __launch_bounds__(RT_BLOCK *GG) k_flux(rt_geom m, const double *__restrict__ U,
-                                                        const double *__restrict__ grad, double *__restrict__ phi,
-                                                        double ct, double dt, int second_order,
-                                                        double *__restrict__ part_out, double *__restrict__ part_in) {
-  __shared__ double sm_out[GG][RT_BLOCK / 32], sm_in[GG][RT_BLOCK / 32];
-  const int64_t C = m.C, F = m.F;
-  const int64_t q = (int64_t)blockIdx.x * RT_BLOCK + threadIdx.x;
-  const int g = threadIdx.y;
-  double b_out = 0.0, b_in = 0.0;
-  if (q < F) {
-    const double *Ug = U + (size_t)4 * g * C, *gg = grad + (size_t)12 * g * C;
-    const int32_t l = m.L[q], r = m.R[q];
-    const double4 fc = ld4(m.faceC + 4 * q);
-    const double n[3] = {m.faceN[3 * q], m.faceN[3 * q + 1], m.faceN[3 * q + 2]};
-    const double A = fc.w;
-    const double4 sl = ld4(m.cellS + 4 * (int64_t)l);
-    double UL[4], UR[4];
-    double Vr = 0.0, Nr = 0.0;
-    extrapolate(Ug, gg, l, fc.x - sl.x, fc.y - sl.y, fc.z - sl.z, second_order, UL);
-    if (r >= 0) {
-      const double4 sr = ld4(m.cellS + 4 * (int64_t)r);
-      Vr = sr.w;
-      extrapolate(Ug, gg, r, rt_wrap(fc.x - sr.x, m.box[0], m.per[0]), rt_wrap(fc.y - sr.y, m.box[1], m.per[1]),
-                  rt_wrap(fc.z - sr.z, m.box[2], m.per[2]), second_order, UR);
-      Nr = Ug[4 * (int64_t)r];
-    } else if (r == RT_BC_OUTFLOW) { UR[0] = UR[1] = UR[2] = UR[3] = 0.0; }  // vacuum ghost
-    else if (r == RT_BC_REFLECT) {
-      const double p = 2.0 * (UL[1] * n[0] + UL[2] * n[1] + UL[3] * n[2]);
-      UR[0] = UL[0]; UR[1] = UL[1] - p * n[0]; UR[2] = UL[2] - p * n[1]; UR[3] = UL[3] - p * n[2];
-    } else {
-      const double4 gs = ld4(m.ghost + ((size_t)(RT_BC_DIRICHLET0 - r) * m.G + g) * 4);
-      UR[0] = gs.x; UR[1] = gs.y; UR[2] = gs.z; UR[3] = gs.w;
+template <int G, bool SECOND>
+__global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restrict__ Uin, const double *__restrict__ grad,
+                                               const double *U0, double *Uout, const int32_t *__restrict__ srcidx,
+                                               const double *__restrict__ srcrate, int nsrc, double ca, double cb, double dt,
+                                               double ct, double n_floor, double *__restrict__ part_floor,
+                                               double *__restrict__ part_out, double *__restrict__ part_in) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ double red[32];
+  double *sPhi = reinterpret_cast<double *>(smem_raw);       // [G][smax][4]  A * (Phi_N, Phi_F)
+  double *sR = sPhi + (size_t)4 * G * m.smax;                // [TC][G][RT_REC]  U (4) + gradients (12)
+  double *sS = sR + (size_t)RT_REC * G * m.TC;               // [TC][4]  (s, V)
+  const int64_t C = m.C;
+  const int64_t c0 = (int64_t)blockIdx.x * m.TC;
+  const int ncell = (int)(c0 + m.TC < C ? m.TC : C - c0);
+  const int64_t fbase = m.fo[c0];
+  const int nown = (int)(m.fo[c0 + ncell] - fbase);
+  const int64_t ib = m.inco[blockIdx.x];
+  const int ns = nown + (int)(m.inco[blockIdx.x + 1] - ib);
+  const int smax = m.smax;
+  // stage the tile's cells
+  for (int x = threadIdx.x; x < ncell * G; x += blockDim.x)
+    *reinterpret_cast<double4 *>(sR + RT_REC * x) = ld4(Uin + 4 * (c0 * G + x));
+  if (SECOND)
+    for (int u = threadIdx.x; u < ncell * G * 3; u += blockDim.x) {
+      const int x = u / 3, part = u - 3 * x;
+      *reinterpret_cast<double4 *>(sR + RT_REC * x + 4 + 4 * part) = ld4(grad + 4 * (3 * c0 * G + u));
     }
-    double PL[3], PR[3];
-    pressure_dot_n(UL, n, ct, PL);
-    pressure_dot_n(UR, n, ct, PR);
-    double ph[4];
-    ph[0] = 0.5 * ((UL[1] + UR[1]) * n[0] + (UL[2] + UR[2]) * n[1] + (UL[3] + UR[3]) * n[2]) - 0.5 * ct * (UR[0] - UL[0]);
-    const double hc2 = 0.5 * ct * ct, hc = 0.5 * ct;
-#pragma unroll
-    for (int a = 0; a < 3; a++) ph[1 + a] = hc2 * (PL[a] + PR[a]) - hc * (UR[1 + a] - UL[1 + a]);
-    // donor cap (S11): the donor cannot lose more photons than it holds through this face in dt;
-    // only the number flux is clamped (continuous in the state; Phi_F is left alone)
-    if (ph[0] > 0.0) {
-      const double lim = Ug[4 * (int64_t)l] * sl.w / (dt * A);
-      if (ph[0] > lim) ph[0] = lim;
-    } else if (ph[0] < 0.0 && r >= 0) {
-      const double lim = Nr * Vr / (dt * A);
-      if (-ph[0] > lim) ph[0] = -lim;
-    }
-    st4(phi + ((size_t)g * F + q) * 4, A * ph[0], A * ph[1], A * ph[2], A * ph[3]);
-    if (r == RT_BC_OUTFLOW) b_out = A * ph[0];
-    else if (r <= RT_BC_DIRICHLET0) b_in = -A * ph[0];
-  }
-  // boundary ledgers: fixed-order block sums, one row per block
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    b_out += __shfl_down_sync(0xffffffffu, b_out, o);
-    b_in += __shfl_down_sync(0xffffffffu, b_in, o);
-  }
-  if ((threadIdx.x & 31) == 0) { sm_out[g][threadIdx.x >> 5] = b_out; sm_in[g][threadIdx.x >> 5] = b_in; }
+  for (int x = threadIdx.x; x < ncell; x += blockDim.x) *reinterpret_cast<double4 *>(sS + 4 * x) = ld4(m.cellS + 4 * (c0 + x));
   __syncthreads();
-  if (threadIdx.x == 0) {
-    double so = 0.0, si = 0.0;
-    for (int k = 0; k < RT_BLOCK / 32; k++) { so += sm_out[g][k]; si += sm_in[g][k]; }
-    part_out[(size_t)blockIdx.x * m.G + g] = so;
-    part_in[(size_t)blockIdx.x * m.G + g] = si;
-  }
-}
 
-template <int GG, int LPC>
-__global__ void __launch_bounds__(RT_BLOCK *GG) k_update(rt_geom m, const double *Ucur, const double *U0,
-                                                          const double *__restrict__ phi, double *Uout,
-                                                          const int32_t *__restrict__ srcidx,
-                                                          const double *__restrict__ srcrate, int nsrc, double ca,
-                                                          double cb, double dt, double ct, double n_floor,
-                                                          double *__restrict__ part_floor) {
-  constexpr int CPB = RT_BLOCK / LPC;
-  __shared__ double sm[GG][RT_BLOCK / 32];
-  const int64_t C = m.C, F = m.F;
-  const int lane = threadIdx.x % LPC;
-  const int64_t i = (int64_t)blockIdx.x * CPB + threadIdx.x / LPC;
-  const int g = threadIdx.y;
-  const bool live = i < C;
-  const int64_t ic = live ? i : C - 1;
-  const double *pg = phi + (size_t)4 * g * F;
-  double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-  const int64_t f0 = m.fo[ic], r0 = m.ro[ic];
-  const int nown = (int)(m.fo[ic + 1] - f0), nr = (int)(m.ro[ic + 1] - r0);
-#pragma unroll 2
-  for (int k = lane; k < nown; k += LPC) {
-    const double4 p = ld4(pg + 4 * (f0 + k));
-    s0 += p.x; s1 += p.y; s2 += p.z; s3 += p.w;
+  // ---- a3: one thread per face slot, all groups
+  double b_out[G], b_in[G];
+#pragma unroll
+  for (int g = 0; g < G; g++) b_out[g] = b_in[g] = 0.0;
+  int bnd = 0;
+  const double hc2 = 0.5 * ct * ct, hc = 0.5 * ct;
+  for (int s = threadIdx.x; s < ns; s += blockDim.x) {
+    const int64_t q = s < nown ? fbase + s : (int64_t)m.incf[ib + (s - nown)];
+    const double4 fc = ld4(m.faceC + 4 * q), fn = ld4(m.faceN + 4 * q);
+    int32_t l, r;
+    rt_unpack_lr(fn.w, l, r);
+    const double n[3] = {fn.x, fn.y, fn.z};
+    const double A = fc.w;
+    const unsigned ll = (unsigned)(l - (int32_t)c0), rl = (unsigned)(r - (int32_t)c0);
+    const bool l_in = ll < (unsigned)ncell, r_in = r >= 0 && rl < (unsigned)ncell;
+    const double4 sl = l_in ? ld4(sS + 4 * ll) : ld4(m.cellS + 4 * (int64_t)l);
+    const double rLx = fc.x - sl.x, rLy = fc.y - sl.y, rLz = fc.z - sl.z;
+    double rRx = 0.0, rRy = 0.0, rRz = 0.0, Vr = 0.0;
+    if (r >= 0) {
+      const double4 sr = r_in ? ld4(sS + 4 * rl) : ld4(m.cellS + 4 * (int64_t)r);
+      Vr = sr.w;
+      rRx = rt_wrap(fc.x - sr.x, m.box[0], m.per[0]); rRy = rt_wrap(fc.y - sr.y, m.box[1], m.per[1]);
+      rRz = rt_wrap(fc.z - sr.z, m.box[2], m.per[2]);
+    }
+    const double capL = sl.w / (dt * A), capR = Vr / (dt * A);
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+      double UL[4], UR[4], NL, NR = 0.0;
+      if (l_in) { const double *p = sR + RT_REC * ((int)ll * G + g); extrapolate<SECOND>(p, p + 4, rLx, rLy, rLz, UL, NL); }
+      else { const int64_t x = (int64_t)l * G + g; extrapolate<SECOND>(Uin + 4 * x, grad + 12 * x, rLx, rLy, rLz, UL, NL); }
+      if (r >= 0) {
+        if (r_in) { const double *p = sR + RT_REC * ((int)rl * G + g); extrapolate<SECOND>(p, p + 4, rRx, rRy, rRz, UR, NR); }
+        else { const int64_t x = (int64_t)r * G + g; extrapolate<SECOND>(Uin + 4 * x, grad + 12 * x, rRx, rRy, rRz, UR, NR); }
+      } else if (r == RT_BC_OUTFLOW) { UR[0] = UR[1] = UR[2] = UR[3] = 0.0; }  // vacuum ghost
+      else if (r == RT_BC_REFLECT) {
+        const double p = 2.0 * (UL[1] * n[0] + UL[2] * n[1] + UL[3] * n[2]);
+        UR[0] = UL[0]; UR[1] = UL[1] - p * n[0]; UR[2] = UL[2] - p * n[1]; UR[3] = UL[3] - p * n[2];
+      } else {
+        const double4 gs = ld4(m.ghost + ((size_t)(RT_BC_DIRICHLET0 - r) * G + g) * 4);
+        UR[0] = gs.x; UR[1] = gs.y; UR[2] = gs.z; UR[3] = gs.w;
+      }
+      double PL[3], PR[3], ph[4];
+      pressure_dot_n(UL, n, ct, PL);
+      pressure_dot_n(UR, n, ct, PR);
+      ph[0] = 0.5 * ((UL[1] + UR[1]) * n[0] + (UL[2] + UR[2]) * n[1] + (UL[3] + UR[3]) * n[2]) - hc * (UR[0] - UL[0]);
+#pragma unroll
+      for (int a = 0; a < 3; a++) ph[1 + a] = hc2 * (PL[a] + PR[a]) - hc * (UR[1 + a] - UL[1 + a]);
+      // donor cap (S11): the donor cannot lose more photons than it holds through this face in dt;
+      // only the number flux is clamped (continuous in the state; Phi_F is left alone)
+      if (ph[0] > 0.0) {
+        const double lim = NL * capL;
+        if (ph[0] > lim) ph[0] = lim;
+      } else if (ph[0] < 0.0 && r >= 0) {
+        const double lim = NR * capR;
+        if (-ph[0] > lim) ph[0] = -lim;
+      }
+      st4(sPhi + 4 * ((size_t)g * smax + s), A * ph[0], A * ph[1], A * ph[2], A * ph[3]);
+      if (r == RT_BC_OUTFLOW) { b_out[g] += A * ph[0]; bnd = 1; }
+      else if (r <= RT_BC_DIRICHLET0) { b_in[g] -= A * ph[0]; bnd = 1; }
+    }
   }
-#pragma unroll 2
-  for (int k = lane; k < nr; k += LPC) {
-    const double4 p = ld4(pg + 4 * (int64_t)m.rl[r0 + k]);
-    s0 -= p.x; s1 -= p.y; s2 -= p.z; s3 -= p.w;
+  // boundary ledgers: fixed-order block sums, one row per tile (the barrier also ends phase a3)
+  if (__syncthreads_or(bnd)) {
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+      const double so = block_sum(b_out[g], red), si = block_sum(b_in[g], red);
+      if (threadIdx.x == 0) { part_out[(size_t)blockIdx.x * G + g] = so; part_in[(size_t)blockIdx.x * G + g] = si; }
+    }
+  } else if (threadIdx.x < G) {
+    part_out[(size_t)blockIdx.x * G + threadIdx.x] = 0.0;
+    part_in[(size_t)blockIdx.x * G + threadIdx.x] = 0.0;
   }
-  s0 = lanes_sum<LPC>(s0); s1 = lanes_sum<LPC>(s1); s2 = lanes_sum<LPC>(s2); s3 = lanes_sum<LPC>(s3);
-  double fl = 0.0;
-  if (live && lane == 0) {
-    const double V = m.cellS[4 * i + 3];
-    double R[4] = {-s0 / V, -s1 / V, -s2 / V, -s3 / V};
+
+  // ---- a4: one thread per (cell, group): gather the cell's faces in list order, update
+  double fl[G];
+#pragma unroll
+  for (int g = 0; g < G; g++) fl[g] = 0.0;
+  int floored = 0;
+  for (int item = threadIdx.x; item < ncell * G; item += blockDim.x) {
+    const int il = item / G, g = item - il * G;
+    const int64_t i = c0 + il;
+    const int s0 = (int)(m.fo[i] - fbase), no = (int)(m.fo[i + 1] - m.fo[i]);
+    const int64_t r0 = m.ro[i];
+    const int nr = (int)(m.ro[i + 1] - r0);
+    const uint16_t *rs = m.rslot + r0;
+    const double *pg = sPhi + 4 * (size_t)g * smax;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+#pragma unroll 4
+    for (int k = 0; k < no; k++) {
+      const double4 p = ld4(pg + 4 * (s0 + k));
+      a0 += p.x; a1 += p.y; a2 += p.z; a3 += p.w;
+    }
+#pragma unroll 4
+    for (int k = 0; k < nr; k++) {
+      const double4 p = ld4(pg + 4 * (int)rs[k]);
+      a0 -= p.x; a1 -= p.y; a2 -= p.z; a3 -= p.w;
+    }
+    const double V = sS[4 * il + 3];
+    double R[4] = {-a0 / V, -a1 / V, -a2 / V, -a3 / V};
     const int32_t si = srcidx[i];
     if (si >= 0) R[0] += srcrate[(size_t)g * nsrc + si] / V;  // isotropic source (S5)
-    const size_t o = ((size_t)g * C + i) * 4;
-    const double4 uc = ld4(Ucur + o), u0 = ld4(U0 + o);
+    const size_t o = 4 * ((size_t)i * G + g);
+    const double4 uc = ld4(sR + RT_REC * item), u0 = ld4(U0 + o);
     double Un[4] = {ca * u0.x + cb * (uc.x + dt * R[0]), ca * u0.y + cb * (uc.y + dt * R[1]),
                     ca * u0.z + cb * (uc.z + dt * R[2]), ca * u0.w + cb * (uc.w + dt * R[3])};
-    if (Un[0] < n_floor) { fl = V * (n_floor - Un[0]); Un[0] = n_floor; }
-    const double fn = sqrt(Un[1] * Un[1] + Un[2] * Un[2] + Un[3] * Un[3]), lim = ct * Un[0];
-    if (fn > lim) { const double sc = lim / fn; Un[1] *= sc; Un[2] *= sc; Un[3] *= sc; }
+    if (Un[0] < n_floor) {
+      const double add = V * (n_floor - Un[0]);
+#pragma unroll
+      for (int gg = 0; gg < G; gg++) if (gg == g) fl[gg] += add;
+      Un[0] = n_floor; floored = 1;
+    }
+    const double fnorm = sqrt(Un[1] * Un[1] + Un[2] * Un[2] + Un[3] * Un[3]), lim = ct * Un[0];
+    if (fnorm > lim) { const double sc = lim / fnorm; Un[1] *= sc; Un[2] *= sc; Un[3] *= sc; }
     st4(Uout + o, Un[0], Un[1], Un[2], Un[3]);
   }
+  if (__syncthreads_or(floored)) {
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) fl += __shfl_down_sync(0xffffffffu, fl, o);
-  if ((threadIdx.x & 31) == 0) sm[g][threadIdx.x >> 5] = fl;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    double t = 0.0;
-    for (int k = 0; k < RT_BLOCK / 32; k++) t += sm[g][k];
-    part_floor[(size_t)blockIdx.x * m.G + g] = t;
-  }
+    for (int g = 0; g < G; g++) {
+      const double t = block_sum(fl[g], red);
+      if (threadIdx.x == 0) part_floor[(size_t)blockIdx.x * G + g] = t;
+    }
+  } else if (threadIdx.x < G) part_floor[(size_t)blockIdx.x * G + threadIdx.x] = 0.0;
 }
 
+// ------------------------------------------------------------------ ledgers
 // acc[slot][g] += weight * sum_rows part[row][g]; one block per (array, g); fixed order.
 struct reduce_job { const double *part; int64_t nrows; double weight; int slot; };
 __global__ void __launch_bounds__(1024) k_reduce(reduce_job j0, reduce_job j1, int G, rt_dev_ledger *led) {
@@ -343,12 +376,12 @@ __global__ void __launch_bounds__(1024) k_reduce(reduce_job j0, reduce_job j1, i
 
 // stored photons per block: part[row][g] = sum_cells V N
 template <int GG>
-__global__ void __launch_bounds__(RT_BLOCK *GG) k_stored(int64_t C, int G, const double *__restrict__ U,
+__global__ void __launch_bounds__(RT_BLOCK *GG) k_stored(int64_t C, const double *__restrict__ U,
                                                           const double *__restrict__ cellS, double *__restrict__ part) {
   __shared__ double sm[GG][RT_BLOCK / 32];
   const int64_t i = (int64_t)blockIdx.x * RT_BLOCK + threadIdx.x;
   const int g = threadIdx.y;
-  double v = i < C ? cellS[4 * i + 3] * U[((size_t)g * C + i) * 4] : 0.0;
+  double v = i < C ? cellS[4 * i + 3] * U[((size_t)i * GG + g) * 4] : 0.0;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
   if ((threadIdx.x & 31) == 0) sm[g][threadIdx.x >> 5] = v;
@@ -356,7 +389,7 @@ __global__ void __launch_bounds__(RT_BLOCK *GG) k_stored(int64_t C, int G, const
   if (threadIdx.x == 0) {
     double t = 0.0;
     for (int k = 0; k < RT_BLOCK / 32; k++) t += sm[g][k];
-    part[(size_t)blockIdx.x * G + g] = t;
+    part[(size_t)blockIdx.x * GG + g] = t;
   }
 }
 
@@ -387,51 +420,71 @@ __global__ void k_set_sources(int nsrc, const int32_t *__restrict__ cell, const 
 
 // ------------------------------------------------------------------ host-side launchers
 static inline unsigned blocks_for(int64_t n, int per_block) { return (unsigned)((n + per_block - 1) / per_block); }
-#define DISPATCH_G(Gv, KERNEL, grid, block, stream, ...)                                  \
+#define DISPATCH_G(Gv, KERNEL, grid, block, smem, stream, ...)                            \
   switch (Gv) {                                                                           \
-    case 1: KERNEL(1)<<<grid, block, 0, stream>>>(__VA_ARGS__); break;                    \
-    case 2: KERNEL(2)<<<grid, block, 0, stream>>>(__VA_ARGS__); break;                    \
-    case 3: KERNEL(3)<<<grid, block, 0, stream>>>(__VA_ARGS__); break;                    \
-    case 4: KERNEL(4)<<<grid, block, 0, stream>>>(__VA_ARGS__); break;                    \
-    case 5: KERNEL(5)<<<grid, block, 0, stream>>>(__VA_ARGS__); break;                    \
-    case 6: KERNEL(6)<<<grid, block, 0, stream>>>(__VA_ARGS__); break;                    \
-    case 7: KERNEL(7)<<<grid, block, 0, stream>>>(__VA_ARGS__); break;                    \
-    default: KERNEL(8)<<<grid, block, 0, stream>>>(__VA_ARGS__); break;                   \
+    case 1: KERNEL(1)<<<grid, block, smem, stream>>>(__VA_ARGS__); break;                 \
+    case 2: KERNEL(2)<<<grid, block, smem, stream>>>(__VA_ARGS__); break;                 \
+    case 3: KERNEL(3)<<<grid, block, smem, stream>>>(__VA_ARGS__); break;                 \
+    case 4: KERNEL(4)<<<grid, block, smem, stream>>>(__VA_ARGS__); break;                 \
+    case 5: KERNEL(5)<<<grid, block, smem, stream>>>(__VA_ARGS__); break;                 \
+    case 6: KERNEL(6)<<<grid, block, smem, stream>>>(__VA_ARGS__); break;                 \
+    case 7: KERNEL(7)<<<grid, block, smem, stream>>>(__VA_ARGS__); break;                 \
+    default: KERNEL(8)<<<grid, block, smem, stream>>>(__VA_ARGS__); break;                \
   }
-#define K_GRAD1(g) k_grad<g, 1>
-#define K_GRAD2(g) k_grad<g, 2>
-#define K_GRAD4(g) k_grad<g, 4>
-#define K_GRAD8(g) k_grad<g, 8>
-#define K_FLUX(g) k_flux<g>
-#define K_UPD1(g) k_update<g, 1>
-#define K_UPD2(g) k_update<g, 2>
-#define K_UPD4(g) k_update<g, 4>
-#define K_UPD8(g) k_update<g, 8>
+#define K_GRAD(g) k_grad<g>
+#define K_STAGE2(g) k_stage<g, true>
+#define K_STAGE1(g) k_stage<g, false>
 #define K_STORED(g) k_stored<g>
-#define DISPATCH_LPC(lpc, Gv, K1, K2, K4, K8, cells, block, stream, ...)                               \
-  switch (lpc) {                                                                                       \
-    case 1: DISPATCH_G(Gv, K1, blocks_for(cells, RT_BLOCK), block, stream, __VA_ARGS__); break;        \
-    case 2: DISPATCH_G(Gv, K2, blocks_for(cells, RT_BLOCK / 2), block, stream, __VA_ARGS__); break;    \
-    case 4: DISPATCH_G(Gv, K4, blocks_for(cells, RT_BLOCK / 4), block, stream, __VA_ARGS__); break;    \
-    default: DISPATCH_G(Gv, K8, blocks_for(cells, RT_BLOCK / 8), block, stream, __VA_ARGS__); break;   \
+
+// the tile kernels need more than the default 48 KB of dynamic shared memory
+template <class K>
+static cudaError_t allow_smem(K kernel, size_t bytes) {
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+#define SET_SMEM_G(Gv, KERNEL, bytes, err)                      \
+  switch (Gv) {                                                 \
+    case 1: err = allow_smem(KERNEL(1), bytes); break;          \
+    case 2: err = allow_smem(KERNEL(2), bytes); break;          \
+    case 3: err = allow_smem(KERNEL(3), bytes); break;          \
+    case 4: err = allow_smem(KERNEL(4), bytes); break;          \
+    case 5: err = allow_smem(KERNEL(5), bytes); break;          \
+    case 6: err = allow_smem(KERNEL(6), bytes); break;          \
+    case 7: err = allow_smem(KERNEL(7), bytes); break;          \
+    default: err = allow_smem(KERNEL(8), bytes); break;         \
   }
+
+int rt_transport_configure(rt_ctx *c) {
+  cudaError_t e = cudaSuccess;
+  const size_t sg = rt_smem_grad(c->TC, c->G, c->smax), ss = rt_smem_stage(c->TC, c->G, c->smax);
+  SET_SMEM_G(c->G, K_GRAD, sg, e);
+  if (e == cudaSuccess) SET_SMEM_G(c->G, K_STAGE2, ss, e);
+  if (e == cudaSuccess) SET_SMEM_G(c->G, K_STAGE1, ss, e);
+  if (e != cudaSuccess) return rt_fail(c, RT_ECUDA, "cudaFuncSetAttribute(shared memory): %s", cudaGetErrorString(e));
+  return RT_OK;
+}
+
+// threads per tile block: one per (cell, group), a whole number of warps, at most 256
+static int tile_threads(const rt_ctx *c) {
+  int n = ((c->TC * c->G + 31) / 32) * 32;
+  return n > 256 ? 256 : (n < 64 ? 64 : n);
+}
 
 rt_geom rt_geom_of(const rt_ctx *c) {
   const rt_layout &l = c->lay;
   rt_geom m;
-  m.C = c->C; m.F = c->F; m.G = c->G;
+  m.C = c->C; m.F = c->F; m.G = c->G; m.TC = c->TC; m.smax = c->smax;
   m.cellS = rt_ptr<double>(c, l.cellS); m.Minv = rt_ptr<double>(c, l.Minv);
   m.faceC = rt_ptr<double>(c, l.faceC); m.faceN = rt_ptr<double>(c, l.faceN); m.faceW = rt_ptr<double>(c, l.faceW);
-  m.L = rt_ptr<int32_t>(c, l.L); m.R = rt_ptr<int32_t>(c, l.R);
-  m.rl = rt_ptr<int32_t>(c, l.rl); m.rn = rt_ptr<int32_t>(c, l.rn); m.fo = rt_ptr<int64_t>(c, l.fo); m.ro = rt_ptr<int64_t>(c, l.ro);
+  m.fo = rt_ptr<int64_t>(c, l.fo); m.ro = rt_ptr<int64_t>(c, l.ro); m.inco = rt_ptr<int64_t>(c, l.inco);
+  m.incf = rt_ptr<int32_t>(c, l.incf); m.rslot = rt_ptr<uint16_t>(c, l.rslot);
   m.ghost = rt_ptr<double>(c, l.ghost);
   for (int a = 0; a < 3; a++) { m.box[a] = c->box[a]; m.per[a] = c->per[a]; }
   return m;
 }
 
 int rt_launch_gradients(rt_ctx *c, const double *U) {
-  DISPATCH_LPC(lpc_grad(), c->G, K_GRAD1, K_GRAD2, K_GRAD4, K_GRAD8, c->C, dim3(RT_BLOCK, c->G), c->stream, rt_geom_of(c),
-               U, rt_ptr<double>(c, c->lay.grad));
+  DISPATCH_G(c->G, K_GRAD, (unsigned)c->T, tile_threads(c), rt_smem_grad(c->TC, c->G, c->smax), c->stream, rt_geom_of(c), U,
+             rt_ptr<double>(c, c->lay.grad));
   c->launches++;
   return RT_OK;
 }
@@ -449,31 +502,30 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
   const rt_layout &l = c->lay;
   const rt_geom m = rt_geom_of(c);
   const int G = c->G;
-  double *grad = rt_ptr<double>(c, l.grad), *phi = rt_ptr<double>(c, l.phi);
+  double *grad = rt_ptr<double>(c, l.grad);
   double *part = rt_ptr<double>(c, l.part);
-  const int64_t nbu = blocks_for(c->C, RT_BLOCK / lpc_upd());
   const int64_t nchem = blocks_for(c->C, RT_CHEM_BLOCK);
-  double *p_floor = part + (size_t)G * nchem, *p_out = p_floor + (size_t)G * nbu, *p_in = p_out + (size_t)G * l.nbf;
-  const int second = c->par.order >= 2;
-  if (second) {
+  double *p_floor = part + (size_t)G * nchem, *p_out = p_floor + (size_t)G * c->T, *p_in = p_out + (size_t)G * c->T;
+  const int nt = tile_threads(c);
+  const size_t ss = rt_smem_stage(c->TC, G, c->smax);
+  if (c->par.order >= 2) {
     rt_prof_begin(c, RT_K_GRAD);
-    DISPATCH_LPC(lpc_grad(), G, K_GRAD1, K_GRAD2, K_GRAD4, K_GRAD8, c->C, dim3(RT_BLOCK, G), c->stream, m, Uin, grad);
+    DISPATCH_G(G, K_GRAD, (unsigned)c->T, nt, rt_smem_grad(c->TC, G, c->smax), c->stream, m, Uin, grad);
     rt_prof_end(c);
     c->launches++;
+    rt_prof_begin(c, RT_K_UPDATE);
+    DISPATCH_G(G, K_STAGE2, (unsigned)c->T, nt, ss, c->stream, m, Uin, grad, U0, Uout, rt_ptr<int32_t>(c, l.srcidx),
+               rt_ptr<double>(c, l.srcrate), c->nsrc, ca, cb, dt, c->par.ctilde, c->par.n_floor, p_floor, p_out, p_in);
+    rt_prof_end(c);
+  } else {
+    rt_prof_begin(c, RT_K_UPDATE);
+    DISPATCH_G(G, K_STAGE1, (unsigned)c->T, nt, ss, c->stream, m, Uin, grad, U0, Uout, rt_ptr<int32_t>(c, l.srcidx),
+               rt_ptr<double>(c, l.srcrate), c->nsrc, ca, cb, dt, c->par.ctilde, c->par.n_floor, p_floor, p_out, p_in);
+    rt_prof_end(c);
   }
-  rt_prof_begin(c, RT_K_FLUX);
-  DISPATCH_G(G, K_FLUX, (unsigned)l.nbf, dim3(RT_BLOCK, G), c->stream, m, Uin, grad, phi, c->par.ctilde, dt, second, p_out,
-             p_in);
-  rt_prof_end(c);
   c->launches++;
-  reduce2(c, {p_out, l.nbf, wl * dt, 1}, {p_in, l.nbf, wl * dt, 2}, 2);
-  rt_prof_begin(c, RT_K_UPDATE);
-  DISPATCH_LPC(lpc_upd(), G, K_UPD1, K_UPD2, K_UPD4, K_UPD8, c->C, dim3(RT_BLOCK, G), c->stream, m, Uin, U0, phi, Uout,
-               rt_ptr<int32_t>(c, l.srcidx), rt_ptr<double>(c, l.srcrate), c->nsrc, ca, cb, dt, c->par.ctilde,
-               c->par.n_floor, p_floor);
-  rt_prof_end(c);
-  c->launches++;
-  reduce2(c, {p_floor, nbu, wf, 3}, {p_floor, nbu, wf, 3}, 1);
+  reduce2(c, {p_out, c->T, wl * dt, 1}, {p_in, c->T, wl * dt, 2}, 2);
+  reduce2(c, {p_floor, c->T, wf, 3}, {p_floor, c->T, wf, 3}, 1);
 }
 
 int rt_launch_step(rt_ctx *c, double dt) {
@@ -514,7 +566,7 @@ int rt_launch_step(rt_ctx *c, double dt) {
 int rt_launch_stored(rt_ctx *c) {
   const rt_layout &l = c->lay;
   double *part = rt_ptr<double>(c, l.part);
-  DISPATCH_G(c->G, K_STORED, (unsigned)l.nbc, dim3(RT_BLOCK, c->G), c->stream, c->C, c->G, rt_ptr<double>(c, l.Ua),
+  DISPATCH_G(c->G, K_STORED, (unsigned)l.nbc, dim3(RT_BLOCK, c->G), 0, c->stream, c->C, rt_ptr<double>(c, l.Ua),
              rt_ptr<double>(c, l.cellS), part);
   c->launches++;
   reduce2(c, {part, l.nbc, 1.0, 4}, {part, l.nbc, 1.0, 4}, 1);

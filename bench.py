@@ -138,14 +138,21 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------ algorithmic bytes
-def algorithmic_bytes(C, F, NR, G, heun=True, chem=True):
-    """Bytes each kernel must move per launch if every array is read or written once."""
-    grad = 32 * G * C + (24 + 24 + 8) * F + 4 * NR + 16 * C + 24 * C + 48 * C + 96 * G * C
-    flux = 32 * G * C + 96 * G * C + (8 + 24 + 24 + 8) * F + 24 * C + 8 * C + 32 * G * F
-    update = 32 * G * F + 8 * F + 4 * NR + 16 * C + 64 * G * C + 8 * C + 4 * C + 32 * G * C
+def algorithmic_bytes(C, F, NR, G, heun=True, chem=True, order=2):
+    """Bytes each kernel must move per launch if every array it needs is read or written once
+    (neighbour gathers served by L2/shared memory; faces shared by two tiles counted once)."""
+    # a2 gradient pass: U in, grad out, per face (w, ids) + (c, A), per r-entry slot id, per cell
+    # Minv, (s, V), two list offsets
+    grad = 32 * G * C + 96 * G * C + 64 * F + 2 * NR + (48 + 32 + 16) * C
+    # a3+a4 stage pass: U and grad in, U out, U0 in (read in both stages), per face (c, A) + (n, ids),
+    # per r-entry slot id, per cell (s, V), two list offsets, source index
+    stage = (32 + 96 + 32 + 32) * G * C + 64 * F + 2 * NR + (32 + 16 + 4) * C
+    if order < 2:
+        stage -= 96 * G * C
     chemb = 64 * G * C + 64 * C + 16 * C
-    per_sub = (2 if heun else 1) * (grad + flux + update) + (chemb if chem else 0)
-    return {"grad": grad, "flux": flux, "update": update, "chem": chemb, "subcycle": per_sub}
+    per_stage = (grad if order >= 2 else 0) + stage
+    per_sub = (2 if heun else 1) * per_stage + (chemb if chem else 0)
+    return {"grad": grad, "stage": stage, "chem": chemb, "subcycle": per_sub}
 
 
 def main():
@@ -193,6 +200,7 @@ def main():
     w.mesh = None
     torch.cuda.empty_cache()
     s.init(w.state, w.sources)
+    tiles = s.tile_info()
     t_build = time.perf_counter() - t_build
     stored0 = None
     s.step(w.dt, args.warmup)
@@ -268,9 +276,10 @@ def main():
         peak, peak_src = float(json.load(open(peaks_file))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     else:
         peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
-    ab = algorithmic_bytes(C, F, NR, G, bool(w.params.heun), w.params.chem_mode != 0)
+    ab = algorithmic_bytes(C, F, NR, G, bool(w.params.heun), w.params.chem_mode != 0, int(w.params.order))
     kern = {}
-    for k in ("chem", "grad", "flux", "update", "reduce"):
+    prof["stage"] = prof["update"]   # class 3 = flux + update of one Heun stage (k_stage)
+    for k in ("chem", "grad", "stage", "reduce"):
         tms, cnt = prof[k]
         if cnt == 0:
             continue
@@ -304,7 +313,7 @@ def main():
             "config": {"workload": workload_name(c, n), "cells": C, "faces": F, "groups": G,
                        "chem_mode": int(w.params.chem_mode), "dt": w.dt, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2 (%.1f GB of state and geometry per subcycle)" % (ab["subcycle"] / 1e9),
-                       "build_s": t_build},
+                       "build_s": t_build, "tiles": tiles},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "kernels": kern,
             "cpu_baseline": cpu,
             "ledger": {"substeps_total": int(led["substeps_total"]), "substeps_max": int(led["substeps_max"]),

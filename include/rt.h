@@ -143,11 +143,17 @@ int rt_download(rt_ctx *ctx, rt_state *out, rt_ledger *ledger);
 /* Number of kernels the context has launched since rt_create (for bench.py's gpu_launches). */
 int64_t rt_kernel_launches(const rt_ctx *ctx);
 
+/* The tile decomposition rt_mesh_upload chose, for reports: out[0] cells per tile,
+ * out[1] number of tiles, out[2] largest number of face slots of a tile, out[3] faces evaluated a
+ * second time because their two cells lie in different tiles.  HOST array of 4.  Needs a mesh. */
+int rt_tile_info(const rt_ctx *ctx, int64_t *out);
+
 /* Per-kernel timing with CUDA events recorded on the context's stream around every launch of
  * rt_step.  rt_profile(ctx, 1) starts recording, rt_profile(ctx, 0) stops.  rt_profile_read
  * synchronises and returns, per kernel class (0 chemistry, 1 gradient, 2 face flux, 3 update,
  * 4 ledger reduction, 5 other), the summed milliseconds and the number of launches since the last
- * read; ms and count are HOST arrays of 6. */
+ * read; ms and count are HOST arrays of 6.  Class 2 is empty since the face fluxes are
+ * evaluated inside the update kernel (class 3 = flux + update of one Heun stage). */
 int rt_profile(rt_ctx *ctx, int enable);
 int rt_profile_read(rt_ctx *ctx, double *ms, int64_t *count);
 

@@ -85,6 +85,13 @@ const char *rt_last_error(const rt_ctx *c) { return c ? c->err : "null context";
 
 int64_t rt_kernel_launches(const rt_ctx *c) { return c ? c->launches : 0; }
 
+int rt_tile_info(const rt_ctx *c, int64_t *out) {
+  if (!c || !out) return RT_EINVAL;
+  if (!c->have_mesh) return RT_ESTATE;
+  out[0] = c->TC; out[1] = c->T; out[2] = c->smax; out[3] = c->ninc;
+  return RT_OK;
+}
+
 size_t rt_workspace_bytes(int64_t ncell, int64_t nface, int ngroup, int flags) {
   (void)flags;
   if (ncell < 1 || nface < 1 || ngroup < 1 || ngroup > RT_MAXG || ncell > 0x7fffffffLL || nface > 0x7fffffffLL) return 0;

@@ -56,6 +56,7 @@ struct rt_ctx {
   int TC;             // cells per tile
   int64_t T;          // number of tiles
   int smax;           // largest slot count of any tile
+  int rmax;           // largest r-list entry count of any tile
   int64_t ninc;       // total incoming faces over all tiles
   double box[3];
   int per[3];
@@ -83,9 +84,13 @@ void rt_prof_end(rt_ctx *c);
 
 // dynamic shared memory of the two tile kernels (rt_transport.cu) for a tile of TC cells whose
 // slot count is at most smax
-static inline size_t rt_smem_grad(int TC, int G, int smax) { return (size_t)64 * smax + (size_t)32 * TC * G; }
-static inline size_t rt_smem_stage(int TC, int G, int smax) {
-  return (size_t)32 * G * smax + (size_t)RT_REC * 8 * TC * G + (size_t)32 * TC;
+// (rmax: most r-list entries of any tile; the face-list tables are two int[TC+1] and uint16[rmax])
+static inline size_t rt_smem_tables(int TC, int rmax) { return ((size_t)8 * (TC + 1) + (size_t)2 * rmax + 15) & ~(size_t)15; }
+static inline size_t rt_smem_grad(int TC, int G, int smax, int rmax) {
+  return (size_t)64 * smax + (size_t)32 * TC * G + rt_smem_tables(TC, rmax);
+}
+static inline size_t rt_smem_stage(int TC, int G, int smax, int rmax) {
+  return (size_t)32 * G * smax + (size_t)RT_REC * 8 * TC * G + (size_t)32 * TC + rt_smem_tables(TC, rmax);
 }
 #define RT_SMEM_MAX 232448     // 227 KB: the most one block may have on sm_100
 #define RT_SMEM_TARGET 110000  // two blocks per SM

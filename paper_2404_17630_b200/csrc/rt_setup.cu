@@ -221,8 +221,8 @@ __global__ void k_tile_count(int64_t C, int TC, const int64_t *ro, const int32_t
   cellInc[i] = n;
 }
 // per tile: exclusive prefix of cellInc over its cells (in place), the tile's total, max slots
-__global__ void k_tile_scan(int64_t C, int TC, int64_t T, const int64_t *fo, int32_t *cellInc, int64_t *tileInc,
-                            int *maxSlots) {
+__global__ void k_tile_scan(int64_t C, int TC, int64_t T, const int64_t *fo, const int64_t *ro, int32_t *cellInc,
+                            int64_t *tileInc, int *maxSlots) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= T) return;
   const int64_t c0 = t * TC, c1 = c0 + TC < C ? c0 + TC : C;
@@ -231,6 +231,8 @@ __global__ void k_tile_scan(int64_t C, int TC, int64_t T, const int64_t *fo, int
   tileInc[t] = run;
   const int64_t slots = fo[c1] - fo[c0] + run;
   atomicMax(maxSlots, slots > 0x7fffffff ? 0x7fffffff : (int)slots);
+  const int64_t nrt = ro[c1] - ro[c0];
+  atomicMax(maxSlots + 1, nrt > 0x7fffffff ? 0x7fffffff : (int)nrt);
 }
 __global__ void k_tile_fill(int64_t C, int TC, const int64_t *fo, const int64_t *ro, const int32_t *rl, const int32_t *rn,
                             const int32_t *cellInc, const int64_t *inco, int32_t *incf, uint16_t *rslot) {
@@ -363,14 +365,15 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
       const size_t limit = pass == 0 ? RT_SMEM_TARGET : RT_SMEM_MAX;
       for (int TC = tc0; TC >= RT_MIN_TILE; TC /= 2) {
         const int64_t T = (C + TC - 1) / TC;
-        RT_CUDA(c, cudaMemsetAsync(maxSlots, 0, sizeof(int), st));
+        RT_CUDA(c, cudaMemsetAsync(maxSlots, 0, 2 * sizeof(int), st));
         k_tile_count<<<nblk(C), SETUP_BLOCK, 0, st>>>(C, TC, ro, rn, cellInc);
-        k_tile_scan<<<nblk(T), SETUP_BLOCK, 0, st>>>(C, TC, T, fo, cellInc, tileInc, maxSlots);
-        int smax = 0;
-        RT_CUDA(c, cudaMemcpyAsync(&smax, maxSlots, sizeof(int), cudaMemcpyDeviceToHost, st));
+        k_tile_scan<<<nblk(T), SETUP_BLOCK, 0, st>>>(C, TC, T, fo, ro, cellInc, tileInc, maxSlots);
+        int mx[2] = {0, 0};
+        RT_CUDA(c, cudaMemcpyAsync(mx, maxSlots, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
         RT_CUDA(c, cudaStreamSynchronize(st));
-        if (smax < 65536 && rt_smem_stage(TC, c->G, smax) <= limit && rt_smem_grad(TC, c->G, smax) <= limit) {
-          best = TC; best_smax = smax;
+        const int smax = mx[0], rmax = mx[1];
+        if (smax < 65536 && rt_smem_stage(TC, c->G, smax, rmax) <= limit && rt_smem_grad(TC, c->G, smax, rmax) <= limit) {
+          best = TC; best_smax = smax; c->rmax = rmax;
           break;
         }
       }

@@ -1,9 +1,10 @@
 // a2-a4: the transport kernels of one Heun stage, one thread block per tile of TC consecutive
 // cells of the Peano-Hilbert order (layout and tile tables: rt_internal.cuh).
-//   k_grad   stages the tile's face records (eq (15) prefactors, face centres, neighbour ids) and
-//            its cells' U in shared memory with coalesced loads; then one thread per (cell, group)
-//            sums the second term of eq (15) over the cell's faces, multiplies by the stored
-//            inverse matrix and runs the slope limiter
+//   k_grad   stages the tile's face records (eq (15) prefactors, face centres, neighbour ids), its
+//            cells' U and its face-list tables in shared memory with coalesced loads; then one
+//            thread per (cell, group) sums the second term of eq (15) over the cell's faces,
+//            multiplies by the stored inverse matrix and runs the slope limiter
+//
 //   k_stage  stages the tile's U and gradients in shared memory; one thread per face slot
 //            extrapolates both cells to the face centre, evaluates the M1 closure and the global
 //            Lax-Friedrichs flux with signal speed c~ and the donor cap for every group, and
@@ -11,14 +12,36 @@
 //            (cell, group) sums the cell's face list in fixed order, adds the source, does the Heun
 //            combine, the floor and |F| <= c~ N (S3, S11, S12).  The fluxes
 //            never go to HBM; a face shared by two tiles is evaluated by both.
+// fp64 throughout.  Reciprocals and the closure's square root use MUFU seeds + two Newton steps
+// (relative error ~1e-16, no special-case branches: all arguments are positive and normal).
 #include "rt_internal.cuh"
 #include "rt_kernels.cuh"
-
-typedef unsigned long long u64;
 
 __device__ __forceinline__ double4 ld4(const double *p) { return *reinterpret_cast<const double4 *>(p); }
 __device__ __forceinline__ void st4(double *p, double a, double b, double c, double d) {
   *reinterpret_cast<double4 *>(p) = make_double4(a, b, c, d);
+}
+__device__ __forceinline__ double dmax2(double a, double b) { return a > b ? a : b; }
+__device__ __forceinline__ double dmin2(double a, double b) { return a < b ? a : b; }
+
+// 1/x for positive normal x: MUFU.RCP64H seed, two Newton steps
+__device__ __forceinline__ double fast_rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  return fma(r, e, r);
+}
+// sqrt(x) for positive normal x: MUFU.RSQ64H seed, two coupled Newton steps (g -> sqrt x, h -> 1/(2 sqrt x))
+__device__ __forceinline__ double fast_sqrt(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double g = x * y, h = 0.5 * y;
+  double r = fma(-h, g, 0.5);
+  g = fma(g, r, g); h = fma(h, r, h);
+  r = fma(-h, g, 0.5);
+  return fma(g, r, g);
 }
 
 // neighbour or ghost state seen across a boundary face with right code `code` (S13)
@@ -48,13 +71,39 @@ __device__ __forceinline__ double block_sum(double v, double *red) {
   return t;
 }
 
+// per-tile face-list tables staged in shared memory: for local cell x, its owned slots are
+// so[x]..so[x+1], its r-list entries sr[ro_l[x]..ro_l[x+1]] (slot numbers)
+struct tile_tables { int *so, *rol; uint16_t *sr; };
+__device__ __forceinline__ tile_tables stage_tables(const rt_geom &m, unsigned char *base, int64_t c0, int ncell,
+                                                    int64_t fbase) {
+  tile_tables t;
+  t.so = reinterpret_cast<int *>(base);
+  t.rol = t.so + (m.TC + 1);
+  t.sr = reinterpret_cast<uint16_t *>(t.rol + (m.TC + 1));
+  const int64_t rbase = m.ro[c0];
+  for (int x = threadIdx.x; x <= ncell; x += blockDim.x) {
+    t.so[x] = (int)(m.fo[c0 + x] - fbase);
+    t.rol[x] = (int)(m.ro[c0 + x] - rbase);
+  }
+  const int nrt = (int)(m.ro[c0 + ncell] - rbase);
+  for (int k = threadIdx.x; k < nrt; k += blockDim.x) t.sr[k] = m.rslot[rbase + k];
+  return t;
+}
+
+// min-image of a face-centre offset: |d| < 1.5 L always (the face touches the cell)
+__device__ __forceinline__ double wrap1(double d, double L, int per) {
+  const double h = 0.5 * L;
+  const double w = d > h ? d - L : (d < -h ? d + L : d);
+  return per ? w : d;
+}
+
 // ------------------------------------------------------------------ a2: gradients + limiter
 template <int G>
 __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restrict__ U, double *__restrict__ grad) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double *sW = reinterpret_cast<double *>(smem_raw);  // [smax][4]  (w, L|R)
-  double *sC = sW + (size_t)4 * m.smax;               // [smax][4]  (c, A)
-  double *sU = sC + (size_t)4 * m.smax;               // [TC][G][4]
+  double *sC = sW + 4 * m.smax;                       // [smax][4]  (c, A)
+  double *sU = sC + 4 * m.smax;                       // [TC][G][4]
   const int64_t C = m.C;
   const int64_t c0 = (int64_t)blockIdx.x * m.TC;
   const int ncell = (int)(c0 + m.TC < C ? m.TC : C - c0);
@@ -62,16 +111,20 @@ __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restric
   const int nown = (int)(m.fo[c0 + ncell] - fbase);
   const int64_t ib = m.inco[blockIdx.x];
   const int ns = nown + (int)(m.inco[blockIdx.x + 1] - ib);
-  // stage the slot records and the tile's U
+  // stage the slot records, the tile's U and the face-list tables
   for (int s = threadIdx.x; s < ns; s += blockDim.x) {
     const int64_t q = s < nown ? fbase + s : (int64_t)m.incf[ib + (s - nown)];
     *reinterpret_cast<double4 *>(sW + 4 * s) = ld4(m.faceW + 4 * q);
     *reinterpret_cast<double4 *>(sC + 4 * s) = ld4(m.faceC + 4 * q);
   }
-  for (int x = threadIdx.x; x < ncell * G; x += blockDim.x)
-    *reinterpret_cast<double4 *>(sU + 4 * x) = ld4(U + 4 * (c0 * G + x));
+  {
+    const double *Ut = U + 4 * c0 * G;
+    for (int x = threadIdx.x; x < ncell * G; x += blockDim.x) *reinterpret_cast<double4 *>(sU + 4 * x) = ld4(Ut + 4 * x);
+  }
+  const tile_tables tt = stage_tables(m, reinterpret_cast<unsigned char *>(sU + 4 * m.TC * G), c0, ncell, fbase);
   __syncthreads();
 
+  const int32_t c0i = (int32_t)c0;
   for (int item = threadIdx.x; item < ncell * G; item += blockDim.x) {
     const int il = item / G, g = item - il * G;
     const int64_t i = c0 + il;
@@ -79,14 +132,14 @@ __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restric
     double b[4][3], hi[4] = {Ui.x, Ui.y, Ui.z, Ui.w}, lo[4] = {Ui.x, Ui.y, Ui.z, Ui.w};
 #pragma unroll
     for (int v = 0; v < 4; v++) b[v][0] = b[v][1] = b[v][2] = 0.0;
-    const int s0 = (int)(m.fo[i] - fbase), no = (int)(m.fo[i + 1] - m.fo[i]);
-    const int64_t r0 = m.ro[i];
-    const int nr = (int)(m.ro[i + 1] - r0);
-    const uint16_t *rs = m.rslot + r0;
+    const int s0 = tt.so[il], s1 = tt.so[il + 1];
+    const int r0 = tt.rol[il], r1 = tt.rol[il + 1];
+    const double *Ug = U + 4 * g;  // neighbour j outside the tile: Ug + 4 G j
 
     auto neighbour = [&](int32_t j) -> double4 {
-      const unsigned jl = (unsigned)(j - (int32_t)c0);
-      return jl < (unsigned)ncell ? ld4(sU + 4 * ((int)jl * G + g)) : ld4(U + 4 * ((int64_t)j * G + g));
+      const unsigned jl = (unsigned)(j - c0i);
+      const double *p = jl < (unsigned)ncell ? sU + 4 * ((int)jl * G + g) : Ug + (int64_t)(4 * G) * j;
+      return ld4(p);
     };
     auto accumulate = [&](const double4 Uj, double wx, double wy, double wz) {
       const double d0 = Uj.x - Ui.x, d1 = Uj.y - Ui.y, d2 = Uj.z - Ui.z, d3 = Uj.w - Ui.w;
@@ -94,22 +147,22 @@ __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restric
       b[1][0] += wx * d1; b[1][1] += wy * d1; b[1][2] += wz * d1;
       b[2][0] += wx * d2; b[2][1] += wy * d2; b[2][2] += wz * d2;
       b[3][0] += wx * d3; b[3][1] += wy * d3; b[3][2] += wz * d3;
-      hi[0] = fmax(hi[0], Uj.x); hi[1] = fmax(hi[1], Uj.y); hi[2] = fmax(hi[2], Uj.z); hi[3] = fmax(hi[3], Uj.w);
-      lo[0] = fmin(lo[0], Uj.x); lo[1] = fmin(lo[1], Uj.y); lo[2] = fmin(lo[2], Uj.z); lo[3] = fmin(lo[3], Uj.w);
+      hi[0] = dmax2(hi[0], Uj.x); hi[1] = dmax2(hi[1], Uj.y); hi[2] = dmax2(hi[2], Uj.z); hi[3] = dmax2(hi[3], Uj.w);
+      lo[0] = dmin2(lo[0], Uj.x); lo[1] = dmin2(lo[1], Uj.y); lo[2] = dmin2(lo[2], Uj.z); lo[3] = dmin2(lo[3], Uj.w);
     };
     // first pass: sum_f w_f (phi_j - phi_i), min/max.  Owned faces: the cell is the left one.
 #pragma unroll 2
-    for (int k = 0; k < no; k++) {
-      const double4 w = ld4(sW + 4 * (s0 + k));
+    for (int s = s0; s < s1; s++) {
+      const double4 w = ld4(sW + 4 * s);
       int32_t l, j;
       rt_unpack_lr(w.w, l, j);
-      const double4 Uj = j >= 0 ? neighbour(j) : ghost_for_gradient(j, Ui, m.faceN, fbase + s0 + k, m.ghost, G, g);
+      const double4 Uj = j >= 0 ? neighbour(j) : ghost_for_gradient(j, Ui, m.faceN, fbase + s, m.ghost, G, g);
       accumulate(Uj, w.x, w.y, w.z);
     }
     // faces where the cell is the right one: d = s_L - s_R, so the prefactor changes sign
 #pragma unroll 2
-    for (int k = 0; k < nr; k++) {
-      const double4 w = ld4(sW + 4 * (int)rs[k]);
+    for (int k = r0; k < r1; k++) {
+      const double4 w = ld4(sW + 4 * (int)tt.sr[k]);
       int32_t j, r;
       rt_unpack_lr(w.w, j, r);
       accumulate(neighbour(j), -w.x, -w.y, -w.z);
@@ -131,28 +184,28 @@ __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restric
 #pragma unroll
       for (int v = 0; v < 4; v++) {
         const double d = gr[v][0] * rx + gr[v][1] * ry + gr[v][2] * rz;
-        dmax[v] = fmax(dmax[v], d); dmin[v] = fmin(dmin[v], d);
+        dmax[v] = dmax2(dmax[v], d); dmin[v] = dmin2(dmin[v], d);
       }
     };
 #pragma unroll 2
-    for (int k = 0; k < no; k++) {
-      const double4 c = ld4(sC + 4 * (s0 + k));  // already in this cell's frame
+    for (int s = s0; s < s1; s++) {
+      const double4 c = ld4(sC + 4 * s);  // already in this cell's frame
       extremes(c.x - si.x, c.y - si.y, c.z - si.z);
     }
 #pragma unroll 2
-    for (int k = 0; k < nr; k++) {
-      const double4 c = ld4(sC + 4 * (int)rs[k]);
-      extremes(rt_wrap(c.x - si.x, m.box[0], m.per[0]), rt_wrap(c.y - si.y, m.box[1], m.per[1]),
-               rt_wrap(c.z - si.z, m.box[2], m.per[2]));
+    for (int k = r0; k < r1; k++) {
+      const double4 c = ld4(sC + 4 * (int)tt.sr[k]);
+      extremes(wrap1(c.x - si.x, m.box[0], m.per[0]), wrap1(c.y - si.y, m.box[1], m.per[1]),
+               wrap1(c.z - si.z, m.box[2], m.per[2]));
     }
-    double *out = grad + (size_t)12 * (i * G + g);
+    double *out = grad + 12 * (i * G + g);
     const double Uiv[4] = {Ui.x, Ui.y, Ui.z, Ui.w};
     double o[12];
 #pragma unroll
     for (int v = 0; v < 4; v++) {
       double a = 1.0;
-      if (dmax[v] > 0.0) a = fmin(a, (hi[v] - Uiv[v]) / dmax[v]);
-      if (dmin[v] < 0.0) a = fmin(a, (lo[v] - Uiv[v]) / dmin[v]);
+      if (dmax[v] > 0.0) a = dmin2(a, (hi[v] - Uiv[v]) / dmax[v]);
+      if (dmin[v] < 0.0) a = dmin2(a, (lo[v] - Uiv[v]) / dmin[v]);
       o[3 * v] = a * gr[v][0]; o[3 * v + 1] = a * gr[v][1]; o[3 * v + 2] = a * gr[v][2];
     }
     st4(out, o[0], o[1], o[2], o[3]); st4(out + 4, o[4], o[5], o[6], o[7]); st4(out + 8, o[8], o[9], o[10], o[11]);
@@ -160,15 +213,19 @@ __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restric
 }
 
 // ------------------------------------------------------------------ a3 + a4: fluxes and update
-// N D.n for the M1 closure (S1), lab frame: D = (1-chi)/2 I + (3 chi - 1)/2 nF nF^T
+// N D.n for the M1 closure (S1), lab frame, D = (1-chi)/2 I + (3 chi - 1)/2 nF nF^T with
+// chi = (3+4f^2)/(5+2s), s = sqrt(4-3f^2), f = min(1, |F|/(c~ N)).  Written with one square root and
+// two reciprocals: with m = max(|F|^2, (c~N)^2), f^2 = |F|^2/m, and since
+// 3 chi - 1 = 6 f^2/(2+s):  (1-chi)/2 = 1/3 - f^2/(2+s),  (3chi-1)/2 N /|F|^2 = 3 N/((2+s) m).
 __device__ __forceinline__ void pressure_dot_n(const double U[4], const double n[3], double ct, double out[3]) {
   const double f2n = U[1] * U[1] + U[2] * U[2] + U[3] * U[3];
-  const double fn = sqrt(f2n);
-  const double f = fmin(1.0, fn / fmax(ct * U[0], 1e-300));
-  const double chi = (3.0 + 4.0 * f * f) / (5.0 + 2.0 * sqrt(4.0 - 3.0 * f * f));
-  const double a = 0.5 * (1.0 - chi) * U[0];
-  double bb = 0.0;
-  if (f2n > 0.0) bb = 0.5 * (3.0 * chi - 1.0) * U[0] * (U[1] * n[0] + U[2] * n[1] + U[3] * n[2]) / f2n;
+  const double cN = ct * U[0];
+  const double mm = dmax2(dmax2(f2n, cN * cN), 1e-290);
+  const double rm = fast_rcp(mm);
+  const double f2 = f2n * rm;
+  const double r2 = fast_rcp(2.0 + fast_sqrt(fma(-3.0, f2, 4.0)));
+  const double a = fma(-f2, r2, 1.0 / 3.0) * U[0];
+  const double bb = 3.0 * U[0] * (U[1] * n[0] + U[2] * n[1] + U[3] * n[2]) * (rm * r2);
   out[0] = a * n[0] + bb * U[1]; out[1] = a * n[1] + bb * U[2]; out[2] = a * n[2] + bb * U[3];
 }
 
@@ -197,9 +254,9 @@ __global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restri
                                                double *__restrict__ part_out, double *__restrict__ part_in) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ double red[32];
-  double *sPhi = reinterpret_cast<double *>(smem_raw);       // [G][smax][4]  A * (Phi_N, Phi_F)
-  double *sR = sPhi + (size_t)4 * G * m.smax;                // [TC][G][RT_REC]  U (4) + gradients (12)
-  double *sS = sR + (size_t)RT_REC * G * m.TC;               // [TC][4]  (s, V)
+  double *sPhi = reinterpret_cast<double *>(smem_raw);  // [G][smax][4]  A * (Phi_N, Phi_F)
+  double *sR = sPhi + 4 * G * m.smax;                   // [TC][G][RT_REC]  U (4) + gradients (12)
+  double *sS = sR + RT_REC * G * m.TC;                  // [TC][4]  (s, V)
   const int64_t C = m.C;
   const int64_t c0 = (int64_t)blockIdx.x * m.TC;
   const int ncell = (int)(c0 + m.TC < C ? m.TC : C - c0);
@@ -208,15 +265,19 @@ __global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restri
   const int64_t ib = m.inco[blockIdx.x];
   const int ns = nown + (int)(m.inco[blockIdx.x + 1] - ib);
   const int smax = m.smax;
-  // stage the tile's cells
-  for (int x = threadIdx.x; x < ncell * G; x += blockDim.x)
-    *reinterpret_cast<double4 *>(sR + RT_REC * x) = ld4(Uin + 4 * (c0 * G + x));
-  if (SECOND)
-    for (int u = threadIdx.x; u < ncell * G * 3; u += blockDim.x) {
-      const int x = u / 3, part = u - 3 * x;
-      *reinterpret_cast<double4 *>(sR + RT_REC * x + 4 + 4 * part) = ld4(grad + 4 * (3 * c0 * G + u));
-    }
-  for (int x = threadIdx.x; x < ncell; x += blockDim.x) *reinterpret_cast<double4 *>(sS + 4 * x) = ld4(m.cellS + 4 * (c0 + x));
+  // stage the tile's cells and face-list tables
+  {
+    const double *Ut = Uin + 4 * c0 * G, *gt = grad + 12 * c0 * G;
+    for (int x = threadIdx.x; x < ncell * G; x += blockDim.x) *reinterpret_cast<double4 *>(sR + RT_REC * x) = ld4(Ut + 4 * x);
+    if (SECOND)
+      for (int u = threadIdx.x; u < ncell * G * 3; u += blockDim.x) {
+        const int x = u / 3, part = u - 3 * x;
+        *reinterpret_cast<double4 *>(sR + RT_REC * x + 4 + 4 * part) = ld4(gt + 4 * u);
+      }
+    const double *St = m.cellS + 4 * c0;
+    for (int x = threadIdx.x; x < ncell; x += blockDim.x) *reinterpret_cast<double4 *>(sS + 4 * x) = ld4(St + 4 * x);
+  }
+  const tile_tables tt = stage_tables(m, reinterpret_cast<unsigned char *>(sS + 4 * m.TC), c0, ncell, fbase);
   __syncthreads();
 
   // ---- a3: one thread per face slot, all groups
@@ -225,6 +286,7 @@ __global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restri
   for (int g = 0; g < G; g++) b_out[g] = b_in[g] = 0.0;
   int bnd = 0;
   const double hc2 = 0.5 * ct * ct, hc = 0.5 * ct;
+  const int32_t c0i = (int32_t)c0;
   for (int s = threadIdx.x; s < ns; s += blockDim.x) {
     const int64_t q = s < nown ? fbase + s : (int64_t)m.incf[ib + (s - nown)];
     const double4 fc = ld4(m.faceC + 4 * q), fn = ld4(m.faceN + 4 * q);
@@ -232,27 +294,33 @@ __global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restri
     rt_unpack_lr(fn.w, l, r);
     const double n[3] = {fn.x, fn.y, fn.z};
     const double A = fc.w;
-    const unsigned ll = (unsigned)(l - (int32_t)c0), rl = (unsigned)(r - (int32_t)c0);
-    const bool l_in = ll < (unsigned)ncell, r_in = r >= 0 && rl < (unsigned)ncell;
-    const double4 sl = l_in ? ld4(sS + 4 * ll) : ld4(m.cellS + 4 * (int64_t)l);
+    const unsigned ll = (unsigned)(l - c0i), rl = (unsigned)(r - c0i);
+    const bool l_in = ll < (unsigned)ncell, r_in = rl < (unsigned)ncell;  // r < 0 gives a huge rl
+    // per-group rows of the two cells: shared memory for tile cells, global memory for the halo
+    const double *puL = l_in ? sR + RT_REC * G * (int)ll : Uin + (int64_t)(4 * G) * l;
+    const double *pgL = l_in ? puL + 4 : grad + (int64_t)(12 * G) * l;
+    const int suL = l_in ? RT_REC : 4, sgL = l_in ? RT_REC : 12;
+    const double4 sl = ld4(l_in ? sS + 4 * (int)ll : m.cellS + 4 * (int64_t)l);
     const double rLx = fc.x - sl.x, rLy = fc.y - sl.y, rLz = fc.z - sl.z;
+    const int rr = r >= 0 ? r : 0;
+    const double *puR = r_in ? sR + RT_REC * G * (int)rl : Uin + (int64_t)(4 * G) * rr;
+    const double *pgR = r_in ? puR + 4 : grad + (int64_t)(12 * G) * rr;
+    const int suR = r_in ? RT_REC : 4, sgR = r_in ? RT_REC : 12;
     double rRx = 0.0, rRy = 0.0, rRz = 0.0, Vr = 0.0;
     if (r >= 0) {
-      const double4 sr = r_in ? ld4(sS + 4 * rl) : ld4(m.cellS + 4 * (int64_t)r);
+      const double4 sr = ld4(r_in ? sS + 4 * (int)rl : m.cellS + 4 * (int64_t)r);
       Vr = sr.w;
-      rRx = rt_wrap(fc.x - sr.x, m.box[0], m.per[0]); rRy = rt_wrap(fc.y - sr.y, m.box[1], m.per[1]);
-      rRz = rt_wrap(fc.z - sr.z, m.box[2], m.per[2]);
+      rRx = wrap1(fc.x - sr.x, m.box[0], m.per[0]); rRy = wrap1(fc.y - sr.y, m.box[1], m.per[1]);
+      rRz = wrap1(fc.z - sr.z, m.box[2], m.per[2]);
     }
-    const double capL = sl.w / (dt * A), capR = Vr / (dt * A);
+    const double rdtA = fast_rcp(dt * A);
+    const double capL = sl.w * rdtA, capR = Vr * rdtA;
 #pragma unroll
     for (int g = 0; g < G; g++) {
       double UL[4], UR[4], NL, NR = 0.0;
-      if (l_in) { const double *p = sR + RT_REC * ((int)ll * G + g); extrapolate<SECOND>(p, p + 4, rLx, rLy, rLz, UL, NL); }
-      else { const int64_t x = (int64_t)l * G + g; extrapolate<SECOND>(Uin + 4 * x, grad + 12 * x, rLx, rLy, rLz, UL, NL); }
-      if (r >= 0) {
-        if (r_in) { const double *p = sR + RT_REC * ((int)rl * G + g); extrapolate<SECOND>(p, p + 4, rRx, rRy, rRz, UR, NR); }
-        else { const int64_t x = (int64_t)r * G + g; extrapolate<SECOND>(Uin + 4 * x, grad + 12 * x, rRx, rRy, rRz, UR, NR); }
-      } else if (r == RT_BC_OUTFLOW) { UR[0] = UR[1] = UR[2] = UR[3] = 0.0; }  // vacuum ghost
+      extrapolate<SECOND>(puL + suL * g, pgL + sgL * g, rLx, rLy, rLz, UL, NL);
+      if (r >= 0) extrapolate<SECOND>(puR + suR * g, pgR + sgR * g, rRx, rRy, rRz, UR, NR);
+      else if (r == RT_BC_OUTFLOW) { UR[0] = UR[1] = UR[2] = UR[3] = 0.0; }  // vacuum ghost
       else if (r == RT_BC_REFLECT) {
         const double p = 2.0 * (UL[1] * n[0] + UL[2] * n[1] + UL[3] * n[2]);
         UR[0] = UL[0]; UR[1] = UL[1] - p * n[0]; UR[2] = UL[2] - p * n[1]; UR[3] = UL[3] - p * n[2];
@@ -268,14 +336,9 @@ __global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restri
       for (int a = 0; a < 3; a++) ph[1 + a] = hc2 * (PL[a] + PR[a]) - hc * (UR[1 + a] - UL[1 + a]);
       // donor cap (S11): the donor cannot lose more photons than it holds through this face in dt;
       // only the number flux is clamped (continuous in the state; Phi_F is left alone)
-      if (ph[0] > 0.0) {
-        const double lim = NL * capL;
-        if (ph[0] > lim) ph[0] = lim;
-      } else if (ph[0] < 0.0 && r >= 0) {
-        const double lim = NR * capR;
-        if (-ph[0] > lim) ph[0] = -lim;
-      }
-      st4(sPhi + 4 * ((size_t)g * smax + s), A * ph[0], A * ph[1], A * ph[2], A * ph[3]);
+      if (ph[0] > 0.0) ph[0] = dmin2(ph[0], NL * capL);
+      else if (r >= 0) ph[0] = -dmin2(-ph[0], NR * capR);
+      st4(sPhi + 4 * (g * smax + s), A * ph[0], A * ph[1], A * ph[2], A * ph[3]);
       if (r == RT_BC_OUTFLOW) { b_out[g] += A * ph[0]; bnd = 1; }
       else if (r <= RT_BC_DIRICHLET0) { b_in[g] -= A * ph[0]; bnd = 1; }
     }
@@ -300,38 +363,36 @@ __global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restri
   for (int item = threadIdx.x; item < ncell * G; item += blockDim.x) {
     const int il = item / G, g = item - il * G;
     const int64_t i = c0 + il;
-    const int s0 = (int)(m.fo[i] - fbase), no = (int)(m.fo[i + 1] - m.fo[i]);
-    const int64_t r0 = m.ro[i];
-    const int nr = (int)(m.ro[i + 1] - r0);
-    const uint16_t *rs = m.rslot + r0;
-    const double *pg = sPhi + 4 * (size_t)g * smax;
+    const int s0 = tt.so[il], s1 = tt.so[il + 1];
+    const int r0 = tt.rol[il], r1 = tt.rol[il + 1];
+    const double *pg = sPhi + 4 * g * smax;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
 #pragma unroll 4
-    for (int k = 0; k < no; k++) {
-      const double4 p = ld4(pg + 4 * (s0 + k));
+    for (int s = s0; s < s1; s++) {
+      const double4 p = ld4(pg + 4 * s);
       a0 += p.x; a1 += p.y; a2 += p.z; a3 += p.w;
     }
 #pragma unroll 4
-    for (int k = 0; k < nr; k++) {
-      const double4 p = ld4(pg + 4 * (int)rs[k]);
+    for (int k = r0; k < r1; k++) {
+      const double4 p = ld4(pg + 4 * (int)tt.sr[k]);
       a0 -= p.x; a1 -= p.y; a2 -= p.z; a3 -= p.w;
     }
     const double V = sS[4 * il + 3];
-    double R[4] = {-a0 / V, -a1 / V, -a2 / V, -a3 / V};
+    const double kk = dt * fast_rcp(V);  // dt / V
     const int32_t si = srcidx[i];
-    if (si >= 0) R[0] += srcrate[(size_t)g * nsrc + si] / V;  // isotropic source (S5)
-    const size_t o = 4 * ((size_t)i * G + g);
+    if (si >= 0) a0 -= srcrate[(size_t)g * nsrc + si];  // isotropic source (S5): + dt Ndot / V on N
+    const int64_t o = 4 * (i * G + g);
     const double4 uc = ld4(sR + RT_REC * item), u0 = ld4(U0 + o);
-    double Un[4] = {ca * u0.x + cb * (uc.x + dt * R[0]), ca * u0.y + cb * (uc.y + dt * R[1]),
-                    ca * u0.z + cb * (uc.z + dt * R[2]), ca * u0.w + cb * (uc.w + dt * R[3])};
+    double Un[4] = {ca * u0.x + cb * fma(-kk, a0, uc.x), ca * u0.y + cb * fma(-kk, a1, uc.y),
+                    ca * u0.z + cb * fma(-kk, a2, uc.z), ca * u0.w + cb * fma(-kk, a3, uc.w)};
     if (Un[0] < n_floor) {
       const double add = V * (n_floor - Un[0]);
 #pragma unroll
       for (int gg = 0; gg < G; gg++) if (gg == g) fl[gg] += add;
       Un[0] = n_floor; floored = 1;
     }
-    const double fnorm = sqrt(Un[1] * Un[1] + Un[2] * Un[2] + Un[3] * Un[3]), lim = ct * Un[0];
-    if (fnorm > lim) { const double sc = lim / fnorm; Un[1] *= sc; Un[2] *= sc; Un[3] *= sc; }
+    const double f2 = Un[1] * Un[1] + Un[2] * Un[2] + Un[3] * Un[3], lim = ct * Un[0];
+    if (f2 > lim * lim) { const double sc = lim / sqrt(f2); Un[1] *= sc; Un[2] *= sc; Un[3] *= sc; }
     st4(Uout + o, Un[0], Un[1], Un[2], Un[3]);
   }
   if (__syncthreads_or(floored)) {
@@ -455,7 +516,7 @@ static cudaError_t allow_smem(K kernel, size_t bytes) {
 
 int rt_transport_configure(rt_ctx *c) {
   cudaError_t e = cudaSuccess;
-  const size_t sg = rt_smem_grad(c->TC, c->G, c->smax), ss = rt_smem_stage(c->TC, c->G, c->smax);
+  const size_t sg = rt_smem_grad(c->TC, c->G, c->smax, c->rmax), ss = rt_smem_stage(c->TC, c->G, c->smax, c->rmax);
   SET_SMEM_G(c->G, K_GRAD, sg, e);
   if (e == cudaSuccess) SET_SMEM_G(c->G, K_STAGE2, ss, e);
   if (e == cudaSuccess) SET_SMEM_G(c->G, K_STAGE1, ss, e);
@@ -483,7 +544,7 @@ rt_geom rt_geom_of(const rt_ctx *c) {
 }
 
 int rt_launch_gradients(rt_ctx *c, const double *U) {
-  DISPATCH_G(c->G, K_GRAD, (unsigned)c->T, tile_threads(c), rt_smem_grad(c->TC, c->G, c->smax), c->stream, rt_geom_of(c), U,
+  DISPATCH_G(c->G, K_GRAD, (unsigned)c->T, tile_threads(c), rt_smem_grad(c->TC, c->G, c->smax, c->rmax), c->stream, rt_geom_of(c), U,
              rt_ptr<double>(c, c->lay.grad));
   c->launches++;
   return RT_OK;
@@ -507,10 +568,10 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
   const int64_t nchem = blocks_for(c->C, RT_CHEM_BLOCK);
   double *p_floor = part + (size_t)G * nchem, *p_out = p_floor + (size_t)G * c->T, *p_in = p_out + (size_t)G * c->T;
   const int nt = tile_threads(c);
-  const size_t ss = rt_smem_stage(c->TC, G, c->smax);
+  const size_t ss = rt_smem_stage(c->TC, G, c->smax, c->rmax);
   if (c->par.order >= 2) {
     rt_prof_begin(c, RT_K_GRAD);
-    DISPATCH_G(G, K_GRAD, (unsigned)c->T, nt, rt_smem_grad(c->TC, G, c->smax), c->stream, m, Uin, grad);
+    DISPATCH_G(G, K_GRAD, (unsigned)c->T, nt, rt_smem_grad(c->TC, G, c->smax, c->rmax), c->stream, m, Uin, grad);
     rt_prof_end(c);
     c->launches++;
     rt_prof_begin(c, RT_K_UPDATE);

@@ -72,6 +72,8 @@ def lib():
         L.rt_download.argtypes = [_vp, ctypes.POINTER(rt_state), ctypes.POINTER(rt_ledger)]
         L.rt_kernel_launches.restype = ctypes.c_int64
         L.rt_kernel_launches.argtypes = [_vp]
+        L.rt_tile_info.restype = ctypes.c_int
+        L.rt_tile_info.argtypes = [_vp, _vp]
         L.rt_debug_gradients.restype = ctypes.c_int
         L.rt_debug_gradients.argtypes = [_vp, ctypes.c_int, _vp, _vp]
         L.rt_profile.restype = ctypes.c_int
@@ -292,6 +294,11 @@ class Solver:
         _check(self.h, lib().rt_profile_read(self.h, _vp(ms.ctypes.data), _vp(cnt.ctypes.data)), "rt_profile_read")
         names = ("chem", "grad", "flux", "update", "reduce", "other")
         return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(names)}
+
+    def tile_info(self):
+        out = np.zeros(4, dtype=np.int64)
+        _check(self.h, lib().rt_tile_info(self.h, _vp(out.ctypes.data)), "rt_tile_info")
+        return {"cells_per_tile": int(out[0]), "tiles": int(out[1]), "max_slots": int(out[2]), "refaces": int(out[3])}
 
     def launches(self):
         return int(lib().rt_kernel_launches(self.h))

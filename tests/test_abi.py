@@ -1,0 +1,49 @@
+"""The C-ABI library loads without a GPU and exports every symbol include/rt.h declares; the host-side
+argument checks that need no device answer with error codes, not exceptions.  CPU only."""
+import ctypes
+import os
+import re
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "rt.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(rt_[a-z_]+)\s*\(", src)))
+
+
+def test_header_declares_the_north_star_calls():
+    names = declared_functions()
+    for n in ("rt_create", "rt_workspace_bytes", "rt_mesh_upload", "rt_state_init", "rt_step", "rt_download",
+              "rt_last_error", "rt_destroy"):
+        assert n in names
+
+
+def test_library_exports_every_declared_symbol():
+    from paper_2404_17630_b200.build import build_rt
+    L = ctypes.CDLL(build_rt())
+    for n in declared_functions():
+        assert hasattr(L, n), n
+
+
+def test_binding_has_the_same_names():
+    from paper_2404_17630_b200 import rt
+    for n in ("rt_create", "rt_workspace_bytes", "rt_mesh_upload", "rt_state_init", "rt_step", "rt_download",
+              "rt_last_error", "rt_destroy"):
+        assert callable(getattr(rt, n))
+
+
+def test_workspace_bytes_and_null_arguments_need_no_device():
+    from paper_2404_17630_b200 import rt
+    L = rt.lib()
+    assert rt.rt_workspace_bytes(0, 10, 1) == 0
+    assert rt.rt_workspace_bytes(10, 10, 9) == 0
+    small, big = rt.rt_workspace_bytes(10 ** 6, 3 * 10 ** 6, 1), rt.rt_workspace_bytes(10 ** 6, 3 * 10 ** 6, 8)
+    assert 0 < small < big
+    # config 4 (384^3 cells, 7.72 faces per cell, 3 groups) must fit the 180 GB of one B200
+    assert rt.rt_workspace_bytes(384 ** 3, int(7.72 * 384 ** 3), 3) < 150e9
+    assert L.rt_step(None, 1.0, 1) == -1          # RT_EINVAL, no abort
+    assert L.rt_download(None, None, None) == -1
+    assert L.rt_last_error(None) == b"null context"
+    L.rt_destroy(None)

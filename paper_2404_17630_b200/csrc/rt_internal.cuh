@@ -14,7 +14,8 @@
 //   tiles: TC consecutive cells (a compact blob of the Hilbert curve) are one thread block's
 //     work.  A tile's "slots" are its owned faces (slot s = face - fo[c0]) followed by its
 //     incoming faces (right cell in the tile, owner in an earlier tile), listed in
-//     incf[inco[t]..inco[t+1]].  rslot[k] is the slot of r-list entry k inside its cell's tile,
+//     incf[inco[t]..inco[t+1]].  hl[fo[i]+ro[i] ..] is cell i's half-face list: the slot of each of
+//     its faces inside its tile (owned faces first; bit 15 set where the cell is the right one),
 //     so a cell finds every one of its faces in the tile's shared-memory slot arrays.
 //   state, cell-major so that a tile is one contiguous run:
 //     Ua, Ub [C][G][4] = (N, Fx, Fy, Fz); grad [C][G][12] (field-major, then direction);
@@ -39,7 +40,7 @@ struct rt_dev_ledger {  // accumulators on the device (value + compensation)
 };
 
 struct rt_layout {
-  size_t perm, iperm, cellS, Minv, faceC, faceN, faceW, L, R, fo, ro, rl, rn, rslot, incf, inco, ghost, led;
+  size_t perm, iperm, cellS, Minv, faceC, faceN, faceW, L, R, fo, ro, rl, rn, hl, incf, inco, ghost, led;
   size_t Ua, Ub, grad, xHII, xHeII, xHeIII, eth, nH, kappa, srcidx, srcrate, part, scratch_end;
   size_t temp;        // start of the setup-time scratch (aliases the state region)
   size_t total;
@@ -56,7 +57,7 @@ struct rt_ctx {
   int TC;             // cells per tile
   int64_t T;          // number of tiles
   int smax;           // largest slot count of any tile
-  int rmax;           // largest r-list entry count of any tile
+  int hmax;           // largest half-face count of any tile
   int64_t ninc;       // total incoming faces over all tiles
   double box[3];
   int per[3];
@@ -84,13 +85,14 @@ void rt_prof_end(rt_ctx *c);
 
 // dynamic shared memory of the two tile kernels (rt_transport.cu) for a tile of TC cells whose
 // slot count is at most smax
-// (rmax: most r-list entries of any tile; the face-list tables are two int[TC+1] and uint16[rmax])
-static inline size_t rt_smem_tables(int TC, int rmax) { return ((size_t)8 * (TC + 1) + (size_t)2 * rmax + 15) & ~(size_t)15; }
-static inline size_t rt_smem_grad(int TC, int G, int smax, int rmax) {
-  return (size_t)64 * smax + (size_t)32 * TC * G + rt_smem_tables(TC, rmax);
+// (hmax: most half-faces of any tile; the face-list tables are int[TC+1] and uint16[hmax])
+static inline size_t rt_smem_tables(int TC, int hmax) { return ((size_t)4 * (TC + 1) + (size_t)2 * hmax + 15) & ~(size_t)15; }
+static inline size_t rt_smem_grad(int TC, int G, int smax, int hmax) {
+  return (size_t)64 * smax + (size_t)32 * TC * G + rt_smem_tables(TC, hmax);
 }
-static inline size_t rt_smem_stage(int TC, int G, int smax, int rmax) {
-  return (size_t)32 * G * smax + (size_t)RT_REC * 8 * TC * G + (size_t)32 * TC + rt_smem_tables(TC, rmax);
+static inline size_t rt_smem_stage(int TC, int G, int smax, int hmax) {
+  const int per_slot = 32 * G > 64 ? 32 * G : 64;  // A*Phi of every group, or the staged face record before it
+  return (size_t)per_slot * smax + (size_t)RT_REC * 8 * TC * G + (size_t)32 * TC + rt_smem_tables(TC, hmax);
 }
 #define RT_SMEM_MAX 232448     // 227 KB: the most one block may have on sm_100
 #define RT_SMEM_TARGET 110000  // two blocks per SM

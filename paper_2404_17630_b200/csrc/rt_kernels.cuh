@@ -15,7 +15,7 @@ struct rt_geom {
   const double *cellS, *Minv, *faceC, *faceN, *faceW;
   const int64_t *fo, *ro, *inco;
   const int32_t *incf;
-  const uint16_t *rslot;
+  const uint16_t *hl;
   const double *ghost;
   double box[3];
   int per[3];

@@ -231,22 +231,26 @@ __global__ void k_tile_scan(int64_t C, int TC, int64_t T, const int64_t *fo, con
   tileInc[t] = run;
   const int64_t slots = fo[c1] - fo[c0] + run;
   atomicMax(maxSlots, slots > 0x7fffffff ? 0x7fffffff : (int)slots);
-  const int64_t nrt = ro[c1] - ro[c0];
-  atomicMax(maxSlots + 1, nrt > 0x7fffffff ? 0x7fffffff : (int)nrt);
+  const int64_t nh = fo[c1] - fo[c0] + ro[c1] - ro[c0];
+  atomicMax(maxSlots + 1, nh > 0x7fffffff ? 0x7fffffff : (int)nh);
 }
 __global__ void k_tile_fill(int64_t C, int TC, const int64_t *fo, const int64_t *ro, const int32_t *rl, const int32_t *rn,
-                            const int32_t *cellInc, const int64_t *inco, int32_t *incf, uint16_t *rslot) {
+                            const int32_t *cellInc, const int64_t *inco, int32_t *incf, uint16_t *hl) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= C) return;
   const int64_t t = i / TC, c0 = t * TC, c1 = c0 + TC < C ? c0 + TC : C;
   const int64_t fbase = fo[c0], nown = fo[c1] - fbase;
+  uint16_t *h = hl + fo[i] + ro[i];  // the cell's half-face list: owned slots, then r-list slots with bit 15 set
+  for (int64_t q = fo[i]; q < fo[i + 1]; q++) *h++ = (uint16_t)(q - fbase);
   int j = cellInc[i];
   for (int64_t k = ro[i]; k < ro[i + 1]; k++) {
+    int slot;
     if (rn[k] < c0) {
       incf[inco[t] + j] = rl[k];
-      rslot[k] = (uint16_t)(nown + j);
+      slot = (int)(nown + j);
       j++;
-    } else rslot[k] = (uint16_t)(rl[k] - fbase);
+    } else slot = (int)(rl[k] - fbase);
+    *h++ = (uint16_t)(slot | 0x8000);
   }
 }
 
@@ -371,9 +375,9 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
         int mx[2] = {0, 0};
         RT_CUDA(c, cudaMemcpyAsync(mx, maxSlots, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
         RT_CUDA(c, cudaStreamSynchronize(st));
-        const int smax = mx[0], rmax = mx[1];
-        if (smax < 65536 && rt_smem_stage(TC, c->G, smax, rmax) <= limit && rt_smem_grad(TC, c->G, smax, rmax) <= limit) {
-          best = TC; best_smax = smax; c->rmax = rmax;
+        const int smax = mx[0], hmax = mx[1];
+        if (smax < 32768 && rt_smem_stage(TC, c->G, smax, hmax) <= limit && rt_smem_grad(TC, c->G, smax, hmax) <= limit) {
+          best = TC; best_smax = smax; c->hmax = hmax;
           break;
         }
       }
@@ -385,7 +389,7 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
     RT_CUDA(c, cudaMemsetAsync(tileInc + c->T, 0, 8, st));
     RT_CUDA(c, cub::DeviceScan::ExclusiveSum(cub_tmp, b, tileInc, inco, c->T + 1, st));
     k_tile_fill<<<nblk(C), SETUP_BLOCK, 0, st>>>(C, best, fo, ro, rl, rn, cellInc, inco, rt_ptr<int32_t>(c, lay.incf),
-                                                 rt_ptr<uint16_t>(c, lay.rslot));
+                                                 rt_ptr<uint16_t>(c, lay.hl));
     RT_CUDA(c, cudaMemcpyAsync(&c->ninc, inco + c->T, 8, cudaMemcpyDeviceToHost, st));
   }
   if (m->nghost > 0)
@@ -411,7 +415,7 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G) {
   l.faceC = take(32 * F); l.faceN = take(32 * F); l.faceW = take(32 * F);
   l.L = take(4 * F); l.R = take(4 * F);
   l.fo = take(8 * (C + 1)); l.ro = take(8 * (C + 1)); l.rl = take(4 * F); l.rn = take(4 * F);
-  l.rslot = take(2 * F); l.incf = take(4 * F); l.inco = take(8 * (l.max_tiles + 2));
+  l.hl = take(4 * F); l.incf = take(4 * F); l.inco = take(8 * (l.max_tiles + 2));
   l.ghost = take(8 * 4 * RT_MAXG * 64);
   l.led = take(sizeof(rt_dev_ledger));
   l.temp = o;

@@ -14,6 +14,7 @@
 //            never go to HBM; a face shared by two tiles is evaluated by both.
 // fp64 throughout.  Reciprocals and the closure's square root use MUFU seeds + two Newton steps
 // (relative error ~1e-16, no special-case branches: all arguments are positive and normal).
+#include <stdlib.h>
 #include "rt_internal.cuh"
 #include "rt_kernels.cuh"
 
@@ -71,22 +72,18 @@ __device__ __forceinline__ double block_sum(double v, double *red) {
   return t;
 }
 
-// per-tile face-list tables staged in shared memory: for local cell x, its owned slots are
-// so[x]..so[x+1], its r-list entries sr[ro_l[x]..ro_l[x+1]] (slot numbers)
-struct tile_tables { int *so, *rol; uint16_t *sr; };
-__device__ __forceinline__ tile_tables stage_tables(const rt_geom &m, unsigned char *base, int64_t c0, int ncell,
-                                                    int64_t fbase) {
+// per-tile face-list tables staged in shared memory: local cell x has the half-faces
+// hl[ho[x]..ho[x+1]]: slot number, bit 15 set where the cell is the face's right cell
+struct tile_tables { int *ho; uint16_t *hl; };
+__device__ __forceinline__ tile_tables stage_tables(const rt_geom &m, unsigned char *base, int64_t c0, int ncell) {
   tile_tables t;
-  t.so = reinterpret_cast<int *>(base);
-  t.rol = t.so + (m.TC + 1);
-  t.sr = reinterpret_cast<uint16_t *>(t.rol + (m.TC + 1));
-  const int64_t rbase = m.ro[c0];
-  for (int x = threadIdx.x; x <= ncell; x += blockDim.x) {
-    t.so[x] = (int)(m.fo[c0 + x] - fbase);
-    t.rol[x] = (int)(m.ro[c0 + x] - rbase);
-  }
-  const int nrt = (int)(m.ro[c0 + ncell] - rbase);
-  for (int k = threadIdx.x; k < nrt; k += blockDim.x) t.sr[k] = m.rslot[rbase + k];
+  t.ho = reinterpret_cast<int *>(base);
+  t.hl = reinterpret_cast<uint16_t *>(t.ho + (m.TC + 1));
+  const int64_t hbase = m.fo[c0] + m.ro[c0];
+  for (int x = threadIdx.x; x <= ncell; x += blockDim.x) t.ho[x] = (int)(m.fo[c0 + x] + m.ro[c0 + x] - hbase);
+  const int nh = (int)(m.fo[c0 + ncell] + m.ro[c0 + ncell] - hbase);
+  const uint16_t *src = m.hl + hbase;
+  for (int k = threadIdx.x; k < nh; k += blockDim.x) t.hl[k] = src[k];
   return t;
 }
 
@@ -121,7 +118,7 @@ __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restric
     const double *Ut = U + 4 * c0 * G;
     for (int x = threadIdx.x; x < ncell * G; x += blockDim.x) *reinterpret_cast<double4 *>(sU + 4 * x) = ld4(Ut + 4 * x);
   }
-  const tile_tables tt = stage_tables(m, reinterpret_cast<unsigned char *>(sU + 4 * m.TC * G), c0, ncell, fbase);
+  const tile_tables tt = stage_tables(m, reinterpret_cast<unsigned char *>(sU + 4 * m.TC * G), c0, ncell);
   __syncthreads();
 
   const int32_t c0i = (int32_t)c0;
@@ -132,16 +129,27 @@ __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restric
     double b[4][3], hi[4] = {Ui.x, Ui.y, Ui.z, Ui.w}, lo[4] = {Ui.x, Ui.y, Ui.z, Ui.w};
 #pragma unroll
     for (int v = 0; v < 4; v++) b[v][0] = b[v][1] = b[v][2] = 0.0;
-    const int s0 = tt.so[il], s1 = tt.so[il + 1];
-    const int r0 = tt.rol[il], r1 = tt.rol[il + 1];
+    const int h0 = tt.ho[il], h1 = tt.ho[il + 1];
     const double *Ug = U + 4 * g;  // neighbour j outside the tile: Ug + 4 G j
 
-    auto neighbour = [&](int32_t j) -> double4 {
-      const unsigned jl = (unsigned)(j - c0i);
-      const double *p = jl < (unsigned)ncell ? sU + 4 * ((int)jl * G + g) : Ug + (int64_t)(4 * G) * j;
-      return ld4(p);
-    };
-    auto accumulate = [&](const double4 Uj, double wx, double wy, double wz) {
+    // first pass over the cell's half-faces: sum_f w_f (phi_j - phi_i), min/max.  Where the cell is
+    // the face's right cell, d = s_L - s_R: the stored prefactor changes sign, the neighbour is L.
+#pragma unroll 2
+    for (int k = h0; k < h1; k++) {
+      const unsigned e = tt.hl[k];
+      const int s = (int)(e & 0x7fffu);
+      const bool right = e >= 0x8000u;
+      const double4 w = ld4(sW + 4 * s);
+      int32_t l, r;
+      rt_unpack_lr(w.w, l, r);
+      const int32_t j = right ? l : r;
+      const double sg = right ? -1.0 : 1.0;
+      double4 Uj;
+      if (j >= 0) {
+        const unsigned jl = (unsigned)(j - c0i);
+        Uj = ld4(jl < (unsigned)ncell ? sU + 4 * ((int)jl * G + g) : Ug + (int64_t)(4 * G) * j);
+      } else Uj = ghost_for_gradient(j, Ui, m.faceN, fbase + s, m.ghost, G, g);
+      const double wx = sg * w.x, wy = sg * w.y, wz = sg * w.z;
       const double d0 = Uj.x - Ui.x, d1 = Uj.y - Ui.y, d2 = Uj.z - Ui.z, d3 = Uj.w - Ui.w;
       b[0][0] += wx * d0; b[0][1] += wy * d0; b[0][2] += wz * d0;
       b[1][0] += wx * d1; b[1][1] += wy * d1; b[1][2] += wz * d1;
@@ -149,23 +157,6 @@ __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restric
       b[3][0] += wx * d3; b[3][1] += wy * d3; b[3][2] += wz * d3;
       hi[0] = dmax2(hi[0], Uj.x); hi[1] = dmax2(hi[1], Uj.y); hi[2] = dmax2(hi[2], Uj.z); hi[3] = dmax2(hi[3], Uj.w);
       lo[0] = dmin2(lo[0], Uj.x); lo[1] = dmin2(lo[1], Uj.y); lo[2] = dmin2(lo[2], Uj.z); lo[3] = dmin2(lo[3], Uj.w);
-    };
-    // first pass: sum_f w_f (phi_j - phi_i), min/max.  Owned faces: the cell is the left one.
-#pragma unroll 2
-    for (int s = s0; s < s1; s++) {
-      const double4 w = ld4(sW + 4 * s);
-      int32_t l, j;
-      rt_unpack_lr(w.w, l, j);
-      const double4 Uj = j >= 0 ? neighbour(j) : ghost_for_gradient(j, Ui, m.faceN, fbase + s, m.ghost, G, g);
-      accumulate(Uj, w.x, w.y, w.z);
-    }
-    // faces where the cell is the right one: d = s_L - s_R, so the prefactor changes sign
-#pragma unroll 2
-    for (int k = r0; k < r1; k++) {
-      const double4 w = ld4(sW + 4 * (int)tt.sr[k]);
-      int32_t j, r;
-      rt_unpack_lr(w.w, j, r);
-      accumulate(neighbour(j), -w.x, -w.y, -w.z);
     }
     const double *Mi = m.Minv + 6 * i;
     const double m00 = Mi[0], m01 = Mi[1], m02 = Mi[2], m11 = Mi[3], m12 = Mi[4], m22 = Mi[5];
@@ -180,23 +171,18 @@ __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restric
     // attained at the largest D_f (division is monotone), so only the extremes are kept.
     const double4 si = ld4(m.cellS + 4 * i);
     double dmax[4] = {0, 0, 0, 0}, dmin[4] = {0, 0, 0, 0};
-    auto extremes = [&](double rx, double ry, double rz) {
+    // (the stored face centre is in the left cell's frame: min-image it for the right cell;
+    // for the left cell the wrap is the identity)
+#pragma unroll 2
+    for (int k = h0; k < h1; k++) {
+      const double4 c = ld4(sC + 4 * (int)(tt.hl[k] & 0x7fffu));
+      const double rx = wrap1(c.x - si.x, m.box[0], m.per[0]), ry = wrap1(c.y - si.y, m.box[1], m.per[1]),
+                   rz = wrap1(c.z - si.z, m.box[2], m.per[2]);
 #pragma unroll
       for (int v = 0; v < 4; v++) {
         const double d = gr[v][0] * rx + gr[v][1] * ry + gr[v][2] * rz;
         dmax[v] = dmax2(dmax[v], d); dmin[v] = dmin2(dmin[v], d);
       }
-    };
-#pragma unroll 2
-    for (int s = s0; s < s1; s++) {
-      const double4 c = ld4(sC + 4 * s);  // already in this cell's frame
-      extremes(c.x - si.x, c.y - si.y, c.z - si.z);
-    }
-#pragma unroll 2
-    for (int k = r0; k < r1; k++) {
-      const double4 c = ld4(sC + 4 * (int)tt.sr[k]);
-      extremes(wrap1(c.x - si.x, m.box[0], m.per[0]), wrap1(c.y - si.y, m.box[1], m.per[1]),
-               wrap1(c.z - si.z, m.box[2], m.per[2]));
     }
     double *out = grad + 12 * (i * G + g);
     const double Uiv[4] = {Ui.x, Ui.y, Ui.z, Ui.w};
@@ -254,8 +240,10 @@ __global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restri
                                                double *__restrict__ part_out, double *__restrict__ part_in) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ double red[32];
-  double *sPhi = reinterpret_cast<double *>(smem_raw);  // [G][smax][4]  A * (Phi_N, Phi_F)
-  double *sR = sPhi + 4 * G * m.smax;                   // [TC][G][RT_REC]  U (4) + gradients (12)
+  constexpr int PS = 4 * G > 8 ? 4 * G : 8;             // doubles per slot
+  double *sPhi = reinterpret_cast<double *>(smem_raw);  // [smax][PS]: the staged face record (c, A), (n, L|R),
+                                                        // overwritten by its owner thread with A * (Phi_N, Phi_F)[G]
+  double *sR = sPhi + PS * m.smax;                      // [TC][G][RT_REC]  U (4) + gradients (12)
   double *sS = sR + RT_REC * G * m.TC;                  // [TC][4]  (s, V)
   const int64_t C = m.C;
   const int64_t c0 = (int64_t)blockIdx.x * m.TC;
@@ -264,8 +252,12 @@ __global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restri
   const int nown = (int)(m.fo[c0 + ncell] - fbase);
   const int64_t ib = m.inco[blockIdx.x];
   const int ns = nown + (int)(m.inco[blockIdx.x + 1] - ib);
-  const int smax = m.smax;
-  // stage the tile's cells and face-list tables
+  // stage the face records, the tile's cells and the face-list tables
+  for (int s = threadIdx.x; s < ns; s += blockDim.x) {
+    const int64_t q = s < nown ? fbase + s : (int64_t)m.incf[ib + (s - nown)];
+    *reinterpret_cast<double4 *>(sPhi + PS * s) = ld4(m.faceC + 4 * q);
+    *reinterpret_cast<double4 *>(sPhi + PS * s + 4) = ld4(m.faceN + 4 * q);
+  }
   {
     const double *Ut = Uin + 4 * c0 * G, *gt = grad + 12 * c0 * G;
     for (int x = threadIdx.x; x < ncell * G; x += blockDim.x) *reinterpret_cast<double4 *>(sR + RT_REC * x) = ld4(Ut + 4 * x);
@@ -277,7 +269,7 @@ __global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restri
     const double *St = m.cellS + 4 * c0;
     for (int x = threadIdx.x; x < ncell; x += blockDim.x) *reinterpret_cast<double4 *>(sS + 4 * x) = ld4(St + 4 * x);
   }
-  const tile_tables tt = stage_tables(m, reinterpret_cast<unsigned char *>(sS + 4 * m.TC), c0, ncell, fbase);
+  const tile_tables tt = stage_tables(m, reinterpret_cast<unsigned char *>(sS + 4 * m.TC), c0, ncell);
   __syncthreads();
 
   // ---- a3: one thread per face slot, all groups
@@ -288,8 +280,7 @@ __global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restri
   const double hc2 = 0.5 * ct * ct, hc = 0.5 * ct;
   const int32_t c0i = (int32_t)c0;
   for (int s = threadIdx.x; s < ns; s += blockDim.x) {
-    const int64_t q = s < nown ? fbase + s : (int64_t)m.incf[ib + (s - nown)];
-    const double4 fc = ld4(m.faceC + 4 * q), fn = ld4(m.faceN + 4 * q);
+    const double4 fc = ld4(sPhi + PS * s), fn = ld4(sPhi + PS * s + 4);
     int32_t l, r;
     rt_unpack_lr(fn.w, l, r);
     const double n[3] = {fn.x, fn.y, fn.z};
@@ -338,7 +329,7 @@ __global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restri
       // only the number flux is clamped (continuous in the state; Phi_F is left alone)
       if (ph[0] > 0.0) ph[0] = dmin2(ph[0], NL * capL);
       else if (r >= 0) ph[0] = -dmin2(-ph[0], NR * capR);
-      st4(sPhi + 4 * (g * smax + s), A * ph[0], A * ph[1], A * ph[2], A * ph[3]);
+      st4(sPhi + PS * s + 4 * g, A * ph[0], A * ph[1], A * ph[2], A * ph[3]);
       if (r == RT_BC_OUTFLOW) { b_out[g] += A * ph[0]; bnd = 1; }
       else if (r <= RT_BC_DIRICHLET0) { b_in[g] -= A * ph[0]; bnd = 1; }
     }
@@ -363,19 +354,15 @@ __global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restri
   for (int item = threadIdx.x; item < ncell * G; item += blockDim.x) {
     const int il = item / G, g = item - il * G;
     const int64_t i = c0 + il;
-    const int s0 = tt.so[il], s1 = tt.so[il + 1];
-    const int r0 = tt.rol[il], r1 = tt.rol[il + 1];
-    const double *pg = sPhi + 4 * g * smax;
+    const int h0 = tt.ho[il], h1 = tt.ho[il + 1];
+    const double *pg = sPhi + 4 * g;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
 #pragma unroll 4
-    for (int s = s0; s < s1; s++) {
-      const double4 p = ld4(pg + 4 * s);
-      a0 += p.x; a1 += p.y; a2 += p.z; a3 += p.w;
-    }
-#pragma unroll 4
-    for (int k = r0; k < r1; k++) {
-      const double4 p = ld4(pg + 4 * (int)tt.sr[k]);
-      a0 -= p.x; a1 -= p.y; a2 -= p.z; a3 -= p.w;
+    for (int k = h0; k < h1; k++) {
+      const unsigned e = tt.hl[k];
+      const double4 p = ld4(pg + PS * (int)(e & 0x7fffu));
+      const double sg = e >= 0x8000u ? -1.0 : 1.0;  // the flux leaves the left cell and enters the right one
+      a0 = fma(sg, p.x, a0); a1 = fma(sg, p.y, a1); a2 = fma(sg, p.z, a2); a3 = fma(sg, p.w, a3);
     }
     const double V = sS[4 * il + 3];
     const double kk = dt * fast_rcp(V);  // dt / V
@@ -500,7 +487,10 @@ static inline unsigned blocks_for(int64_t n, int per_block) { return (unsigned)(
 // the tile kernels need more than the default 48 KB of dynamic shared memory
 template <class K>
 static cudaError_t allow_smem(K kernel, size_t bytes) {
-  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  if (e != cudaSuccess) return e;
+  // as many blocks per SM as shared memory allows: take the largest carve-out
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
 }
 #define SET_SMEM_G(Gv, KERNEL, bytes, err)                      \
   switch (Gv) {                                                 \
@@ -516,7 +506,7 @@ static cudaError_t allow_smem(K kernel, size_t bytes) {
 
 int rt_transport_configure(rt_ctx *c) {
   cudaError_t e = cudaSuccess;
-  const size_t sg = rt_smem_grad(c->TC, c->G, c->smax, c->rmax), ss = rt_smem_stage(c->TC, c->G, c->smax, c->rmax);
+  const size_t sg = rt_smem_grad(c->TC, c->G, c->smax, c->hmax), ss = rt_smem_stage(c->TC, c->G, c->smax, c->hmax);
   SET_SMEM_G(c->G, K_GRAD, sg, e);
   if (e == cudaSuccess) SET_SMEM_G(c->G, K_STAGE2, ss, e);
   if (e == cudaSuccess) SET_SMEM_G(c->G, K_STAGE1, ss, e);
@@ -524,10 +514,14 @@ int rt_transport_configure(rt_ctx *c) {
   return RT_OK;
 }
 
-// threads per tile block: one per (cell, group), a whole number of warps, at most 256
+// threads per tile block: a whole number of warps, at most 256 (the kernels' launch bound);
+// RT_TILE_THREADS in the environment overrides the default for experiments
 static int tile_threads(const rt_ctx *c) {
-  int n = ((c->TC * c->G + 31) / 32) * 32;
-  return n > 256 ? 256 : (n < 64 ? 64 : n);
+  static int env = -1;
+  if (env < 0) { const char *e = getenv("RT_TILE_THREADS"); env = e ? atoi(e) : 0; }
+  int n = env > 0 ? env : 256;
+  n = ((n + 31) / 32) * 32;
+  return n > 256 ? 256 : (n < 32 ? 32 : n);
 }
 
 rt_geom rt_geom_of(const rt_ctx *c) {
@@ -537,14 +531,14 @@ rt_geom rt_geom_of(const rt_ctx *c) {
   m.cellS = rt_ptr<double>(c, l.cellS); m.Minv = rt_ptr<double>(c, l.Minv);
   m.faceC = rt_ptr<double>(c, l.faceC); m.faceN = rt_ptr<double>(c, l.faceN); m.faceW = rt_ptr<double>(c, l.faceW);
   m.fo = rt_ptr<int64_t>(c, l.fo); m.ro = rt_ptr<int64_t>(c, l.ro); m.inco = rt_ptr<int64_t>(c, l.inco);
-  m.incf = rt_ptr<int32_t>(c, l.incf); m.rslot = rt_ptr<uint16_t>(c, l.rslot);
+  m.incf = rt_ptr<int32_t>(c, l.incf); m.hl = rt_ptr<uint16_t>(c, l.hl);
   m.ghost = rt_ptr<double>(c, l.ghost);
   for (int a = 0; a < 3; a++) { m.box[a] = c->box[a]; m.per[a] = c->per[a]; }
   return m;
 }
 
 int rt_launch_gradients(rt_ctx *c, const double *U) {
-  DISPATCH_G(c->G, K_GRAD, (unsigned)c->T, tile_threads(c), rt_smem_grad(c->TC, c->G, c->smax, c->rmax), c->stream, rt_geom_of(c), U,
+  DISPATCH_G(c->G, K_GRAD, (unsigned)c->T, tile_threads(c), rt_smem_grad(c->TC, c->G, c->smax, c->hmax), c->stream, rt_geom_of(c), U,
              rt_ptr<double>(c, c->lay.grad));
   c->launches++;
   return RT_OK;
@@ -568,10 +562,10 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
   const int64_t nchem = blocks_for(c->C, RT_CHEM_BLOCK);
   double *p_floor = part + (size_t)G * nchem, *p_out = p_floor + (size_t)G * c->T, *p_in = p_out + (size_t)G * c->T;
   const int nt = tile_threads(c);
-  const size_t ss = rt_smem_stage(c->TC, G, c->smax, c->rmax);
+  const size_t ss = rt_smem_stage(c->TC, G, c->smax, c->hmax);
   if (c->par.order >= 2) {
     rt_prof_begin(c, RT_K_GRAD);
-    DISPATCH_G(G, K_GRAD, (unsigned)c->T, nt, rt_smem_grad(c->TC, G, c->smax, c->rmax), c->stream, m, Uin, grad);
+    DISPATCH_G(G, K_GRAD, (unsigned)c->T, nt, rt_smem_grad(c->TC, G, c->smax, c->hmax), c->stream, m, Uin, grad);
     rt_prof_end(c);
     c->launches++;
     rt_prof_begin(c, RT_K_UPDATE);

@@ -278,8 +278,11 @@ def main():
         peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
     ab = algorithmic_bytes(C, F, NR, G, bool(w.params.heun), w.params.chem_mode != 0, int(w.params.order))
     kern = {}
-    prof["stage"] = prof["update"]   # class 3 = flux + update of one Heun stage (k_stage)
-    for k in ("chem", "grad", "stage", "reduce"):
+    # one Heun stage's a3 + a4 = k_flux (class 2) followed by k_finish (class 3): reported separately
+    # and, as "stage", together (the algorithmic bytes of a3 + a4 are those of the pair)
+    prof["finish"] = prof["update"]
+    prof["stage"] = (prof["flux"][0] + prof["update"][0], prof["flux"][1])
+    for k in ("chem", "grad", "stage", "flux", "finish", "reduce"):
         tms, cnt = prof[k]
         if cnt == 0:
             continue

@@ -145,7 +145,9 @@ int64_t rt_kernel_launches(const rt_ctx *ctx);
 
 /* The tile decomposition rt_mesh_upload chose, for reports: out[0] cells per tile,
  * out[1] number of tiles, out[2] largest number of face slots of a tile, out[3] faces evaluated a
- * second time because their two cells lie in different tiles.  HOST array of 4.  Needs a mesh. */
+ * second time because their two cells lie in different tiles, out[4] largest halo (cells outside a
+ * tile that touch it) of a tile, out[5] halo cells summed over the tiles, out[6] largest per-tile
+ * table in 32-bit words, out[7] all per-tile tables in 32-bit words.  HOST array of 8.  Needs a mesh. */
 int rt_tile_info(const rt_ctx *ctx, int64_t *out);
 
 /* Per-kernel timing with CUDA events recorded on the context's stream around every launch of

@@ -89,6 +89,7 @@ int rt_tile_info(const rt_ctx *c, int64_t *out) {
   if (!c || !out) return RT_EINVAL;
   if (!c->have_mesh) return RT_ESTATE;
   out[0] = c->TC; out[1] = c->T; out[2] = c->smax; out[3] = c->ninc;
+  out[4] = c->hmax; out[5] = c->nhalo; out[6] = c->bmax; out[7] = c->blob_words;
   return RT_OK;
 }
 

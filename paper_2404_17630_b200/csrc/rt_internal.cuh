@@ -5,18 +5,36 @@
 //     cellS[C][4] = (sx, sy, sz, V); Minv[C][6] (symmetric inverse of sum_f A n n^T, eq (15))
 //   faces sorted by owner (= left cell, the lower new id), then by right id, boundary faces last;
 //   every face array is [F][4] doubles = one aligned 32-byte sector per face:
-//     faceC = (cx, cy, cz, A)     centroid in the left cell's frame and area
-//     faceN = (nx, ny, nz, L|R)   unit normal L -> R; the fourth slot holds the two int32 ids
-//     faceW = (wx, wy, wz, L|R)   w = A d/|d|^2, d = s_R - s_L: prefactor of eq (15)'s second
-//                                 term
+//     faceC = (cx, cy, cz, A)     centroid relative to the left cell's centroid (min-image) and area
+//     faceN = (nx, ny, nz, 0)     unit normal L -> R
+//     faceW = (wx, wy, wz, kappa) w = A d/|d|^2, d = s_R - s_L: prefactor of eq (15)'s second
+//                                 term; kappa = |d|^2/A, so the face centroid relative
+//                                 to the right cell is c - kappa w
 //   cell -> faces: owned faces are the contiguous range fo[i]..fo[i+1]; the faces
 //     where the cell is the right one are r-list entries ro[i]..ro[i+1] (ascending face id)
 //   tiles: TC consecutive cells (a compact blob of the Hilbert curve) are one thread block's
 //     work.  A tile's "slots" are its owned faces (slot s = face - fo[c0]) followed by its
-//     incoming faces (right cell in the tile, owner in an earlier tile), listed in
-//     incf[inco[t]..inco[t+1]].  hl[fo[i]+ro[i] ..] is cell i's half-face list: the slot of each of
-//     its faces inside its tile (owned faces first; bit 15 set where the cell is the right one),
-//     so a cell finds every one of its faces in the tile's shared-memory slot arrays.
+//     incoming faces (right cell in the tile, owner in an earlier tile).  Its "halo" is the sorted
+//     list of the cells outside the tile that touch one of its slots; a cell of the tile has the
+//     local id x = i - c0, halo cell k the local id TC + k.  Per tile one descriptor (rt_tile) and
+//     one contiguous blob of 32-bit words (16-byte aligned, a whole number of 16-byte chunks):
+//       ho[TC+1]   offset of each cell's half-face list inside hl
+//       hl[nhf]    half-faces, cell by cell, owned faces first:
+//                    bits 0-14 slot, bit 15 set where the cell is the face's right cell,
+//                    bits 16-31 local id of the cell across the face or a boundary code
+//       slr[nown]  per owned slot: bits 0-15 local id of the left cell, bits 16-31 local id of the
+//                    right cell or a boundary code (0x10000 + right, i.e. 0xFFFF outflow, 0xFFFE
+//                    reflective, 0xFFFD - k Dirichlet ghost k); local ids stay below 0xFF00
+//       halo[nh]   global ids of the halo cells, ascending: the first nb lie before the tile
+//                  ("backward"), the others after it ("forward")
+//       incf[ninc] global face ids of the incoming slots
+//       outs[nout] the owned slots whose right cell lies in a later tile ("outgoing"), ascending;
+//                  the tile writes their fluxes to rows xbase .. xbase + nout of xphi
+//     so a thread block stages everything its tile touches in shared memory with asynchronous
+//     copies and then computes from shared memory alone.  Every face's flux is evaluated once, by
+//     the tile of its left cell (k_flux), which also updates the cells all of whose faces it has.
+//     The other cells ("incomplete": k2cell[n2]) get the fluxes of their incoming faces from
+//     xphi[ninc][G][4] in k_finish: rows k2row[k2off[k] .. k2off[k+1]] for cell k2cell[k].
 //   state, cell-major so that a tile is one contiguous run:
 //     Ua, Ub [C][G][4] = (N, Fx, Fy, Fz); grad [C][G][12] (field-major, then direction);
 //     xHII, xHeII, xHeIII, eth, nH, kappa [C]
@@ -40,8 +58,10 @@ struct rt_dev_ledger {  // accumulators on the device (value + compensation)
 };
 
 struct rt_layout {
-  size_t perm, iperm, cellS, Minv, faceC, faceN, faceW, L, R, fo, ro, rl, rn, hl, incf, inco, ghost, led;
-  size_t Ua, Ub, grad, xHII, xHeII, xHeIII, eth, nH, kappa, srcidx, srcrate, part, scratch_end;
+  size_t perm, iperm, cellS, Minv, faceC, faceN, faceW, L, R, fo, ro, rl, rn, tiles, blob, xphi, k2cell, k2off, k2row, ghost, led;
+  size_t Ua, Ub, grad, pacc, xHII, xHeII, xHeIII, eth, nH, kappa, srcidx, srcrate, part, scratch_end;
+  size_t blob_bytes;  // capacity of the blob region
+  int64_t xcap;       // rows [G][4] of xphi
   size_t temp;        // start of the setup-time scratch (aliases the state region)
   size_t total;
   int64_t nbc;        // blocks of RT_BLOCK cells (partial-sum rows of k_stored)
@@ -57,8 +77,14 @@ struct rt_ctx {
   int TC;             // cells per tile
   int64_t T;          // number of tiles
   int smax;           // largest slot count of any tile
-  int hmax;           // largest half-face count of any tile
+  int hmax;           // largest halo (cells outside the tile touching it) of any tile
+  int fmax;           // largest forward halo of any tile
+  int omax;           // most owned faces of any tile
+  int64_t n2;         // cells with at least one incoming face
+  int bmax;           // largest blob of any tile, in 32-bit words
   int64_t ninc;       // total incoming faces over all tiles
+  int64_t nhalo;      // total halo cells over all tiles
+  int64_t blob_words; // total blob size
   double box[3];
   int per[3];
   int nghost;
@@ -83,19 +109,31 @@ enum { RT_K_CHEM = 0, RT_K_GRAD = 1, RT_K_FLUX = 2, RT_K_UPDATE = 3, RT_K_REDUCE
 void rt_prof_begin(rt_ctx *c, int cls);
 void rt_prof_end(rt_ctx *c);
 
-// dynamic shared memory of the two tile kernels (rt_transport.cu) for a tile of TC cells whose
-// slot count is at most smax
-// (hmax: most half-faces of any tile; the face-list tables are int[TC+1] and uint16[hmax])
-static inline size_t rt_smem_tables(int TC, int hmax) { return ((size_t)4 * (TC + 1) + (size_t)2 * hmax + 15) & ~(size_t)15; }
-static inline size_t rt_smem_grad(int TC, int G, int smax, int hmax) {
-  return (size_t)64 * smax + (size_t)32 * TC * G + rt_smem_tables(TC, hmax);
+// one tile's descriptor (32 bytes)
+struct rt_tile {
+  int64_t fbase;  // first owned face = fo[c0]
+  int64_t blob;   // first word of the tile's blob
+  int64_t xbase;  // first row of xphi the tile publishes
+  int32_t nown, ninc, nh, nhf;  // owned faces, incoming faces, halo cells, half-faces
+  int32_t nb, nout, n2, pad;    // backward halo cells, outgoing faces, cells with incoming faces
+};
+#define RT_TILE_LIMIT 2048  // most owned faces / r-list entries / halo candidates of a tile the builder handles
+__host__ __device__ static inline int rt_blob_words(int TC, int nhf, int nown, int nh, int ninc, int nout) {
+  return (TC + 1 + nhf + nown + nh + ninc + nout + 3) & ~3;
 }
-static inline size_t rt_smem_stage(int TC, int G, int smax, int hmax) {
-  const int per_slot = 32 * G > 64 ? 32 * G : 64;  // A*Phi of every group, or the staged face record before it
-  return (size_t)per_slot * smax + (size_t)RT_REC * 8 * TC * G + (size_t)32 * TC + rt_smem_tables(TC, hmax);
+
+// dynamic shared memory of the two tile kernels (rt_transport.cu) for tiles of TC cells with at
+// most smax slots, hmax halo cells (k_grad) / forward halo cells (k_stage) and bmax blob words
+static inline size_t rt_smem_grad(int TC, int G, int smax, int hmax, int bmax) {
+  return (size_t)4 * bmax + (size_t)64 * smax + (size_t)32 * G * (TC + hmax) + (size_t)48 * TC;
+}
+static inline size_t rt_smem_flux(int TC, int G, int omax, int fmax, int bmax) {
+  const int planes = G > 3 ? G : 3;  // three face records per slot, overwritten by A*Phi of every group
+  return (size_t)4 * bmax + (size_t)32 * planes * omax + (size_t)(128 * G + 32) * (TC + fmax) + (size_t)32 * G * TC +
+         (size_t)16 * ((TC + 3) / 4);
 }
 #define RT_SMEM_MAX 232448     // 227 KB: the most one block may have on sm_100
-#define RT_SMEM_TARGET 110000  // two blocks per SM
+#define RT_SMEM_TARGET 115000  // two blocks per SM (228 KB per SM, 1 KB reserved per block)
 
 template <class T>
 static inline T *rt_ptr(const rt_ctx *c, size_t off) { return (T *)(c->ws + off); }

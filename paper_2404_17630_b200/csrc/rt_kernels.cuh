@@ -13,13 +13,13 @@ struct rt_chem_par {
 struct rt_geom {
   int64_t C, F;
   const double *cellS, *Minv, *faceC, *faceN, *faceW;
-  const int64_t *fo, *ro, *inco;
-  const int32_t *incf;
-  const uint16_t *hl;
+  const rt_tile *tiles;
+  const uint32_t *blob;
+  double *xphi;          // [ninc][G][4] fluxes of the faces that cross tile boundaries
   const double *ghost;
   double box[3];
   int per[3];
-  int G, TC, smax;
+  int G, TC, smax, omax, hmax, fmax, bmax;
 };
 
 // the two int32 ids packed in the fourth slot of a faceN / faceW record

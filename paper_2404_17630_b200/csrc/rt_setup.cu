@@ -107,7 +107,7 @@ __global__ void k_gather_faces(geom_in g, int64_t C, int64_t F, const int32_t *o
   bool flip = (iperm[g.left[f]] != l);
   if (flip) r = iperm[g.left[f]];
   L[q] = l; R[q] = r;
-  faceN[4 * q + 3] = rt_pack_lr(l, r);
+  faceN[4 * q + 3] = 0.0;
   faceC[4 * q + 3] = g.area[f];
   double sg = flip ? -1.0 : 1.0;
   double b[3] = {bx, by, bz};
@@ -115,7 +115,7 @@ __global__ void k_gather_faces(geom_in g, int64_t C, int64_t F, const int32_t *o
   for (int a = 0; a < 3; a++) {
     faceN[4 * q + a] = sg * g.normal[a * F + f];
     double sl = cellS[4 * (int64_t)l + a];
-    faceC[4 * q + a] = sl + rt_wrap(g.fcentroid[a * F + f] - sl, b[a], per[a]);  // left cell's frame
+    faceC[4 * q + a] = rt_wrap(g.fcentroid[a * F + f] - sl, b[a], per[a]);  // relative to the left cell's centroid
   }
 }
 
@@ -147,7 +147,9 @@ __global__ void k_rlist(const uint64_t *keys, int64_t NR, const int32_t *L, int3
 }
 
 // per-face prefactor of eq (15)'s second term, seen from the left cell: w = A d/|d|^2,
-// d = s_R - s_L measured through the face; boundary faces use the mirror point (S13)
+// d = s_R - s_L measured through the face; boundary faces use the mirror point (S13).
+// faceW = (w, kappa) with kappa = |d|^2 / A, so that d = kappa w: the face centre seen from the
+// right cell is (c - s_L) - kappa w, without a min-image test in the kernels.
 __global__ void k_face_geom(int64_t C, int64_t F, const double *cellS, const double *faceC, const double *faceN,
                             const int32_t *L, const int32_t *R, double bx, double by, double bz, int p0, int p1, int p2,
                             double *faceW) {
@@ -159,19 +161,20 @@ __global__ void k_face_geom(int64_t C, int64_t F, const double *cellS, const dou
   double d[3];
   if (r >= 0) {
     for (int a = 0; a < 3; a++) {
-      double c = faceC[4 * q + a];
-      d[a] = (c - cellS[4 * (int64_t)l + a]) - rt_wrap(c - cellS[4 * (int64_t)r + a], b[a], per[a]);
+      double rl = faceC[4 * q + a];
+      double c = cellS[4 * (int64_t)l + a] + rl;
+      d[a] = rl - rt_wrap(c - cellS[4 * (int64_t)r + a], b[a], per[a]);
     }
   } else {
     double n[3] = {faceN[4 * q], faceN[4 * q + 1], faceN[4 * q + 2]};
     double p = 0.0;
-    for (int a = 0; a < 3; a++) p += (faceC[4 * q + a] - cellS[4 * (int64_t)l + a]) * n[a];
+    for (int a = 0; a < 3; a++) p += faceC[4 * q + a] * n[a];
     for (int a = 0; a < 3; a++) d[a] = 2.0 * p * n[a];
   }
   double d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
   double k = faceC[4 * q + 3] / d2;
   for (int a = 0; a < 3; a++) faceW[4 * q + a] = k * d[a];
-  faceW[4 * q + 3] = rt_pack_lr(l, r);
+  faceW[4 * q + 3] = d2 / faceC[4 * q + 3];
 }
 
 // per cell: M = sum_f A n n^T (n = d/|d| = w/|w|), its inverse, and the closure check
@@ -209,49 +212,196 @@ __global__ void k_cell_geom(int64_t C, int64_t F, const double *faceC, const dou
 }
 
 
-// ---- tiles: incoming-face lists and per-cell slot numbers (layout: rt_internal.cuh)
-// number of r-list entries of cell i whose owner lies in an earlier tile (they come first: the
-// r-list is sorted by face id = by owner)
-__global__ void k_tile_count(int64_t C, int TC, const int64_t *ro, const int32_t *rn, int32_t *cellInc) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= C) return;
-  const int32_t c0 = (int32_t)((i / TC) * TC);
-  int n = 0;
-  for (int64_t k = ro[i]; k < ro[i + 1]; k++) n += rn[k] < c0;
-  cellInc[i] = n;
+// ---- tiles: descriptors and blobs (layout: rt_internal.cuh).  One block per tile.
+// MODE 0 measures (blob words per tile, maxima), MODE 1 writes.
+#define TILE_BT 128
+struct tile_max { int ns, no, nh, nf, words, overflow, pad[2]; };
+
+__device__ inline int halo_pos(const int32_t *halo, int nh, int32_t id) {
+  int lo = 0, hi = nh;
+  while (lo < hi) { const int mid = (lo + hi) >> 1; if (halo[mid] < id) lo = mid + 1; else hi = mid; }
+  return lo;
 }
-// per tile: exclusive prefix of cellInc over its cells (in place), the tile's total, max slots
-__global__ void k_tile_scan(int64_t C, int TC, int64_t T, const int64_t *fo, const int64_t *ro, int32_t *cellInc,
-                            int64_t *tileInc, int *maxSlots) {
+
+template <int MODE>
+__global__ void __launch_bounds__(TILE_BT) k_tile_build(int64_t C, int TC, const int64_t *fo, const int64_t *ro,
+                                                        const int32_t *R, const int32_t *rl, const int32_t *rn,
+                                                        int64_t *tsize, int64_t *xcnt, int64_t *icnt, int64_t *n2cnt,
+                                                        tile_max *mx, const int64_t *boff, const int64_t *xoff,
+                                                        const int64_t *ibase, const int64_t *k2base, rt_tile *tiles,
+                                                        uint32_t *blob, int32_t *faceX, int32_t *k2cell, int32_t *k2off) {
+  typedef cub::BlockScan<int, TILE_BT> Scan;
+  __shared__ typename Scan::TempStorage scan_tmp;
+  __shared__ int32_t s_cand[RT_TILE_LIMIT], s_rank[RT_TILE_LIMIT], s_halo[RT_TILE_LIMIT];
+  __shared__ int s_nc, s_run;
+  const int64_t t = blockIdx.x;
+  const int64_t c0 = t * TC, c1 = c0 + TC < C ? c0 + TC : C;
+  const int ncell = (int)(c1 - c0);
+  const int64_t fbase = fo[c0], rbase = ro[c0];
+  const int64_t nown64 = fo[c1] - fbase, nr64 = ro[c1] - rbase;
+  if (nown64 > RT_TILE_LIMIT || nr64 > RT_TILE_LIMIT) {
+    if (threadIdx.x == 0) { atomicMax(&mx->overflow, 1); if (MODE == 0) { tsize[t] = 0; xcnt[t] = 0; icnt[t] = 0; n2cnt[t] = 0; } }
+    return;
+  }
+  const int nown = (int)nown64, nr = (int)nr64;
+  if (threadIdx.x == 0) { s_nc = 0; s_run = 0; }
+  __syncthreads();
+  // incoming faces: r-list entries whose owner lies in an earlier tile, ranked in r-list order
+  for (int k0 = 0; k0 < nr; k0 += TILE_BT) {
+    const int k = k0 + threadIdx.x;
+    const int flag = k < nr && rn[rbase + k] < c0;
+    int pos, tot;
+    Scan(scan_tmp).ExclusiveSum(flag, pos, tot);
+    const int base = s_run;
+    if (k < nr) s_rank[k] = flag ? base + pos : -1;
+    __syncthreads();
+    if (threadIdx.x == 0) s_run = base + tot;
+    __syncthreads();
+  }
+  const int ninc = s_run;
+  // halo candidates: the far cell of every face that leaves the tile
+  for (int s = threadIdx.x; s < nown; s += TILE_BT) {
+    const int32_t r = R[fbase + s];
+    if (r >= c1) { const int p = atomicAdd(&s_nc, 1); if (p < RT_TILE_LIMIT) s_cand[p] = r; }
+  }
+  for (int k = threadIdx.x; k < nr; k += TILE_BT)
+    if (s_rank[k] >= 0) { const int p = atomicAdd(&s_nc, 1); if (p < RT_TILE_LIMIT) s_cand[p] = rn[rbase + k]; }
+  __syncthreads();
+  const int nc = s_nc;
+  if (nc > RT_TILE_LIMIT) {
+    if (threadIdx.x == 0) { atomicMax(&mx->overflow, 1); if (MODE == 0) { tsize[t] = 0; xcnt[t] = 0; icnt[t] = 0; n2cnt[t] = 0; } }
+    return;
+  }
+  int np2 = 1;
+  while (np2 < nc) np2 <<= 1;
+  for (int k = nc + threadIdx.x; k < np2; k += TILE_BT) s_cand[k] = 0x7fffffff;
+  __syncthreads();
+  for (int size = 2; size <= np2; size <<= 1)  // bitonic sort, ascending
+    for (int stride = size >> 1; stride > 0; stride >>= 1) {
+      for (int k = threadIdx.x; k < np2; k += TILE_BT) {
+        const int j = k ^ stride;
+        if (j > k) {
+          const int32_t a = s_cand[k], b = s_cand[j];
+          const bool up = (k & size) == 0;
+          if ((a > b) == up) { s_cand[k] = b; s_cand[j] = a; }
+        }
+      }
+      __syncthreads();
+    }
+  if (threadIdx.x == 0) s_run = 0;
+  __syncthreads();
+  for (int k0 = 0; k0 < nc; k0 += TILE_BT) {  // unique
+    const int k = k0 + threadIdx.x;
+    const int flag = k < nc && (k == 0 || s_cand[k] != s_cand[k - 1]);
+    int pos, tot;
+    Scan(scan_tmp).ExclusiveSum(flag, pos, tot);
+    const int base = s_run;
+    if (flag) s_halo[base + pos] = s_cand[k];
+    __syncthreads();
+    if (threadIdx.x == 0) s_run = base + tot;
+    __syncthreads();
+  }
+  const int nh = s_run, nhf = nown + nr, ns = nown + ninc;
+  const int nb = halo_pos(s_halo, nh, (int32_t)c0);  // halo cells before the tile
+  __syncthreads();
+  // outgoing faces (right cell in a later tile), ranked in face order; s_cand is free again
+  if (threadIdx.x == 0) s_run = 0;
+  __syncthreads();
+  for (int k0 = 0; k0 < nown; k0 += TILE_BT) {
+    const int k = k0 + threadIdx.x;
+    const int flag = k < nown && R[fbase + k] >= c1;
+    int pos, tot;
+    Scan(scan_tmp).ExclusiveSum(flag, pos, tot);
+    const int base = s_run;
+    if (k < nown) s_cand[k] = flag ? base + pos : -1;
+    __syncthreads();
+    if (threadIdx.x == 0) s_run = base + tot;
+    __syncthreads();
+  }
+  const int nout = s_run;
+  // cells with at least one incoming face ("incomplete": k_finish adds those fluxes), in cell
+  // order; a cell's incoming faces have consecutive ranks
+  __syncthreads();
+  if (threadIdx.x == 0) s_run = 0;
+  __syncthreads();
+  for (int x0 = 0; x0 < ncell; x0 += TILE_BT) {
+    const int x = x0 + threadIdx.x;
+    int first = -1;
+    if (x < ncell)
+      for (int64_t k = ro[c0 + x]; k < ro[c0 + x + 1] && first < 0; k++) first = s_rank[k - rbase];
+    const int flag = first >= 0;
+    int pos, tot;
+    Scan(scan_tmp).ExclusiveSum(flag, pos, tot);
+    const int base = s_run;
+    if (MODE == 1 && flag) {
+      k2cell[k2base[t] + base + pos] = (int32_t)(c0 + x);
+      k2off[k2base[t] + base + pos] = (int32_t)(ibase[t] + first);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) s_run = base + tot;
+    __syncthreads();
+  }
+  const int n2 = s_run;
+  const int words = rt_blob_words(TC, nhf, nown, nh, ninc, nout);
+  if (MODE == 0) {
+    if (threadIdx.x == 0) {
+      tsize[t] = words; xcnt[t] = nout; icnt[t] = ninc; n2cnt[t] = n2;
+      atomicMax(&mx->ns, ns); atomicMax(&mx->no, nown); atomicMax(&mx->nh, nh); atomicMax(&mx->nf, nh - nb); atomicMax(&mx->words, words);
+      if (TC + nh >= 0xFF00 || ns > 0x7fff) atomicMax(&mx->overflow, 1);
+    }
+    return;
+  }
+  if (threadIdx.x == 0) {
+    rt_tile d;
+    d.fbase = fbase; d.blob = boff[t]; d.xbase = xoff[t]; d.nown = nown; d.ninc = ninc; d.nh = nh; d.nhf = nhf;
+    d.nb = nb; d.nout = nout; d.n2 = n2; d.pad = 0;
+    tiles[t] = d;
+    if (t == (int64_t)gridDim.x - 1) k2off[k2base[t] + n2] = (int32_t)(ibase[t] + ninc);  // end of the last cell's rows
+  }
+  uint32_t *ho = blob + boff[t], *hl = ho + TC + 1, *slr = hl + nhf, *halo = slr + nown, *incf = halo + nh;
+  uint32_t *outs = incf + ninc;
+  for (int k = threadIdx.x; k < nown; k += TILE_BT)
+    if (s_cand[k] >= 0) { outs[s_cand[k]] = (uint32_t)k; faceX[fbase + k] = (int32_t)(xoff[t] + s_cand[k]); }
+  auto local_of = [&](int32_t id) -> uint32_t {  // id >= 0
+    return id >= c0 && id < c1 ? (uint32_t)(id - c0) : (uint32_t)(TC + halo_pos(s_halo, nh, id));
+  };
+  for (int x = threadIdx.x; x <= TC; x += TILE_BT) {
+    const int64_t i = c0 + (x < ncell ? x : ncell);
+    ho[x] = (uint32_t)((fo[i] - fbase) + (ro[i] - rbase));
+  }
+  for (int x = threadIdx.x; x < ncell; x += TILE_BT) {
+    const int64_t i = c0 + x;
+    uint32_t *h = hl + (fo[i] - fbase) + (ro[i] - rbase);
+    for (int64_t q = fo[i]; q < fo[i + 1]; q++) {  // owned slots: left = this cell
+      const int32_t r = R[q];
+      const uint32_t nbr = r >= 0 ? local_of(r) : (uint32_t)(0x10000 + r);
+      *h++ = (nbr << 16) | (uint32_t)(q - fbase);
+      slr[q - fbase] = (nbr << 16) | (uint32_t)x;
+    }
+    for (int64_t k = ro[i]; k < ro[i + 1]; k++) {
+      const int rk = s_rank[k - rbase];
+      const uint32_t slot = rk >= 0 ? (uint32_t)(nown + rk) : (uint32_t)(rl[k] - fbase);
+      *h++ = (local_of(rn[k]) << 16) | 0x8000u | slot;
+      if (rk >= 0) incf[rk] = (uint32_t)rl[k];
+    }
+  }
+  for (int k = threadIdx.x; k < nh; k += TILE_BT) halo[k] = (uint32_t)s_halo[k];
+  for (int k = TC + 1 + nhf + nown + nh + ninc + nout + threadIdx.x; k < words; k += TILE_BT) ho[k] = 0;
+}
+
+// k2row: the xphi row of every incoming face, tile by tile in rank order (= cell by cell)
+__global__ void __launch_bounds__(TILE_BT) k_tile_rows(int TC, const rt_tile *tiles, const uint32_t *blob, const int64_t *ibase,
+                                                       const int32_t *faceX, int32_t *k2row) {
+  const rt_tile d = tiles[blockIdx.x];
+  const uint32_t *incf = blob + d.blob + TC + 1 + d.nhf + d.nown + d.nh;
+  for (int j = threadIdx.x; j < d.ninc; j += TILE_BT) k2row[ibase[blockIdx.x] + j] = faceX[incf[j]];
+}
+
+__global__ void k_tile_totals(int64_t T, const rt_tile *tiles, unsigned long long *tot) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= T) return;
-  const int64_t c0 = t * TC, c1 = c0 + TC < C ? c0 + TC : C;
-  int run = 0;
-  for (int64_t i = c0; i < c1; i++) { int n = cellInc[i]; cellInc[i] = run; run += n; }
-  tileInc[t] = run;
-  const int64_t slots = fo[c1] - fo[c0] + run;
-  atomicMax(maxSlots, slots > 0x7fffffff ? 0x7fffffff : (int)slots);
-  const int64_t nh = fo[c1] - fo[c0] + ro[c1] - ro[c0];
-  atomicMax(maxSlots + 1, nh > 0x7fffffff ? 0x7fffffff : (int)nh);
-}
-__global__ void k_tile_fill(int64_t C, int TC, const int64_t *fo, const int64_t *ro, const int32_t *rl, const int32_t *rn,
-                            const int32_t *cellInc, const int64_t *inco, int32_t *incf, uint16_t *hl) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= C) return;
-  const int64_t t = i / TC, c0 = t * TC, c1 = c0 + TC < C ? c0 + TC : C;
-  const int64_t fbase = fo[c0], nown = fo[c1] - fbase;
-  uint16_t *h = hl + fo[i] + ro[i];  // the cell's half-face list: owned slots, then r-list slots with bit 15 set
-  for (int64_t q = fo[i]; q < fo[i + 1]; q++) *h++ = (uint16_t)(q - fbase);
-  int j = cellInc[i];
-  for (int64_t k = ro[i]; k < ro[i + 1]; k++) {
-    int slot;
-    if (rn[k] < c0) {
-      incf[inco[t] + j] = rl[k];
-      slot = (int)(nown + j);
-      j++;
-    } else slot = (int)(rl[k] - fbase);
-    *h++ = (uint16_t)(slot | 0x8000);
-  }
+  atomicAdd(tot, (unsigned long long)tiles[t].ninc);
+  atomicAdd(tot + 1, (unsigned long long)tiles[t].nh);
 }
 
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -263,7 +413,7 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
   // carve the scratch region
   size_t o = lay.temp;
   auto take = [&](size_t bytes) { size_t r = o; o = align256(o + bytes); return r; };
-  const int64_t NM = C > F ? C : F;
+  const int64_t NM = (C > F ? C : F) > 4 * (lay.max_tiles + 2) ? (C > F ? C : F) : 4 * (lay.max_tiles + 2);
   uint64_t *k0 = rt_ptr<uint64_t>(c, take(8 * NM)), *k1 = rt_ptr<uint64_t>(c, take(8 * NM));
   int32_t *v0 = rt_ptr<int32_t>(c, take(4 * NM)), *v1 = rt_ptr<int32_t>(c, take(4 * NM));
   int *flags = rt_ptr<int>(c, take(256));
@@ -354,43 +504,74 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
                                                c->per[0], c->per[1], c->per[2], faceW);
   k_cell_geom<<<nblk(C), SETUP_BLOCK, 0, st>>>(C, F, faceC, faceN, faceW, fo, ro, rl, rt_ptr<double>(c, lay.Minv), flags);
   RT_CUDA(c, cudaMemcpyAsync(&hflags, flags, sizeof(int), cudaMemcpyDeviceToHost, st));
-  // 5. tiles: the largest tile size (halving from RT_TILE_CELLS, default 64) whose shared memory fits
+  // 5. tiles: the largest tile size (from RT_TILE_CELLS, default 64, downwards) whose shared memory
+  // lets RT_TILE_BLOCKS (default 2) thread blocks of k_flux share an SM; failing that, the largest
+  // that fits one block
   {
-    int32_t *cellInc = v0;
-    int64_t *tileInc = (int64_t *)k0;
-    int *maxSlots = flags + 1;
+    const int64_t Tmax = lay.max_tiles + 2;
+    int64_t *tsize = (int64_t *)k0, *xcnt = tsize + Tmax, *icnt = xcnt + Tmax, *n2cnt = icnt + Tmax;
+    int64_t *boff = (int64_t *)k1, *xoff = boff + Tmax, *ibase = xoff + Tmax, *k2base = ibase + Tmax;
+    int32_t *faceX = v0;
+    tile_max *mx = (tile_max *)(flags + 4);
     const int32_t *rn = rt_ptr<int32_t>(c, lay.rn);
-    int64_t *inco = rt_ptr<int64_t>(c, lay.inco);
     const char *env = getenv("RT_TILE_CELLS");
     int tc0 = env ? atoi(env) : 64;
     if (tc0 < RT_MIN_TILE || tc0 > 1024) tc0 = 64;
-    int best = 0, best_smax = 0;
+    env = getenv("RT_TILE_BLOCKS");
+    int nblocks = env ? atoi(env) : 2;
+    if (nblocks < 1 || nblocks > 8) nblocks = 2;
+    int best = 0;
+    tile_max hm;
+    memset(&hm, 0, sizeof hm);
     for (int pass = 0; pass < 2 && !best; pass++) {
-      const size_t limit = pass == 0 ? RT_SMEM_TARGET : RT_SMEM_MAX;
-      for (int TC = tc0; TC >= RT_MIN_TILE; TC /= 2) {
+      const size_t limit = pass == 0 ? (size_t)(233472 / nblocks - 1024 - 512) : RT_SMEM_MAX;
+      for (int TC = tc0; TC >= RT_MIN_TILE; TC -= TC > 32 ? 8 : 4) {
         const int64_t T = (C + TC - 1) / TC;
-        RT_CUDA(c, cudaMemsetAsync(maxSlots, 0, 2 * sizeof(int), st));
-        k_tile_count<<<nblk(C), SETUP_BLOCK, 0, st>>>(C, TC, ro, rn, cellInc);
-        k_tile_scan<<<nblk(T), SETUP_BLOCK, 0, st>>>(C, TC, T, fo, ro, cellInc, tileInc, maxSlots);
-        int mx[2] = {0, 0};
-        RT_CUDA(c, cudaMemcpyAsync(mx, maxSlots, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+        RT_CUDA(c, cudaMemsetAsync(mx, 0, sizeof(tile_max), st));
+        k_tile_build<0><<<(unsigned)T, TILE_BT, 0, st>>>(C, TC, fo, ro, R, rl, rn, tsize, xcnt, icnt, n2cnt, mx, nullptr, nullptr,
+                                                        nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+        RT_CUDA(c, cudaMemcpyAsync(&hm, mx, sizeof(tile_max), cudaMemcpyDeviceToHost, st));
         RT_CUDA(c, cudaStreamSynchronize(st));
-        const int smax = mx[0], hmax = mx[1];
-        if (smax < 32768 && rt_smem_stage(TC, c->G, smax, hmax) <= limit && rt_smem_grad(TC, c->G, smax, hmax) <= limit) {
-          best = TC; best_smax = smax; c->hmax = hmax;
+        if (!hm.overflow && rt_smem_flux(TC, c->G, hm.no, hm.nf, hm.words) <= limit &&
+            rt_smem_grad(TC, c->G, hm.ns, hm.nh, hm.words) <= (limit > RT_SMEM_TARGET ? limit : RT_SMEM_TARGET)) {
+          best = TC;
           break;
         }
       }
     }
     if (!best) return rt_fail(c, RT_EMESH, "a cell has too many faces for one thread block's shared memory");
-    c->TC = best; c->smax = best_smax; c->T = (C + best - 1) / best;
-    // tileInc / cellInc hold the accepted tile size's counts (the loop stops at the first fit)
-    size_t b = cub_bytes;
-    RT_CUDA(c, cudaMemsetAsync(tileInc + c->T, 0, 8, st));
-    RT_CUDA(c, cub::DeviceScan::ExclusiveSum(cub_tmp, b, tileInc, inco, c->T + 1, st));
-    k_tile_fill<<<nblk(C), SETUP_BLOCK, 0, st>>>(C, best, fo, ro, rl, rn, cellInc, inco, rt_ptr<int32_t>(c, lay.incf),
-                                                 rt_ptr<uint16_t>(c, lay.hl));
-    RT_CUDA(c, cudaMemcpyAsync(&c->ninc, inco + c->T, 8, cudaMemcpyDeviceToHost, st));
+    c->TC = best; c->smax = hm.ns; c->omax = hm.no; c->hmax = hm.nh; c->fmax = hm.nf; c->bmax = hm.words;
+    c->T = (C + best - 1) / best;
+    // the count arrays hold the accepted tile size's values (the loop stops at the first fit)
+    int64_t *cnt[4] = {tsize, xcnt, icnt, n2cnt}, *off[4] = {boff, xoff, ibase, k2base};
+    for (int a = 0; a < 4; a++) {
+      size_t b = cub_bytes;
+      RT_CUDA(c, cudaMemsetAsync(cnt[a] + c->T, 0, 8, st));
+      RT_CUDA(c, cub::DeviceScan::ExclusiveSum(cub_tmp, b, cnt[a], off[a], c->T + 1, st));
+    }
+    RT_CUDA(c, cudaMemcpyAsync(&c->blob_words, boff + c->T, 8, cudaMemcpyDeviceToHost, st));
+    RT_CUDA(c, cudaMemcpyAsync(&c->ninc, xoff + c->T, 8, cudaMemcpyDeviceToHost, st));
+    RT_CUDA(c, cudaMemcpyAsync(&c->n2, k2base + c->T, 8, cudaMemcpyDeviceToHost, st));
+    RT_CUDA(c, cudaStreamSynchronize(st));
+    if ((size_t)c->blob_words * 4 > lay.blob_bytes)
+      return rt_fail(c, RT_ENOMEM, "tile tables need %lld bytes, the workspace holds %zu", (long long)c->blob_words * 4,
+                     lay.blob_bytes);
+    if (c->ninc > lay.xcap)
+      return rt_fail(c, RT_ENOMEM, "%lld faces cross tile boundaries, the workspace holds the fluxes of %lld",
+                     (long long)c->ninc, (long long)lay.xcap);
+    rt_tile *tiles = rt_ptr<rt_tile>(c, lay.tiles);
+    uint32_t *blob = rt_ptr<uint32_t>(c, lay.blob);
+    k_tile_build<1><<<(unsigned)c->T, TILE_BT, 0, st>>>(C, best, fo, ro, R, rl, rn, nullptr, nullptr, nullptr, nullptr, mx, boff,
+                                                       xoff, ibase, k2base, tiles, blob, faceX,
+                                                       rt_ptr<int32_t>(c, lay.k2cell), rt_ptr<int32_t>(c, lay.k2off));
+    k_tile_rows<<<(unsigned)c->T, TILE_BT, 0, st>>>(best, tiles, blob, ibase, faceX, rt_ptr<int32_t>(c, lay.k2row));
+    // (tsize is dead after the scan: reuse its first words for the halo total)
+    RT_CUDA(c, cudaMemsetAsync(tsize, 0, 16, st));
+    k_tile_totals<<<nblk(c->T), SETUP_BLOCK, 0, st>>>(c->T, tiles, (unsigned long long *)tsize);
+    int64_t tot[2] = {0, 0};
+    RT_CUDA(c, cudaMemcpyAsync(tot, tsize, 16, cudaMemcpyDeviceToHost, st));
+    RT_CUDA(c, cudaStreamSynchronize(st));
+    c->nhalo = tot[1];
   }
   if (m->nghost > 0)
     RT_CUDA(c, cudaMemcpyAsync(rt_ptr<double>(c, lay.ghost), m->ghost_state, sizeof(double) * m->nghost * 4 * c->G,
@@ -415,18 +596,29 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G) {
   l.faceC = take(32 * F); l.faceN = take(32 * F); l.faceW = take(32 * F);
   l.L = take(4 * F); l.R = take(4 * F);
   l.fo = take(8 * (C + 1)); l.ro = take(8 * (C + 1)); l.rl = take(4 * F); l.rn = take(4 * F);
-  l.hl = take(4 * F); l.incf = take(4 * F); l.inco = take(8 * (l.max_tiles + 2));
+  // tile tables: descriptors for the smallest tile size; blobs bounded by
+  // sum_t (TC + 4) + half-faces (<= 2F) + slots (<= 2F) + halo (<= 2F) + incoming (<= F) words
+  l.tiles = take(sizeof(rt_tile) * (size_t)(l.max_tiles + 1));
+  l.blob_bytes = 4 * (8 * (size_t)F + 2 * (size_t)C + 5 * (size_t)l.max_tiles + 2048);
+  l.blob = take(l.blob_bytes);
+  // fluxes of the faces that cross tile boundaries, written by the owner tile (<= 60 % of the
+  // faces; rt_mesh_upload fails with RT_ENOMEM on a mesh whose tiles need more)
+  l.xcap = (int64_t)(0.6 * (double)F) + 1024;
+  l.xphi = take(32 * (size_t)G * (size_t)l.xcap);
+  // cells with incoming faces and the xphi rows of those faces (k_finish)
+  l.k2cell = take(4 * (size_t)C); l.k2off = take(4 * ((size_t)C + 1)); l.k2row = take(4 * (size_t)l.xcap);
   l.ghost = take(8 * 4 * RT_MAXG * 64);
   l.led = take(sizeof(rt_dev_ledger));
   l.temp = o;
   l.Ua = take(32 * (size_t)G * C); l.Ub = take(32 * (size_t)G * C);
   l.grad = take(96 * (size_t)G * C);
+  l.pacc = take(32 * (size_t)G * C);  // partial flux sums of the cells with incoming faces
   l.xHII = take(8 * C); l.xHeII = take(8 * C); l.xHeIII = take(8 * C); l.eth = take(8 * C); l.nH = take(8 * C);
   l.kappa = take(8 * C);
-  l.srcidx = take(4 * C);
+  l.srcidx = take(4 * C + 64);  // (+ padding: the tile kernels copy whole 16-byte chunks)
   l.srcrate = take(8 * (size_t)G * 65536);
   // partial sums: chem absorbed [<= 4 nbc + 1][G]; per tile: floor, outflow, inflow [max_tiles][G] each
-  l.part = take(8 * (size_t)G * (5 * l.nbc + 3 * l.max_tiles + 16));
+  l.part = take(8 * (size_t)G * (5 * l.nbc + 3 * l.max_tiles + (size_t)G * l.nbc + 32));
   l.scratch_end = o;
   // setup scratch aliases the state region; make sure it fits (incl. staging of a host mesh)
   int64_t NM = C > F ? C : F;

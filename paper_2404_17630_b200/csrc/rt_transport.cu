@@ -22,6 +22,8 @@ __device__ __forceinline__ double4 ld4(const double *p) { return *reinterpret_ca
 __device__ __forceinline__ void st4(double *p, double a, double b, double c, double d) {
   *reinterpret_cast<double4 *>(p) = make_double4(a, b, c, d);
 }
+// x with its sign bit xor-ed with sgn (0 or 0x80000000): an integer operation, not an fp64 multiply
+__device__ __forceinline__ double flip_sign(double x, int sgn) { return __hiloint2double(__double2hiint(x) ^ sgn, __double2loint(x)); }
 __device__ __forceinline__ double dmax2(double a, double b) { return a > b ? a : b; }
 __device__ __forceinline__ double dmin2(double a, double b) { return a < b ? a : b; }
 
@@ -72,84 +74,124 @@ __device__ __forceinline__ double block_sum(double v, double *red) {
   return t;
 }
 
-// per-tile face-list tables staged in shared memory: local cell x has the half-faces
-// hl[ho[x]..ho[x+1]]: slot number, bit 15 set where the cell is the face's right cell
-struct tile_tables { int *ho; uint16_t *hl; };
-__device__ __forceinline__ tile_tables stage_tables(const rt_geom &m, unsigned char *base, int64_t c0, int ncell) {
-  tile_tables t;
-  t.ho = reinterpret_cast<int *>(base);
-  t.hl = reinterpret_cast<uint16_t *>(t.ho + (m.TC + 1));
-  const int64_t hbase = m.fo[c0] + m.ro[c0];
-  for (int x = threadIdx.x; x <= ncell; x += blockDim.x) t.ho[x] = (int)(m.fo[c0 + x] + m.ro[c0 + x] - hbase);
-  const int nh = (int)(m.fo[c0 + ncell] + m.ro[c0 + ncell] - hbase);
-  const uint16_t *src = m.hl + hbase;
-  for (int k = threadIdx.x; k < nh; k += blockDim.x) t.hl[k] = src[k];
-  return t;
+// asynchronous 16-byte global -> shared copies (LDGSTS) for the gathers: the data never passes
+// through registers, so one thread keeps many copies in flight; they bypass L1
+__device__ __forceinline__ void cp16(void *dst, const void *src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+// n consecutive 16-byte chunks
+template <int N>
+__device__ __forceinline__ void cp_run(double *dst, const double *src) {
+#pragma unroll
+  for (int c = 0; c < N; c++) cp16(dst + 2 * c, src + 2 * c);
 }
 
-// min-image of a face-centre offset: |d| < 1.5 L always (the face touches the cell)
-__device__ __forceinline__ double wrap1(double d, double L, int per) {
-  const double h = 0.5 * L;
-  const double w = d > h ? d - L : (d < -h ? d + L : d);
-  return per ? w : d;
+// bulk asynchronous global -> shared copies (TMA, cp.async.bulk) for the long contiguous runs: one instruction moves a whole
+// contiguous run (16-byte aligned, a multiple of 16 bytes) and reports to an mbarrier, so staging a
+// tile costs a handful of instructions instead of one per 16 bytes
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+// one arrival that also announces `bytes` of bulk copies still to land in this phase
+__device__ __forceinline__ void mbar_expect(uint64_t *bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@!p bra WAIT_%=;\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar) {
+  if (bytes == 0) return;
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+// a tile's blob in shared memory (layout: rt_internal.cuh)
+struct tile_view {
+  int64_t c0, fbase, xbase;
+  int ncell, nown, ninc, ns, nh, nhf, nb, nout, words;
+  const uint32_t *ho, *hl, *slr, *halo, *incf, *outs;  // in shared memory
+  const uint32_t *blob;                                // in global memory
+};
+__device__ __forceinline__ tile_view view_tile(const rt_geom &m, const uint32_t *sB, unsigned tile) {
+  const rt_tile d = m.tiles[tile];
+  tile_view v;
+  v.c0 = (int64_t)tile * m.TC;
+  v.ncell = (int)(v.c0 + m.TC < m.C ? m.TC : m.C - v.c0);
+  v.fbase = d.fbase; v.xbase = d.xbase; v.nown = d.nown; v.ninc = d.ninc; v.ns = d.nown + d.ninc; v.nh = d.nh; v.nhf = d.nhf;
+  v.nb = d.nb; v.nout = d.nout;
+  v.words = rt_blob_words(m.TC, v.nhf, v.nown, v.nh, v.ninc, v.nout);
+  v.ho = sB; v.hl = v.ho + m.TC + 1; v.slr = v.hl + v.nhf; v.halo = v.slr + v.nown; v.incf = v.halo + v.nh;
+  v.outs = v.incf + v.ninc;
+  v.blob = m.blob + d.blob;
+  return v;
 }
 
 // ------------------------------------------------------------------ a2: gradients + limiter
 template <int G>
 __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restrict__ U, double *__restrict__ grad) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double *sW = reinterpret_cast<double *>(smem_raw);  // [smax][4]  (w, L|R)
-  double *sC = sW + 4 * m.smax;                       // [smax][4]  (c, A)
-  double *sU = sC + 4 * m.smax;                       // [TC][G][4]
-  const int64_t C = m.C;
-  const int64_t c0 = (int64_t)blockIdx.x * m.TC;
-  const int ncell = (int)(c0 + m.TC < C ? m.TC : C - c0);
-  const int64_t fbase = m.fo[c0];
-  const int nown = (int)(m.fo[c0 + ncell] - fbase);
-  const int64_t ib = m.inco[blockIdx.x];
-  const int ns = nown + (int)(m.inco[blockIdx.x + 1] - ib);
-  // stage the slot records, the tile's U and the face-list tables
-  for (int s = threadIdx.x; s < ns; s += blockDim.x) {
-    const int64_t q = s < nown ? fbase + s : (int64_t)m.incf[ib + (s - nown)];
-    *reinterpret_cast<double4 *>(sW + 4 * s) = ld4(m.faceW + 4 * q);
-    *reinterpret_cast<double4 *>(sC + 4 * s) = ld4(m.faceC + 4 * q);
+  __shared__ __align__(8) uint64_t bar;
+  uint32_t *sB = reinterpret_cast<uint32_t *>(smem_raw);  // the tile's blob
+  double *sW = reinterpret_cast<double *>(sB + m.bmax);   // [smax][4]  (w, kappa)
+  double *sC = sW + 4 * m.smax;                           // [smax][4]  (c - s_L, A)
+  double *sU = sC + 4 * m.smax;                           // [(TC + hmax) G][4]  tile cells, then halo cells
+  double *sM = sU + 4 * G * (m.TC + m.hmax);              // [TC][6]
+  const tile_view v = view_tile(m, sB, blockIdx.x);
+  const int tid = threadIdx.x, nt = blockDim.x;
+  if (tid == 0) mbar_init(&bar, 1);
+  __syncthreads();
+  // round 1: what the descriptor locates: the blob, the owned faces and the tile's own cells
+  if (tid == 0) {
+    mbar_expect(&bar, 4u * v.words + 64u * v.nown + (32u * G + 48u) * v.ncell);
+    bulk_g2s(sB, v.blob, 4u * v.words, &bar);
+    bulk_g2s(sW, m.faceW + 4 * v.fbase, 32u * v.nown, &bar);
+    bulk_g2s(sC, m.faceC + 4 * v.fbase, 32u * v.nown, &bar);
+    bulk_g2s(sU, U + 4 * G * v.c0, 32u * G * v.ncell, &bar);
+    bulk_g2s(sM, m.Minv + 6 * v.c0, 48u * v.ncell, &bar);
   }
-  {
-    const double *Ut = U + 4 * c0 * G;
-    for (int x = threadIdx.x; x < ncell * G; x += blockDim.x) *reinterpret_cast<double4 *>(sU + 4 * x) = ld4(Ut + 4 * x);
+  mbar_wait(&bar, 0);
+  // round 2: what the blob locates: halo cells and incoming faces
+  // (gathers of 32 to 96 bytes: 16-byte asynchronous copies, one halo cell / incoming face per thread)
+  for (int h = tid; h < v.nh; h += nt) cp_run<2 * G>(sU + 4 * G * (m.TC + h), U + (int64_t)(4 * G) * v.halo[h]);
+  for (int j = tid; j < v.ninc; j += nt) {
+    const int64_t q = v.incf[j];
+    cp_run<2>(sW + 4 * (v.nown + j), m.faceW + 4 * q);
+    cp_run<2>(sC + 4 * (v.nown + j), m.faceC + 4 * q);
   }
-  const tile_tables tt = stage_tables(m, reinterpret_cast<unsigned char *>(sU + 4 * m.TC * G), c0, ncell);
+  cp_wait_all();
   __syncthreads();
 
-  const int32_t c0i = (int32_t)c0;
-  for (int item = threadIdx.x; item < ncell * G; item += blockDim.x) {
+  for (int item = tid; item < v.ncell * G; item += nt) {
     const int il = item / G, g = item - il * G;
-    const int64_t i = c0 + il;
     const double4 Ui = ld4(sU + 4 * item);
     double b[4][3], hi[4] = {Ui.x, Ui.y, Ui.z, Ui.w}, lo[4] = {Ui.x, Ui.y, Ui.z, Ui.w};
 #pragma unroll
-    for (int v = 0; v < 4; v++) b[v][0] = b[v][1] = b[v][2] = 0.0;
-    const int h0 = tt.ho[il], h1 = tt.ho[il + 1];
-    const double *Ug = U + 4 * g;  // neighbour j outside the tile: Ug + 4 G j
-
+    for (int w = 0; w < 4; w++) b[w][0] = b[w][1] = b[w][2] = 0.0;
+    const int h0 = (int)v.ho[il], h1 = (int)v.ho[il + 1];
+    const double *Ug = sU + 4 * g;
     // first pass over the cell's half-faces: sum_f w_f (phi_j - phi_i), min/max.  Where the cell is
-    // the face's right cell, d = s_L - s_R: the stored prefactor changes sign, the neighbour is L.
+    // the face's right cell, d = s_L - s_R: the stored prefactor changes sign.
 #pragma unroll 2
     for (int k = h0; k < h1; k++) {
-      const unsigned e = tt.hl[k];
+      const uint32_t e = v.hl[k];
       const int s = (int)(e & 0x7fffu);
-      const bool right = e >= 0x8000u;
+      const uint32_t nb = e >> 16;
+      const int sgn = (int)((e & 0x8000u) << 16);  // sign bit where the cell is the right one
       const double4 w = ld4(sW + 4 * s);
-      int32_t l, r;
-      rt_unpack_lr(w.w, l, r);
-      const int32_t j = right ? l : r;
-      const double sg = right ? -1.0 : 1.0;
       double4 Uj;
-      if (j >= 0) {
-        const unsigned jl = (unsigned)(j - c0i);
-        Uj = ld4(jl < (unsigned)ncell ? sU + 4 * ((int)jl * G + g) : Ug + (int64_t)(4 * G) * j);
-      } else Uj = ghost_for_gradient(j, Ui, m.faceN, fbase + s, m.ghost, G, g);
-      const double wx = sg * w.x, wy = sg * w.y, wz = sg * w.z;
+      if (nb < 0xFF00u) Uj = ld4(Ug + 4 * G * (int)nb);
+      else Uj = ghost_for_gradient((int)nb - 0x10000, Ui, m.faceN, v.fbase + s, m.ghost, G, g);
+      const double wx = flip_sign(w.x, sgn), wy = flip_sign(w.y, sgn), wz = flip_sign(w.z, sgn);
       const double d0 = Uj.x - Ui.x, d1 = Uj.y - Ui.y, d2 = Uj.z - Ui.z, d3 = Uj.w - Ui.w;
       b[0][0] += wx * d0; b[0][1] += wy * d0; b[0][2] += wz * d0;
       b[1][0] += wx * d1; b[1][1] += wy * d1; b[1][2] += wz * d1;
@@ -158,41 +200,42 @@ __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restric
       hi[0] = dmax2(hi[0], Uj.x); hi[1] = dmax2(hi[1], Uj.y); hi[2] = dmax2(hi[2], Uj.z); hi[3] = dmax2(hi[3], Uj.w);
       lo[0] = dmin2(lo[0], Uj.x); lo[1] = dmin2(lo[1], Uj.y); lo[2] = dmin2(lo[2], Uj.z); lo[3] = dmin2(lo[3], Uj.w);
     }
-    const double *Mi = m.Minv + 6 * i;
+    const double *Mi = sM + 6 * il;
     const double m00 = Mi[0], m01 = Mi[1], m02 = Mi[2], m11 = Mi[3], m12 = Mi[4], m22 = Mi[5];
     double gr[4][3];
 #pragma unroll
-    for (int v = 0; v < 4; v++) {
-      gr[v][0] = m00 * b[v][0] + m01 * b[v][1] + m02 * b[v][2];
-      gr[v][1] = m01 * b[v][0] + m11 * b[v][1] + m12 * b[v][2];
-      gr[v][2] = m02 * b[v][0] + m12 * b[v][1] + m22 * b[v][2];
+    for (int w = 0; w < 4; w++) {
+      gr[w][0] = m00 * b[w][0] + m01 * b[w][1] + m02 * b[w][2];
+      gr[w][1] = m01 * b[w][0] + m11 * b[w][1] + m12 * b[w][2];
+      gr[w][2] = m02 * b[w][0] + m12 * b[w][1] + m22 * b[w][2];
     }
     // second pass: extreme extrapolated increments at the face centres.  min_f (hi-phi)/D_f is
     // attained at the largest D_f (division is monotone), so only the extremes are kept.
-    const double4 si = ld4(m.cellS + 4 * i);
+    // The stored face centre is relative to the left cell; seen from the right cell it is
+    // c - d with d = kappa w (rt_internal.cuh).
     double dmax[4] = {0, 0, 0, 0}, dmin[4] = {0, 0, 0, 0};
-    // (the stored face centre is in the left cell's frame: min-image it for the right cell;
-    // for the left cell the wrap is the identity)
 #pragma unroll 2
     for (int k = h0; k < h1; k++) {
-      const double4 c = ld4(sC + 4 * (int)(tt.hl[k] & 0x7fffu));
-      const double rx = wrap1(c.x - si.x, m.box[0], m.per[0]), ry = wrap1(c.y - si.y, m.box[1], m.per[1]),
-                   rz = wrap1(c.z - si.z, m.box[2], m.per[2]);
+      const uint32_t e = v.hl[k];
+      const int s = (int)(e & 0x7fffu);
+      const double4 c = ld4(sC + 4 * s), w = ld4(sW + 4 * s);
+      const double kr = (e & 0x8000u) ? -w.w : 0.0;
+      const double rx = fma(kr, w.x, c.x), ry = fma(kr, w.y, c.y), rz = fma(kr, w.z, c.z);
 #pragma unroll
-      for (int v = 0; v < 4; v++) {
-        const double d = gr[v][0] * rx + gr[v][1] * ry + gr[v][2] * rz;
-        dmax[v] = dmax2(dmax[v], d); dmin[v] = dmin2(dmin[v], d);
+      for (int f = 0; f < 4; f++) {
+        const double d = gr[f][0] * rx + gr[f][1] * ry + gr[f][2] * rz;
+        dmax[f] = dmax2(dmax[f], d); dmin[f] = dmin2(dmin[f], d);
       }
     }
-    double *out = grad + 12 * (i * G + g);
+    double *out = grad + 12 * ((v.c0 + il) * G + g);
     const double Uiv[4] = {Ui.x, Ui.y, Ui.z, Ui.w};
     double o[12];
 #pragma unroll
-    for (int v = 0; v < 4; v++) {
+    for (int w = 0; w < 4; w++) {
       double a = 1.0;
-      if (dmax[v] > 0.0) a = dmin2(a, (hi[v] - Uiv[v]) / dmax[v]);
-      if (dmin[v] < 0.0) a = dmin2(a, (lo[v] - Uiv[v]) / dmin[v]);
-      o[3 * v] = a * gr[v][0]; o[3 * v + 1] = a * gr[v][1]; o[3 * v + 2] = a * gr[v][2];
+      if (dmax[w] > 0.0) a = dmin2(a, (hi[w] - Uiv[w]) / dmax[w]);
+      if (dmin[w] < 0.0) a = dmin2(a, (lo[w] - Uiv[w]) / dmin[w]);
+      o[3 * w] = a * gr[w][0]; o[3 * w + 1] = a * gr[w][1]; o[3 * w + 2] = a * gr[w][2];
     }
     st4(out, o[0], o[1], o[2], o[3]); st4(out + 4, o[4], o[5], o[6], o[7]); st4(out + 8, o[8], o[9], o[10], o[11]);
   }
@@ -216,10 +259,10 @@ __device__ __forceinline__ void pressure_dot_n(const double U[4], const double n
 }
 
 // U_face = U_i + grad U_i . r  (linear extrapolation to the centre of the interface)
-// pu: the cell's (N, Fx, Fy, Fz); pg: its 12 gradient components (field-major); shared or global
+// rec: the cell's (N, Fx, Fy, Fz) followed by its 12 gradient components (field-major), in shared memory
 template <bool SECOND>
-__device__ __forceinline__ void extrapolate(const double *pu, const double *pg, double rx, double ry, double rz,
-                                            double Uo[4], double &Ncentre) {
+__device__ __forceinline__ void extrapolate(const double *pu, const double *pg, double rx, double ry, double rz, double Uo[4],
+                                            double &Ncentre) {
   const double4 u = ld4(pu);
   Ncentre = u.x;
   Uo[0] = u.x; Uo[1] = u.y; Uo[2] = u.z; Uo[3] = u.w;
@@ -232,163 +275,251 @@ __device__ __forceinline__ void extrapolate(const double *pu, const double *pg, 
   }
 }
 
+// the end of a4 for one (cell, group): a = sum_f s_if A_f Phi_f; source, Heun combine, floor, |F| <= c~ N
+// (S3, S5, S11, S12).  Returns the photons the floor added (0 if none).
+struct update_par { double ca, cb, dt, ct, n_floor; };
+__device__ __forceinline__ double finish_cell(double a0, double a1, double a2, double a3, double V, double src,
+                                              const double4 uc, const double4 u0, const update_par &p, double *out) {
+  const double kk = p.dt * fast_rcp(V);  // dt / V
+  a0 -= src;                              // isotropic source (S5): + dt Ndot / V on N
+  double Un[4] = {p.ca * u0.x + p.cb * fma(-kk, a0, uc.x), p.ca * u0.y + p.cb * fma(-kk, a1, uc.y),
+                  p.ca * u0.z + p.cb * fma(-kk, a2, uc.z), p.ca * u0.w + p.cb * fma(-kk, a3, uc.w)};
+  double add = 0.0;
+  if (Un[0] < p.n_floor) { add = V * (p.n_floor - Un[0]); Un[0] = p.n_floor; }
+  const double f2 = Un[1] * Un[1] + Un[2] * Un[2] + Un[3] * Un[3], lim = p.ct * Un[0];
+  if (f2 > lim * lim) { const double sc = lim / sqrt(f2); Un[1] *= sc; Un[2] *= sc; Un[3] *= sc; }
+  st4(out, Un[0], Un[1], Un[2], Un[3]);
+  return add;
+}
+
 template <int G, bool SECOND>
-__global__ void __launch_bounds__(256) k_stage(rt_geom m, const double *__restrict__ Uin, const double *__restrict__ grad,
-                                               const double *U0, double *Uout, const int32_t *__restrict__ srcidx,
-                                               const double *__restrict__ srcrate, int nsrc, double ca, double cb, double dt,
-                                               double ct, double n_floor, double *__restrict__ part_floor,
-                                               double *__restrict__ part_out, double *__restrict__ part_in) {
+__global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__restrict__ Uin, const double *__restrict__ grad,
+                                                 const double *U0, double *Uout, const int32_t *__restrict__ srcidx,
+                                                 const double *__restrict__ srcrate, int nsrc, update_par up,
+                                                 double *__restrict__ pacc, double *__restrict__ part_floor,
+                                                 double *__restrict__ part_out, double *__restrict__ part_in) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ double red[32];
-  constexpr int PS = 4 * G > 8 ? 4 * G : 8;             // doubles per slot
-  double *sPhi = reinterpret_cast<double *>(smem_raw);  // [smax][PS]: the staged face record (c, A), (n, L|R),
-                                                        // overwritten by its owner thread with A * (Phi_N, Phi_F)[G]
-  double *sR = sPhi + PS * m.smax;                      // [TC][G][RT_REC]  U (4) + gradients (12)
-  double *sS = sR + RT_REC * G * m.TC;                  // [TC][4]  (s, V)
-  const int64_t C = m.C;
-  const int64_t c0 = (int64_t)blockIdx.x * m.TC;
-  const int ncell = (int)(c0 + m.TC < C ? m.TC : C - c0);
-  const int64_t fbase = m.fo[c0];
-  const int nown = (int)(m.fo[c0 + ncell] - fbase);
-  const int64_t ib = m.inco[blockIdx.x];
-  const int ns = nown + (int)(m.inco[blockIdx.x + 1] - ib);
-  // stage the face records, the tile's cells and the face-list tables
-  for (int s = threadIdx.x; s < ns; s += blockDim.x) {
-    const int64_t q = s < nown ? fbase + s : (int64_t)m.incf[ib + (s - nown)];
-    *reinterpret_cast<double4 *>(sPhi + PS * s) = ld4(m.faceC + 4 * q);
-    *reinterpret_cast<double4 *>(sPhi + PS * s + 4) = ld4(m.faceN + 4 * q);
+  __shared__ __align__(8) uint64_t bar;
+  constexpr int NP = G > 3 ? G : 3;                        // planes of [omax][4]
+  const int NE = m.TC + m.fmax;                            // tile cells, then forward halo cells
+  const int OM = m.omax;
+  uint32_t *sB = reinterpret_cast<uint32_t *>(smem_raw);   // the tile's blob
+  double *sF = reinterpret_cast<double *>(sB + m.bmax);    // [NP][omax][4]: planes 0-2 hold the staged face records
+                                                           // (c, A), (n, -), (w, kappa); a slot's warp then
+                                                           // overwrites plane g with A * (Phi_N, Phi_F) of group g
+  double *sU = sF + 4 * NP * OM;                           // [NE][G][4]
+  double *sG = sU + 4 * G * NE;                            // [NE][G][12]
+  double *sS = sG + 12 * G * NE;                           // [NE][4]  (s, V)
+  double *sU0 = sS + 4 * NE;                               // [TC][G][4]  U^n of the tile's cells
+  int32_t *sSrc = reinterpret_cast<int32_t *>(sU0 + 4 * G * m.TC);  // [TC] source index or -1
+  const unsigned tile = blockIdx.x;
+  const tile_view v = view_tile(m, sB, tile);
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const double dt = up.dt, ct = up.ct;
+  if (tid == 0) mbar_init(&bar, 1);
+  __syncthreads();
+  // round 1: what the descriptor locates: the blob, the owned faces and the tile's own cells
+  if (tid == 0) {
+    const unsigned nsb = (4u * v.ncell + 15u) & ~15u;  // srcidx is padded
+    mbar_expect(&bar, 4u * v.words + 96u * v.nown + ((SECOND ? 128u : 32u) * G + 32u + 32u * G) * v.ncell + nsb);
+    bulk_g2s(sB, v.blob, 4u * v.words, &bar);
+    bulk_g2s(sF, m.faceC + 4 * v.fbase, 32u * v.nown, &bar);
+    bulk_g2s(sF + 4 * OM, m.faceN + 4 * v.fbase, 32u * v.nown, &bar);
+    bulk_g2s(sF + 8 * OM, m.faceW + 4 * v.fbase, 32u * v.nown, &bar);
+    bulk_g2s(sU, Uin + 4 * G * v.c0, 32u * G * v.ncell, &bar);
+    if (SECOND) bulk_g2s(sG, grad + 12 * G * v.c0, 96u * G * v.ncell, &bar);
+    bulk_g2s(sS, m.cellS + 4 * v.c0, 32u * v.ncell, &bar);
+    bulk_g2s(sU0, U0 + 4 * G * v.c0, 32u * G * v.ncell, &bar);
+    bulk_g2s(sSrc, srcidx + v.c0, nsb, &bar);
   }
-  {
-    const double *Ut = Uin + 4 * c0 * G, *gt = grad + 12 * c0 * G;
-    for (int x = threadIdx.x; x < ncell * G; x += blockDim.x) *reinterpret_cast<double4 *>(sR + RT_REC * x) = ld4(Ut + 4 * x);
-    if (SECOND)
-      for (int u = threadIdx.x; u < ncell * G * 3; u += blockDim.x) {
-        const int x = u / 3, part = u - 3 * x;
-        *reinterpret_cast<double4 *>(sR + RT_REC * x + 4 + 4 * part) = ld4(gt + 4 * u);
-      }
-    const double *St = m.cellS + 4 * c0;
-    for (int x = threadIdx.x; x < ncell; x += blockDim.x) *reinterpret_cast<double4 *>(sS + 4 * x) = ld4(St + 4 * x);
+  mbar_wait(&bar, 0);
+  // round 2: what the blob locates: the forward halo cells (right cells of the outgoing faces)
+  const int nf = v.nh - v.nb;
+  // (gathers of 32 to 288 bytes: 16-byte asynchronous copies; a halo cell's gradients are split over G threads)
+  for (int k = tid; k < nf * (G + 1); k += nt) {
+    const int h = k / (G + 1), part = k - h * (G + 1);
+    const int64_t id = v.halo[v.nb + h];
+    if (part < G) {
+      if (SECOND) cp_run<6>(sG + 12 * (G * (m.TC + h) + part), grad + 12 * (G * id + part));
+    } else {
+      cp_run<2 * G>(sU + 4 * G * (m.TC + h), Uin + (int64_t)(4 * G) * id);
+      cp_run<2>(sS + 4 * (m.TC + h), m.cellS + 4 * id);
+    }
   }
-  const tile_tables tt = stage_tables(m, reinterpret_cast<unsigned char *>(sS + 4 * m.TC), c0, ncell);
+  cp_wait_all();
   __syncthreads();
 
-  // ---- a3: one thread per face slot, all groups
-  double b_out[G], b_in[G];
-#pragma unroll
-  for (int g = 0; g < G; g++) b_out[g] = b_in[g] = 0.0;
+  // ---- a3: one lane per (face slot, group); a slot's groups sit in one warp, which reads the staged
+  // face record before any of its lanes overwrites it with the fluxes
+  constexpr int SPW = 32 / G;  // slots per warp pass
+  const int lane = tid & 31, warp = tid >> 5, nw = nt >> 5;
+  const int sl = lane / G, g = lane - sl * G;
+  double b_out = 0.0, b_in = 0.0;
   int bnd = 0;
   const double hc2 = 0.5 * ct * ct, hc = 0.5 * ct;
-  const int32_t c0i = (int32_t)c0;
-  for (int s = threadIdx.x; s < ns; s += blockDim.x) {
-    const double4 fc = ld4(sPhi + PS * s), fn = ld4(sPhi + PS * s + 4);
-    int32_t l, r;
-    rt_unpack_lr(fn.w, l, r);
+  for (int sb = warp * SPW; sb < v.nown; sb += nw * SPW) {
+    const int s = sb + sl;
+    const bool on = sl < SPW && s < v.nown;
+    double4 fc = make_double4(0, 0, 0, 1), fn = make_double4(0, 0, 0, 0), fw = make_double4(0, 0, 0, 0);
+    uint32_t lr = 0;
+    if (on) { fc = ld4(sF + 4 * s); fn = ld4(sF + 4 * (OM + s)); fw = ld4(sF + 4 * (2 * OM + s)); lr = v.slr[s]; }
+    __syncwarp();
+    if (!on) continue;
+    const int xl = (int)(lr & 0xffffu);
+    int xr = (int)(lr >> 16);
+    const bool rin = xr < 0xFF00;
+    if (rin && xr >= m.TC) xr -= v.nb;  // forward halo cells follow the tile's cells in sU / sG / sS
+    const int r = rin ? 0 : xr - 0x10000;  // boundary code (negative) where the face has no right cell
     const double n[3] = {fn.x, fn.y, fn.z};
     const double A = fc.w;
-    const unsigned ll = (unsigned)(l - c0i), rl = (unsigned)(r - c0i);
-    const bool l_in = ll < (unsigned)ncell, r_in = rl < (unsigned)ncell;  // r < 0 gives a huge rl
-    // per-group rows of the two cells: shared memory for tile cells, global memory for the halo
-    const double *puL = l_in ? sR + RT_REC * G * (int)ll : Uin + (int64_t)(4 * G) * l;
-    const double *pgL = l_in ? puL + 4 : grad + (int64_t)(12 * G) * l;
-    const int suL = l_in ? RT_REC : 4, sgL = l_in ? RT_REC : 12;
-    const double4 sl = ld4(l_in ? sS + 4 * (int)ll : m.cellS + 4 * (int64_t)l);
-    const double rLx = fc.x - sl.x, rLy = fc.y - sl.y, rLz = fc.z - sl.z;
-    const int rr = r >= 0 ? r : 0;
-    const double *puR = r_in ? sR + RT_REC * G * (int)rl : Uin + (int64_t)(4 * G) * rr;
-    const double *pgR = r_in ? puR + 4 : grad + (int64_t)(12 * G) * rr;
-    const int suR = r_in ? RT_REC : 4, sgR = r_in ? RT_REC : 12;
-    double rRx = 0.0, rRy = 0.0, rRz = 0.0, Vr = 0.0;
-    if (r >= 0) {
-      const double4 sr = ld4(r_in ? sS + 4 * (int)rl : m.cellS + 4 * (int64_t)r);
-      Vr = sr.w;
-      rRx = wrap1(fc.x - sr.x, m.box[0], m.per[0]); rRy = wrap1(fc.y - sr.y, m.box[1], m.per[1]);
-      rRz = wrap1(fc.z - sr.z, m.box[2], m.per[2]);
-    }
     const double rdtA = fast_rcp(dt * A);
-    const double capL = sl.w * rdtA, capR = Vr * rdtA;
+    const double capL = sS[4 * xl + 3] * rdtA;
+    double UL[4], UR[4], NL, NR = 0.0, capR = 0.0;
+    // the face centre relative to the left cell is stored; relative to the right cell it is c - kappa w
+    extrapolate<SECOND>(sU + 4 * (xl * G + g), sG + 12 * (xl * G + g), fc.x, fc.y, fc.z, UL, NL);
+    if (rin) {
+      capR = sS[4 * xr + 3] * rdtA;
+      const double rRx = fma(-fw.w, fw.x, fc.x), rRy = fma(-fw.w, fw.y, fc.y), rRz = fma(-fw.w, fw.z, fc.z);
+      extrapolate<SECOND>(sU + 4 * (xr * G + g), sG + 12 * (xr * G + g), rRx, rRy, rRz, UR, NR);
+    } else if (r == RT_BC_OUTFLOW) { UR[0] = UR[1] = UR[2] = UR[3] = 0.0; }  // vacuum ghost
+    else if (r == RT_BC_REFLECT) {
+      const double p = 2.0 * (UL[1] * n[0] + UL[2] * n[1] + UL[3] * n[2]);
+      UR[0] = UL[0]; UR[1] = UL[1] - p * n[0]; UR[2] = UL[2] - p * n[1]; UR[3] = UL[3] - p * n[2];
+    } else {
+      const double4 gs = ld4(m.ghost + ((size_t)(RT_BC_DIRICHLET0 - r) * G + g) * 4);
+      UR[0] = gs.x; UR[1] = gs.y; UR[2] = gs.z; UR[3] = gs.w;
+    }
+    double PL[3], PR[3], ph[4];
+    pressure_dot_n(UL, n, ct, PL);
+    pressure_dot_n(UR, n, ct, PR);
+    ph[0] = 0.5 * ((UL[1] + UR[1]) * n[0] + (UL[2] + UR[2]) * n[1] + (UL[3] + UR[3]) * n[2]) - hc * (UR[0] - UL[0]);
 #pragma unroll
-    for (int g = 0; g < G; g++) {
-      double UL[4], UR[4], NL, NR = 0.0;
-      extrapolate<SECOND>(puL + suL * g, pgL + sgL * g, rLx, rLy, rLz, UL, NL);
-      if (r >= 0) extrapolate<SECOND>(puR + suR * g, pgR + sgR * g, rRx, rRy, rRz, UR, NR);
-      else if (r == RT_BC_OUTFLOW) { UR[0] = UR[1] = UR[2] = UR[3] = 0.0; }  // vacuum ghost
-      else if (r == RT_BC_REFLECT) {
-        const double p = 2.0 * (UL[1] * n[0] + UL[2] * n[1] + UL[3] * n[2]);
-        UR[0] = UL[0]; UR[1] = UL[1] - p * n[0]; UR[2] = UL[2] - p * n[1]; UR[3] = UL[3] - p * n[2];
-      } else {
-        const double4 gs = ld4(m.ghost + ((size_t)(RT_BC_DIRICHLET0 - r) * G + g) * 4);
-        UR[0] = gs.x; UR[1] = gs.y; UR[2] = gs.z; UR[3] = gs.w;
-      }
-      double PL[3], PR[3], ph[4];
-      pressure_dot_n(UL, n, ct, PL);
-      pressure_dot_n(UR, n, ct, PR);
-      ph[0] = 0.5 * ((UL[1] + UR[1]) * n[0] + (UL[2] + UR[2]) * n[1] + (UL[3] + UR[3]) * n[2]) - hc * (UR[0] - UL[0]);
-#pragma unroll
-      for (int a = 0; a < 3; a++) ph[1 + a] = hc2 * (PL[a] + PR[a]) - hc * (UR[1 + a] - UL[1 + a]);
-      // donor cap (S11): the donor cannot lose more photons than it holds through this face in dt;
-      // only the number flux is clamped (continuous in the state; Phi_F is left alone)
-      if (ph[0] > 0.0) ph[0] = dmin2(ph[0], NL * capL);
-      else if (r >= 0) ph[0] = -dmin2(-ph[0], NR * capR);
-      st4(sPhi + PS * s + 4 * g, A * ph[0], A * ph[1], A * ph[2], A * ph[3]);
-      if (r == RT_BC_OUTFLOW) { b_out[g] += A * ph[0]; bnd = 1; }
-      else if (r <= RT_BC_DIRICHLET0) { b_in[g] -= A * ph[0]; bnd = 1; }
+    for (int a = 0; a < 3; a++) ph[1 + a] = hc2 * (PL[a] + PR[a]) - hc * (UR[1 + a] - UL[1 + a]);
+    // donor cap (S11): the donor cannot lose more photons than it holds through this face in dt;
+    // only the number flux is clamped (continuous in the state; Phi_F is left alone)
+    if (ph[0] > 0.0) ph[0] = dmin2(ph[0], NL * capL);
+    else if (rin) ph[0] = -dmin2(-ph[0], NR * capR);
+    st4(sF + 4 * (g * OM + s), A * ph[0], A * ph[1], A * ph[2], A * ph[3]);
+    if (r == RT_BC_OUTFLOW) { b_out += A * ph[0]; bnd = 1; }
+    else if (r <= RT_BC_DIRICHLET0) { b_in -= A * ph[0]; bnd = 1; }
+  }
+  __syncthreads();  // every owned slot holds its fluxes
+  // the outgoing faces' fluxes go to xphi for the tiles of their right cells (k_finish)
+  {
+    double *xo = m.xphi + (size_t)(4 * G) * v.xbase;
+    for (int k = tid; k < 2 * G * v.nout; k += nt) {
+      const int j = k / (2 * G), c = k - j * (2 * G);
+      *reinterpret_cast<double2 *>(xo + 2 * k) =
+          *reinterpret_cast<const double2 *>(sF + 4 * ((c >> 1) * OM + (int)v.outs[j]) + 2 * (c & 1));
     }
   }
-  // boundary ledgers: fixed-order block sums, one row per tile (the barrier also ends phase a3)
+  // boundary ledgers: fixed-order block sums, one row per tile
   if (__syncthreads_or(bnd)) {
 #pragma unroll
-    for (int g = 0; g < G; g++) {
-      const double so = block_sum(b_out[g], red), si = block_sum(b_in[g], red);
-      if (threadIdx.x == 0) { part_out[(size_t)blockIdx.x * G + g] = so; part_in[(size_t)blockIdx.x * G + g] = si; }
+    for (int gg = 0; gg < G; gg++) {
+      const double so = block_sum(g == gg ? b_out : 0.0, red), si = block_sum(g == gg ? b_in : 0.0, red);
+      if (tid == 0) { part_out[(size_t)tile * G + gg] = so; part_in[(size_t)tile * G + gg] = si; }
     }
-  } else if (threadIdx.x < G) {
-    part_out[(size_t)blockIdx.x * G + threadIdx.x] = 0.0;
-    part_in[(size_t)blockIdx.x * G + threadIdx.x] = 0.0;
+  } else if (tid < G) {
+    part_out[(size_t)tile * G + tid] = 0.0;
+    part_in[(size_t)tile * G + tid] = 0.0;
   }
 
-  // ---- a4: one thread per (cell, group): gather the cell's faces in list order, update
+  // ---- a4: P lanes per (cell, group) gather the cell's faces (lane p takes entries p, p + P, ... of
+  // the list, the partial sums are combined in a fixed order).  A cell all of whose faces are the
+  // tile's is updated here; one with incoming faces leaves its partial sum in pacc for k_finish
+  // (Uout may be U^n itself, which k_finish still needs)
   double fl[G];
 #pragma unroll
-  for (int g = 0; g < G; g++) fl[g] = 0.0;
+  for (int gg = 0; gg < G; gg++) fl[gg] = 0.0;
   int floored = 0;
-  for (int item = threadIdx.x; item < ncell * G; item += blockDim.x) {
-    const int il = item / G, g = item - il * G;
-    const int64_t i = c0 + il;
-    const int h0 = tt.ho[il], h1 = tt.ho[il + 1];
-    const double *pg = sPhi + 4 * g;
+  const int P = nt >= 4 * m.TC * G ? 4 : (nt >= 2 * m.TC * G ? 2 : 1);
+  const int nitem = v.ncell * G;
+  for (int base = 0; base < nitem * P; base += nt) {  // (nt is a multiple of 32, P divides 32: whole warps iterate together)
+    const int e = base + tid;
+    const int item = e / P, p = e - item * P;
+    const bool on = item < nitem;
+    const int il = on ? item / G : 0, ig = on ? item - il * G : 0;
+    const int h0 = on ? (int)v.ho[il] : 0, h1 = on ? (int)v.ho[il + 1] : 0;
+    const double *pg = sF + 4 * ig * OM;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-#pragma unroll 4
-    for (int k = h0; k < h1; k++) {
-      const unsigned e = tt.hl[k];
-      const double4 p = ld4(pg + PS * (int)(e & 0x7fffu));
-      const double sg = e >= 0x8000u ? -1.0 : 1.0;  // the flux leaves the left cell and enters the right one
-      a0 = fma(sg, p.x, a0); a1 = fma(sg, p.y, a1); a2 = fma(sg, p.z, a2); a3 = fma(sg, p.w, a3);
+    int incomplete = 0;
+#pragma unroll 2
+    for (int k = h0 + p; k < h1; k += P) {
+      const uint32_t w = v.hl[k];
+      const int s = (int)(w & 0x7fffu);
+      if (s >= v.nown) { incomplete = 1; continue; }  // incoming: its owner tile has the flux
+      const double4 q = ld4(pg + 4 * s);
+      const int sgn = (int)((w & 0x8000u) << 16);  // the flux leaves the left cell and enters the right one
+      a0 += flip_sign(q.x, sgn); a1 += flip_sign(q.y, sgn); a2 += flip_sign(q.z, sgn); a3 += flip_sign(q.w, sgn);
     }
-    const double V = sS[4 * il + 3];
-    const double kk = dt * fast_rcp(V);  // dt / V
-    const int32_t si = srcidx[i];
-    if (si >= 0) a0 -= srcrate[(size_t)g * nsrc + si];  // isotropic source (S5): + dt Ndot / V on N
-    const int64_t o = 4 * (i * G + g);
-    const double4 uc = ld4(sR + RT_REC * item), u0 = ld4(U0 + o);
-    double Un[4] = {ca * u0.x + cb * fma(-kk, a0, uc.x), ca * u0.y + cb * fma(-kk, a1, uc.y),
-                    ca * u0.z + cb * fma(-kk, a2, uc.z), ca * u0.w + cb * fma(-kk, a3, uc.w)};
-    if (Un[0] < n_floor) {
-      const double add = V * (n_floor - Un[0]);
+    for (int o = 1; o < P; o <<= 1) {
+      a0 += __shfl_xor_sync(0xffffffffu, a0, o); a1 += __shfl_xor_sync(0xffffffffu, a1, o);
+      a2 += __shfl_xor_sync(0xffffffffu, a2, o); a3 += __shfl_xor_sync(0xffffffffu, a3, o);
+      incomplete |= __shfl_xor_sync(0xffffffffu, incomplete, o);
+    }
+    if (!on || p != 0) continue;
+    if (incomplete) { st4(pacc + 4 * (v.c0 * G + item), a0, a1, a2, a3); continue; }
+    const int32_t si = sSrc[il];
+    const double src = si >= 0 ? srcrate[(size_t)ig * nsrc + si] : 0.0;
+    const double add = finish_cell(a0, a1, a2, a3, sS[4 * il + 3], src, ld4(sU + 4 * item), ld4(sU0 + 4 * item), up,
+                                   Uout + 4 * (v.c0 * G + item));
+    if (add != 0.0) {
 #pragma unroll
-      for (int gg = 0; gg < G; gg++) if (gg == g) fl[gg] += add;
-      Un[0] = n_floor; floored = 1;
+      for (int gg = 0; gg < G; gg++) if (gg == ig) fl[gg] += add;
+      floored = 1;
     }
-    const double f2 = Un[1] * Un[1] + Un[2] * Un[2] + Un[3] * Un[3], lim = ct * Un[0];
-    if (f2 > lim * lim) { const double sc = lim / sqrt(f2); Un[1] *= sc; Un[2] *= sc; Un[3] *= sc; }
-    st4(Uout + o, Un[0], Un[1], Un[2], Un[3]);
   }
   if (__syncthreads_or(floored)) {
 #pragma unroll
-    for (int g = 0; g < G; g++) {
-      const double t = block_sum(fl[g], red);
-      if (threadIdx.x == 0) part_floor[(size_t)blockIdx.x * G + g] = t;
+    for (int gg = 0; gg < G; gg++) {
+      const double t = block_sum(fl[gg], red);
+      if (tid == 0) part_floor[(size_t)tile * G + gg] = t;
     }
-  } else if (threadIdx.x < G) part_floor[(size_t)blockIdx.x * G + threadIdx.x] = 0.0;
+  } else if (tid < G) part_floor[(size_t)tile * G + tid] = 0.0;
+}
+
+// a4 for the cells with incoming faces: pacc holds their partial sums (k_flux); subtract the
+// incoming fluxes (the cell is their right cell) in list order and finish the update.
+// One thread per (cell, group); part_floor: one row per block.
+#define RT_FIN_BLOCK 128
+template <int G>
+__global__ void __launch_bounds__(RT_FIN_BLOCK) k_finish(int64_t n2, const int32_t *__restrict__ k2cell,
+                                                         const int32_t *__restrict__ k2off, const int32_t *__restrict__ k2row,
+                                                         const double *__restrict__ xphi, const double *__restrict__ pacc,
+                                                         const double *__restrict__ cellS,
+                                                         const double *__restrict__ Uin, const double *U0, double *Uout,
+                                                         const int32_t *__restrict__ srcidx, const double *__restrict__ srcrate,
+                                                         int nsrc, update_par up, double *__restrict__ part_floor) {
+  __shared__ double red[32];
+  const int64_t item = (int64_t)blockIdx.x * RT_FIN_BLOCK + threadIdx.x;
+  const int64_t k = item / G;
+  const int g = (int)(item - k * G);
+  double add = 0.0;
+  if (k < n2) {
+    const int64_t i = k2cell[k];
+    const int r0 = k2off[k], r1 = k2off[k + 1];
+    double *out = Uout + 4 * (i * G + g);
+    double4 a = ld4(pacc + 4 * (i * G + g));
+    const double *xg = xphi + 4 * g;
+#pragma unroll 4
+    for (int r = r0; r < r1; r++) {
+      const double4 p = ld4(xg + (size_t)(4 * G) * k2row[r]);
+      a.x -= p.x; a.y -= p.y; a.z -= p.z; a.w -= p.w;
+    }
+    const int32_t si = srcidx[i];
+    const double src = si >= 0 ? srcrate[(size_t)g * nsrc + si] : 0.0;
+    add = finish_cell(a.x, a.y, a.z, a.w, cellS[4 * i + 3], src, ld4(Uin + 4 * (i * G + g)), ld4(U0 + 4 * (i * G + g)), up, out);
+  }
+  // fixed-order block sums per group
+  const int any = __syncthreads_or(add != 0.0);
+#pragma unroll
+  for (int gg = 0; gg < G; gg++) {
+    double t = 0.0;
+    if (any) t = block_sum(g == gg ? add : 0.0, red);
+    if (threadIdx.x == 0) part_floor[(size_t)blockIdx.x * G + gg] = t;
+  }
 }
 
 // ------------------------------------------------------------------ ledgers
@@ -405,6 +536,13 @@ __global__ void __launch_bounds__(1024) k_reduce(reduce_job j0, reduce_job j1, i
     c += fabs(s) >= fabs(x) ? (s - t) + x : (x - t) + s;
     s = t;
   }
+  if (gridDim.y == 1 && j1.part != j0.part)  // one job made of two partial-sum arrays
+    for (int64_t r = threadIdx.x; r < j1.nrows; r += 1024) {
+      const double x = j1.part[(size_t)r * G + g];
+      const double t = s + x;
+      c += fabs(s) >= fabs(x) ? (s - t) + x : (x - t) + s;
+      s = t;
+    }
   sm[threadIdx.x] = s + c;
   __syncthreads();
   for (int o = 512; o > 0; o >>= 1) {
@@ -480,8 +618,9 @@ static inline unsigned blocks_for(int64_t n, int per_block) { return (unsigned)(
     default: KERNEL(8)<<<grid, block, smem, stream>>>(__VA_ARGS__); break;                \
   }
 #define K_GRAD(g) k_grad<g>
-#define K_STAGE2(g) k_stage<g, true>
-#define K_STAGE1(g) k_stage<g, false>
+#define K_FLUX2(g) k_flux<g, true>
+#define K_FLUX1(g) k_flux<g, false>
+#define K_FINISH(g) k_finish<g>
 #define K_STORED(g) k_stored<g>
 
 // the tile kernels need more than the default 48 KB of dynamic shared memory
@@ -506,39 +645,45 @@ static cudaError_t allow_smem(K kernel, size_t bytes) {
 
 int rt_transport_configure(rt_ctx *c) {
   cudaError_t e = cudaSuccess;
-  const size_t sg = rt_smem_grad(c->TC, c->G, c->smax, c->hmax), ss = rt_smem_stage(c->TC, c->G, c->smax, c->hmax);
+  const size_t sg = rt_smem_grad(c->TC, c->G, c->smax, c->hmax, c->bmax), ss = rt_smem_flux(c->TC, c->G, c->omax, c->fmax, c->bmax);
   SET_SMEM_G(c->G, K_GRAD, sg, e);
-  if (e == cudaSuccess) SET_SMEM_G(c->G, K_STAGE2, ss, e);
-  if (e == cudaSuccess) SET_SMEM_G(c->G, K_STAGE1, ss, e);
+  if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX2, ss, e);
+  if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX1, ss, e);
   if (e != cudaSuccess) return rt_fail(c, RT_ECUDA, "cudaFuncSetAttribute(shared memory): %s", cudaGetErrorString(e));
   return RT_OK;
 }
 
-// threads per tile block: a whole number of warps, at most 256 (the kernels' launch bound);
-// RT_TILE_THREADS in the environment overrides the default for experiments
-static int tile_threads(const rt_ctx *c) {
+// threads per tile block (a whole number of warps, at most 256, the kernels' launch bound).
+// k_grad has one thread per (cell, group); k_stage one lane per (slot, group), several passes.
+// RT_TILE_THREADS / RT_GRAD_THREADS in the environment override the defaults for experiments.
+static int env_int(const char *name) { const char *e = getenv(name); return e ? atoi(e) : 0; }
+static int round_threads(int n) { n = ((n + 31) / 32) * 32; return n > 256 ? 256 : (n < 32 ? 32 : n); }
+static int tile_threads(const rt_ctx *) {
   static int env = -1;
-  if (env < 0) { const char *e = getenv("RT_TILE_THREADS"); env = e ? atoi(e) : 0; }
-  int n = env > 0 ? env : 256;
-  n = ((n + 31) / 32) * 32;
-  return n > 256 ? 256 : (n < 32 ? 32 : n);
+  if (env < 0) env = env_int("RT_TILE_THREADS");
+  return round_threads(env > 0 ? env : 256);
+}
+static int grad_threads(const rt_ctx *c) {
+  static int env = -1;
+  if (env < 0) env = env_int("RT_GRAD_THREADS");
+  return round_threads(env > 0 ? env : c->TC * c->G);
 }
 
 rt_geom rt_geom_of(const rt_ctx *c) {
   const rt_layout &l = c->lay;
   rt_geom m;
-  m.C = c->C; m.F = c->F; m.G = c->G; m.TC = c->TC; m.smax = c->smax;
+  m.C = c->C; m.F = c->F; m.G = c->G; m.TC = c->TC; m.smax = c->smax; m.omax = c->omax; m.hmax = c->hmax; m.fmax = c->fmax; m.bmax = c->bmax;
   m.cellS = rt_ptr<double>(c, l.cellS); m.Minv = rt_ptr<double>(c, l.Minv);
   m.faceC = rt_ptr<double>(c, l.faceC); m.faceN = rt_ptr<double>(c, l.faceN); m.faceW = rt_ptr<double>(c, l.faceW);
-  m.fo = rt_ptr<int64_t>(c, l.fo); m.ro = rt_ptr<int64_t>(c, l.ro); m.inco = rt_ptr<int64_t>(c, l.inco);
-  m.incf = rt_ptr<int32_t>(c, l.incf); m.hl = rt_ptr<uint16_t>(c, l.hl);
+  m.tiles = rt_ptr<rt_tile>(c, l.tiles); m.blob = rt_ptr<uint32_t>(c, l.blob);
+  m.xphi = rt_ptr<double>(c, l.xphi);
   m.ghost = rt_ptr<double>(c, l.ghost);
   for (int a = 0; a < 3; a++) { m.box[a] = c->box[a]; m.per[a] = c->per[a]; }
   return m;
 }
 
 int rt_launch_gradients(rt_ctx *c, const double *U) {
-  DISPATCH_G(c->G, K_GRAD, (unsigned)c->T, tile_threads(c), rt_smem_grad(c->TC, c->G, c->smax, c->hmax), c->stream, rt_geom_of(c), U,
+  DISPATCH_G(c->G, K_GRAD, (unsigned)c->T, grad_threads(c), rt_smem_grad(c->TC, c->G, c->smax, c->hmax, c->bmax), c->stream, rt_geom_of(c), U,
              rt_ptr<double>(c, c->lay.grad));
   c->launches++;
   return RT_OK;
@@ -560,27 +705,39 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
   double *grad = rt_ptr<double>(c, l.grad);
   double *part = rt_ptr<double>(c, l.part);
   const int64_t nchem = blocks_for(c->C, RT_CHEM_BLOCK);
+  const int64_t nfin = (c->n2 * G + RT_FIN_BLOCK - 1) / RT_FIN_BLOCK;
   double *p_floor = part + (size_t)G * nchem, *p_out = p_floor + (size_t)G * c->T, *p_in = p_out + (size_t)G * c->T;
+  double *p_floor2 = p_in + (size_t)G * c->T;
   const int nt = tile_threads(c);
-  const size_t ss = rt_smem_stage(c->TC, G, c->smax, c->hmax);
+  const size_t ss = rt_smem_flux(c->TC, G, c->omax, c->fmax, c->bmax);
+  const update_par up = {ca, cb, dt, c->par.ctilde, c->par.n_floor};
+  double *pacc = rt_ptr<double>(c, l.pacc);
+  const int32_t *srcidx = rt_ptr<int32_t>(c, l.srcidx);
+  const double *srcrate = rt_ptr<double>(c, l.srcrate);
   if (c->par.order >= 2) {
     rt_prof_begin(c, RT_K_GRAD);
-    DISPATCH_G(G, K_GRAD, (unsigned)c->T, nt, rt_smem_grad(c->TC, G, c->smax, c->hmax), c->stream, m, Uin, grad);
+    DISPATCH_G(G, K_GRAD, (unsigned)c->T, grad_threads(c), rt_smem_grad(c->TC, G, c->smax, c->hmax, c->bmax), c->stream, m, Uin, grad);
     rt_prof_end(c);
     c->launches++;
-    rt_prof_begin(c, RT_K_UPDATE);
-    DISPATCH_G(G, K_STAGE2, (unsigned)c->T, nt, ss, c->stream, m, Uin, grad, U0, Uout, rt_ptr<int32_t>(c, l.srcidx),
-               rt_ptr<double>(c, l.srcrate), c->nsrc, ca, cb, dt, c->par.ctilde, c->par.n_floor, p_floor, p_out, p_in);
+    rt_prof_begin(c, RT_K_FLUX);
+    DISPATCH_G(G, K_FLUX2, (unsigned)c->T, nt, ss, c->stream, m, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
     rt_prof_end(c);
   } else {
-    rt_prof_begin(c, RT_K_UPDATE);
-    DISPATCH_G(G, K_STAGE1, (unsigned)c->T, nt, ss, c->stream, m, Uin, grad, U0, Uout, rt_ptr<int32_t>(c, l.srcidx),
-               rt_ptr<double>(c, l.srcrate), c->nsrc, ca, cb, dt, c->par.ctilde, c->par.n_floor, p_floor, p_out, p_in);
+    rt_prof_begin(c, RT_K_FLUX);
+    DISPATCH_G(G, K_FLUX1, (unsigned)c->T, nt, ss, c->stream, m, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
     rt_prof_end(c);
   }
   c->launches++;
+  if (nfin > 0) {
+    rt_prof_begin(c, RT_K_UPDATE);
+    DISPATCH_G(G, K_FINISH, (unsigned)nfin, RT_FIN_BLOCK, 0, c->stream, c->n2, rt_ptr<int32_t>(c, l.k2cell),
+               rt_ptr<int32_t>(c, l.k2off), rt_ptr<int32_t>(c, l.k2row), m.xphi, pacc, m.cellS, Uin, U0, Uout, srcidx, srcrate, c->nsrc, up,
+               p_floor2);
+    rt_prof_end(c);
+    c->launches++;
+  }
   reduce2(c, {p_out, c->T, wl * dt, 1}, {p_in, c->T, wl * dt, 2}, 2);
-  reduce2(c, {p_floor, c->T, wf, 3}, {p_floor, c->T, wf, 3}, 1);
+  reduce2(c, {p_floor, c->T, wf, 3}, {nfin > 0 ? p_floor2 : p_floor, nfin, wf, 3}, 1);
 }
 
 int rt_launch_step(rt_ctx *c, double dt) {

@@ -3,6 +3,8 @@
 // loop runs in registers with no main-memory access inside the iterations.
 // Formulas: readings S17-S24 of DESIGN.md (the paper defers them to Kannan+19); rate fits:
 // DESIGN.md appendix A.
+#include <cub/cub.cuh>
+#include <stdlib.h>
 #include "rt_internal.cuh"
 #include "rt_kernels.cuh"
 
@@ -16,35 +18,44 @@ struct rate_set {
   double cool_neu[3];              // cooling per n_e n_X for X = HI, HeI, HeII (coll. ionisation + excitation)
 };
 
-__device__ inline double recomb_fit(double lam) {
-  return 2.753e-14 * lam * sqrt(lam) / pow(1.0 + pow(lam * (1.0 / 2.74), 0.407), 2.242);
+// The fits are products of powers of T; every power is taken as exp(c log x) from ONE log T
+// (log lambda_i = log(2 T_i) - log T), which costs a third of pow() and agrees with it to ~1e-14
+// relative (|c log x| <= 40): far inside the parity tolerance, and the sub-step controller's
+// decisions only differ where f sits within 1e-14 of its threshold.
+// 2.753e-14 lam^1.5 / (1 + (lam/2.74)^0.407)^2.242
+__device__ inline double recomb_fit(double loglam) {
+  const double u = exp(0.407 * (loglam - 1.007957920399979));  // log 2.74
+  return 2.753e-14 * exp(1.5 * loglam - 2.242 * log(1.0 + u));
 }
-__device__ inline double recomb_cool_fit(double T, double lam) {
-  return 3.435e-30 * T * pow(lam, 1.970) / pow(1.0 + pow(lam * (1.0 / 2.250), 0.376), 3.720);
+// 3.435e-30 T lam^1.970 / (1 + (lam/2.250)^0.376)^3.720
+__device__ inline double recomb_cool_fit(double T, double loglam) {
+  const double u = exp(0.376 * (loglam - 0.8109302162163288));  // log 2.25
+  return 3.435e-30 * T * exp(1.970 * loglam - 3.720 * log(1.0 + u));
 }
 
 template <bool THERMAL>
 __device__ inline void eval_rates(double T, double aB_override, rate_set &r) {
-  const double iT = 1.0 / T;
-  const double lHI = 2.0 * 157807.0 * iT, lHeI = 2.0 * 285335.0 * iT, lHeII = 2.0 * 631515.0 * iT;
+  const double iT = 1.0 / T, logT = log(T);
+  // log(2 T_i) for T_HI = 157807, T_HeI = 285335, T_HeII = 631515 K
+  const double llHI = 12.662275226919286 - logT, llHeI = 13.254566388120152 - logT, llHeII = 14.049024154019651 - logT;
   const double sq = sqrt(T), q = 1.0 / (1.0 + sqrt(T * 1.0e-5));
   const double eHI = exp(-157809.1 * iT), eHeI = exp(-285335.4 * iT), eHeII = exp(-631515.0 * iT);
   const double sqq = sq * q;
-  r.aHII = aB_override > 0.0 ? aB_override : recomb_fit(lHI);
-  r.aHeII = 1.26e-14 * pow(lHeI, 0.75);
-  r.aHeIII = 2.0 * recomb_fit(lHeII);
+  r.aHII = aB_override > 0.0 ? aB_override : recomb_fit(llHI);
+  r.aHeII = 1.26e-14 * exp(0.75 * llHeI);
+  r.aHeIII = 2.0 * recomb_fit(llHeII);
   r.bHI = 5.85e-11 * sqq * eHI;
   r.bHeI = 2.38e-11 * sqq * eHeI;
   r.bHeII = 5.68e-12 * sqq * eHeII;
   if (THERMAL) {
-    const double lt = log10(T);
+    const double lt = logT * 0.43429448190325176;  // log10 T
     const double brem = 1.42e-27 * (1.1 + 0.34 * exp(-(5.5 - lt) * (5.5 - lt) * (1.0 / 3.0))) * sq;
-    r.cool_ion[0] = recomb_cool_fit(T, lHI) + brem;
+    r.cool_ion[0] = recomb_cool_fit(T, llHI) + brem;
     r.cool_ion[1] = KB_CGS * T * r.aHeII + brem;
-    r.cool_ion[2] = 8.0 * recomb_cool_fit(T, lHeII) + 4.0 * brem;
+    r.cool_ion[2] = 8.0 * recomb_cool_fit(T, llHeII) + 4.0 * brem;
     r.cool_neu[0] = 1.27e-21 * sqq * eHI + 7.50e-19 * exp(-118348.0 * iT) * q;
     r.cool_neu[1] = 9.38e-22 * sqq * eHeI;
-    r.cool_neu[2] = 4.95e-22 * sqq * eHeII + 5.54e-17 * pow(T, -0.397) * exp(-473638.0 * iT) * q;
+    r.cool_neu[2] = 4.95e-22 * sqq * eHeII + 5.54e-17 * exp(-0.397 * logT - 473638.0 * iT) * q;
   }
 }
 
@@ -52,11 +63,16 @@ template <int G>
 struct cell_state {
   double N[G], Fx[G], Fy[G], Fz[G], xHII, xHeII, xHeIII, e;
 };
+// what a trial sub-step proposes: the photon attenuation factors and the new chemistry state
+template <int G>
+struct trial_out {
+  double inv[G], xHII, xHeII, xHeIII, e;
+};
 
 // one trial sub-step of size h from s into o; returns the controller's f (C1-C7)
 template <int G, bool THERMAL>
 __device__ inline double trial(const rt_chem_par &P, const cell_state<G> &s, double nH, double h, const rate_set &r,
-                               cell_state<G> &o) {
+                               trial_out<G> &o) {
   const double y = P.y_he, nHe = y * nH;
   const double xe = s.xHII + y * (s.xHeII + 2.0 * s.xHeIII);
   const double ne = nH * xe;
@@ -67,9 +83,9 @@ __device__ inline double trial(const rt_chem_par &P, const cell_state<G> &s, dou
     const double k0 = P.sigma[g][0] * nHI, k1 = P.sigma[g][1] * nHeI, k2 = P.sigma[g][2] * nHeII;
     const double k = k0 + k1 + k2;
     const double inv = 1.0 / (1.0 + h * P.ctilde * k);
-    o.N[g] = s.N[g] * inv; o.Fx[g] = s.Fx[g] * inv; o.Fy[g] = s.Fy[g] * inv; o.Fz[g] = s.Fz[g] * inv;
+    o.inv[g] = inv;
     if (k > 0.0) {
-      const double dNk = (s.N[g] - o.N[g]) / k;
+      const double dNk = (s.N[g] - s.N[g] * inv) / k;
       const double a0 = dNk * k0, a1 = dNk * k1, a2 = dNk * k2;
       pHI += a0; pHeI += a1; pHeII += a2;
       if (THERMAL) heat += a0 * P.eps[g][0] + a1 * P.eps[g][1] + a2 * P.eps[g][2];
@@ -122,115 +138,223 @@ __device__ inline double block_sum(double v) {
   return v;
 }
 
-template <int G, int MODE>
+// what a cell whose sub-stepping is not finished carries to the next pass (the cells
+// that need many sub-steps are compacted and continued by later passes, so that a few slow cells
+// do not hold back the warps of the fast ones)
+struct chem_carry {
+  double *t, *h;      // time reached, next sub-step (negative: it is the clipped last one)
+  int32_t *attempts;  // trials so far
+};
+
+// One pass of the sub-stepping.  FIRST: every cell, starting at t = 0, h = dt; otherwise the cells
+// list[0 .. *count) with the carried (t, h).  A cell stops after `cap` trials in this pass
+// (cap <= 0: no limit) and is flagged for the next pass.  One warp per block; warps stride over the
+// cells; part_abs has one row per 32 consecutive entries (fixed order: deterministic ledger).
+template <int G, int MODE, bool FIRST>
 __global__ void __launch_bounds__(RT_CHEM_BLOCK) k_chem(rt_chem_par P, int64_t C, double dt, double *__restrict__ U,
                                                    double *__restrict__ xHII, double *__restrict__ xHeII,
                                                    double *__restrict__ xHeIII, double *__restrict__ eth,
                                                    const double *__restrict__ nHv, const double *__restrict__ cellS,
                                                    const double *__restrict__ kappa, double *__restrict__ part_abs,
-                                                   rt_dev_ledger *led) {
+                                                   rt_dev_ledger *led, const int32_t *__restrict__ list,
+                                                   const int *__restrict__ count, int cap, chem_carry carry,
+                                                   uint8_t *__restrict__ flag) {
   constexpr bool THERMAL = (MODE == RT_CHEM_HHE_THERMAL);
   static_assert(RT_CHEM_BLOCK == 32, "block_sum assumes one warp");
-  const int64_t i = (int64_t)blockIdx.x * RT_CHEM_BLOCK + threadIdx.x;
-  const bool live = i < C;
-  double absd[G];
+  const int64_t n = FIRST ? C : (int64_t)*count;
+  unsigned long long wsum_att = 0, wmax_att = 0;
+  int wcap = 0;
+  for (int64_t row = blockIdx.x; row * RT_CHEM_BLOCK < n; row += gridDim.x) {
+    const int64_t idx = row * RT_CHEM_BLOCK + threadIdx.x;
+    const bool live = idx < n;
+    double absd[G];
 #pragma unroll
-  for (int g = 0; g < G; g++) absd[g] = 0.0;
-  unsigned long long attempts = 0;
-  int capped = 0;
-  if (live) {
-    cell_state<G> s;
+    for (int g = 0; g < G; g++) absd[g] = 0.0;
+    if (live) {
+      const int64_t i = FIRST ? idx : (int64_t)list[idx];
+      cell_state<G> s;
 #pragma unroll
-    for (int g = 0; g < G; g++) {
-      const double4 u = *reinterpret_cast<const double4 *>(U + ((size_t)i * G + g) * 4);
-      s.N[g] = u.x; s.Fx[g] = u.y; s.Fy[g] = u.z; s.Fz[g] = u.w;
-      absd[g] = s.N[g];
-    }
-    if (MODE == RT_CHEM_FIXED_OPACITY) {
-      // one implicit step of the absorption terms of eqs (6)-(7): N' = N/(1 + dt c kappa)
-      const double den = 1.0 + dt * P.ctilde * kappa[i];
-#pragma unroll
-      for (int g = 0; g < G; g++) { s.N[g] /= den; s.Fx[g] /= den; s.Fy[g] /= den; s.Fz[g] /= den; }
-    } else {
-      const double nH = nHv[i];
-      s.xHII = xHII[i]; s.xHeII = xHeII[i]; s.xHeIII = xHeIII[i]; s.e = eth[i];
-      rate_set r;
-      if (!THERMAL) eval_rates<false>(P.T_fixed, P.alphaB_override, r);
-      // controller of PAPER.md:238: start with h = dt; reject if f > 0.1 and shrink by f_s/f; on
-      // accept scale by f_s/f but at most double; the last step is clipped to end at dt
-      double t = 0.0, h = dt;
-      bool last = true, stale = true;  // rates depend on the state only: a retry reuses them
-      while (true) {
-        if ((long long)attempts >= P.max_substeps) { capped = 1; break; }
-        if (THERMAL && stale) {
-          stale = false;
-          const double xe = s.xHII + P.y_he * (s.xHeII + 2.0 * s.xHeIII);
-          const double T = (2.0 / 3.0) * s.e / (KB_CGS * (nH * (1.0 + P.y_he + xe)));
-          eval_rates<true>(T, P.alphaB_override, r);
-        }
-        cell_state<G> o;
-        const double f = trial<G, THERMAL>(P, s, nH, h, r, o);
-        attempts++;
-        if (f > P.f_accept) { h = h * P.f_target / f; last = false; continue; }
-        s = o;
-        stale = true;
-        if (last) break;
-        t += h;
-        h = h * fmin(2.0, P.f_target / fmax(f, 1e-300));
-        if (h >= dt - t) { h = dt - t; last = true; }
+      for (int g = 0; g < G; g++) {
+        const double4 u = *reinterpret_cast<const double4 *>(U + ((size_t)i * G + g) * 4);
+        s.N[g] = u.x; s.Fx[g] = u.y; s.Fy[g] = u.z; s.Fz[g] = u.w;
+        absd[g] = s.N[g];
       }
-      xHII[i] = s.xHII; xHeII[i] = s.xHeII; xHeIII[i] = s.xHeIII;
-      if (THERMAL) eth[i] = s.e;
+      bool unfinished = false;
+      if (MODE == RT_CHEM_FIXED_OPACITY) {
+        // one implicit step of the absorption terms of eqs (6)-(7): N' = N/(1 + dt c kappa)
+        const double den = 1.0 + dt * P.ctilde * kappa[i];
+#pragma unroll
+        for (int g = 0; g < G; g++) { s.N[g] /= den; s.Fx[g] /= den; s.Fy[g] /= den; s.Fz[g] /= den; }
+      } else {
+        const double nH = nHv[i];
+        s.xHII = xHII[i]; s.xHeII = xHeII[i]; s.xHeIII = xHeIII[i]; s.e = eth[i];
+        rate_set r;
+        if (!THERMAL) eval_rates<false>(P.T_fixed, P.alphaB_override, r);
+        // controller of PAPER.md:238: start with h = dt; reject if f > 0.1 and shrink by f_s/f; on
+        // accept scale by f_s/f but at most double; the last step is clipped to end at dt
+        double t = 0.0, h = dt;
+        bool last = true, stale = true;  // rates depend on the state only: a retry reuses them
+        long long attempts = 0;
+        if (!FIRST) {
+          t = carry.t[i];
+          h = carry.h[i];
+          last = h < 0.0;
+          h = fabs(h);
+          attempts = carry.attempts[i];
+        }
+        int here = 0, capped = 0;
+        bool done = false;
+        while (true) {
+          if (attempts >= P.max_substeps) { capped = 1; done = true; break; }
+          if (cap > 0 && here >= cap) break;
+          if (THERMAL && stale) {
+            stale = false;
+            const double xe = s.xHII + P.y_he * (s.xHeII + 2.0 * s.xHeIII);
+            const double T = (2.0 / 3.0) * s.e / (KB_CGS * (nH * (1.0 + P.y_he + xe)));
+            eval_rates<true>(T, P.alphaB_override, r);
+          }
+          trial_out<G> o;
+          const double f = trial<G, THERMAL>(P, s, nH, h, r, o);
+          attempts++; here++;
+          if (f > P.f_accept) { h = h * P.f_target / f; last = false; continue; }
+#pragma unroll
+          for (int g = 0; g < G; g++) { s.N[g] *= o.inv[g]; s.Fx[g] *= o.inv[g]; s.Fy[g] *= o.inv[g]; s.Fz[g] *= o.inv[g]; }
+          s.xHII = o.xHII; s.xHeII = o.xHeII; s.xHeIII = o.xHeIII; s.e = o.e;
+          stale = true;
+          if (last) { done = true; break; }
+          t += h;
+          h = h * fmin(2.0, P.f_target / fmax(f, 1e-300));
+          if (h >= dt - t) { h = dt - t; last = true; }
+        }
+        xHII[i] = s.xHII; xHeII[i] = s.xHeII; xHeIII[i] = s.xHeIII;
+        if (THERMAL) eth[i] = s.e;
+        wsum_att += (unsigned long long)here;
+        if (done) {
+          wmax_att = (unsigned long long)attempts > wmax_att ? (unsigned long long)attempts : wmax_att;
+          wcap += capped;
+        } else {
+          unfinished = true;
+          carry.t[i] = t; carry.h[i] = last ? -h : h; carry.attempts[i] = (int32_t)attempts;
+        }
+      }
+      if (flag) flag[idx] = unfinished ? 1 : 0;
+      const double V = cellS[4 * i + 3];
+#pragma unroll
+      for (int g = 0; g < G; g++) {
+        *reinterpret_cast<double4 *>(U + ((size_t)i * G + g) * 4) = make_double4(s.N[g], s.Fx[g], s.Fy[g], s.Fz[g]);
+        absd[g] = V * (absd[g] - s.N[g]);
+      }
     }
-    const double V = cellS[4 * i + 3];
 #pragma unroll
     for (int g = 0; g < G; g++) {
-      *reinterpret_cast<double4 *>(U + ((size_t)i * G + g) * 4) = make_double4(s.N[g], s.Fx[g], s.Fy[g], s.Fz[g]);
-      absd[g] = V * (absd[g] - s.N[g]);
+      const double tsum = block_sum(absd[g]);
+      if (threadIdx.x == 0) part_abs[(size_t)row * G + g] = tsum;
     }
-  }
-#pragma unroll
-  for (int g = 0; g < G; g++) {
-    const double t = block_sum(absd[g]);
-    if (threadIdx.x == 0) part_abs[(size_t)blockIdx.x * G + g] = t;
   }
   if (MODE != RT_CHEM_FIXED_OPACITY) {
     // integer counters: order-independent, so atomics keep the result deterministic
-    unsigned long long wsum = attempts, wmax = attempts;
-    int wcap = capped;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-      wsum += __shfl_down_sync(0xffffffffu, wsum, o);
-      unsigned long long m = __shfl_down_sync(0xffffffffu, wmax, o);
-      wmax = m > wmax ? m : wmax;
+      wsum_att += __shfl_down_sync(0xffffffffu, wsum_att, o);
+      unsigned long long mm = __shfl_down_sync(0xffffffffu, wmax_att, o);
+      wmax_att = mm > wmax_att ? mm : wmax_att;
       wcap += __shfl_down_sync(0xffffffffu, wcap, o);
     }
     if ((threadIdx.x & 31) == 0) {
-      atomicAdd(&led->substeps_total, wsum);
-      atomicMax(&led->substeps_max, wmax);
+      if (wsum_att) atomicAdd(&led->substeps_total, wsum_att);
+      if (wmax_att) atomicMax(&led->substeps_max, wmax_att);
       if (wcap) atomicAdd(&led->cells_hit_cap, (unsigned long long)wcap);
     }
   }
 }
 
-template <int G>
-static void launch_chem_g(rt_ctx *c, const rt_chem_par &P, double dt, double *U) {
+// caps of the passes: RT_CHEM_CAPS="1,8" means pass 0 makes one trial per cell, pass 1 up to 8 more
+// for the cells still unfinished, and a last pass finishes the rest (default "1,8")
+static int chem_caps(int *caps, int maxn) {
+  static int cached[8], ncached = -1;
+  if (ncached < 0) {
+    ncached = 0;
+    const char *e = getenv("RT_CHEM_CAPS");
+    if (!e) e = "1,8";
+    while (*e && ncached < 6) {
+      const int v = atoi(e);
+      if (v > 0) cached[ncached++] = v;
+      while (*e && *e != ',') e++;
+      if (*e == ',') e++;
+    }
+  }
+  int n = 0;
+  for (; n < ncached && n < maxn; n++) caps[n] = cached[n];
+  return n;
+}
+
+template <int G, int MODE>
+static void launch_chem_mode(rt_ctx *c, const rt_chem_par &P, double dt, double *U) {
   const rt_layout &l = c->lay;
-  dim3 grid((unsigned)((c->C + RT_CHEM_BLOCK - 1) / RT_CHEM_BLOCK)), block(RT_CHEM_BLOCK);
+  const int64_t C = c->C;
+  const unsigned nrows = (unsigned)((C + RT_CHEM_BLOCK - 1) / RT_CHEM_BLOCK);
   double *part = rt_ptr<double>(c, l.part);
-#define CHEM_ARGS P, c->C, dt, U, rt_ptr<double>(c, l.xHII), rt_ptr<double>(c, l.xHeII), rt_ptr<double>(c, l.xHeIII), \
-      rt_ptr<double>(c, l.eth), rt_ptr<double>(c, l.nH), rt_ptr<double>(c, l.cellS), rt_ptr<double>(c, l.kappa), part, \
-      rt_ptr<rt_dev_ledger>(c, l.led)
-  switch (c->par.chem_mode) {
-    case RT_CHEM_FIXED_OPACITY: k_chem<G, RT_CHEM_FIXED_OPACITY><<<grid, block, 0, c->stream>>>(CHEM_ARGS); break;
-    case RT_CHEM_H_ISOTHERMAL: k_chem<G, RT_CHEM_H_ISOTHERMAL><<<grid, block, 0, c->stream>>>(CHEM_ARGS); break;
-    default: k_chem<G, RT_CHEM_HHE_THERMAL><<<grid, block, 0, c->stream>>>(CHEM_ARGS); break;
+  rt_dev_ledger *led = rt_ptr<rt_dev_ledger>(c, l.led);
+  chem_carry carry = {rt_ptr<double>(c, l.chem_t), rt_ptr<double>(c, l.chem_h), rt_ptr<int32_t>(c, l.chem_att)};
+  uint8_t *flags = rt_ptr<uint8_t>(c, l.chem_flag);
+  int32_t *lists[2] = {rt_ptr<int32_t>(c, l.chem_list), rt_ptr<int32_t>(c, l.chem_list) + C};
+  int *count = rt_ptr<int>(c, l.chem_count);
+#define CHEM_ARGS P, C, dt, U, rt_ptr<double>(c, l.xHII), rt_ptr<double>(c, l.xHeII), rt_ptr<double>(c, l.xHeIII), \
+      rt_ptr<double>(c, l.eth), rt_ptr<double>(c, l.nH), rt_ptr<double>(c, l.cellS), rt_ptr<double>(c, l.kappa)
+  int caps[8];
+  const int ncap = MODE == RT_CHEM_FIXED_OPACITY ? 0 : chem_caps(caps, 8);
+  // pass 0: every cell
+  rt_prof_begin(c, RT_K_CHEM);
+  k_chem<G, MODE, true><<<nrows, RT_CHEM_BLOCK, 0, c->stream>>>(CHEM_ARGS, part, led, nullptr, nullptr, ncap > 0 ? caps[0] : 0, carry,
+                                                              ncap > 0 ? flags : nullptr);
+  rt_prof_end(c);
+  c->launches++;
+  rt_reduce2(c, {part, nrows, 1.0, 0, nullptr}, {part, nrows, 1.0, 0, nullptr}, 1);
+  // later passes: compact the unfinished cells (order kept: deterministic), continue them
+  unsigned grid = (unsigned)(c->nsm > 0 ? c->nsm : 148) * 32u;
+  if (grid > nrows) grid = nrows;
+  for (int p = 1; p <= ncap; p++) {
+    size_t bytes = l.chem_cub_bytes;
+    rt_prof_begin(c, RT_K_CHEM);
+    if (p == 1)
+      cub::DeviceSelect::Flagged(rt_ptr<void>(c, l.chem_cub), bytes, cub::CountingInputIterator<int32_t>(0), flags, lists[1], count,
+                                 (int)C, c->stream);
+    else
+      cub::DeviceSelect::Flagged(rt_ptr<void>(c, l.chem_cub), bytes, lists[(p - 1) & 1], flags, lists[p & 1], count, (int)C,
+                                 c->stream);
+    cudaMemsetAsync(flags, 0, (size_t)C, c->stream);  // entries beyond the new count must not be selected again
+    double *part_p = part + (size_t)p * G * nrows;
+    k_chem<G, MODE, false><<<grid, RT_CHEM_BLOCK, 0, c->stream>>>(CHEM_ARGS, part_p, led, lists[p & 1], count, p < ncap ? caps[p] : 0,
+                                                               carry, flags);
+    rt_prof_end(c);
+    c->launches += 2;
+    rt_reduce2(c, {part_p, 0, 1.0, 0, count}, {part_p, 0, 1.0, 0, count}, 1);
   }
 #undef CHEM_ARGS
 }
 
+template <int G>
+static void launch_chem_g(rt_ctx *c, const rt_chem_par &P, double dt, double *U) {
+  switch (c->par.chem_mode) {
+    case RT_CHEM_FIXED_OPACITY: launch_chem_mode<G, RT_CHEM_FIXED_OPACITY>(c, P, dt, U); break;
+    case RT_CHEM_H_ISOTHERMAL: launch_chem_mode<G, RT_CHEM_H_ISOTHERMAL>(c, P, dt, U); break;
+    default: launch_chem_mode<G, RT_CHEM_HHE_THERMAL>(c, P, dt, U); break;
+  }
+}
+
+size_t rt_chem_cub_bytes(int64_t C) {
+  size_t bytes = 0;
+  cub::DeviceSelect::Flagged(nullptr, bytes, (const int32_t *)nullptr, (const uint8_t *)nullptr, (int32_t *)nullptr, (int *)nullptr,
+                             (int)C);
+  return bytes + 256;
+}
+
 void rt_launch_chem(rt_ctx *c, const rt_chem_par &P, double dt, double *U) {
-  rt_prof_begin(c, RT_K_CHEM);
+  if (c->nsm <= 0) {
+    int n = 0;
+    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, c->device);
+    c->nsm = n > 0 ? n : 1;
+  }
   switch (c->G) {
     case 1: launch_chem_g<1>(c, P, dt, U); break;
     case 2: launch_chem_g<2>(c, P, dt, U); break;
@@ -241,6 +365,4 @@ void rt_launch_chem(rt_ctx *c, const rt_chem_par &P, double dt, double *U) {
     case 7: launch_chem_g<7>(c, P, dt, U); break;
     default: launch_chem_g<8>(c, P, dt, U); break;
   }
-  rt_prof_end(c);
-  c->launches++;
 }

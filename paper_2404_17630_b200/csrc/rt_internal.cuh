@@ -48,6 +48,7 @@
 #ifndef RT_BLOCK
 #define RT_BLOCK 128
 #endif
+#define RT_CHEM_MAXPASS 8  // sub-stepping passes (rt_chem.cu): partial-sum rows are reserved for each
 #define RT_CHEM_BLOCK 32  // one warp per block: a slow cell holds back 31 others, not 127
 #define RT_REC 18        // doubles per (cell, group) row of U + gradients in shared memory (16 + 2 pad: bank spread)
 #define RT_MIN_TILE 8     // smallest tile size rt_mesh_upload will fall back to
@@ -59,6 +60,7 @@ struct rt_dev_ledger {  // accumulators on the device (value + compensation)
 
 struct rt_layout {
   size_t perm, iperm, cellS, Minv, faceC, faceN, faceW, L, R, fo, ro, rl, rn, tiles, blob, xphi, k2cell, k2off, k2row, ghost, led;
+  size_t chem_t, chem_h, chem_att, chem_flag, chem_list, chem_count, chem_cub, chem_cub_bytes;
   size_t Ua, Ub, grad, pacc, xHII, xHeII, xHeIII, eth, nH, kappa, srcidx, srcrate, part, scratch_end;
   size_t blob_bytes;  // capacity of the blob region
   int64_t xcap;       // rows [G][4] of xphi
@@ -80,6 +82,7 @@ struct rt_ctx {
   int hmax;           // largest halo (cells outside the tile touching it) of any tile
   int fmax;           // largest forward halo of any tile
   int omax;           // most owned faces of any tile
+  int nsm;            // multiprocessors of the device (0 until first needed)
   int64_t n2;         // cells with at least one incoming face
   int bmax;           // largest blob of any tile, in 32-bit words
   int64_t ninc;       // total incoming faces over all tiles

@@ -37,5 +37,9 @@ __device__ __forceinline__ void rt_unpack_lr(double d, int32_t &l, int32_t &r) {
   r = (int32_t)(uint32_t)(u >> 32);
 }
 
-void rt_launch_chem(rt_ctx *c, const rt_chem_par &P, double dt, double *U);
+void rt_launch_chem(rt_ctx *c, const rt_chem_par &P, double dt, double *U);  // all passes + their ledger reductions
+size_t rt_chem_cub_bytes(int64_t C);
+// acc[slot][g] += weight * sum_rows part[row][g]; nrows = ceil(*ncount / 32) if ncount is given
+struct reduce_job { const double *part; int64_t nrows; double weight; int slot; const int *ncount; };
+void rt_reduce2(rt_ctx *c, reduce_job a, reduce_job b, int njobs);
 rt_geom rt_geom_of(const rt_ctx *c);

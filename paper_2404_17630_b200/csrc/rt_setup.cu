@@ -618,7 +618,12 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G) {
   l.srcidx = take(4 * C + 64);  // (+ padding: the tile kernels copy whole 16-byte chunks)
   l.srcrate = take(8 * (size_t)G * 65536);
   // partial sums: chem absorbed [<= 4 nbc + 1][G]; per tile: floor, outflow, inflow [max_tiles][G] each
-  l.part = take(8 * (size_t)G * (5 * l.nbc + 3 * l.max_tiles + (size_t)G * l.nbc + 32));
+  l.part = take(8 * (size_t)G * ((4 * RT_CHEM_MAXPASS + 1) * l.nbc + 3 * l.max_tiles + (size_t)G * l.nbc + 64));
+  // sub-stepping passes of the chemistry: carried (t, h, attempts), flags, two index lists, cub scratch
+  l.chem_t = take(8 * (size_t)C); l.chem_h = take(8 * (size_t)C); l.chem_att = take(4 * (size_t)C);
+  l.chem_flag = take((size_t)C + 64); l.chem_list = take(8 * (size_t)C); l.chem_count = take(256);
+  l.chem_cub_bytes = rt_chem_cub_bytes(C);
+  l.chem_cub = take(l.chem_cub_bytes);
   l.scratch_end = o;
   // setup scratch aliases the state region; make sure it fits (incl. staging of a host mesh)
   int64_t NM = C > F ? C : F;

@@ -524,10 +524,11 @@ __global__ void __launch_bounds__(RT_FIN_BLOCK) k_finish(int64_t n2, const int32
 
 // ------------------------------------------------------------------ ledgers
 // acc[slot][g] += weight * sum_rows part[row][g]; one block per (array, g); fixed order.
-struct reduce_job { const double *part; int64_t nrows; double weight; int slot; };
 __global__ void __launch_bounds__(1024) k_reduce(reduce_job j0, reduce_job j1, int G, rt_dev_ledger *led) {
   __shared__ double sm[1024];
-  const reduce_job j = blockIdx.y == 0 ? j0 : j1;
+  reduce_job j = blockIdx.y == 0 ? j0 : j1;
+  if (j.ncount) j.nrows = ((int64_t)*j.ncount + 31) / 32;
+  if (j1.ncount) j1.nrows = ((int64_t)*j1.ncount + 31) / 32;
   const int g = blockIdx.x;
   double s = 0.0, c = 0.0;
   for (int64_t r = threadIdx.x; r < j.nrows; r += 1024) {  // Neumaier per thread
@@ -689,7 +690,7 @@ int rt_launch_gradients(rt_ctx *c, const double *U) {
   return RT_OK;
 }
 
-static void reduce2(rt_ctx *c, reduce_job a, reduce_job b, int njobs) {
+void rt_reduce2(rt_ctx *c, reduce_job a, reduce_job b, int njobs) {
   rt_prof_begin(c, RT_K_REDUCE);
   k_reduce<<<dim3(c->G, njobs), 1024, 0, c->stream>>>(a, b, c->G, rt_ptr<rt_dev_ledger>(c, c->lay.led));
   rt_prof_end(c);
@@ -706,7 +707,7 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
   double *part = rt_ptr<double>(c, l.part);
   const int64_t nchem = blocks_for(c->C, RT_CHEM_BLOCK);
   const int64_t nfin = (c->n2 * G + RT_FIN_BLOCK - 1) / RT_FIN_BLOCK;
-  double *p_floor = part + (size_t)G * nchem, *p_out = p_floor + (size_t)G * c->T, *p_in = p_out + (size_t)G * c->T;
+  double *p_floor = part + (size_t)G * nchem * RT_CHEM_MAXPASS, *p_out = p_floor + (size_t)G * c->T, *p_in = p_out + (size_t)G * c->T;
   double *p_floor2 = p_in + (size_t)G * c->T;
   const int nt = tile_threads(c);
   const size_t ss = rt_smem_flux(c->TC, G, c->omax, c->fmax, c->bmax);
@@ -736,8 +737,8 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
     rt_prof_end(c);
     c->launches++;
   }
-  reduce2(c, {p_out, c->T, wl * dt, 1}, {p_in, c->T, wl * dt, 2}, 2);
-  reduce2(c, {p_floor, c->T, wf, 3}, {nfin > 0 ? p_floor2 : p_floor, nfin, wf, 3}, 1);
+  rt_reduce2(c, {p_out, c->T, wl * dt, 1, nullptr}, {p_in, c->T, wl * dt, 2, nullptr}, 2);
+  rt_reduce2(c, {p_floor, c->T, wf, 3, nullptr}, {nfin > 0 ? p_floor2 : p_floor, nfin, wf, 3, nullptr}, 1);
 }
 
 int rt_launch_step(rt_ctx *c, double dt) {
@@ -751,8 +752,6 @@ int rt_launch_step(rt_ctx *c, double dt) {
     for (int g = 0; g < RT_MAXG; g++)
       for (int j = 0; j < 3; j++) { P.sigma[g][j] = c->par.sigma[g][j]; P.eps[g][j] = c->par.eps_heat[g][j]; }
     rt_launch_chem(c, P, dt, Ua);
-    const int64_t nchem = blocks_for(c->C, RT_CHEM_BLOCK);
-    reduce2(c, {rt_ptr<double>(c, l.part), nchem, 1.0, 0}, {rt_ptr<double>(c, l.part), nchem, 1.0, 0}, 1);
   }
   double tot[RT_MAXG];
   for (int g = 0; g < c->G; g++) tot[g] = dt * c->src_total[g];
@@ -781,7 +780,7 @@ int rt_launch_stored(rt_ctx *c) {
   DISPATCH_G(c->G, K_STORED, (unsigned)l.nbc, dim3(RT_BLOCK, c->G), 0, c->stream, c->C, rt_ptr<double>(c, l.Ua),
              rt_ptr<double>(c, l.cellS), part);
   c->launches++;
-  reduce2(c, {part, l.nbc, 1.0, 4}, {part, l.nbc, 1.0, 4}, 1);
+  rt_reduce2(c, {part, l.nbc, 1.0, 4, nullptr}, {part, l.nbc, 1.0, 4, nullptr}, 1);
   return RT_OK;
 }
 

@@ -37,6 +37,7 @@ extern "C" {
 
 enum { RT_OK = 0, RT_EINVAL = -1, RT_ENOMEM = -2, RT_ECUDA = -3, RT_ESTATE = -4, RT_EMESH = -5 };
 enum { RT_MEM_HOST = 0, RT_MEM_DEVICE = 1 };
+enum { RT_WS_DEVICE_MESH = 1 }; /* flags of rt_workspace_bytes */
 /* rt_mesh.right codes for boundary faces (reading S13) */
 enum { RT_BC_OUTFLOW = -1, RT_BC_REFLECT = -2, RT_BC_DIRICHLET0 = -3 /* -3-k: ghost state k */ };
 enum { RT_CHEM_NONE = 0, RT_CHEM_FIXED_OPACITY = 1, RT_CHEM_H_ISOTHERMAL = 2, RT_CHEM_HHE_THERMAL = 3 };
@@ -115,7 +116,8 @@ typedef struct {
 int rt_create(rt_ctx **out, int device, void *cuda_stream);
 
 /* Bytes of device workspace rt_mesh_upload needs for this problem size (0 on invalid sizes).
- * flags: reserved, pass 0. */
+ * flags: 0, or RT_WS_DEVICE_MESH if the mesh arrays passed to rt_mesh_upload will be DEVICE
+ * pointers (no staging space for a host mesh is reserved then: 88 bytes per face less). */
 size_t rt_workspace_bytes(int64_t ncell, int64_t nface, int ngroup, int flags);
 
 /* Validates the mesh (index ranges, positive volumes and areas, unit normals, closed cells:

@@ -94,9 +94,8 @@ int rt_tile_info(const rt_ctx *c, int64_t *out) {
 }
 
 size_t rt_workspace_bytes(int64_t ncell, int64_t nface, int ngroup, int flags) {
-  (void)flags;
   if (ncell < 1 || nface < 1 || ngroup < 1 || ngroup > RT_MAXG || ncell > 0x7fffffffLL || nface > 0x7fffffffLL) return 0;
-  return rt_make_layout(ncell, nface, ngroup).total;
+  return rt_make_layout(ncell, nface, ngroup, flags).total;
 }
 
 int rt_mesh_upload(rt_ctx *c, const rt_mesh *m, void *ws, size_t bytes) {
@@ -117,7 +116,7 @@ int rt_mesh_upload(rt_ctx *c, const rt_mesh *m, void *ws, size_t bytes) {
   RT_CUDA(c, cudaSetDevice(c->device));
   c->C = m->ncell; c->F = m->nface; c->G = m->ngroup; c->nghost = m->nghost;
   for (int a = 0; a < 3; a++) { c->box[a] = m->box[a]; c->per[a] = m->periodic[a] != 0; }
-  c->lay = rt_make_layout(c->C, c->F, c->G);
+  c->lay = rt_make_layout(c->C, c->F, c->G, m->mem_kind == RT_MEM_DEVICE ? RT_WS_DEVICE_MESH : 0);
   if (bytes < c->lay.total)
     return rt_fail(c, RT_ENOMEM, "workspace has %zu bytes, rt_workspace_bytes says %zu", bytes, c->lay.total);
   c->ws = (char *)ws;

@@ -59,7 +59,7 @@ struct rt_dev_ledger {  // accumulators on the device (value + compensation)
 };
 
 struct rt_layout {
-  size_t perm, iperm, cellS, Minv, faceC, faceN, faceW, L, R, fo, ro, rl, rn, tiles, blob, xphi, k2cell, k2off, k2row, ghost, led;
+  size_t perm, iperm, cellS, Minv, faceC, faceN, faceW, fo, ro, tiles, blob, xphi, k2cell, k2off, k2row, ghost, led;
   size_t chem_t, chem_h, chem_att, chem_flag, chem_list, chem_count, chem_cub, chem_cub_bytes;
   size_t Ua, Ub, grad, pacc, xHII, xHeII, xHeIII, eth, nH, kappa, srcidx, srcrate, part, scratch_end;
   size_t blob_bytes;  // capacity of the blob region
@@ -141,7 +141,7 @@ static inline size_t rt_smem_flux(int TC, int G, int omax, int fmax, int bmax) {
 template <class T>
 static inline T *rt_ptr(const rt_ctx *c, size_t off) { return (T *)(c->ws + off); }
 
-rt_layout rt_make_layout(int64_t C, int64_t F, int G);
+rt_layout rt_make_layout(int64_t C, int64_t F, int G, int flags);
 
 int rt_fail(rt_ctx *c, int code, const char *fmt, ...);
 #define RT_CUDA(c, call)                                                                          \

@@ -416,6 +416,9 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
   const int64_t NM = (C > F ? C : F) > 4 * (lay.max_tiles + 2) ? (C > F ? C : F) : 4 * (lay.max_tiles + 2);
   uint64_t *k0 = rt_ptr<uint64_t>(c, take(8 * NM)), *k1 = rt_ptr<uint64_t>(c, take(8 * NM));
   int32_t *v0 = rt_ptr<int32_t>(c, take(4 * NM)), *v1 = rt_ptr<int32_t>(c, take(4 * NM));
+  // left / right ids of the sorted faces and the right lists: only the setup needs them
+  int32_t *L = rt_ptr<int32_t>(c, take(4 * F)), *R = rt_ptr<int32_t>(c, take(4 * F));
+  int32_t *rl = rt_ptr<int32_t>(c, take(4 * F)), *rn = rt_ptr<int32_t>(c, take(4 * F));
   int *flags = rt_ptr<int>(c, take(256));
   size_t cub_bytes = 0;
   {
@@ -473,9 +476,7 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
   // 2. faces by owner
   double *faceC = rt_ptr<double>(c, lay.faceC), *faceN = rt_ptr<double>(c, lay.faceN);
   double *faceW = rt_ptr<double>(c, lay.faceW);
-  int32_t *L = rt_ptr<int32_t>(c, lay.L), *R = rt_ptr<int32_t>(c, lay.R);
   int64_t *fo = rt_ptr<int64_t>(c, lay.fo), *ro = rt_ptr<int64_t>(c, lay.ro);
-  int32_t *rl = rt_ptr<int32_t>(c, lay.rl);
   {
     k_face_keys<<<nblk(F), SETUP_BLOCK, 0, st>>>(g, F, iperm, k0, v0);
     cub::DoubleBuffer<uint64_t> dk(k0, k1);
@@ -497,7 +498,7 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
     RT_CUDA(c, cudaMemcpyAsync(&NR, ro + C, 8, cudaMemcpyDeviceToHost, st));
     RT_CUDA(c, cudaStreamSynchronize(st));
     c->NR = NR;
-    if (NR > 0) k_rlist<<<nblk(NR), SETUP_BLOCK, 0, st>>>(dk.Current(), NR, L, rl, rt_ptr<int32_t>(c, lay.rn));
+    if (NR > 0) k_rlist<<<nblk(NR), SETUP_BLOCK, 0, st>>>(dk.Current(), NR, L, rl, rn);
   }
   // 4. geometry of eq (15)
   k_face_geom<<<nblk(F), SETUP_BLOCK, 0, st>>>(C, F, cellS, faceC, faceN, L, R, c->box[0], c->box[1], c->box[2],
@@ -513,7 +514,6 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
     int64_t *boff = (int64_t *)k1, *xoff = boff + Tmax, *ibase = xoff + Tmax, *k2base = ibase + Tmax;
     int32_t *faceX = v0;
     tile_max *mx = (tile_max *)(flags + 4);
-    const int32_t *rn = rt_ptr<int32_t>(c, lay.rn);
     const char *env = getenv("RT_TILE_CELLS");
     int tc0 = env ? atoi(env) : 64;
     if (tc0 < RT_MIN_TILE || tc0 > 1024) tc0 = 64;
@@ -585,7 +585,7 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
   return RT_OK;
 }
 
-rt_layout rt_make_layout(int64_t C, int64_t F, int G) {
+rt_layout rt_make_layout(int64_t C, int64_t F, int G, int flags) {
   rt_layout l;
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t r = o; o = align256(o + bytes); return r; };
@@ -594,16 +594,15 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G) {
   l.perm = take(4 * C); l.iperm = take(4 * C);
   l.cellS = take(32 * C); l.Minv = take(48 * C);
   l.faceC = take(32 * F); l.faceN = take(32 * F); l.faceW = take(32 * F);
-  l.L = take(4 * F); l.R = take(4 * F);
-  l.fo = take(8 * (C + 1)); l.ro = take(8 * (C + 1)); l.rl = take(4 * F); l.rn = take(4 * F);
+  l.fo = take(8 * (C + 1)); l.ro = take(8 * (C + 1));
   // tile tables: descriptors for the smallest tile size; blobs bounded by
   // sum_t (TC + 4) + half-faces (<= 2F) + slots (<= 2F) + halo (<= 2F) + incoming (<= F) words
   l.tiles = take(sizeof(rt_tile) * (size_t)(l.max_tiles + 1));
-  l.blob_bytes = 4 * (8 * (size_t)F + 2 * (size_t)C + 5 * (size_t)l.max_tiles + 2048);
+  l.blob_bytes = 4 * ((size_t)(5.5 * (double)F) + 2 * (size_t)C + 5 * (size_t)l.max_tiles + 2048);
   l.blob = take(l.blob_bytes);
-  // fluxes of the faces that cross tile boundaries, written by the owner tile (<= 60 % of the
+  // fluxes of the faces that cross tile boundaries, written by the owner tile (<= 56 % of the
   // faces; rt_mesh_upload fails with RT_ENOMEM on a mesh whose tiles need more)
-  l.xcap = (int64_t)(0.6 * (double)F) + 1024;
+  l.xcap = (int64_t)(0.56 * (double)F) + 1024;
   l.xphi = take(32 * (size_t)G * (size_t)l.xcap);
   // cells with incoming faces and the xphi rows of those faces (k_finish)
   l.k2cell = take(4 * (size_t)C); l.k2off = take(4 * ((size_t)C + 1)); l.k2row = take(4 * (size_t)l.xcap);
@@ -627,7 +626,8 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G) {
   l.scratch_end = o;
   // setup scratch aliases the state region; make sure it fits (incl. staging of a host mesh)
   int64_t NM = C > F ? C : F;
-  size_t need = 24 * (size_t)NM + 4096 + (size_t)(64 << 20) + 88 * (size_t)F + 32 * (size_t)C + 16 * 256;
+  const size_t staging = (flags & RT_WS_DEVICE_MESH) ? 0 : 88 * (size_t)F + 32 * (size_t)C;
+  size_t need = 24 * (size_t)NM + 4096 + (size_t)(64 << 20) + 16 * (size_t)F + staging + 32 * 256;
   if (l.temp + need > o) o = align256(l.temp + need);
   l.total = o;
   return l;

@@ -12,6 +12,7 @@ import numpy as np
 
 RT_MAXG = 8
 RT_MEM_HOST, RT_MEM_DEVICE = 0, 1
+RT_WS_DEVICE_MESH = 1
 LEDGER_ROWS = ("stored", "injected", "absorbed", "outflow", "inflow_bc", "floor_added")
 _vp = ctypes.c_void_p
 
@@ -137,6 +138,10 @@ def _check(h, rc, what):
         raise RTError("%s failed (%d): %s" % (what, rc, rt_last_error(h)))
 
 
+def _on_device(mesh):
+    return _kind(mesh.volume) == RT_MEM_DEVICE
+
+
 def rt_mesh_upload(h, mesh, ngroup, ghost_state, workspace):
     """mesh: object with the attributes of inputs.mesh.Mesh (numpy or torch arrays)."""
     keep = [_prep(getattr(mesh, k), np.float64) for k in ("volume", "centroid", "area", "normal", "fcentroid")]
@@ -249,7 +254,7 @@ class Solver:
         if stream is None:
             stream = torch.cuda.current_stream(self.dev).cuda_stream
         self.h = rt_create(device, stream)
-        nbytes = rt_workspace_bytes(self.C, self.F, self.G)
+        nbytes = rt_workspace_bytes(self.C, self.F, self.G, RT_WS_DEVICE_MESH if _on_device(mesh) else 0)
         if nbytes == 0:
             raise RTError("rt_workspace_bytes rejected the sizes")
         self.workspace = torch.empty((nbytes + 7) // 8, dtype=torch.float64, device=self.dev)

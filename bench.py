@@ -94,6 +94,22 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------ replicas: timing over ranks
+def max_over_ranks(x, dist, device):
+    """The slowest rank's value (device-timed milliseconds or seconds); x itself without a group."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(world, C, G, steps, ms):
+    """Whole-job throughput of `world` independent replicas (replicas only)."""
+    return world * C * G * steps / (ms * 1e-3)
+
+
 # ------------------------------------------------------------------ clocks
 class ClockSampler:
     Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
@@ -228,11 +244,8 @@ def main():
     s.profile(False)
     launches = s.launches() - l0
     clocks = sampler.stop(tw0, tw1)
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * C * G * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms, dist, "cuda")
+    value = aggregate_value(world, C, G, args.steps, ms)
 
     # ---- ledger sanity after the timed region (photon budget closes)
     led = s.ledger()
@@ -258,10 +271,7 @@ def main():
             rt.rt_download(s.h, host, False, G)
         torch.cuda.synchronize()
         el = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([el], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            el = float(t.item())
+        el = max_over_ranks(el, dist, "cuda")
         e2e = {"value": world * C * G * args.e2e_steps / el, "unit": UNIT, "h2d_bytes_per_step": (4 * G + 5) * 8 * C,
                "d2h_bytes_per_step": (4 * G + 4) * 8 * C, "steps": args.e2e_steps, "ms_per_step": el / args.e2e_steps * 1e3}
 
@@ -294,11 +304,18 @@ def main():
             d["frac_of_hbm_peak"] = d["GBps"] / peak
         kern[k] = d
     dom = max((k for k in kern if k in ab), key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"])
+    # (kern["stage"] is the pair k_flux + k_finish: avg_ms is the pair's time per stage)
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
+    # capture of this workload (profiles/traffic.csv, written from profiles/r1_ncu_full_*.md); for
+    # the stage pair it is k_flux's (k_finish's metric passes failed in that capture)
     traffic = None
-    tf = os.path.join(ROOT, "profiles", "traffic.json")
+    tf = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tf):
-        traffic = json.load(open(tf)).get(workload_name(c, n), {}).get(dom)
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["GBps"], "peak": peak, "unit": "GB/s",
+        for ln in open(tf).read().splitlines()[1:]:
+            wl, kn, by = ln.split(",")
+            if wl == workload_name(c, n) and kn == {"stage": "flux"}.get(dom, dom):
+                traffic = float(by)
+    roofline = {"bound": "hbm", "kernel": {"stage": "stage = k_flux + k_finish (a3 + a4 of one Heun stage)"}.get(dom, dom), "achieved": kern[dom]["GBps"], "peak": peak, "unit": "GB/s",
                 "frac": kern[dom]["GBps"] / peak, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": ab[dom],
                 "subcycle": {"algorithmic_bytes": ab["subcycle"], "GBps": ab["subcycle"] * args.steps / (ms * 1e-3) / 1e9,

@@ -1,17 +1,18 @@
-// a2-a4: the transport kernels of one Heun stage, one thread block per tile of TC consecutive
-// cells of the Peano-Hilbert order (layout and tile tables: rt_internal.cuh).
-//   k_grad   stages the tile's face records (eq (15) prefactors, face centres, neighbour ids), its
-//            cells' U and its face-list tables in shared memory with coalesced loads; then one
-//            thread per (cell, group) sums the second term of eq (15) over the cell's faces,
-//            multiplies by the stored inverse matrix and runs the slope limiter
-//
-//   k_stage  stages the tile's U and gradients in shared memory; one thread per face slot
-//            extrapolates both cells to the face centre, evaluates the M1 closure and the global
-//            Lax-Friedrichs flux with signal speed c~ and the donor cap for every group, and
-//            leaves A*Phi in shared memory; after a barrier one thread per
-//            (cell, group) sums the cell's face list in fixed order, adds the source, does the Heun
-//            combine, the floor and |F| <= c~ N (S3, S11, S12).  The fluxes
-//            never go to HBM; a face shared by two tiles is evaluated by both.
+// a2-a4: the transport kernels of one Heun stage.  A thread block works on one tile of TC consecutive
+// cells of the Peano-Hilbert order; everything the tile touches (its cells, its faces, the cells
+// across its faces, its index tables: layout in rt_internal.cuh) is staged in shared memory with
+// asynchronous copies (TMA bulk copies for the contiguous runs, 16-byte LDGSTS for the gathers)
+// and the arithmetic then runs from shared memory alone.
+//   k_grad    one thread per (cell, group): the second term of eq (15) summed over the cell's
+//             faces, times the stored inverse matrix, then the slope limiter
+//   k_flux    a3: one lane per (owned face, group) extrapolates both cells to the face centre,
+//             evaluates the M1 closure, the global Lax-Friedrichs flux with signal speed c~ and the
+//             donor cap, and leaves A*Phi in shared memory.  Every face is
+//             evaluated once, by the tile of its left cell; fluxes of faces whose right cell lies in
+//             a later tile also go to xphi.  a4: the tile's cells sum their faces in list order; a
+//             cell all of whose faces are the tile's gets the source, the Heun combine, the floor
+//             and |F| <= c~ N here (S3, S11, S12)
+//   k_finish  a4 for the other cells: adds the fluxes of the faces owned by earlier tiles (xphi)
 // fp64 throughout.  Reciprocals and the closure's square root use MUFU seeds + two Newton steps
 // (relative error ~1e-16, no special-case branches: all arguments are positive and normal).
 #include <stdlib.h>

@@ -20,6 +20,7 @@ struct rt_geom {
   double box[3];
   int per[3];
   int G, TC, smax, omax, hmax, fmax, bmax;
+  int prefetch_tiles;    // the tile kernels ask L2 for the data of tile t + prefetch_tiles
 };
 
 // the two int32 ids packed in the fourth slot of a faceN / faceW record

@@ -116,6 +116,12 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned by
                : "memory");
 }
 
+// asks L2 to fetch a contiguous run (a tile that a later block will stage)
+__device__ __forceinline__ void bulk_prefetch_l2(const void *src, unsigned bytes) {
+  if (bytes == 0) return;
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+
 // a tile's blob in shared memory (layout: rt_internal.cuh)
 struct tile_view {
   int64_t c0, fbase, xbase;
@@ -139,9 +145,9 @@ __device__ __forceinline__ tile_view view_tile(const rt_geom &m, const uint32_t 
 
 // ------------------------------------------------------------------ a2: gradients + limiter
 template <int G>
-__global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restrict__ U, double *__restrict__ grad) {
+__global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__restrict__ U, double *__restrict__ grad) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  __shared__ __align__(8) uint64_t bar;
+  __shared__ __align__(8) uint64_t bar, bar_blob;
   uint32_t *sB = reinterpret_cast<uint32_t *>(smem_raw);  // the tile's blob
   double *sW = reinterpret_cast<double *>(sB + m.bmax);   // [smax][4]  (w, kappa)
   double *sC = sW + 4 * m.smax;                           // [smax][4]  (c - s_L, A)
@@ -149,18 +155,31 @@ __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restric
   double *sM = sU + 4 * G * (m.TC + m.hmax);              // [TC][6]
   const tile_view v = view_tile(m, sB, blockIdx.x);
   const int tid = threadIdx.x, nt = blockDim.x;
-  if (tid == 0) mbar_init(&bar, 1);
+  if (tid == 0) { mbar_init(&bar, 1); mbar_init(&bar_blob, 1); }
   __syncthreads();
   // round 1: what the descriptor locates: the blob, the owned faces and the tile's own cells
   if (tid == 0) {
-    mbar_expect(&bar, 4u * v.words + 64u * v.nown + (32u * G + 48u) * v.ncell);
-    bulk_g2s(sB, v.blob, 4u * v.words, &bar);
+    mbar_expect(&bar_blob, 4u * v.words);
+    bulk_g2s(sB, v.blob, 4u * v.words, &bar_blob);
+    mbar_expect(&bar, 64u * v.nown + (32u * G + 48u) * v.ncell);
     bulk_g2s(sW, m.faceW + 4 * v.fbase, 32u * v.nown, &bar);
     bulk_g2s(sC, m.faceC + 4 * v.fbase, 32u * v.nown, &bar);
     bulk_g2s(sU, U + 4 * G * v.c0, 32u * G * v.ncell, &bar);
     bulk_g2s(sM, m.Minv + 6 * v.c0, 48u * v.ncell, &bar);
+    // a tile that starts a few gridfuls later: pull its contiguous runs into L2 now
+    const int64_t tp = (int64_t)blockIdx.x + m.prefetch_tiles;
+    if (tp < (int64_t)gridDim.x) {
+      const rt_tile dp = m.tiles[tp];
+      const int64_t cp = tp * m.TC;
+      const unsigned nc = (unsigned)(cp + m.TC < m.C ? m.TC : m.C - cp);
+      bulk_prefetch_l2(m.blob + dp.blob, 4u * rt_blob_words(m.TC, dp.nhf, dp.nown, dp.nh, dp.ninc, dp.nout));
+      bulk_prefetch_l2(m.faceW + 4 * dp.fbase, 32u * dp.nown);
+      bulk_prefetch_l2(m.faceC + 4 * dp.fbase, 32u * dp.nown);
+      bulk_prefetch_l2(U + 4 * G * cp, 32u * G * nc);
+      bulk_prefetch_l2(m.Minv + 6 * cp, 48u * nc);
+    }
   }
-  mbar_wait(&bar, 0);
+  mbar_wait(&bar_blob, 0);
   // round 2: what the blob locates: halo cells and incoming faces
   // (gathers of 32 to 96 bytes: 16-byte asynchronous copies, one halo cell / incoming face per thread)
   for (int h = tid; h < v.nh; h += nt) cp_run<2 * G>(sU + 4 * G * (m.TC + h), U + (int64_t)(4 * G) * v.halo[h]);
@@ -169,6 +188,7 @@ __global__ void __launch_bounds__(256) k_grad(rt_geom m, const double *__restric
     cp_run<2>(sW + 4 * (v.nown + j), m.faceW + 4 * q);
     cp_run<2>(sC + 4 * (v.nown + j), m.faceC + 4 * q);
   }
+  mbar_wait(&bar, 0);
   cp_wait_all();
   __syncthreads();
 
@@ -301,7 +321,7 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
                                                  double *__restrict__ part_out, double *__restrict__ part_in) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ double red[32];
-  __shared__ __align__(8) uint64_t bar;
+  __shared__ __align__(8) uint64_t bar, bar_blob;
   constexpr int NP = G > 3 ? G : 3;                        // planes of [omax][4]
   const int NE = m.TC + m.fmax;                            // tile cells, then forward halo cells
   const int OM = m.omax;
@@ -318,13 +338,14 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
   const tile_view v = view_tile(m, sB, tile);
   const int tid = threadIdx.x, nt = blockDim.x;
   const double dt = up.dt, ct = up.ct;
-  if (tid == 0) mbar_init(&bar, 1);
+  if (tid == 0) { mbar_init(&bar, 1); mbar_init(&bar_blob, 1); }
   __syncthreads();
   // round 1: what the descriptor locates: the blob, the owned faces and the tile's own cells
   if (tid == 0) {
     const unsigned nsb = (4u * v.ncell + 15u) & ~15u;  // srcidx is padded
-    mbar_expect(&bar, 4u * v.words + 96u * v.nown + ((SECOND ? 128u : 32u) * G + 32u + 32u * G) * v.ncell + nsb);
-    bulk_g2s(sB, v.blob, 4u * v.words, &bar);
+    mbar_expect(&bar_blob, 4u * v.words);
+    bulk_g2s(sB, v.blob, 4u * v.words, &bar_blob);
+    mbar_expect(&bar, 96u * v.nown + ((SECOND ? 128u : 32u) * G + 32u + 32u * G) * v.ncell + nsb);
     bulk_g2s(sF, m.faceC + 4 * v.fbase, 32u * v.nown, &bar);
     bulk_g2s(sF + 4 * OM, m.faceN + 4 * v.fbase, 32u * v.nown, &bar);
     bulk_g2s(sF + 8 * OM, m.faceW + 4 * v.fbase, 32u * v.nown, &bar);
@@ -333,8 +354,23 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
     bulk_g2s(sS, m.cellS + 4 * v.c0, 32u * v.ncell, &bar);
     bulk_g2s(sU0, U0 + 4 * G * v.c0, 32u * G * v.ncell, &bar);
     bulk_g2s(sSrc, srcidx + v.c0, nsb, &bar);
+    // a tile that starts a few gridfuls later: pull its contiguous runs into L2 now
+    const int64_t tp = (int64_t)blockIdx.x + m.prefetch_tiles;
+    if (tp < (int64_t)gridDim.x) {
+      const rt_tile dp = m.tiles[tp];
+      const int64_t cp = tp * m.TC;
+      const unsigned nc = (unsigned)(cp + m.TC < m.C ? m.TC : m.C - cp);
+      bulk_prefetch_l2(m.blob + dp.blob, 4u * rt_blob_words(m.TC, dp.nhf, dp.nown, dp.nh, dp.ninc, dp.nout));
+      bulk_prefetch_l2(m.faceC + 4 * dp.fbase, 32u * dp.nown);
+      bulk_prefetch_l2(m.faceN + 4 * dp.fbase, 32u * dp.nown);
+      bulk_prefetch_l2(m.faceW + 4 * dp.fbase, 32u * dp.nown);
+      bulk_prefetch_l2(Uin + 4 * G * cp, 32u * G * nc);
+      if (SECOND) bulk_prefetch_l2(grad + 12 * G * cp, 96u * G * nc);
+      bulk_prefetch_l2(m.cellS + 4 * cp, 32u * nc);
+      bulk_prefetch_l2(U0 + 4 * G * cp, 32u * G * nc);
+    }
   }
-  mbar_wait(&bar, 0);
+  mbar_wait(&bar_blob, 0);
   // round 2: what the blob locates: the forward halo cells (right cells of the outgoing faces)
   const int nf = v.nh - v.nb;
   // (gathers of 32 to 288 bytes: 16-byte asynchronous copies; a halo cell's gradients are split over G threads)
@@ -348,6 +384,7 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
       cp_run<2>(sS + 4 * (m.TC + h), m.cellS + 4 * id);
     }
   }
+  mbar_wait(&bar, 0);
   cp_wait_all();
   __syncthreads();
 
@@ -532,19 +569,23 @@ __global__ void __launch_bounds__(1024) k_reduce(reduce_job j0, reduce_job j1, i
   if (j1.ncount) j1.nrows = ((int64_t)*j1.ncount + 31) / 32;
   const int g = blockIdx.x;
   double s = 0.0, c = 0.0;
-  for (int64_t r = threadIdx.x; r < j.nrows; r += 1024) {  // Neumaier per thread
-    const double x = j.part[(size_t)r * G + g];
-    const double t = s + x;
-    c += fabs(s) >= fabs(x) ? (s - t) + x : (x - t) + s;
-    s = t;
-  }
-  if (gridDim.y == 1 && j1.part != j0.part)  // one job made of two partial-sum arrays
-    for (int64_t r = threadIdx.x; r < j1.nrows; r += 1024) {
-      const double x = j1.part[(size_t)r * G + g];
-      const double t = s + x;
-      c += fabs(s) >= fabs(x) ? (s - t) + x : (x - t) + s;
-      s = t;
+  // Neumaier per thread over rows tid, tid + 1024, ...: eight loads in flight, added in row order
+  // (a padding zero changes neither the sum nor the compensation)
+  auto sum_rows = [&](const double *part, int64_t nrows) {
+    for (int64_t r = threadIdx.x; r < nrows; r += 8 * 1024) {
+      double x[8];
+#pragma unroll
+      for (int u = 0; u < 8; u++) { const int64_t rr = r + 1024 * u; x[u] = rr < nrows ? part[(size_t)rr * G + g] : 0.0; }
+#pragma unroll
+      for (int u = 0; u < 8; u++) {
+        const double t = s + x[u];
+        c += fabs(s) >= fabs(x[u]) ? (s - t) + x[u] : (x[u] - t) + s;
+        s = t;
+      }
     }
+  };
+  sum_rows(j.part, j.nrows);
+  if (gridDim.y == 1 && j1.part != j0.part) sum_rows(j1.part, j1.nrows);  // one job made of two partial-sum arrays
   sm[threadIdx.x] = s + c;
   __syncthreads();
   for (int o = 512; o > 0; o >>= 1) {
@@ -665,10 +706,11 @@ static int tile_threads(const rt_ctx *) {
   if (env < 0) env = env_int("RT_TILE_THREADS");
   return round_threads(env > 0 ? env : 256);
 }
-static int grad_threads(const rt_ctx *c) {
+static int grad_threads(const rt_ctx *c) {  // one thread per (cell, group), at most k_grad's launch bound
   static int env = -1;
   if (env < 0) env = env_int("RT_GRAD_THREADS");
-  return round_threads(env > 0 ? env : c->TC * c->G);
+  const int n = round_threads(env > 0 ? env : c->TC * c->G);
+  return n > 192 ? 192 : n;
 }
 
 rt_geom rt_geom_of(const rt_ctx *c) {
@@ -679,6 +721,11 @@ rt_geom rt_geom_of(const rt_ctx *c) {
   m.faceC = rt_ptr<double>(c, l.faceC); m.faceN = rt_ptr<double>(c, l.faceN); m.faceW = rt_ptr<double>(c, l.faceW);
   m.tiles = rt_ptr<rt_tile>(c, l.tiles); m.blob = rt_ptr<uint32_t>(c, l.blob);
   m.xphi = rt_ptr<double>(c, l.xphi);
+  {
+    static int ahead = -1;
+    if (ahead < 0) { const char *e = getenv("RT_PREFETCH_TILES"); ahead = e ? atoi(e) : 600; }
+    m.prefetch_tiles = ahead > 0 ? ahead : (1 << 30);
+  }
   m.ghost = rt_ptr<double>(c, l.ghost);
   for (int a = 0; a < 3; a++) { m.box[a] = c->box[a]; m.per[a] = c->per[a]; }
   return m;

@@ -84,7 +84,8 @@ struct rt_ctx {
   int omax;           // most owned faces of any tile
   int nsm;            // multiprocessors of the device (0 until first needed)
   int64_t n2;         // cells with at least one incoming face
-  int bmax;           // largest blob of any tile, in 32-bit words
+  int bmax;           // largest blob of any tile, in 32-bit words (without the header)
+  int bstride;        // words between the blobs of consecutive tiles
   int64_t ninc;       // total incoming faces over all tiles
   int64_t nhalo;      // total halo cells over all tiles
   int64_t blob_words; // total blob size
@@ -120,6 +121,7 @@ struct rt_tile {
   int32_t nown, ninc, nh, nhf;  // owned faces, incoming faces, halo cells, half-faces
   int32_t nb, nout, n2, pad;    // backward halo cells, outgoing faces, cells with incoming faces
 };
+#define RT_BLOB_HEAD 12     // 32-bit words of the descriptor copy at the start of a blob
 #define RT_TILE_LIMIT 2048  // most owned faces / r-list entries / halo candidates of a tile the builder handles
 __host__ __device__ static inline int rt_blob_words(int TC, int nhf, int nown, int nh, int ninc, int nout) {
   return (TC + 1 + nhf + nown + nh + ninc + nout + 3) & ~3;

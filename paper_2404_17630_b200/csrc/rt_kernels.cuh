@@ -19,7 +19,7 @@ struct rt_geom {
   const double *ghost;
   double box[3];
   int per[3];
-  int G, TC, smax, omax, hmax, fmax, bmax;
+  int G, TC, smax, omax, hmax, fmax, bmax, bstride;
   int prefetch_tiles;    // the tile kernels ask L2 for the data of tile t + prefetch_tiles
 };
 

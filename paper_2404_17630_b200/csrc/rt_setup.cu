@@ -227,7 +227,7 @@ template <int MODE>
 __global__ void __launch_bounds__(TILE_BT) k_tile_build(int64_t C, int TC, const int64_t *fo, const int64_t *ro,
                                                         const int32_t *R, const int32_t *rl, const int32_t *rn,
                                                         int64_t *tsize, int64_t *xcnt, int64_t *icnt, int64_t *n2cnt,
-                                                        tile_max *mx, const int64_t *boff, const int64_t *xoff,
+                                                        tile_max *mx, int64_t bstride, const int64_t *xoff,
                                                         const int64_t *ibase, const int64_t *k2base, rt_tile *tiles,
                                                         uint32_t *blob, int32_t *faceX, int32_t *k2cell, int32_t *k2off) {
   typedef cub::BlockScan<int, TILE_BT> Scan;
@@ -353,12 +353,13 @@ __global__ void __launch_bounds__(TILE_BT) k_tile_build(int64_t C, int TC, const
   }
   if (threadIdx.x == 0) {
     rt_tile d;
-    d.fbase = fbase; d.blob = boff[t]; d.xbase = xoff[t]; d.nown = nown; d.ninc = ninc; d.nh = nh; d.nhf = nhf;
+    d.fbase = fbase; d.blob = t * bstride; d.xbase = xoff[t]; d.nown = nown; d.ninc = ninc; d.nh = nh; d.nhf = nhf;
     d.nb = nb; d.nout = nout; d.n2 = n2; d.pad = 0;
     tiles[t] = d;
+    *reinterpret_cast<rt_tile *>(blob + t * bstride) = d;  // the blob starts with a copy of the descriptor
     if (t == (int64_t)gridDim.x - 1) k2off[k2base[t] + n2] = (int32_t)(ibase[t] + ninc);  // end of the last cell's rows
   }
-  uint32_t *ho = blob + boff[t], *hl = ho + TC + 1, *slr = hl + nhf, *halo = slr + nown, *incf = halo + nh;
+  uint32_t *ho = blob + t * bstride + RT_BLOB_HEAD, *hl = ho + TC + 1, *slr = hl + nhf, *halo = slr + nown, *incf = halo + nh;
   uint32_t *outs = incf + ninc;
   for (int k = threadIdx.x; k < nown; k += TILE_BT)
     if (s_cand[k] >= 0) { outs[s_cand[k]] = (uint32_t)k; faceX[fbase + k] = (int32_t)(xoff[t] + s_cand[k]); }
@@ -393,7 +394,7 @@ __global__ void __launch_bounds__(TILE_BT) k_tile_build(int64_t C, int TC, const
 __global__ void __launch_bounds__(TILE_BT) k_tile_rows(int TC, const rt_tile *tiles, const uint32_t *blob, const int64_t *ibase,
                                                        const int32_t *faceX, int32_t *k2row) {
   const rt_tile d = tiles[blockIdx.x];
-  const uint32_t *incf = blob + d.blob + TC + 1 + d.nhf + d.nown + d.nh;
+  const uint32_t *incf = blob + d.blob + RT_BLOB_HEAD + TC + 1 + d.nhf + d.nown + d.nh;
   for (int j = threadIdx.x; j < d.ninc; j += TILE_BT) k2row[ibase[blockIdx.x] + j] = faceX[incf[j]];
 }
 
@@ -528,7 +529,7 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
       for (int TC = tc0; TC >= RT_MIN_TILE; TC -= TC > 32 ? 8 : 4) {
         const int64_t T = (C + TC - 1) / TC;
         RT_CUDA(c, cudaMemsetAsync(mx, 0, sizeof(tile_max), st));
-        k_tile_build<0><<<(unsigned)T, TILE_BT, 0, st>>>(C, TC, fo, ro, R, rl, rn, tsize, xcnt, icnt, n2cnt, mx, nullptr, nullptr,
+        k_tile_build<0><<<(unsigned)T, TILE_BT, 0, st>>>(C, TC, fo, ro, R, rl, rn, tsize, xcnt, icnt, n2cnt, mx, 0, nullptr,
                                                         nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
         RT_CUDA(c, cudaMemcpyAsync(&hm, mx, sizeof(tile_max), cudaMemcpyDeviceToHost, st));
         RT_CUDA(c, cudaStreamSynchronize(st));
@@ -549,7 +550,9 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
       RT_CUDA(c, cudaMemsetAsync(cnt[a] + c->T, 0, 8, st));
       RT_CUDA(c, cub::DeviceScan::ExclusiveSum(cub_tmp, b, cnt[a], off[a], c->T + 1, st));
     }
-    RT_CUDA(c, cudaMemcpyAsync(&c->blob_words, boff + c->T, 8, cudaMemcpyDeviceToHost, st));
+    // blobs at a fixed stride, so that a kernel finds a tile's blob without reading its descriptor first
+    c->bstride = (hm.words + RT_BLOB_HEAD + 3) & ~3;
+    c->blob_words = (int64_t)c->bstride * c->T;
     RT_CUDA(c, cudaMemcpyAsync(&c->ninc, xoff + c->T, 8, cudaMemcpyDeviceToHost, st));
     RT_CUDA(c, cudaMemcpyAsync(&c->n2, k2base + c->T, 8, cudaMemcpyDeviceToHost, st));
     RT_CUDA(c, cudaStreamSynchronize(st));
@@ -561,7 +564,7 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
                      (long long)c->ninc, (long long)lay.xcap);
     rt_tile *tiles = rt_ptr<rt_tile>(c, lay.tiles);
     uint32_t *blob = rt_ptr<uint32_t>(c, lay.blob);
-    k_tile_build<1><<<(unsigned)c->T, TILE_BT, 0, st>>>(C, best, fo, ro, R, rl, rn, nullptr, nullptr, nullptr, nullptr, mx, boff,
+    k_tile_build<1><<<(unsigned)c->T, TILE_BT, 0, st>>>(C, best, fo, ro, R, rl, rn, nullptr, nullptr, nullptr, nullptr, mx, c->bstride,
                                                        xoff, ibase, k2base, tiles, blob, faceX,
                                                        rt_ptr<int32_t>(c, lay.k2cell), rt_ptr<int32_t>(c, lay.k2off));
     k_tile_rows<<<(unsigned)c->T, TILE_BT, 0, st>>>(best, tiles, blob, ibase, faceX, rt_ptr<int32_t>(c, lay.k2row));
@@ -598,7 +601,7 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G, int flags) {
   // tile tables: descriptors for the smallest tile size; blobs bounded by
   // sum_t (TC + 4) + half-faces (<= 2F) + slots (<= 2F) + halo (<= 2F) + incoming (<= F) words
   l.tiles = take(sizeof(rt_tile) * (size_t)(l.max_tiles + 1));
-  l.blob_bytes = 4 * ((size_t)(5.5 * (double)F) + 2 * (size_t)C + 5 * (size_t)l.max_tiles + 2048);
+  l.blob_bytes = 4 * ((size_t)(6.5 * (double)F) + 2 * (size_t)C + 5 * (size_t)l.max_tiles + 2048);
   l.blob = take(l.blob_bytes);
   // fluxes of the faces that cross tile boundaries, written by the owner tile (<= 56 % of the
   // faces; rt_mesh_upload fails with RT_ENOMEM on a mesh whose tiles need more)

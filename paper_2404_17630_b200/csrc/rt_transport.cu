@@ -129,17 +129,18 @@ struct tile_view {
   const uint32_t *ho, *hl, *slr, *halo, *incf, *outs;  // in shared memory
   const uint32_t *blob;                                // in global memory
 };
+// the view of a tile whose blob (header + tables) has landed in shared memory at sB
 __device__ __forceinline__ tile_view view_tile(const rt_geom &m, const uint32_t *sB, unsigned tile) {
-  const rt_tile d = m.tiles[tile];
+  const rt_tile d = *reinterpret_cast<const rt_tile *>(sB);
   tile_view v;
   v.c0 = (int64_t)tile * m.TC;
   v.ncell = (int)(v.c0 + m.TC < m.C ? m.TC : m.C - v.c0);
   v.fbase = d.fbase; v.xbase = d.xbase; v.nown = d.nown; v.ninc = d.ninc; v.ns = d.nown + d.ninc; v.nh = d.nh; v.nhf = d.nhf;
   v.nb = d.nb; v.nout = d.nout;
   v.words = rt_blob_words(m.TC, v.nhf, v.nown, v.nh, v.ninc, v.nout);
-  v.ho = sB; v.hl = v.ho + m.TC + 1; v.slr = v.hl + v.nhf; v.halo = v.slr + v.nown; v.incf = v.halo + v.nh;
+  v.ho = sB + RT_BLOB_HEAD; v.hl = v.ho + m.TC + 1; v.slr = v.hl + v.nhf; v.halo = v.slr + v.nown; v.incf = v.halo + v.nh;
   v.outs = v.incf + v.ninc;
-  v.blob = m.blob + d.blob;
+  v.blob = m.blob + (size_t)tile * m.bstride;
   return v;
 }
 
@@ -148,19 +149,24 @@ template <int G>
 __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__restrict__ U, double *__restrict__ grad) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar, bar_blob;
-  uint32_t *sB = reinterpret_cast<uint32_t *>(smem_raw);  // the tile's blob
-  double *sW = reinterpret_cast<double *>(sB + m.bmax);   // [smax][4]  (w, kappa)
+  uint32_t *sB = reinterpret_cast<uint32_t *>(smem_raw);    // the tile's blob
+  double *sW = reinterpret_cast<double *>(sB + m.bstride);  // [smax][4]  (w, kappa)
   double *sC = sW + 4 * m.smax;                           // [smax][4]  (c - s_L, A)
   double *sU = sC + 4 * m.smax;                           // [(TC + hmax) G][4]  tile cells, then halo cells
   double *sM = sU + 4 * G * (m.TC + m.hmax);              // [TC][6]
-  const tile_view v = view_tile(m, sB, blockIdx.x);
   const int tid = threadIdx.x, nt = blockDim.x;
   if (tid == 0) { mbar_init(&bar, 1); mbar_init(&bar_blob, 1); }
   __syncthreads();
-  // round 1: what the descriptor locates: the blob, the owned faces and the tile's own cells
+  // round 1: the tile's blob sits at a fixed stride: header (descriptor) + tables
   if (tid == 0) {
-    mbar_expect(&bar_blob, 4u * v.words);
-    bulk_g2s(sB, v.blob, 4u * v.words, &bar_blob);
+    mbar_expect(&bar_blob, 4u * m.bstride);
+    bulk_g2s(sB, m.blob + (size_t)blockIdx.x * m.bstride, 4u * m.bstride, &bar_blob);
+  }
+  mbar_wait(&bar_blob, 0);
+  const tile_view v = view_tile(m, sB, blockIdx.x);
+  // round 2: what the descriptor locates (bulk copies: owned faces, the tile's own cells) and what the
+  // tables locate (gathers: halo cells, incoming faces), all in flight together
+  if (tid == 0) {
     mbar_expect(&bar, 64u * v.nown + (32u * G + 48u) * v.ncell);
     bulk_g2s(sW, m.faceW + 4 * v.fbase, 32u * v.nown, &bar);
     bulk_g2s(sC, m.faceC + 4 * v.fbase, 32u * v.nown, &bar);
@@ -172,14 +178,13 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
       const rt_tile dp = m.tiles[tp];
       const int64_t cp = tp * m.TC;
       const unsigned nc = (unsigned)(cp + m.TC < m.C ? m.TC : m.C - cp);
-      bulk_prefetch_l2(m.blob + dp.blob, 4u * rt_blob_words(m.TC, dp.nhf, dp.nown, dp.nh, dp.ninc, dp.nout));
+      bulk_prefetch_l2(m.blob + (size_t)tp * m.bstride, 4u * m.bstride);
       bulk_prefetch_l2(m.faceW + 4 * dp.fbase, 32u * dp.nown);
       bulk_prefetch_l2(m.faceC + 4 * dp.fbase, 32u * dp.nown);
       bulk_prefetch_l2(U + 4 * G * cp, 32u * G * nc);
       bulk_prefetch_l2(m.Minv + 6 * cp, 48u * nc);
     }
   }
-  mbar_wait(&bar_blob, 0);
   // round 2: what the blob locates: halo cells and incoming faces
   // (gathers of 32 to 96 bytes: 16-byte asynchronous copies, one halo cell / incoming face per thread)
   for (int h = tid; h < v.nh; h += nt) cp_run<2 * G>(sU + 4 * G * (m.TC + h), U + (int64_t)(4 * G) * v.halo[h]);
@@ -326,7 +331,7 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
   const int NE = m.TC + m.fmax;                            // tile cells, then forward halo cells
   const int OM = m.omax;
   uint32_t *sB = reinterpret_cast<uint32_t *>(smem_raw);   // the tile's blob
-  double *sF = reinterpret_cast<double *>(sB + m.bmax);    // [NP][omax][4]: planes 0-2 hold the staged face records
+  double *sF = reinterpret_cast<double *>(sB + m.bstride); // [NP][omax][4]: planes 0-2 hold the staged face records
                                                            // (c, A), (n, -), (w, kappa); a slot's warp then
                                                            // overwrites plane g with A * (Phi_N, Phi_F) of group g
   double *sU = sF + 4 * NP * OM;                           // [NE][G][4]
@@ -335,16 +340,21 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
   double *sU0 = sS + 4 * NE;                               // [TC][G][4]  U^n of the tile's cells
   int32_t *sSrc = reinterpret_cast<int32_t *>(sU0 + 4 * G * m.TC);  // [TC] source index or -1
   const unsigned tile = blockIdx.x;
-  const tile_view v = view_tile(m, sB, tile);
   const int tid = threadIdx.x, nt = blockDim.x;
   const double dt = up.dt, ct = up.ct;
   if (tid == 0) { mbar_init(&bar, 1); mbar_init(&bar_blob, 1); }
   __syncthreads();
-  // round 1: what the descriptor locates: the blob, the owned faces and the tile's own cells
+  // round 1: the tile's blob sits at a fixed stride: header (descriptor) + tables
+  if (tid == 0) {
+    mbar_expect(&bar_blob, 4u * m.bstride);
+    bulk_g2s(sB, m.blob + (size_t)tile * m.bstride, 4u * m.bstride, &bar_blob);
+  }
+  mbar_wait(&bar_blob, 0);
+  const tile_view v = view_tile(m, sB, tile);
+  // round 2: what the descriptor locates (bulk copies: owned faces, the tile's own cells) and what the
+  // tables locate (gathers: forward halo cells), all in flight together
   if (tid == 0) {
     const unsigned nsb = (4u * v.ncell + 15u) & ~15u;  // srcidx is padded
-    mbar_expect(&bar_blob, 4u * v.words);
-    bulk_g2s(sB, v.blob, 4u * v.words, &bar_blob);
     mbar_expect(&bar, 96u * v.nown + ((SECOND ? 128u : 32u) * G + 32u + 32u * G) * v.ncell + nsb);
     bulk_g2s(sF, m.faceC + 4 * v.fbase, 32u * v.nown, &bar);
     bulk_g2s(sF + 4 * OM, m.faceN + 4 * v.fbase, 32u * v.nown, &bar);
@@ -360,7 +370,7 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
       const rt_tile dp = m.tiles[tp];
       const int64_t cp = tp * m.TC;
       const unsigned nc = (unsigned)(cp + m.TC < m.C ? m.TC : m.C - cp);
-      bulk_prefetch_l2(m.blob + dp.blob, 4u * rt_blob_words(m.TC, dp.nhf, dp.nown, dp.nh, dp.ninc, dp.nout));
+      bulk_prefetch_l2(m.blob + (size_t)tp * m.bstride, 4u * m.bstride);
       bulk_prefetch_l2(m.faceC + 4 * dp.fbase, 32u * dp.nown);
       bulk_prefetch_l2(m.faceN + 4 * dp.fbase, 32u * dp.nown);
       bulk_prefetch_l2(m.faceW + 4 * dp.fbase, 32u * dp.nown);
@@ -370,7 +380,6 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
       bulk_prefetch_l2(U0 + 4 * G * cp, 32u * G * nc);
     }
   }
-  mbar_wait(&bar_blob, 0);
   // round 2: what the blob locates: the forward halo cells (right cells of the outgoing faces)
   const int nf = v.nh - v.nb;
   // (gathers of 32 to 288 bytes: 16-byte asynchronous copies; a halo cell's gradients are split over G threads)
@@ -388,22 +397,16 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
   cp_wait_all();
   __syncthreads();
 
-  // ---- a3: one lane per (face slot, group); a slot's groups sit in one warp, which reads the staged
-  // face record before any of its lanes overwrites it with the fluxes
-  constexpr int SPW = 32 / G;  // slots per warp pass
-  const int lane = tid & 31, warp = tid >> 5, nw = nt >> 5;
-  const int sl = lane / G, g = lane - sl * G;
-  double b_out = 0.0, b_in = 0.0;
+  // ---- a3: one thread per owned face: its record is read once into registers (so the thread may
+  // overwrite it in shared memory with the fluxes), then every group in turn
+  double b_out[G], b_in[G];
+#pragma unroll
+  for (int g = 0; g < G; g++) b_out[g] = b_in[g] = 0.0;
   int bnd = 0;
   const double hc2 = 0.5 * ct * ct, hc = 0.5 * ct;
-  for (int sb = warp * SPW; sb < v.nown; sb += nw * SPW) {
-    const int s = sb + sl;
-    const bool on = sl < SPW && s < v.nown;
-    double4 fc = make_double4(0, 0, 0, 1), fn = make_double4(0, 0, 0, 0), fw = make_double4(0, 0, 0, 0);
-    uint32_t lr = 0;
-    if (on) { fc = ld4(sF + 4 * s); fn = ld4(sF + 4 * (OM + s)); fw = ld4(sF + 4 * (2 * OM + s)); lr = v.slr[s]; }
-    __syncwarp();
-    if (!on) continue;
+  for (int s = tid; s < v.nown; s += nt) {
+    const double4 fc = ld4(sF + 4 * s), fn = ld4(sF + 4 * (OM + s)), fw = ld4(sF + 4 * (2 * OM + s));
+    const uint32_t lr = v.slr[s];
     const int xl = (int)(lr & 0xffffu);
     int xr = (int)(lr >> 16);
     const bool rin = xr < 0xFF00;
@@ -413,34 +416,40 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
     const double A = fc.w;
     const double rdtA = fast_rcp(dt * A);
     const double capL = sS[4 * xl + 3] * rdtA;
-    double UL[4], UR[4], NL, NR = 0.0, capR = 0.0;
     // the face centre relative to the left cell is stored; relative to the right cell it is c - kappa w
-    extrapolate<SECOND>(sU + 4 * (xl * G + g), sG + 12 * (xl * G + g), fc.x, fc.y, fc.z, UL, NL);
+    double capR = 0.0, rRx = 0.0, rRy = 0.0, rRz = 0.0;
     if (rin) {
       capR = sS[4 * xr + 3] * rdtA;
-      const double rRx = fma(-fw.w, fw.x, fc.x), rRy = fma(-fw.w, fw.y, fc.y), rRz = fma(-fw.w, fw.z, fc.z);
-      extrapolate<SECOND>(sU + 4 * (xr * G + g), sG + 12 * (xr * G + g), rRx, rRy, rRz, UR, NR);
-    } else if (r == RT_BC_OUTFLOW) { UR[0] = UR[1] = UR[2] = UR[3] = 0.0; }  // vacuum ghost
-    else if (r == RT_BC_REFLECT) {
-      const double p = 2.0 * (UL[1] * n[0] + UL[2] * n[1] + UL[3] * n[2]);
-      UR[0] = UL[0]; UR[1] = UL[1] - p * n[0]; UR[2] = UL[2] - p * n[1]; UR[3] = UL[3] - p * n[2];
-    } else {
-      const double4 gs = ld4(m.ghost + ((size_t)(RT_BC_DIRICHLET0 - r) * G + g) * 4);
-      UR[0] = gs.x; UR[1] = gs.y; UR[2] = gs.z; UR[3] = gs.w;
+      rRx = fma(-fw.w, fw.x, fc.x); rRy = fma(-fw.w, fw.y, fc.y); rRz = fma(-fw.w, fw.z, fc.z);
     }
-    double PL[3], PR[3], ph[4];
-    pressure_dot_n(UL, n, ct, PL);
-    pressure_dot_n(UR, n, ct, PR);
-    ph[0] = 0.5 * ((UL[1] + UR[1]) * n[0] + (UL[2] + UR[2]) * n[1] + (UL[3] + UR[3]) * n[2]) - hc * (UR[0] - UL[0]);
+    const int xrr = rin ? xr : xl;
 #pragma unroll
-    for (int a = 0; a < 3; a++) ph[1 + a] = hc2 * (PL[a] + PR[a]) - hc * (UR[1 + a] - UL[1 + a]);
-    // donor cap (S11): the donor cannot lose more photons than it holds through this face in dt;
-    // only the number flux is clamped (continuous in the state; Phi_F is left alone)
-    if (ph[0] > 0.0) ph[0] = dmin2(ph[0], NL * capL);
-    else if (rin) ph[0] = -dmin2(-ph[0], NR * capR);
-    st4(sF + 4 * (g * OM + s), A * ph[0], A * ph[1], A * ph[2], A * ph[3]);
-    if (r == RT_BC_OUTFLOW) { b_out += A * ph[0]; bnd = 1; }
-    else if (r <= RT_BC_DIRICHLET0) { b_in -= A * ph[0]; bnd = 1; }
+    for (int g = 0; g < G; g++) {
+      double UL[4], UR[4], NL, NR = 0.0;
+      extrapolate<SECOND>(sU + 4 * (xl * G + g), sG + 12 * (xl * G + g), fc.x, fc.y, fc.z, UL, NL);
+      if (rin) extrapolate<SECOND>(sU + 4 * (xrr * G + g), sG + 12 * (xrr * G + g), rRx, rRy, rRz, UR, NR);
+      else if (r == RT_BC_OUTFLOW) { UR[0] = UR[1] = UR[2] = UR[3] = 0.0; }  // vacuum ghost
+      else if (r == RT_BC_REFLECT) {
+        const double p = 2.0 * (UL[1] * n[0] + UL[2] * n[1] + UL[3] * n[2]);
+        UR[0] = UL[0]; UR[1] = UL[1] - p * n[0]; UR[2] = UL[2] - p * n[1]; UR[3] = UL[3] - p * n[2];
+      } else {
+        const double4 gs = ld4(m.ghost + ((size_t)(RT_BC_DIRICHLET0 - r) * G + g) * 4);
+        UR[0] = gs.x; UR[1] = gs.y; UR[2] = gs.z; UR[3] = gs.w;
+      }
+      double PL[3], PR[3], ph[4];
+      pressure_dot_n(UL, n, ct, PL);
+      pressure_dot_n(UR, n, ct, PR);
+      ph[0] = 0.5 * ((UL[1] + UR[1]) * n[0] + (UL[2] + UR[2]) * n[1] + (UL[3] + UR[3]) * n[2]) - hc * (UR[0] - UL[0]);
+#pragma unroll
+      for (int a = 0; a < 3; a++) ph[1 + a] = hc2 * (PL[a] + PR[a]) - hc * (UR[1 + a] - UL[1 + a]);
+      // donor cap (S11): the donor cannot lose more photons than it holds through this face in dt;
+      // only the number flux is clamped (continuous in the state; Phi_F is left alone)
+      if (ph[0] > 0.0) ph[0] = dmin2(ph[0], NL * capL);
+      else if (rin) ph[0] = -dmin2(-ph[0], NR * capR);
+      st4(sF + 4 * (g * OM + s), A * ph[0], A * ph[1], A * ph[2], A * ph[3]);
+      if (r == RT_BC_OUTFLOW) { b_out[g] += A * ph[0]; bnd = 1; }
+      else if (r <= RT_BC_DIRICHLET0) { b_in[g] -= A * ph[0]; bnd = 1; }
+    }
   }
   __syncthreads();  // every owned slot holds its fluxes
   // the outgoing faces' fluxes go to xphi for the tiles of their right cells (k_finish)
@@ -456,7 +465,7 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
   if (__syncthreads_or(bnd)) {
 #pragma unroll
     for (int gg = 0; gg < G; gg++) {
-      const double so = block_sum(g == gg ? b_out : 0.0, red), si = block_sum(g == gg ? b_in : 0.0, red);
+      const double so = block_sum(b_out[gg], red), si = block_sum(b_in[gg], red);
       if (tid == 0) { part_out[(size_t)tile * G + gg] = so; part_in[(size_t)tile * G + gg] = si; }
     }
   } else if (tid < G) {
@@ -688,7 +697,7 @@ static cudaError_t allow_smem(K kernel, size_t bytes) {
 
 int rt_transport_configure(rt_ctx *c) {
   cudaError_t e = cudaSuccess;
-  const size_t sg = rt_smem_grad(c->TC, c->G, c->smax, c->hmax, c->bmax), ss = rt_smem_flux(c->TC, c->G, c->omax, c->fmax, c->bmax);
+  const size_t sg = rt_smem_grad(c->TC, c->G, c->smax, c->hmax, c->bstride), ss = rt_smem_flux(c->TC, c->G, c->omax, c->fmax, c->bstride);
   SET_SMEM_G(c->G, K_GRAD, sg, e);
   if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX2, ss, e);
   if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX1, ss, e);
@@ -716,7 +725,7 @@ static int grad_threads(const rt_ctx *c) {  // one thread per (cell, group), at 
 rt_geom rt_geom_of(const rt_ctx *c) {
   const rt_layout &l = c->lay;
   rt_geom m;
-  m.C = c->C; m.F = c->F; m.G = c->G; m.TC = c->TC; m.smax = c->smax; m.omax = c->omax; m.hmax = c->hmax; m.fmax = c->fmax; m.bmax = c->bmax;
+  m.C = c->C; m.F = c->F; m.G = c->G; m.TC = c->TC; m.smax = c->smax; m.omax = c->omax; m.hmax = c->hmax; m.fmax = c->fmax; m.bmax = c->bmax; m.bstride = c->bstride;
   m.cellS = rt_ptr<double>(c, l.cellS); m.Minv = rt_ptr<double>(c, l.Minv);
   m.faceC = rt_ptr<double>(c, l.faceC); m.faceN = rt_ptr<double>(c, l.faceN); m.faceW = rt_ptr<double>(c, l.faceW);
   m.tiles = rt_ptr<rt_tile>(c, l.tiles); m.blob = rt_ptr<uint32_t>(c, l.blob);
@@ -732,7 +741,7 @@ rt_geom rt_geom_of(const rt_ctx *c) {
 }
 
 int rt_launch_gradients(rt_ctx *c, const double *U) {
-  DISPATCH_G(c->G, K_GRAD, (unsigned)c->T, grad_threads(c), rt_smem_grad(c->TC, c->G, c->smax, c->hmax, c->bmax), c->stream, rt_geom_of(c), U,
+  DISPATCH_G(c->G, K_GRAD, (unsigned)c->T, grad_threads(c), rt_smem_grad(c->TC, c->G, c->smax, c->hmax, c->bstride), c->stream, rt_geom_of(c), U,
              rt_ptr<double>(c, c->lay.grad));
   c->launches++;
   return RT_OK;
@@ -758,14 +767,14 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
   double *p_floor = part + (size_t)G * nchem * RT_CHEM_MAXPASS, *p_out = p_floor + (size_t)G * c->T, *p_in = p_out + (size_t)G * c->T;
   double *p_floor2 = p_in + (size_t)G * c->T;
   const int nt = tile_threads(c);
-  const size_t ss = rt_smem_flux(c->TC, G, c->omax, c->fmax, c->bmax);
+  const size_t ss = rt_smem_flux(c->TC, G, c->omax, c->fmax, c->bstride);
   const update_par up = {ca, cb, dt, c->par.ctilde, c->par.n_floor};
   double *pacc = rt_ptr<double>(c, l.pacc);
   const int32_t *srcidx = rt_ptr<int32_t>(c, l.srcidx);
   const double *srcrate = rt_ptr<double>(c, l.srcrate);
   if (c->par.order >= 2) {
     rt_prof_begin(c, RT_K_GRAD);
-    DISPATCH_G(G, K_GRAD, (unsigned)c->T, grad_threads(c), rt_smem_grad(c->TC, G, c->smax, c->hmax, c->bmax), c->stream, m, Uin, grad);
+    DISPATCH_G(G, K_GRAD, (unsigned)c->T, grad_threads(c), rt_smem_grad(c->TC, G, c->smax, c->hmax, c->bstride), c->stream, m, Uin, grad);
     rt_prof_end(c);
     c->launches++;
     rt_prof_begin(c, RT_K_FLUX);

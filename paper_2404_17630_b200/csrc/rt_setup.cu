@@ -605,7 +605,12 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G, int flags) {
   l.blob = take(l.blob_bytes);
   // fluxes of the faces that cross tile boundaries, written by the owner tile (<= 56 % of the
   // faces; rt_mesh_upload fails with RT_ENOMEM on a mesh whose tiles need more)
-  l.xcap = (int64_t)(0.56 * (double)F) + 1024;
+  {
+    // (small tiles, which only RT_TILE_CELLS asks for, let up to every face cross a tile boundary)
+    const char *env = getenv("RT_TILE_CELLS");
+    const double frac = env && atoi(env) >= RT_MIN_TILE && atoi(env) < 32 ? 1.0 : 0.56;
+    l.xcap = (int64_t)(frac * (double)F) + 1024;
+  }
   l.xphi = take(32 * (size_t)G * (size_t)l.xcap);
   // cells with incoming faces and the xphi rows of those faces (k_finish)
   l.k2cell = take(4 * (size_t)C); l.k2off = take(4 * ((size_t)C + 1)); l.k2row = take(4 * (size_t)l.xcap);

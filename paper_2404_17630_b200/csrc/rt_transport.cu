@@ -48,6 +48,15 @@ __device__ __forceinline__ double fast_sqrt(double x) {
   return fma(g, r, g);
 }
 
+// 1/sqrt(x) for positive normal x: MUFU.RSQ64H seed, two Newton steps
+__device__ __forceinline__ double fast_rsqrt(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double hx = 0.5 * x;
+  y = y * fma(-hx * y, y, 1.5);
+  return y * fma(-hx * y, y, 1.5);
+}
+
 // neighbour or ghost state seen across a boundary face with right code `code` (S13)
 __device__ __forceinline__ double4 ghost_for_gradient(int code, const double4 Ui, const double *faceN, int64_t q,
                                                       const double *ghost, int G, int g) {
@@ -313,7 +322,10 @@ __device__ __forceinline__ double finish_cell(double a0, double a1, double a2, d
   double add = 0.0;
   if (Un[0] < p.n_floor) { add = V * (p.n_floor - Un[0]); Un[0] = p.n_floor; }
   const double f2 = Un[1] * Un[1] + Un[2] * Un[2] + Un[3] * Un[3], lim = p.ct * Un[0];
-  if (f2 > lim * lim) { const double sc = lim / sqrt(f2); Un[1] *= sc; Un[2] *= sc; Un[3] *= sc; }
+  if (f2 > lim * lim) {  // |F| <= c~ N (S12); 1/sqrt from the MUFU seed where f2 is safely normal
+    const double sc = f2 > 1e-280 ? lim * fast_rsqrt(f2) : lim / sqrt(f2);
+    Un[1] *= sc; Un[2] *= sc; Un[3] *= sc;
+  }
   st4(out, Un[0], Un[1], Un[2], Un[3]);
   return add;
 }
@@ -492,7 +504,7 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
     const double *pg = sF + 4 * ig * OM;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
     int incomplete = 0;
-#pragma unroll 2
+#pragma unroll 4
     for (int k = h0 + p; k < h1; k += P) {
       const uint32_t w = v.hl[k];
       const int s = (int)(w & 0x7fffu);

@@ -163,3 +163,74 @@ def test_errors_are_reported_not_thrown_across_the_abi():
     with pytest.raises(rt.RTError, match="workspace has"):
         rt.rt_mesh_upload(h, mesh, 1, None, ws)
     rt.rt_destroy(h)
+
+
+def _regroup(w, G):
+    """The config-2 workload with G frequency groups: cross-sections, heating energies and source
+    shares of the three stock groups spread over G (input generation only, no method arithmetic)."""
+    rs = np.random.RandomState(100 + G)
+    C = w.mesh.ncell
+    pick = np.arange(G) % 3
+    scale = rs.uniform(0.6, 1.4, (G, 1))
+    p = w.params
+    p.ngroup = G
+    p.sigma = cfg.SIGMA3[pick] * scale
+    p.eps_heat = cfg.EPS3[pick] * rs.uniform(0.8, 1.2, (G, 1))
+    share = rs.uniform(0.2, 1.0, G); share /= share.sum()
+    total = w.sources.rate.sum(0)
+    src = cfg.Sources(w.sources.cell, share[:, None] * total[None, :])
+    N = np.repeat(w.state.N[:1], G, 0) * rs.uniform(0.5, 2.0, (G, C))
+    F = rs.randn(G, 3, C) * 0.05 * p.ctilde * N[:, None, :]
+    st = cfg.State(N, F, w.state.xHII, w.state.xHeII, w.state.xHeIII, w.state.eth, w.state.nH)
+    return cfg.Workload(w.name + "_G%d" % G, w.mesh, p, st, src, w.dt)
+
+
+@pytest.mark.parametrize("G", [2, 4, 5, 8])
+def test_other_group_counts(oracle_mod, G):
+    """The kernels are instantiated for 1..8 groups; configs 0-4 only use 1 and 3."""
+    from paper_2404_17630_b200 import rt
+    w = _regroup(cfg.get(2, 8), G)
+    s = rt.Solver(w.mesh, w.params); s.init(w.state, w.sources)
+    s.step(w.dt, 6)
+    dev, _ = s.download(); dev["nH"] = w.state.nH
+    s.step(w.dt, 1)
+    got, lg = s.download()
+    o = oracle_mod.Oracle(w.mesh, w.params); o.set_sources(w.sources); o.set_state(P.as_state(dev))
+    o.step(w.dt, 1)
+    e = P.step_errors(w.mesh, w.params.ctilde, dev, o.get_state(), got)
+    assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
+    assert max(e["xHII"], e["xHeII"], e["xHeIII"]) <= 1e-9 and e["eth"] <= 1e-8, e
+    stored0 = (w.state.N * w.mesh.volume).sum(1)
+    assert P.budget_residual(lg, stored0).max() <= P.TOL_LEDGER
+
+
+@pytest.mark.parametrize("tc", [8, 12, 20])
+def test_small_tiles_many_halos(oracle_mod, monkeypatch, tc):
+    """Forces small tiles (RT_TILE_CELLS): most faces then cross tile boundaries, so the exchange of
+    fluxes through xphi / k_finish and the halo tables carry the result; ragged last tile."""
+    monkeypatch.setenv("RT_TILE_CELLS", str(tc))
+    from paper_2404_17630_b200 import rt
+    w = cfg.get(3, 9)                      # 729 cells: not a multiple of any tile size used here
+    o, s = _pair(oracle_mod, w)
+    assert s.tile_info()["cells_per_tile"] <= tc
+    prev = o.get_state()
+    for _ in range(4):
+        prev = o.get_state()
+        o.step(w.dt, 1); s.step(w.dt, 1)
+    got, lg = s.download()
+    e = P.step_errors(w.mesh, w.params.ctilde, prev, o.get_state(), got)
+    assert e["N"] <= 1e-9 and e["F"] <= 1e-9, e
+    assert P.ledger_errors(o.ledger(), lg) <= 1e-11
+
+
+def test_chemistry_passes_keep_the_per_cell_trial_sequence(oracle_mod):
+    """The sub-stepping runs in passes over compacted lists of unfinished cells (a scheduling choice):
+    every cell must still go through the oracle's sequence of trials, so the counts agree exactly."""
+    from paper_2404_17630_b200 import rt
+    w = cfg.get(2, 8)
+    a = rt.Solver(w.mesh, w.params); a.init(w.state, w.sources); a.step(w.dt, 12)
+    _, la = a.download()
+    o = oracle_mod.Oracle(w.mesh, w.params); o.set_sources(w.sources); o.set_state(w.state)
+    o.step(w.dt, 12)
+    assert la["substeps_total"] == o.ledger()["substeps_total"]
+    assert la["substeps_max"] == o.ledger()["substeps_max"] > 2      # later passes were exercised

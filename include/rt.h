@@ -149,7 +149,11 @@ int64_t rt_kernel_launches(const rt_ctx *ctx);
  * out[1] number of tiles, out[2] largest number of face slots of a tile, out[3] faces evaluated a
  * second time because their two cells lie in different tiles, out[4] largest halo (cells outside a
  * tile that touch it) of a tile, out[5] halo cells summed over the tiles, out[6] largest per-tile
- * table in 32-bit words, out[7] all per-tile tables in 32-bit words.  HOST array of 8.  Needs a mesh. */
+ * table in 32-bit words, out[7] all per-tile tables in 32-bit words, out[8] most owned faces of a
+ * tile, out[9] largest forward halo, out[10] / out[11] dynamic shared memory (bytes) of a block of
+ * the gradient / flux kernel sized for the largest tile; out[12] tiles in the flux kernel's class A
+ * (run with the smaller capacities out[13] owned faces, out[14] forward halo cells and out[15] bytes
+ * of shared memory; the other tiles run in a second launch).  HOST array of 16.  Needs a mesh. */
 int rt_tile_info(const rt_ctx *ctx, int64_t *out);
 
 /* Per-kernel timing with CUDA events recorded on the context's stream around every launch of

@@ -90,6 +90,11 @@ int rt_tile_info(const rt_ctx *c, int64_t *out) {
   if (!c->have_mesh) return RT_ESTATE;
   out[0] = c->TC; out[1] = c->T; out[2] = c->smax; out[3] = c->ninc;
   out[4] = c->hmax; out[5] = c->nhalo; out[6] = c->bmax; out[7] = c->blob_words;
+  out[8] = c->omax; out[9] = c->fmax;
+  out[10] = (int64_t)rt_smem_grad(c->TC, c->G, c->smax, c->hmax, c->bstride);
+  out[11] = (int64_t)rt_smem_flux(c->TC, c->G, c->omax, c->fmax, c->bstride);
+  out[12] = c->nFA; out[13] = c->omaxA; out[14] = c->fmaxA;
+  out[15] = (int64_t)rt_smem_flux(c->TC, c->G, c->omaxA, c->fmaxA, c->bstride);
   return RT_OK;
 }
 

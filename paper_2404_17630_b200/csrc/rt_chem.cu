@@ -154,7 +154,7 @@ template <int G, int MODE, bool FIRST>
 __global__ void __launch_bounds__(RT_CHEM_BLOCK) k_chem(rt_chem_par P, int64_t C, double dt, double *__restrict__ U,
                                                    double *__restrict__ xHII, double *__restrict__ xHeII,
                                                    double *__restrict__ xHeIII, double *__restrict__ eth,
-                                                   const double *__restrict__ nHv, const double *__restrict__ cellS,
+                                                   const double *__restrict__ nHv, const double *__restrict__ cellV,
                                                    const double *__restrict__ kappa, double *__restrict__ part_abs,
                                                    rt_dev_ledger *led, const int32_t *__restrict__ list,
                                                    const int *__restrict__ count, int cap, chem_carry carry,
@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(RT_CHEM_BLOCK) k_chem(rt_chem_par P, int64_t C
         }
       }
       if (flag) flag[idx] = unfinished ? 1 : 0;
-      const double V = cellS[4 * i + 3];
+      const double V = cellV[i];
 #pragma unroll
       for (int g = 0; g < G; g++) {
         *reinterpret_cast<double4 *>(U + ((size_t)i * G + g) * 4) = make_double4(s.N[g], s.Fx[g], s.Fy[g], s.Fz[g]);
@@ -300,7 +300,7 @@ static void launch_chem_mode(rt_ctx *c, const rt_chem_par &P, double dt, double 
   int32_t *lists[2] = {rt_ptr<int32_t>(c, l.chem_list), rt_ptr<int32_t>(c, l.chem_list) + C};
   int *count = rt_ptr<int>(c, l.chem_count);
 #define CHEM_ARGS P, C, dt, U, rt_ptr<double>(c, l.xHII), rt_ptr<double>(c, l.xHeII), rt_ptr<double>(c, l.xHeIII), \
-      rt_ptr<double>(c, l.eth), rt_ptr<double>(c, l.nH), rt_ptr<double>(c, l.cellS), rt_ptr<double>(c, l.kappa)
+      rt_ptr<double>(c, l.eth), rt_ptr<double>(c, l.nH), rt_ptr<double>(c, l.cellV), rt_ptr<double>(c, l.kappa)
   int caps[8];
   const int ncap = MODE == RT_CHEM_FIXED_OPACITY ? 0 : chem_caps(caps, 8);
   // pass 0: every cell

@@ -2,7 +2,7 @@
 //
 // Device data layout (all inside the caller's workspace, fp64, 256-byte aligned blocks).
 //   cells in Peano-Hilbert order p = 0..C-1:   perm[p] = caller's id, iperm = inverse
-//     cellS[C][4] = (sx, sy, sz, V); Minv[C][6] (symmetric inverse of sum_f A n n^T, eq (15))
+//     cellV[C] = V; Minv[C][6] (symmetric inverse of sum_f A n n^T, eq (15))
 //   faces sorted by owner (= left cell, the lower new id), then by right id, boundary faces last;
 //   every face array is [F][4] doubles = one aligned 32-byte sector per face:
 //     faceC = (cx, cy, cz, A)     centroid relative to the left cell's centroid (min-image) and area
@@ -59,7 +59,7 @@ struct rt_dev_ledger {  // accumulators on the device (value + compensation)
 };
 
 struct rt_layout {
-  size_t perm, iperm, cellS, Minv, faceC, faceN, faceW, fo, ro, tiles, blob, xphi, k2cell, k2off, k2row, ghost, led;
+  size_t perm, iperm, cellV, Minv, faceC, faceN, faceW, fo, ro, tiles, blob, tlistG, tlistF, xphi, k2cell, k2off, k2row, ghost, led;
   size_t chem_t, chem_h, chem_att, chem_flag, chem_list, chem_count, chem_cub, chem_cub_bytes;
   size_t Ua, Ub, grad, pacc, xHII, xHeII, xHeIII, eth, nH, kappa, srcidx, srcrate, part, scratch_end;
   size_t blob_bytes;  // capacity of the blob region
@@ -83,6 +83,11 @@ struct rt_ctx {
   int fmax;           // largest forward halo of any tile
   int omax;           // most owned faces of any tile
   int nsm;            // multiprocessors of the device (0 until first needed)
+  // tiles in two classes per kernel: class A = the tiles that fit smaller shared-memory capacities
+  // (more blocks per SM), class B = the others, sized by the maxima above.  tlist*: A tiles first.
+  int64_t nGA, nFA;   // class-A tiles of k_grad / k_flux
+  int smaxA, hmaxA;   // class-A capacities of k_grad
+  int omaxA, fmaxA;   // class-A capacities of k_flux
   int64_t n2;         // cells with at least one incoming face
   int bmax;           // largest blob of any tile, in 32-bit words (without the header)
   int bstride;        // words between the blobs of consecutive tiles
@@ -134,8 +139,8 @@ static inline size_t rt_smem_grad(int TC, int G, int smax, int hmax, int bmax) {
 }
 static inline size_t rt_smem_flux(int TC, int G, int omax, int fmax, int bmax) {
   const int planes = G > 3 ? G : 3;  // three face records per slot, overwritten by A*Phi of every group
-  return (size_t)4 * bmax + (size_t)32 * planes * omax + (size_t)(128 * G + 32) * (TC + fmax) + (size_t)32 * G * TC +
-         (size_t)16 * ((TC + 3) / 4);
+  const int NE = (TC + fmax + 1) & ~1;
+  return (size_t)4 * bmax + (size_t)32 * planes * omax + (size_t)(128 * G + 8) * NE + (size_t)16 * ((TC + 3) / 4);
 }
 #define RT_SMEM_MAX 232448     // 227 KB: the most one block may have on sm_100
 #define RT_SMEM_TARGET 115000  // two blocks per SM (228 KB per SM, 1 KB reserved per block)

@@ -12,7 +12,7 @@ struct rt_chem_par {
 // geometry + tile tables passed by value to the transport kernels (layout: rt_internal.cuh)
 struct rt_geom {
   int64_t C, F;
-  const double *cellS, *Minv, *faceC, *faceN, *faceW;
+  const double *cellV, *Minv, *faceC, *faceN, *faceW;
   const rt_tile *tiles;
   const uint32_t *blob;
   double *xphi;          // [ninc][G][4] fluxes of the faces that cross tile boundaries
@@ -20,6 +20,8 @@ struct rt_geom {
   double box[3];
   int per[3];
   int G, TC, smax, omax, hmax, fmax, bmax, bstride;
+  const int32_t *tlist;  // the launch works on tiles tlist[tbase + blockIdx.x]
+  int64_t tbase;
   int prefetch_tiles;    // the tile kernels ask L2 for the data of tile t + prefetch_tiles
 };
 

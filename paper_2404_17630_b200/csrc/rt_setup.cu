@@ -4,6 +4,7 @@
 #include <cub/cub.cuh>
 #include <string.h>
 #include <stdlib.h>
+#include <vector>
 #include "rt_internal.cuh"
 #include "rt_kernels.cuh"
 
@@ -72,13 +73,14 @@ __global__ void k_cell_keys(const double *centroid, int64_t C, double bx, double
   idx[i] = (int32_t)i;
 }
 
-__global__ void k_permute_cells(geom_in g, int64_t C, const int32_t *perm, int32_t *iperm, double *cellS) {
+__global__ void k_permute_cells(geom_in g, int64_t C, const int32_t *perm, int32_t *iperm, double *cellS, double *cellV) {
   int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= C) return;
   int32_t o = perm[p];
   iperm[o] = (int32_t)p;
   for (int a = 0; a < 3; a++) cellS[4 * p + a] = g.centroid[a * C + o];
   cellS[4 * p + 3] = g.volume[o];
+  cellV[p] = g.volume[o];
 }
 
 __device__ inline uint64_t face_key(int32_t l, int32_t r) {
@@ -398,6 +400,21 @@ __global__ void __launch_bounds__(TILE_BT) k_tile_rows(int TC, const rt_tile *ti
   for (int j = threadIdx.x; j < d.ninc; j += TILE_BT) k2row[ibase[blockIdx.x] + j] = faceX[incf[j]];
 }
 
+// per tile: the four sizes that decide its shared-memory need
+__global__ void k_tile_sizes(int64_t T, const rt_tile *tiles, int32_t *nown, int32_t *nf, int32_t *ns, int32_t *nh) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= T) return;
+  const rt_tile d = tiles[t];
+  nown[t] = d.nown; nf[t] = d.nh - d.nb; ns[t] = d.nown + d.ninc; nh[t] = d.nh;
+}
+// flag[t] = tile fits both capacities (inv: the opposite)
+__global__ void k_tile_fits(int64_t T, const int32_t *a, const int32_t *b, int capa, int capb, int inv, uint8_t *flag) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= T) return;
+  const int fits = a[t] <= capa && b[t] <= capb;
+  flag[t] = (uint8_t)(inv ? !fits : fits);
+}
+
 __global__ void k_tile_totals(int64_t T, const rt_tile *tiles, unsigned long long *tot) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= T) return;
@@ -420,6 +437,7 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
   // left / right ids of the sorted faces and the right lists: only the setup needs them
   int32_t *L = rt_ptr<int32_t>(c, take(4 * F)), *R = rt_ptr<int32_t>(c, take(4 * F));
   int32_t *rl = rt_ptr<int32_t>(c, take(4 * F)), *rn = rt_ptr<int32_t>(c, take(4 * F));
+  double *cellS = rt_ptr<double>(c, take(32 * C));  // (centroid, V) in the new order: the kernels keep only V
   int *flags = rt_ptr<int>(c, take(256));
   size_t cub_bytes = 0;
   {
@@ -463,7 +481,6 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
                    hflags & E_GHOST ? " Dirichlet ghost index >= nghost;" : "", hflags & E_VOL ? " volume <= 0;" : "",
                    hflags & E_AREA ? " area <= 0;" : "", hflags & E_NORMAL ? " normal not unit;" : "");
   int32_t *perm = rt_ptr<int32_t>(c, lay.perm), *iperm = rt_ptr<int32_t>(c, lay.iperm);
-  double *cellS = rt_ptr<double>(c, lay.cellS);
   // 1. cells along the Peano-Hilbert curve
   {
     k_cell_keys<<<nblk(C), SETUP_BLOCK, 0, st>>>(g.centroid, C, c->box[0], c->box[1], c->box[2], k0, v0);
@@ -472,7 +489,7 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
     size_t b = cub_bytes;
     RT_CUDA(c, cub::DeviceRadixSort::SortPairs(cub_tmp, b, dk, dv, C, 0, 63, st));
     RT_CUDA(c, cudaMemcpyAsync(perm, dv.Current(), 4 * C, cudaMemcpyDeviceToDevice, st));
-    k_permute_cells<<<nblk(C), SETUP_BLOCK, 0, st>>>(g, C, perm, iperm, cellS);
+    k_permute_cells<<<nblk(C), SETUP_BLOCK, 0, st>>>(g, C, perm, iperm, cellS, rt_ptr<double>(c, lay.cellV));
   }
   // 2. faces by owner
   double *faceC = rt_ptr<double>(c, lay.faceC), *faceN = rt_ptr<double>(c, lay.faceN);
@@ -516,8 +533,11 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
     int32_t *faceX = v0;
     tile_max *mx = (tile_max *)(flags + 4);
     const char *env = getenv("RT_TILE_CELLS");
-    int tc0 = env ? atoi(env) : 64;
-    if (tc0 < RT_MIN_TILE || tc0 > 1024) tc0 = 64;
+    // (measured on the Voronoi configs with 3 groups: 32 cells per tile with three blocks of k_flux
+    // per SM beat 40 cells with two; with one group a tile's shared memory is small: start at 64)
+    const int tc_default = c->G >= 2 ? 32 : 64;
+    int tc0 = env ? atoi(env) : tc_default;
+    if (tc0 < RT_MIN_TILE || tc0 > 1024) tc0 = tc_default;
     env = getenv("RT_TILE_BLOCKS");
     int nblocks = env ? atoi(env) : 2;
     if (nblocks < 1 || nblocks > 8) nblocks = 2;
@@ -575,6 +595,77 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
     RT_CUDA(c, cudaMemcpyAsync(tot, tsize, 16, cudaMemcpyDeviceToHost, st));
     RT_CUDA(c, cudaStreamSynchronize(st));
     c->nhalo = tot[1];
+    // tile classes: most tiles are much smaller than the largest one, so the kernels run them with
+    // smaller shared-memory capacities (a quantile of the sizes) and more blocks per SM; the few
+    // others run in a second launch with the maxima
+    {
+      const int64_t T = c->T;
+      int32_t *sz[4], *sorted[4];
+      for (int a = 0; a < 4; a++) { sz[a] = (int32_t *)k0 + a * T; sorted[a] = (int32_t *)k1 + a * T; }
+      k_tile_sizes<<<nblk(T), SETUP_BLOCK, 0, st>>>(T, tiles, sz[0], sz[1], sz[2], sz[3]);
+      std::vector<int32_t> hs[4];
+      for (int a = 0; a < 4; a++) {
+        size_t b = cub_bytes;
+        RT_CUDA(c, cub::DeviceRadixSort::SortKeys(cub_tmp, b, sz[a], sorted[a], (int)T, 0, 32, st));
+        hs[a].resize((size_t)T);
+        RT_CUDA(c, cudaMemcpyAsync(hs[a].data(), sorted[a], 4 * (size_t)T, cudaMemcpyDeviceToHost, st));
+      }
+      RT_CUDA(c, cudaStreamSynchronize(st));
+      const double qs[] = {1.0, 0.9995, 0.999, 0.998, 0.995, 0.99, 0.985, 0.98, 0.97, 0.96, 0.95, 0.93, 0.9, 0.87, 0.84, 0.8, 0.75, 0.7};
+      auto quant = [&](const std::vector<int32_t> &v, double q) {
+        int64_t k = (int64_t)(q * (double)T + 0.999999) - 1;
+        if (k < 0) k = 0;
+        if (k >= T) k = T - 1;
+        return (int)v[(size_t)k];
+      };
+      env = getenv("RT_TILE_CLASSES");
+      const bool classes = !(env && atoi(env) == 0);
+      // k_flux: three blocks of 256 threads per SM is what its registers allow
+      c->omaxA = c->omax; c->fmaxA = c->fmax;
+      const size_t lim_flux = 233472 / 3 - 1024 - 512;
+      if (classes && rt_smem_flux(best, c->G, c->omax, c->fmax, c->bstride) > lim_flux)
+        for (double q : qs) {
+          const int o = quant(hs[0], q), f = quant(hs[1], q);
+          if (rt_smem_flux(best, c->G, o, f, c->bstride) <= lim_flux) { c->omaxA = o; c->fmaxA = f; break; }
+        }
+      // k_grad: six blocks, else five (off by default: measured no gain, its registers and the
+      // shared-memory pipeline bound it before occupancy does); RT_GRAD_CLASSES=1 turns it on
+      c->smaxA = c->smax; c->hmaxA = c->hmax;
+      bool done = false;
+      env = getenv("RT_GRAD_CLASSES");
+      const bool gclasses = classes && env && atoi(env) == 1;
+      for (int nb = 6; gclasses && nb >= 5 && !done; nb--) {
+        const size_t lim = 233472 / nb - 1024 - 64;
+        if (rt_smem_grad(best, c->G, c->smax, c->hmax, c->bstride) <= lim) break;
+        for (double q : qs) {
+          if (q < 0.95) break;
+          const int s2 = quant(hs[2], q), h2 = quant(hs[3], q);
+          if (rt_smem_grad(best, c->G, s2, h2, c->bstride) <= lim) { c->smaxA = s2; c->hmaxA = h2; done = true; break; }
+        }
+      }
+      // lists: class-A tiles in ascending order, then the class-B tiles
+      uint8_t *flag = (uint8_t *)v1;
+      int *cnt = (int *)flags + 16;
+      int32_t *lists[2] = {rt_ptr<int32_t>(c, lay.tlistF), rt_ptr<int32_t>(c, lay.tlistG)};
+      const int32_t *sa[2] = {sz[0], sz[2]}, *sb[2] = {sz[1], sz[3]};
+      const int capa[2] = {c->omaxA, c->smaxA}, capb[2] = {c->fmaxA, c->hmaxA};
+      int64_t *nA[2] = {&c->nFA, &c->nGA};
+      for (int k = 0; k < 2; k++) {
+        int hcnt = 0;
+        size_t b = cub_bytes;
+        k_tile_fits<<<nblk(T), SETUP_BLOCK, 0, st>>>(T, sa[k], sb[k], capa[k], capb[k], 0, flag);
+        RT_CUDA(c, cub::DeviceSelect::Flagged(cub_tmp, b, cub::CountingInputIterator<int32_t>(0), flag, lists[k], cnt, (int)T, st));
+        RT_CUDA(c, cudaMemcpyAsync(&hcnt, cnt, sizeof(int), cudaMemcpyDeviceToHost, st));
+        RT_CUDA(c, cudaStreamSynchronize(st));
+        *nA[k] = hcnt;
+        if (hcnt < T) {
+          b = cub_bytes;
+          k_tile_fits<<<nblk(T), SETUP_BLOCK, 0, st>>>(T, sa[k], sb[k], capa[k], capb[k], 1, flag);
+          RT_CUDA(c, cub::DeviceSelect::Flagged(cub_tmp, b, cub::CountingInputIterator<int32_t>(0), flag, lists[k] + hcnt, cnt, (int)T, st));
+        }
+      }
+      RT_CUDA(c, cudaStreamSynchronize(st));
+    }
   }
   if (m->nghost > 0)
     RT_CUDA(c, cudaMemcpyAsync(rt_ptr<double>(c, lay.ghost), m->ghost_state, sizeof(double) * m->nghost * 4 * c->G,
@@ -595,7 +686,7 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G, int flags) {
   l.nbc = (C + RT_BLOCK - 1) / RT_BLOCK;
   l.max_tiles = (C + RT_MIN_TILE - 1) / RT_MIN_TILE;
   l.perm = take(4 * C); l.iperm = take(4 * C);
-  l.cellS = take(32 * C); l.Minv = take(48 * C);
+  l.cellV = take(8 * C + 64); l.Minv = take(48 * C);
   l.faceC = take(32 * F); l.faceN = take(32 * F); l.faceW = take(32 * F);
   l.fo = take(8 * (C + 1)); l.ro = take(8 * (C + 1));
   // tile tables: descriptors for the smallest tile size; blobs bounded by
@@ -603,6 +694,7 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G, int flags) {
   l.tiles = take(sizeof(rt_tile) * (size_t)(l.max_tiles + 1));
   l.blob_bytes = 4 * ((size_t)(6.5 * (double)F) + 2 * (size_t)C + 5 * (size_t)l.max_tiles + 2048);
   l.blob = take(l.blob_bytes);
+  l.tlistG = take(4 * (size_t)(l.max_tiles + 1)); l.tlistF = take(4 * (size_t)(l.max_tiles + 1));
   // fluxes of the faces that cross tile boundaries, written by the owner tile (<= 56 % of the
   // faces; rt_mesh_upload fails with RT_ENOMEM on a mesh whose tiles need more)
   {
@@ -635,7 +727,7 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G, int flags) {
   // setup scratch aliases the state region; make sure it fits (incl. staging of a host mesh)
   int64_t NM = C > F ? C : F;
   const size_t staging = (flags & RT_WS_DEVICE_MESH) ? 0 : 88 * (size_t)F + 32 * (size_t)C;
-  size_t need = 24 * (size_t)NM + 4096 + (size_t)(64 << 20) + 16 * (size_t)F + staging + 32 * 256;
+  size_t need = 24 * (size_t)NM + 4096 + (size_t)(64 << 20) + 16 * (size_t)F + 32 * (size_t)C + staging + 32 * 256;
   if (l.temp + need > o) o = align256(l.temp + need);
   l.total = o;
   return l;

@@ -89,6 +89,9 @@ __device__ __forceinline__ double block_sum(double v, double *red) {
 __device__ __forceinline__ void cp16(void *dst, const void *src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
 }
+__device__ __forceinline__ void cp8(void *dst, const void *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
 __device__ __forceinline__ void cp_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 // n consecutive 16-byte chunks
 template <int N>
@@ -164,15 +167,16 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
   double *sU = sC + 4 * m.smax;                           // [(TC + hmax) G][4]  tile cells, then halo cells
   double *sM = sU + 4 * G * (m.TC + m.hmax);              // [TC][6]
   const int tid = threadIdx.x, nt = blockDim.x;
+  const unsigned tile = (unsigned)m.tlist[m.tbase + blockIdx.x];
   if (tid == 0) { mbar_init(&bar, 1); mbar_init(&bar_blob, 1); }
   __syncthreads();
   // round 1: the tile's blob sits at a fixed stride: header (descriptor) + tables
   if (tid == 0) {
     mbar_expect(&bar_blob, 4u * m.bstride);
-    bulk_g2s(sB, m.blob + (size_t)blockIdx.x * m.bstride, 4u * m.bstride, &bar_blob);
+    bulk_g2s(sB, m.blob + (size_t)tile * m.bstride, 4u * m.bstride, &bar_blob);
   }
   mbar_wait(&bar_blob, 0);
-  const tile_view v = view_tile(m, sB, blockIdx.x);
+  const tile_view v = view_tile(m, sB, tile);
   // round 2: what the descriptor locates (bulk copies: owned faces, the tile's own cells) and what the
   // tables locate (gathers: halo cells, incoming faces), all in flight together
   if (tid == 0) {
@@ -182,8 +186,8 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
     bulk_g2s(sU, U + 4 * G * v.c0, 32u * G * v.ncell, &bar);
     bulk_g2s(sM, m.Minv + 6 * v.c0, 48u * v.ncell, &bar);
     // a tile that starts a few gridfuls later: pull its contiguous runs into L2 now
-    const int64_t tp = (int64_t)blockIdx.x + m.prefetch_tiles;
-    if (tp < (int64_t)gridDim.x) {
+    if ((int64_t)blockIdx.x + m.prefetch_tiles < (int64_t)gridDim.x) {
+      const int64_t tp = m.tlist[m.tbase + blockIdx.x + m.prefetch_tiles];
       const rt_tile dp = m.tiles[tp];
       const int64_t cp = tp * m.TC;
       const unsigned nc = (unsigned)(cp + m.TC < m.C ? m.TC : m.C - cp);
@@ -331,7 +335,7 @@ __device__ __forceinline__ double finish_cell(double a0, double a1, double a2, d
 }
 
 template <int G, bool SECOND>
-__global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__restrict__ Uin, const double *__restrict__ grad,
+__global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__restrict__ Uin, const double *__restrict__ grad,
                                                  const double *U0, double *Uout, const int32_t *__restrict__ srcidx,
                                                  const double *__restrict__ srcrate, int nsrc, update_par up,
                                                  double *__restrict__ pacc, double *__restrict__ part_floor,
@@ -340,7 +344,7 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
   __shared__ double red[32];
   __shared__ __align__(8) uint64_t bar, bar_blob;
   constexpr int NP = G > 3 ? G : 3;                        // planes of [omax][4]
-  const int NE = m.TC + m.fmax;                            // tile cells, then forward halo cells
+  const int NE = (m.TC + m.fmax + 1) & ~1;                 // tile cells, then forward halo cells
   const int OM = m.omax;
   uint32_t *sB = reinterpret_cast<uint32_t *>(smem_raw);   // the tile's blob
   double *sF = reinterpret_cast<double *>(sB + m.bstride); // [NP][omax][4]: planes 0-2 hold the staged face records
@@ -348,10 +352,9 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
                                                            // overwrites plane g with A * (Phi_N, Phi_F) of group g
   double *sU = sF + 4 * NP * OM;                           // [NE][G][4]
   double *sG = sU + 4 * G * NE;                            // [NE][G][12]
-  double *sS = sG + 12 * G * NE;                           // [NE][4]  (s, V)
-  double *sU0 = sS + 4 * NE;                               // [TC][G][4]  U^n of the tile's cells
-  int32_t *sSrc = reinterpret_cast<int32_t *>(sU0 + 4 * G * m.TC);  // [TC] source index or -1
-  const unsigned tile = blockIdx.x;
+  double *sV = sG + 12 * G * NE;                           // [NE]  cell volumes
+  int32_t *sSrc = reinterpret_cast<int32_t *>(sV + NE);    // [TC] source index or -1
+  const unsigned tile = (unsigned)m.tlist[m.tbase + blockIdx.x];
   const int tid = threadIdx.x, nt = blockDim.x;
   const double dt = up.dt, ct = up.ct;
   if (tid == 0) { mbar_init(&bar, 1); mbar_init(&bar_blob, 1); }
@@ -366,19 +369,18 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
   // round 2: what the descriptor locates (bulk copies: owned faces, the tile's own cells) and what the
   // tables locate (gathers: forward halo cells), all in flight together
   if (tid == 0) {
-    const unsigned nsb = (4u * v.ncell + 15u) & ~15u;  // srcidx is padded
-    mbar_expect(&bar, 96u * v.nown + ((SECOND ? 128u : 32u) * G + 32u + 32u * G) * v.ncell + nsb);
+    const unsigned nsb = (4u * v.ncell + 15u) & ~15u, nvb = (8u * v.ncell + 15u) & ~15u;  // srcidx and cellV are padded
+    mbar_expect(&bar, 96u * v.nown + (SECOND ? 128u : 32u) * G * v.ncell + nvb + nsb);
     bulk_g2s(sF, m.faceC + 4 * v.fbase, 32u * v.nown, &bar);
     bulk_g2s(sF + 4 * OM, m.faceN + 4 * v.fbase, 32u * v.nown, &bar);
     bulk_g2s(sF + 8 * OM, m.faceW + 4 * v.fbase, 32u * v.nown, &bar);
     bulk_g2s(sU, Uin + 4 * G * v.c0, 32u * G * v.ncell, &bar);
     if (SECOND) bulk_g2s(sG, grad + 12 * G * v.c0, 96u * G * v.ncell, &bar);
-    bulk_g2s(sS, m.cellS + 4 * v.c0, 32u * v.ncell, &bar);
-    bulk_g2s(sU0, U0 + 4 * G * v.c0, 32u * G * v.ncell, &bar);
+    bulk_g2s(sV, m.cellV + v.c0, nvb, &bar);
     bulk_g2s(sSrc, srcidx + v.c0, nsb, &bar);
     // a tile that starts a few gridfuls later: pull its contiguous runs into L2 now
-    const int64_t tp = (int64_t)blockIdx.x + m.prefetch_tiles;
-    if (tp < (int64_t)gridDim.x) {
+    if ((int64_t)blockIdx.x + m.prefetch_tiles < (int64_t)gridDim.x) {
+      const int64_t tp = m.tlist[m.tbase + blockIdx.x + m.prefetch_tiles];
       const rt_tile dp = m.tiles[tp];
       const int64_t cp = tp * m.TC;
       const unsigned nc = (unsigned)(cp + m.TC < m.C ? m.TC : m.C - cp);
@@ -388,7 +390,6 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
       bulk_prefetch_l2(m.faceW + 4 * dp.fbase, 32u * dp.nown);
       bulk_prefetch_l2(Uin + 4 * G * cp, 32u * G * nc);
       if (SECOND) bulk_prefetch_l2(grad + 12 * G * cp, 96u * G * nc);
-      bulk_prefetch_l2(m.cellS + 4 * cp, 32u * nc);
       bulk_prefetch_l2(U0 + 4 * G * cp, 32u * G * nc);
     }
   }
@@ -402,7 +403,7 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
       if (SECOND) cp_run<6>(sG + 12 * (G * (m.TC + h) + part), grad + 12 * (G * id + part));
     } else {
       cp_run<2 * G>(sU + 4 * G * (m.TC + h), Uin + (int64_t)(4 * G) * id);
-      cp_run<2>(sS + 4 * (m.TC + h), m.cellS + 4 * id);
+      cp8(sV + m.TC + h, m.cellV + id);
     }
   }
   mbar_wait(&bar, 0);
@@ -411,9 +412,6 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
 
   // ---- a3: one thread per owned face: its record is read once into registers (so the thread may
   // overwrite it in shared memory with the fluxes), then every group in turn
-  double b_out[G], b_in[G];
-#pragma unroll
-  for (int g = 0; g < G; g++) b_out[g] = b_in[g] = 0.0;
   int bnd = 0;
   const double hc2 = 0.5 * ct * ct, hc = 0.5 * ct;
   for (int s = tid; s < v.nown; s += nt) {
@@ -427,15 +425,16 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
     const double n[3] = {fn.x, fn.y, fn.z};
     const double A = fc.w;
     const double rdtA = fast_rcp(dt * A);
-    const double capL = sS[4 * xl + 3] * rdtA;
+    const double capL = sV[xl] * rdtA;
     // the face centre relative to the left cell is stored; relative to the right cell it is c - kappa w
     double capR = 0.0, rRx = 0.0, rRy = 0.0, rRz = 0.0;
     if (rin) {
-      capR = sS[4 * xr + 3] * rdtA;
+      capR = sV[xr] * rdtA;
       rRx = fma(-fw.w, fw.x, fc.x); rRy = fma(-fw.w, fw.y, fc.y); rRz = fma(-fw.w, fw.z, fc.z);
     }
     const int xrr = rin ? xr : xl;
-#pragma unroll
+    if (!rin && r != RT_BC_REFLECT) bnd = 1;  // outflow or Dirichlet face: its flux enters a ledger
+#pragma unroll 1
     for (int g = 0; g < G; g++) {
       double UL[4], UR[4], NL, NR = 0.0;
       extrapolate<SECOND>(sU + 4 * (xl * G + g), sG + 12 * (xl * G + g), fc.x, fc.y, fc.z, UL, NL);
@@ -459,8 +458,6 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
       if (ph[0] > 0.0) ph[0] = dmin2(ph[0], NL * capL);
       else if (rin) ph[0] = -dmin2(-ph[0], NR * capR);
       st4(sF + 4 * (g * OM + s), A * ph[0], A * ph[1], A * ph[2], A * ph[3]);
-      if (r == RT_BC_OUTFLOW) { b_out[g] += A * ph[0]; bnd = 1; }
-      else if (r <= RT_BC_DIRICHLET0) { b_in[g] -= A * ph[0]; bnd = 1; }
     }
   }
   __syncthreads();  // every owned slot holds its fluxes
@@ -473,11 +470,21 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
           *reinterpret_cast<const double2 *>(sF + 4 * ((c >> 1) * OM + (int)v.outs[j]) + 2 * (c & 1));
     }
   }
-  // boundary ledgers: fixed-order block sums, one row per tile
+  // boundary ledgers: the number fluxes through the tile's outflow / Dirichlet faces, read back from
+  // the slots; fixed-order block sums, one row per tile
   if (__syncthreads_or(bnd)) {
 #pragma unroll
     for (int gg = 0; gg < G; gg++) {
-      const double so = block_sum(b_out[gg], red), si = block_sum(b_in[gg], red);
+      double b_out = 0.0, b_in = 0.0;
+      for (int s = tid; s < v.nown; s += nt) {
+        const int xr = (int)(v.slr[s] >> 16);
+        if (xr < 0xFF00) continue;
+        const int r = xr - 0x10000;
+        const double aphi = sF[4 * (gg * OM + s)];
+        if (r == RT_BC_OUTFLOW) b_out += aphi;
+        else if (r <= RT_BC_DIRICHLET0) b_in -= aphi;
+      }
+      const double so = block_sum(b_out, red), si = block_sum(b_in, red);
       if (tid == 0) { part_out[(size_t)tile * G + gg] = so; part_in[(size_t)tile * G + gg] = si; }
     }
   } else if (tid < G) {
@@ -502,6 +509,8 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
     const int il = on ? item / G : 0, ig = on ? item - il * G : 0;
     const int h0 = on ? (int)v.ho[il] : 0, h1 = on ? (int)v.ho[il + 1] : 0;
     const double *pg = sF + 4 * ig * OM;
+    // U^n of the cell (the stage buffer itself in stage 1): asked for now, needed after the sum
+    const double4 u0 = on && p == 0 ? ld4(U0 + 4 * (v.c0 * G + item)) : make_double4(0, 0, 0, 0);
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
     int incomplete = 0;
 #pragma unroll 4
@@ -522,7 +531,7 @@ __global__ void __launch_bounds__(256, 2) k_flux(rt_geom m, const double *__rest
     if (incomplete) { st4(pacc + 4 * (v.c0 * G + item), a0, a1, a2, a3); continue; }
     const int32_t si = sSrc[il];
     const double src = si >= 0 ? srcrate[(size_t)ig * nsrc + si] : 0.0;
-    const double add = finish_cell(a0, a1, a2, a3, sS[4 * il + 3], src, ld4(sU + 4 * item), ld4(sU0 + 4 * item), up,
+    const double add = finish_cell(a0, a1, a2, a3, sV[il], src, ld4(sU + 4 * item), u0, up,
                                    Uout + 4 * (v.c0 * G + item));
     if (add != 0.0) {
 #pragma unroll
@@ -547,7 +556,7 @@ template <int G>
 __global__ void __launch_bounds__(RT_FIN_BLOCK) k_finish(int64_t n2, const int32_t *__restrict__ k2cell,
                                                          const int32_t *__restrict__ k2off, const int32_t *__restrict__ k2row,
                                                          const double *__restrict__ xphi, const double *__restrict__ pacc,
-                                                         const double *__restrict__ cellS,
+                                                         const double *__restrict__ cellV,
                                                          const double *__restrict__ Uin, const double *U0, double *Uout,
                                                          const int32_t *__restrict__ srcidx, const double *__restrict__ srcrate,
                                                          int nsrc, update_par up, double *__restrict__ part_floor) {
@@ -569,7 +578,7 @@ __global__ void __launch_bounds__(RT_FIN_BLOCK) k_finish(int64_t n2, const int32
     }
     const int32_t si = srcidx[i];
     const double src = si >= 0 ? srcrate[(size_t)g * nsrc + si] : 0.0;
-    add = finish_cell(a.x, a.y, a.z, a.w, cellS[4 * i + 3], src, ld4(Uin + 4 * (i * G + g)), ld4(U0 + 4 * (i * G + g)), up, out);
+    add = finish_cell(a.x, a.y, a.z, a.w, cellV[i], src, ld4(Uin + 4 * (i * G + g)), ld4(U0 + 4 * (i * G + g)), up, out);
   }
   // fixed-order block sums per group
   const int any = __syncthreads_or(add != 0.0);
@@ -627,11 +636,11 @@ __global__ void __launch_bounds__(1024) k_reduce(reduce_job j0, reduce_job j1, i
 // stored photons per block: part[row][g] = sum_cells V N
 template <int GG>
 __global__ void __launch_bounds__(RT_BLOCK *GG) k_stored(int64_t C, const double *__restrict__ U,
-                                                          const double *__restrict__ cellS, double *__restrict__ part) {
+                                                          const double *__restrict__ cellV, double *__restrict__ part) {
   __shared__ double sm[GG][RT_BLOCK / 32];
   const int64_t i = (int64_t)blockIdx.x * RT_BLOCK + threadIdx.x;
   const int g = threadIdx.y;
-  double v = i < C ? cellS[4 * i + 3] * U[((size_t)i * GG + g) * 4] : 0.0;
+  double v = i < C ? cellV[i] * U[((size_t)i * GG + g) * 4] : 0.0;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
   if ((threadIdx.x & 31) == 0) sm[g][threadIdx.x >> 5] = v;
@@ -738,7 +747,7 @@ rt_geom rt_geom_of(const rt_ctx *c) {
   const rt_layout &l = c->lay;
   rt_geom m;
   m.C = c->C; m.F = c->F; m.G = c->G; m.TC = c->TC; m.smax = c->smax; m.omax = c->omax; m.hmax = c->hmax; m.fmax = c->fmax; m.bmax = c->bmax; m.bstride = c->bstride;
-  m.cellS = rt_ptr<double>(c, l.cellS); m.Minv = rt_ptr<double>(c, l.Minv);
+  m.cellV = rt_ptr<double>(c, l.cellV); m.Minv = rt_ptr<double>(c, l.Minv);
   m.faceC = rt_ptr<double>(c, l.faceC); m.faceN = rt_ptr<double>(c, l.faceN); m.faceW = rt_ptr<double>(c, l.faceW);
   m.tiles = rt_ptr<rt_tile>(c, l.tiles); m.blob = rt_ptr<uint32_t>(c, l.blob);
   m.xphi = rt_ptr<double>(c, l.xphi);
@@ -752,10 +761,21 @@ rt_geom rt_geom_of(const rt_ctx *c) {
   return m;
 }
 
+// the two tile classes of a kernel: class A (most tiles) with the smaller capacities, class B with the maxima
+static void launch_grad(rt_ctx *c, rt_geom m, const double *U, double *grad) {
+  m.tlist = rt_ptr<int32_t>(c, c->lay.tlistG);
+  for (int cls = 0; cls < 2; cls++) {
+    const int64_t n = cls == 0 ? c->nGA : c->T - c->nGA;
+    if (n <= 0) continue;
+    m.tbase = cls == 0 ? 0 : c->nGA;
+    m.smax = cls == 0 ? c->smaxA : c->smax; m.hmax = cls == 0 ? c->hmaxA : c->hmax;
+    DISPATCH_G(c->G, K_GRAD, (unsigned)n, grad_threads(c), rt_smem_grad(c->TC, c->G, m.smax, m.hmax, c->bstride), c->stream, m, U, grad);
+    c->launches++;
+  }
+}
+
 int rt_launch_gradients(rt_ctx *c, const double *U) {
-  DISPATCH_G(c->G, K_GRAD, (unsigned)c->T, grad_threads(c), rt_smem_grad(c->TC, c->G, c->smax, c->hmax, c->bstride), c->stream, rt_geom_of(c), U,
-             rt_ptr<double>(c, c->lay.grad));
-  c->launches++;
+  launch_grad(c, rt_geom_of(c), U, rt_ptr<double>(c, c->lay.grad));
   return RT_OK;
 }
 
@@ -779,29 +799,38 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
   double *p_floor = part + (size_t)G * nchem * RT_CHEM_MAXPASS, *p_out = p_floor + (size_t)G * c->T, *p_in = p_out + (size_t)G * c->T;
   double *p_floor2 = p_in + (size_t)G * c->T;
   const int nt = tile_threads(c);
-  const size_t ss = rt_smem_flux(c->TC, G, c->omax, c->fmax, c->bstride);
   const update_par up = {ca, cb, dt, c->par.ctilde, c->par.n_floor};
   double *pacc = rt_ptr<double>(c, l.pacc);
   const int32_t *srcidx = rt_ptr<int32_t>(c, l.srcidx);
   const double *srcrate = rt_ptr<double>(c, l.srcrate);
   if (c->par.order >= 2) {
     rt_prof_begin(c, RT_K_GRAD);
-    DISPATCH_G(G, K_GRAD, (unsigned)c->T, grad_threads(c), rt_smem_grad(c->TC, G, c->smax, c->hmax, c->bstride), c->stream, m, Uin, grad);
-    rt_prof_end(c);
-    c->launches++;
-    rt_prof_begin(c, RT_K_FLUX);
-    DISPATCH_G(G, K_FLUX2, (unsigned)c->T, nt, ss, c->stream, m, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
-    rt_prof_end(c);
-  } else {
-    rt_prof_begin(c, RT_K_FLUX);
-    DISPATCH_G(G, K_FLUX1, (unsigned)c->T, nt, ss, c->stream, m, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
+    launch_grad(c, m, Uin, grad);
     rt_prof_end(c);
   }
-  c->launches++;
+  rt_prof_begin(c, RT_K_FLUX);
+  {
+    rt_geom mf = m;
+    mf.tlist = rt_ptr<int32_t>(c, l.tlistF);
+    for (int cls = 0; cls < 2; cls++) {
+      const int64_t n = cls == 0 ? c->nFA : c->T - c->nFA;
+      if (n <= 0) continue;
+      mf.tbase = cls == 0 ? 0 : c->nFA;
+      mf.omax = cls == 0 ? c->omaxA : c->omax; mf.fmax = cls == 0 ? c->fmaxA : c->fmax;
+      const size_t sf = rt_smem_flux(c->TC, G, mf.omax, mf.fmax, c->bstride);
+      if (c->par.order >= 2) {
+        DISPATCH_G(G, K_FLUX2, (unsigned)n, nt, sf, c->stream, mf, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
+      } else {
+        DISPATCH_G(G, K_FLUX1, (unsigned)n, nt, sf, c->stream, mf, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
+      }
+      c->launches++;
+    }
+  }
+  rt_prof_end(c);
   if (nfin > 0) {
     rt_prof_begin(c, RT_K_UPDATE);
     DISPATCH_G(G, K_FINISH, (unsigned)nfin, RT_FIN_BLOCK, 0, c->stream, c->n2, rt_ptr<int32_t>(c, l.k2cell),
-               rt_ptr<int32_t>(c, l.k2off), rt_ptr<int32_t>(c, l.k2row), m.xphi, pacc, m.cellS, Uin, U0, Uout, srcidx, srcrate, c->nsrc, up,
+               rt_ptr<int32_t>(c, l.k2off), rt_ptr<int32_t>(c, l.k2row), m.xphi, pacc, m.cellV, Uin, U0, Uout, srcidx, srcrate, c->nsrc, up,
                p_floor2);
     rt_prof_end(c);
     c->launches++;
@@ -847,7 +876,7 @@ int rt_launch_stored(rt_ctx *c) {
   const rt_layout &l = c->lay;
   double *part = rt_ptr<double>(c, l.part);
   DISPATCH_G(c->G, K_STORED, (unsigned)l.nbc, dim3(RT_BLOCK, c->G), 0, c->stream, c->C, rt_ptr<double>(c, l.Ua),
-             rt_ptr<double>(c, l.cellS), part);
+             rt_ptr<double>(c, l.cellV), part);
   c->launches++;
   rt_reduce2(c, {part, l.nbc, 1.0, 4, nullptr}, {part, l.nbc, 1.0, 4, nullptr}, 1);
   return RT_OK;

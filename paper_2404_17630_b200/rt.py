@@ -301,11 +301,14 @@ class Solver:
         return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(names)}
 
     def tile_info(self):
-        out = np.zeros(8, dtype=np.int64)
+        out = np.zeros(16, dtype=np.int64)
         _check(self.h, lib().rt_tile_info(self.h, _vp(out.ctypes.data)), "rt_tile_info")
         return {"cells_per_tile": int(out[0]), "tiles": int(out[1]), "max_slots": int(out[2]), "refaces": int(out[3]),
                 "max_halo": int(out[4]), "halo_cells": int(out[5]), "max_table_words": int(out[6]),
-                "table_words": int(out[7])}
+                "table_words": int(out[7]), "max_owned": int(out[8]), "max_forward_halo": int(out[9]),
+                "smem_grad": int(out[10]), "smem_flux": int(out[11]),
+                "flux_class_a": {"tiles": int(out[12]), "max_owned": int(out[13]), "max_forward_halo": int(out[14]),
+                                 "smem": int(out[15])}}
 
     def launches(self):
         return int(lib().rt_kernel_launches(self.h))

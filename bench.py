@@ -307,14 +307,18 @@ def main():
     # (kern["stage"] is the pair k_flux + k_finish: avg_ms is the pair's time per stage)
     # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
     # capture of this workload (profiles/traffic.csv, written from profiles/r1_ncu_full_*.md); for
-    # the stage pair it is k_flux's (k_finish's metric passes failed in that capture)
+    # the stage pair it is the sum of k_flux (both tile classes) and k_finish
     traffic = None
     tf = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tf):
+        rows = {}
         for ln in open(tf).read().splitlines()[1:]:
             wl, kn, by = ln.split(",")
-            if wl == workload_name(c, n) and kn == {"stage": "flux"}.get(dom, dom):
-                traffic = float(by)
+            if wl == workload_name(c, n):
+                rows[kn] = float(by)
+        parts = {"stage": ("flux", "finish")}.get(dom, (dom,))
+        if all(k in rows for k in parts):
+            traffic = sum(rows[k] for k in parts)
     roofline = {"bound": "hbm", "kernel": {"stage": "stage = k_flux + k_finish (a3 + a4 of one Heun stage)"}.get(dom, dom), "achieved": kern[dom]["GBps"], "peak": peak, "unit": "GB/s",
                 "frac": kern[dom]["GBps"] / peak, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": ab[dom],

@@ -327,7 +327,7 @@ static void launch_chem_mode(rt_ctx *c, const rt_chem_par &P, double dt, double 
     k_chem<G, MODE, false><<<grid, RT_CHEM_BLOCK, 0, c->stream>>>(CHEM_ARGS, part_p, led, lists[p & 1], count, p < ncap ? caps[p] : 0,
                                                                carry, flags);
     rt_prof_end(c);
-    c->launches += 2;
+    c->launches += 3;  // two kernels of the compaction + the pass
     rt_reduce2(c, {part_p, 0, 1.0, 0, count}, {part_p, 0, 1.0, 0, count}, 1);
   }
 #undef CHEM_ARGS

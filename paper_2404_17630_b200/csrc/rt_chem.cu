@@ -151,7 +151,7 @@ struct chem_carry {
 // (cap <= 0: no limit) and is flagged for the next pass.  One warp per block; warps stride over the
 // cells; part_abs has one row per 32 consecutive entries (fixed order: deterministic ledger).
 template <int G, int MODE, bool FIRST>
-__global__ void __launch_bounds__(RT_CHEM_BLOCK) k_chem(rt_chem_par P, int64_t C, double dt, double *__restrict__ U,
+__global__ void __launch_bounds__(RT_CHEM_BLOCK, 16) k_chem(rt_chem_par P, int64_t C, double dt, double *__restrict__ U,
                                                    double *__restrict__ xHII, double *__restrict__ xHeII,
                                                    double *__restrict__ xHeIII, double *__restrict__ eth,
                                                    const double *__restrict__ nHv, const double *__restrict__ cellV,

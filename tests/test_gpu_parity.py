@@ -234,3 +234,19 @@ def test_chemistry_passes_keep_the_per_cell_trial_sequence(oracle_mod):
     o.step(w.dt, 12)
     assert la["substeps_total"] == o.ledger()["substeps_total"]
     assert la["substeps_max"] == o.ledger()["substeps_max"] > 2      # later passes were exercised
+
+
+def test_zero_subcycles_and_zero_sources_leave_the_state_alone():
+    from paper_2404_17630_b200 import rt
+    w = cfg.get(2, 8)
+    none = cfg.Sources(np.zeros(0, np.int32), np.zeros((w.params.ngroup, 0)))
+    s = rt.Solver(w.mesh, w.params); s.init(w.state, none)
+    s.step(w.dt, 0)
+    got, lg = s.download()
+    assert np.array_equal(got["N"], w.state.N) and np.array_equal(got["F"], w.state.F)
+    assert np.array_equal(got["xHII"], w.state.xHII) and np.array_equal(got["eth"], w.state.eth)
+    assert lg["nsub_done"] == 0 and np.all(lg["injected"] == 0.0)
+    s.step(w.dt, 2)                              # no sources: nothing is injected, the budget still closes
+    _, lg = s.download()
+    stored0 = (w.state.N * w.mesh.volume).sum(1)
+    assert np.all(lg["injected"] == 0.0) and P.budget_residual(lg, stored0).max() <= P.TOL_LEDGER

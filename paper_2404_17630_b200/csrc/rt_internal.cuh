@@ -49,6 +49,7 @@
 #define RT_BLOCK 128
 #endif
 #define RT_CHEM_MAXPASS 8  // sub-stepping passes (rt_chem.cu): partial-sum rows are reserved for each
+#define RT_RED_BLOCKS 64   // blocks per (job, group) of k_reduce
 #define RT_CHEM_BLOCK 32  // one warp per block: a slow cell holds back 31 others, not 127
 #define RT_REC 18        // doubles per (cell, group) row of U + gradients in shared memory (16 + 2 pad: bank spread)
 #define RT_MIN_TILE 8     // smallest tile size rt_mesh_upload will fall back to
@@ -56,6 +57,9 @@
 struct rt_dev_ledger {  // accumulators on the device (value + compensation)
   double acc[5][RT_MAXG][2];  // 0 absorbed, 1 outflow, 2 inflow_bc, 3 floor_added, 4 stored (value only)
   unsigned long long substeps_total, substeps_max, cells_hit_cap;
+  // scratch of k_reduce: per (job, group) the chunk sums of its blocks and the count of blocks done
+  double red_tmp[2][RT_MAXG][RT_RED_BLOCKS];
+  unsigned red_cnt[2][RT_MAXG];
 };
 
 struct rt_layout {

@@ -591,31 +591,38 @@ __global__ void __launch_bounds__(RT_FIN_BLOCK) k_finish(int64_t n2, const int32
 }
 
 // ------------------------------------------------------------------ ledgers
-// acc[slot][g] += weight * sum_rows part[row][g]; one block per (array, g); fixed order.
+// acc[slot][g] += weight * sum_rows part[row][g].  Grid (G, jobs, RT_RED_BLOCKS): block z sums a
+// fixed contiguous chunk of the rows (Neumaier per thread, fixed tree), the last block to finish
+// adds the chunk sums in chunk order: the result does not depend on the scheduling.
 __global__ void __launch_bounds__(1024) k_reduce(reduce_job j0, reduce_job j1, int G, rt_dev_ledger *led) {
   __shared__ double sm[1024];
+  __shared__ bool last;
   reduce_job j = blockIdx.y == 0 ? j0 : j1;
   if (j.ncount) j.nrows = ((int64_t)*j.ncount + 31) / 32;
   if (j1.ncount) j1.nrows = ((int64_t)*j1.ncount + 31) / 32;
-  const int g = blockIdx.x;
+  const int g = blockIdx.x, y = blockIdx.y, z = blockIdx.z;
+  // one job may be made of two partial-sum arrays: rows of the first, then rows of the second
+  const bool two = gridDim.y == 1 && j1.part != j0.part;
+  const int64_t n0 = j.nrows, ntot = n0 + (two ? j1.nrows : 0);
+  const int64_t chunk = (ntot + RT_RED_BLOCKS - 1) / RT_RED_BLOCKS;
+  const int64_t r0 = (int64_t)z * chunk, r1 = r0 + chunk < ntot ? r0 + chunk : ntot;
   double s = 0.0, c = 0.0;
-  // Neumaier per thread over rows tid, tid + 1024, ...: eight loads in flight, added in row order
-  // (a padding zero changes neither the sum nor the compensation)
-  auto sum_rows = [&](const double *part, int64_t nrows) {
-    for (int64_t r = threadIdx.x; r < nrows; r += 8 * 1024) {
-      double x[8];
+  // rows r0 + tid, + 1024, ...: eight loads in flight, added in row order (a padding zero changes
+  // neither the sum nor the compensation)
+  for (int64_t r = r0 + threadIdx.x; r < r1; r += 8 * 1024) {
+    double x[8];
 #pragma unroll
-      for (int u = 0; u < 8; u++) { const int64_t rr = r + 1024 * u; x[u] = rr < nrows ? part[(size_t)rr * G + g] : 0.0; }
-#pragma unroll
-      for (int u = 0; u < 8; u++) {
-        const double t = s + x[u];
-        c += fabs(s) >= fabs(x[u]) ? (s - t) + x[u] : (x[u] - t) + s;
-        s = t;
-      }
+    for (int u = 0; u < 8; u++) {
+      const int64_t rr = r + 1024 * u;
+      x[u] = rr < r1 ? (rr < n0 ? j.part[(size_t)rr * G + g] : j1.part[(size_t)(rr - n0) * G + g]) : 0.0;
     }
-  };
-  sum_rows(j.part, j.nrows);
-  if (gridDim.y == 1 && j1.part != j0.part) sum_rows(j1.part, j1.nrows);  // one job made of two partial-sum arrays
+#pragma unroll
+    for (int u = 0; u < 8; u++) {
+      const double t = s + x[u];
+      c += fabs(s) >= fabs(x[u]) ? (s - t) + x[u] : (x[u] - t) + s;
+      s = t;
+    }
+  }
   sm[threadIdx.x] = s + c;
   __syncthreads();
   for (int o = 512; o > 0; o >>= 1) {
@@ -623,13 +630,28 @@ __global__ void __launch_bounds__(1024) k_reduce(reduce_job j0, reduce_job j1, i
     __syncthreads();
   }
   if (threadIdx.x == 0) {
-    double *a = led->acc[j.slot][g];
-    if (j.slot == 4) { a[0] = j.weight * sm[0]; a[1] = 0.0; }
-    else {
-      const double x = j.weight * sm[0], t = a[0] + x;
-      a[1] += fabs(a[0]) >= fabs(x) ? (a[0] - t) + x : (x - t) + a[0];
-      a[0] = t;
-    }
+    led->red_tmp[y][g][z] = sm[0];
+    __threadfence();
+    last = atomicAdd(&led->red_cnt[y][g], 1u) == RT_RED_BLOCKS - 1;
+  }
+  __syncthreads();
+  if (!last || threadIdx.x != 0) return;
+  __threadfence();
+  led->red_cnt[y][g] = 0;
+  double t = 0.0, tc = 0.0;
+  for (int k = 0; k < RT_RED_BLOCKS; k++) {
+    const double x = *(volatile double *)&led->red_tmp[y][g][k];
+    const double u = t + x;
+    tc += fabs(t) >= fabs(x) ? (t - u) + x : (x - u) + t;
+    t = u;
+  }
+  const double total = t + tc;
+  double *a = led->acc[j.slot][g];
+  if (j.slot == 4) { a[0] = j.weight * total; a[1] = 0.0; }
+  else {
+    const double x = j.weight * total, u = a[0] + x;
+    a[1] += fabs(a[0]) >= fabs(x) ? (a[0] - u) + x : (x - u) + a[0];
+    a[0] = u;
   }
 }
 
@@ -781,7 +803,7 @@ int rt_launch_gradients(rt_ctx *c, const double *U) {
 
 void rt_reduce2(rt_ctx *c, reduce_job a, reduce_job b, int njobs) {
   rt_prof_begin(c, RT_K_REDUCE);
-  k_reduce<<<dim3(c->G, njobs), 1024, 0, c->stream>>>(a, b, c->G, rt_ptr<rt_dev_ledger>(c, c->lay.led));
+  k_reduce<<<dim3(c->G, njobs, RT_RED_BLOCKS), 1024, 0, c->stream>>>(a, b, c->G, rt_ptr<rt_dev_ledger>(c, c->lay.led));
   rt_prof_end(c);
   c->launches++;
 }

@@ -533,9 +533,9 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
     int32_t *faceX = v0;
     tile_max *mx = (tile_max *)(flags + 4);
     const char *env = getenv("RT_TILE_CELLS");
-    // (measured on the Voronoi configs with 3 groups: 32 cells per tile with three blocks of k_flux
-    // per SM beat 40 cells with two; with one group a tile's shared memory is small: start at 64)
-    const int tc_default = c->G >= 2 ? 32 : 64;
+    // (measured: with 3 groups on the Voronoi configs 32 cells per tile and three blocks of k_flux per
+    // SM beat 40 cells and two; with one group (128^3 Cartesian) 96 cells beat 64 and equal 128)
+    const int tc_default = c->G >= 2 ? 32 : 96;
     int tc0 = env ? atoi(env) : tc_default;
     if (tc0 < RT_MIN_TILE || tc0 > 1024) tc0 = tc_default;
     env = getenv("RT_TILE_BLOCKS");

@@ -257,9 +257,12 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
     for (int k = h0; k < h1; k++) {
       const uint32_t e = v.hl[k];
       const int s = (int)(e & 0x7fffu);
-      const double4 c = ld4(sC + 4 * s), w = ld4(sW + 4 * s);
-      const double kr = (e & 0x8000u) ? -w.w : 0.0;
-      const double rx = fma(kr, w.x, c.x), ry = fma(kr, w.y, c.y), rz = fma(kr, w.z, c.z);
+      const double4 c = ld4(sC + 4 * s);
+      double rx = c.x, ry = c.y, rz = c.z;
+      if (e & 0x8000u) {  // (a cell's right-side faces come last in its list: mostly uniform across a warp)
+        const double4 w = ld4(sW + 4 * s);
+        rx = fma(-w.w, w.x, rx); ry = fma(-w.w, w.y, ry); rz = fma(-w.w, w.z, rz);
+      }
 #pragma unroll
       for (int f = 0; f < 4; f++) {
         const double d = gr[f][0] * rx + gr[f][1] * ry + gr[f][2] * rz;

@@ -320,10 +320,12 @@ def main():
         if all(k in rows for k in parts):
             traffic = sum(rows[k] for k in parts)
     roofline = {"bound": "hbm", "kernel": {"stage": "stage = k_flux + k_finish (a3 + a4 of one Heun stage)"}.get(dom, dom), "achieved": kern[dom]["GBps"], "peak": peak, "unit": "GB/s",
-                "frac": kern[dom]["GBps"] / peak, "traffic": traffic, "peak_source": peak_src,
+                "frac": kern[dom]["GBps"] / peak, "frac_of_nominal_8TBs": kern[dom]["GBps"] / 8000.0,
+                "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": ab[dom],
                 "subcycle": {"algorithmic_bytes": ab["subcycle"], "GBps": ab["subcycle"] * args.steps / (ms * 1e-3) / 1e9,
                              "frac": ab["subcycle"] * args.steps / (ms * 1e-3) / 1e9 / peak,
+                             "frac_of_nominal_8TBs": ab["subcycle"] * args.steps / (ms * 1e-3) / 1e9 / 8000.0,
                              "bytes_per_cell_group_update": ab["subcycle"] / (C * G)}}
 
     cpu = None

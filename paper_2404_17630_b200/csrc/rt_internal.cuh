@@ -4,12 +4,15 @@
 //   cells in Peano-Hilbert order p = 0..C-1:   perm[p] = caller's id, iperm = inverse
 //     cellV[C] = V; Minv[C][6] (symmetric inverse of sum_f A n n^T, eq (15))
 //   faces sorted by owner (= left cell, the lower new id), then by right id, boundary faces last;
-//   every face array is [F][4] doubles = one aligned 32-byte sector per face:
-//     faceC = (cx, cy, cz, A)     centroid relative to the left cell's centroid (min-image) and area
-//     faceN = (nx, ny, nz, 0)     unit normal L -> R
-//     faceW = (wx, wy, wz, kappa) w = A d/|d|^2, d = s_R - s_L: prefactor of eq (15)'s second
-//                                 term; kappa = |d|^2/A, so the face centroid relative
-//                                 to the right cell is c - kappa w
+//   every face array holds 4 doubles per face, stored as two halves: [F][2] = components 0-1, then
+//   [F][2] = components 2-3, so that consecutive faces (and scattered ones) are read as 16-byte
+//   chunks at a 16-byte stride, which spread over all shared-memory banks (32-byte records read by
+//   one lane each collide two-way at best):
+//     faceC = (cx, cy | cz, A)     centroid relative to the left cell's centroid (min-image) and area
+//     faceN = (nx, ny | nz, 0)     unit normal L -> R
+//     faceW = (wx, wy | wz, kappa) w = A d/|d|^2, d = s_R - s_L: prefactor of eq (15)'s second
+//                                  term; kappa = |d|^2/A, so the face centroid relative
+//                                  to the right cell is c - kappa w
 //   cell -> faces: owned faces are the contiguous range fo[i]..fo[i+1]; the faces
 //     where the cell is the right one are r-list entries ro[i]..ro[i+1] (ascending face id)
 //   tiles: TC consecutive cells (a compact blob of the Hilbert curve) are one thread block's

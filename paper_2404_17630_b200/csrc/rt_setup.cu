@@ -16,6 +16,10 @@ struct geom_in {
   const int32_t *left, *right;
 };
 
+// component a of face q's record: the face arrays are stored as two halves, [F][2] = components
+// 0-1 followed by [F][2] = components 2-3 (rt_internal.cuh)
+#define FA(arr, q, a) (arr)[((a) < 2 ? 0 : 2 * F) + 2 * (int64_t)(q) + ((a) & 1)]
+
 // error flag bits
 enum { E_LEFT = 1, E_RIGHT = 2, E_VOL = 4, E_AREA = 8, E_NORMAL = 16, E_CLOSURE = 32, E_MATRIX = 64, E_GHOST = 128 };
 
@@ -109,15 +113,15 @@ __global__ void k_gather_faces(geom_in g, int64_t C, int64_t F, const int32_t *o
   bool flip = (iperm[g.left[f]] != l);
   if (flip) r = iperm[g.left[f]];
   L[q] = l; R[q] = r;
-  faceN[4 * q + 3] = 0.0;
-  faceC[4 * q + 3] = g.area[f];
+  FA(faceN, q, 3) = 0.0;
+  FA(faceC, q, 3) = g.area[f];
   double sg = flip ? -1.0 : 1.0;
   double b[3] = {bx, by, bz};
   int per[3] = {p0, p1, p2};
   for (int a = 0; a < 3; a++) {
-    faceN[4 * q + a] = sg * g.normal[a * F + f];
+    FA(faceN, q, a) = sg * g.normal[a * F + f];
     double sl = cellS[4 * (int64_t)l + a];
-    faceC[4 * q + a] = rt_wrap(g.fcentroid[a * F + f] - sl, b[a], per[a]);  // relative to the left cell's centroid
+    FA(faceC, q, a) = rt_wrap(g.fcentroid[a * F + f] - sl, b[a], per[a]);  // relative to the left cell's centroid
   }
 }
 
@@ -163,20 +167,20 @@ __global__ void k_face_geom(int64_t C, int64_t F, const double *cellS, const dou
   double d[3];
   if (r >= 0) {
     for (int a = 0; a < 3; a++) {
-      double rl = faceC[4 * q + a];
+      double rl = FA(faceC, q, a);
       double c = cellS[4 * (int64_t)l + a] + rl;
       d[a] = rl - rt_wrap(c - cellS[4 * (int64_t)r + a], b[a], per[a]);
     }
   } else {
-    double n[3] = {faceN[4 * q], faceN[4 * q + 1], faceN[4 * q + 2]};
+    double n[3] = {FA(faceN, q, 0), FA(faceN, q, 1), FA(faceN, q, 2)};
     double p = 0.0;
-    for (int a = 0; a < 3; a++) p += faceC[4 * q + a] * n[a];
+    for (int a = 0; a < 3; a++) p += FA(faceC, q, a) * n[a];
     for (int a = 0; a < 3; a++) d[a] = 2.0 * p * n[a];
   }
   double d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
-  double k = faceC[4 * q + 3] / d2;
-  for (int a = 0; a < 3; a++) faceW[4 * q + a] = k * d[a];
-  faceW[4 * q + 3] = d2 / faceC[4 * q + 3];
+  double k = FA(faceC, q, 3) / d2;
+  for (int a = 0; a < 3; a++) FA(faceW, q, a) = k * d[a];
+  FA(faceW, q, 3) = d2 / FA(faceC, q, 3);
 }
 
 // per cell: M = sum_f A n n^T (n = d/|d| = w/|w|), its inverse, and the closure check
@@ -189,13 +193,13 @@ __global__ void k_cell_geom(int64_t C, int64_t F, const double *faceC, const dou
   for (int64_t k = 0; k < n_own + n_r; k++) {
     int64_t q = k < n_own ? fo[i] + k : rl[ro[i] + (k - n_own)];
     double sg = k < n_own ? 1.0 : -1.0;
-    double a = faceC[4 * q + 3];
-    double wx = faceW[4 * q], wy = faceW[4 * q + 1], wz = faceW[4 * q + 2];
+    double a = FA(faceC, q, 3);
+    double wx = FA(faceW, q, 0), wy = FA(faceW, q, 1), wz = FA(faceW, q, 2);
     double w2 = wx * wx + wy * wy + wz * wz;
     double f = a / w2;  // A n n^T = A w w^T / |w|^2
     m[0] += f * wx * wx; m[1] += f * wx * wy; m[2] += f * wx * wz;
     m[3] += f * wy * wy; m[4] += f * wy * wz; m[5] += f * wz * wz;
-    cl[0] += sg * a * faceN[4 * q]; cl[1] += sg * a * faceN[4 * q + 1]; cl[2] += sg * a * faceN[4 * q + 2];
+    cl[0] += sg * a * FA(faceN, q, 0); cl[1] += sg * a * FA(faceN, q, 1); cl[2] += sg * a * FA(faceN, q, 2);
     sa += a;
   }
   int e = 0;

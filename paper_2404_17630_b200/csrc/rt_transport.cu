@@ -20,6 +20,8 @@
 #include "rt_kernels.cuh"
 
 __device__ __forceinline__ double4 ld4(const double *p) { return *reinterpret_cast<const double4 *>(p); }
+__device__ __forceinline__ double2 ld2(const double *p) { return *reinterpret_cast<const double2 *>(p); }
+__device__ __forceinline__ void st2(double *p, double a, double b) { *reinterpret_cast<double2 *>(p) = make_double2(a, b); }
 __device__ __forceinline__ void st4(double *p, double a, double b, double c, double d) {
   *reinterpret_cast<double4 *>(p) = make_double4(a, b, c, d);
 }
@@ -58,11 +60,12 @@ __device__ __forceinline__ double fast_rsqrt(double x) {
 }
 
 // neighbour or ghost state seen across a boundary face with right code `code` (S13)
-__device__ __forceinline__ double4 ghost_for_gradient(int code, const double4 Ui, const double *faceN, int64_t q,
+__device__ __forceinline__ double4 ghost_for_gradient(int code, const double4 Ui, const double *faceN, int64_t F, int64_t q,
                                                       const double *ghost, int G, int g) {
   if (code == RT_BC_OUTFLOW) return Ui;
   if (code == RT_BC_REFLECT) {
-    const double4 n = ld4(faceN + 4 * q);
+    const double2 n01 = ld2(faceN + 2 * q);
+    const double4 n = make_double4(n01.x, n01.y, faceN[2 * F + 2 * q], 0.0);
     const double p = 2.0 * (Ui.y * n.x + Ui.z * n.y + Ui.w * n.z);
     return make_double4(Ui.x, Ui.y - p * n.x, Ui.z - p * n.y, Ui.w - p * n.z);
   }
@@ -162,9 +165,11 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar, bar_blob;
   uint32_t *sB = reinterpret_cast<uint32_t *>(smem_raw);    // the tile's blob
-  double *sW = reinterpret_cast<double *>(sB + m.bstride);  // [smax][4]  (w, kappa)
-  double *sC = sW + 4 * m.smax;                           // [smax][4]  (c - s_L, A)
-  double *sU = sC + 4 * m.smax;                           // [(TC + hmax) G][4]  tile cells, then halo cells
+  double *sWl = reinterpret_cast<double *>(sB + m.bstride);  // [smax][2]  (wx, wy)      the face records come as
+  double *sWh = sWl + 2 * m.smax;                          // [smax][2]  (wz, kappa)   16-byte halves
+  double *sCl = sWh + 2 * m.smax;                          // [smax][2]  (cx, cy)      (c = centre - s_L)
+  double *sCh = sCl + 2 * m.smax;                          // [smax][2]  (cz, A)
+  double *sU = sCh + 2 * m.smax;                           // [(TC + hmax) G][4]  tile cells, then halo cells
   double *sM = sU + 4 * G * (m.TC + m.hmax);              // [TC][6]
   const int tid = threadIdx.x, nt = blockDim.x;
   const unsigned tile = (unsigned)m.tlist[m.tbase + blockIdx.x];
@@ -181,8 +186,10 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
   // tables locate (gathers: halo cells, incoming faces), all in flight together
   if (tid == 0) {
     mbar_expect(&bar, 64u * v.nown + (32u * G + 48u) * v.ncell);
-    bulk_g2s(sW, m.faceW + 4 * v.fbase, 32u * v.nown, &bar);
-    bulk_g2s(sC, m.faceC + 4 * v.fbase, 32u * v.nown, &bar);
+    bulk_g2s(sWl, m.faceW + 2 * v.fbase, 16u * v.nown, &bar);
+    bulk_g2s(sWh, m.faceW + 2 * m.F + 2 * v.fbase, 16u * v.nown, &bar);
+    bulk_g2s(sCl, m.faceC + 2 * v.fbase, 16u * v.nown, &bar);
+    bulk_g2s(sCh, m.faceC + 2 * m.F + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sU, U + 4 * G * v.c0, 32u * G * v.ncell, &bar);
     bulk_g2s(sM, m.Minv + 6 * v.c0, 48u * v.ncell, &bar);
     // a tile that starts a few gridfuls later: pull its contiguous runs into L2 now
@@ -192,8 +199,10 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
       const int64_t cp = tp * m.TC;
       const unsigned nc = (unsigned)(cp + m.TC < m.C ? m.TC : m.C - cp);
       bulk_prefetch_l2(m.blob + (size_t)tp * m.bstride, 4u * m.bstride);
-      bulk_prefetch_l2(m.faceW + 4 * dp.fbase, 32u * dp.nown);
-      bulk_prefetch_l2(m.faceC + 4 * dp.fbase, 32u * dp.nown);
+      bulk_prefetch_l2(m.faceW + 2 * dp.fbase, 16u * dp.nown);
+      bulk_prefetch_l2(m.faceW + 2 * m.F + 2 * dp.fbase, 16u * dp.nown);
+      bulk_prefetch_l2(m.faceC + 2 * dp.fbase, 16u * dp.nown);
+      bulk_prefetch_l2(m.faceC + 2 * m.F + 2 * dp.fbase, 16u * dp.nown);
       bulk_prefetch_l2(U + 4 * G * cp, 32u * G * nc);
       bulk_prefetch_l2(m.Minv + 6 * cp, 48u * nc);
     }
@@ -203,8 +212,10 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
   for (int h = tid; h < v.nh; h += nt) cp_run<2 * G>(sU + 4 * G * (m.TC + h), U + (int64_t)(4 * G) * v.halo[h]);
   for (int j = tid; j < v.ninc; j += nt) {
     const int64_t q = v.incf[j];
-    cp_run<2>(sW + 4 * (v.nown + j), m.faceW + 4 * q);
-    cp_run<2>(sC + 4 * (v.nown + j), m.faceC + 4 * q);
+    cp16(sWl + 2 * (v.nown + j), m.faceW + 2 * q);
+    cp16(sWh + 2 * (v.nown + j), m.faceW + 2 * m.F + 2 * q);
+    cp16(sCl + 2 * (v.nown + j), m.faceC + 2 * q);
+    cp16(sCh + 2 * (v.nown + j), m.faceC + 2 * m.F + 2 * q);
   }
   mbar_wait(&bar, 0);
   cp_wait_all();
@@ -226,11 +237,12 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
       const int s = (int)(e & 0x7fffu);
       const uint32_t nb = e >> 16;
       const int sgn = (int)((e & 0x8000u) << 16);  // sign bit where the cell is the right one
-      const double4 w = ld4(sW + 4 * s);
+      const double2 wl = ld2(sWl + 2 * s);
+      const double wzz = sWh[2 * s];
       double4 Uj;
       if (nb < 0xFF00u) Uj = ld4(Ug + 4 * G * (int)nb);
-      else Uj = ghost_for_gradient((int)nb - 0x10000, Ui, m.faceN, v.fbase + s, m.ghost, G, g);
-      const double wx = flip_sign(w.x, sgn), wy = flip_sign(w.y, sgn), wz = flip_sign(w.z, sgn);
+      else Uj = ghost_for_gradient((int)nb - 0x10000, Ui, m.faceN, m.F, v.fbase + s, m.ghost, G, g);
+      const double wx = flip_sign(wl.x, sgn), wy = flip_sign(wl.y, sgn), wz = flip_sign(wzz, sgn);
       const double d0 = Uj.x - Ui.x, d1 = Uj.y - Ui.y, d2 = Uj.z - Ui.z, d3 = Uj.w - Ui.w;
       b[0][0] += wx * d0; b[0][1] += wy * d0; b[0][2] += wz * d0;
       b[1][0] += wx * d1; b[1][1] += wy * d1; b[1][2] += wz * d1;
@@ -257,11 +269,11 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
     for (int k = h0; k < h1; k++) {
       const uint32_t e = v.hl[k];
       const int s = (int)(e & 0x7fffu);
-      const double4 c = ld4(sC + 4 * s);
-      double rx = c.x, ry = c.y, rz = c.z;
+      const double2 cl = ld2(sCl + 2 * s);
+      double rx = cl.x, ry = cl.y, rz = sCh[2 * s];
       if (e & 0x8000u) {  // (a cell's right-side faces come last in its list: mostly uniform across a warp)
-        const double4 w = ld4(sW + 4 * s);
-        rx = fma(-w.w, w.x, rx); ry = fma(-w.w, w.y, ry); rz = fma(-w.w, w.z, rz);
+        const double2 wl = ld2(sWl + 2 * s), wh = ld2(sWh + 2 * s);
+        rx = fma(-wh.y, wl.x, rx); ry = fma(-wh.y, wl.y, ry); rz = fma(-wh.y, wh.x, rz);
       }
 #pragma unroll
       for (int f = 0; f < 4; f++) {
@@ -350,9 +362,10 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
   const int NE = (m.TC + m.fmax + 1) & ~1;                 // tile cells, then forward halo cells
   const int OM = m.omax;
   uint32_t *sB = reinterpret_cast<uint32_t *>(smem_raw);   // the tile's blob
-  double *sF = reinterpret_cast<double *>(sB + m.bstride); // [NP][omax][4]: planes 0-2 hold the staged face records
-                                                           // (c, A), (n, -), (w, kappa); a slot's warp then
-                                                           // overwrites plane g with A * (Phi_N, Phi_F) of group g
+  double *sF = reinterpret_cast<double *>(sB + m.bstride); // [2 NP][omax][2]: half-planes 0-5 hold the staged face records
+                                                           // (cx, cy | cz, A), (nx, ny | nz, -), (wx, wy | wz, kappa) as
+                                                           // 16-byte halves; the slot's thread then overwrites
+                                                           // half-planes 2g, 2g + 1 with A * (Phi_N, Phi_F) of group g
   double *sU = sF + 4 * NP * OM;                           // [NE][G][4]
   double *sG = sU + 4 * G * NE;                            // [NE][G][12]
   double *sV = sG + 12 * G * NE;                           // [NE]  cell volumes
@@ -374,9 +387,12 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
   if (tid == 0) {
     const unsigned nsb = (4u * v.ncell + 15u) & ~15u, nvb = (8u * v.ncell + 15u) & ~15u;  // srcidx and cellV are padded
     mbar_expect(&bar, 96u * v.nown + (SECOND ? 128u : 32u) * G * v.ncell + nvb + nsb);
-    bulk_g2s(sF, m.faceC + 4 * v.fbase, 32u * v.nown, &bar);
-    bulk_g2s(sF + 4 * OM, m.faceN + 4 * v.fbase, 32u * v.nown, &bar);
-    bulk_g2s(sF + 8 * OM, m.faceW + 4 * v.fbase, 32u * v.nown, &bar);
+    bulk_g2s(sF, m.faceC + 2 * v.fbase, 16u * v.nown, &bar);
+    bulk_g2s(sF + 2 * OM, m.faceC + 2 * m.F + 2 * v.fbase, 16u * v.nown, &bar);
+    bulk_g2s(sF + 4 * OM, m.faceN + 2 * v.fbase, 16u * v.nown, &bar);
+    bulk_g2s(sF + 6 * OM, m.faceN + 2 * m.F + 2 * v.fbase, 16u * v.nown, &bar);
+    bulk_g2s(sF + 8 * OM, m.faceW + 2 * v.fbase, 16u * v.nown, &bar);
+    bulk_g2s(sF + 10 * OM, m.faceW + 2 * m.F + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sU, Uin + 4 * G * v.c0, 32u * G * v.ncell, &bar);
     if (SECOND) bulk_g2s(sG, grad + 12 * G * v.c0, 96u * G * v.ncell, &bar);
     bulk_g2s(sV, m.cellV + v.c0, nvb, &bar);
@@ -388,9 +404,11 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
       const int64_t cp = tp * m.TC;
       const unsigned nc = (unsigned)(cp + m.TC < m.C ? m.TC : m.C - cp);
       bulk_prefetch_l2(m.blob + (size_t)tp * m.bstride, 4u * m.bstride);
-      bulk_prefetch_l2(m.faceC + 4 * dp.fbase, 32u * dp.nown);
-      bulk_prefetch_l2(m.faceN + 4 * dp.fbase, 32u * dp.nown);
-      bulk_prefetch_l2(m.faceW + 4 * dp.fbase, 32u * dp.nown);
+      for (int hf = 0; hf < 2; hf++) {
+        bulk_prefetch_l2(m.faceC + 2 * m.F * hf + 2 * dp.fbase, 16u * dp.nown);
+        bulk_prefetch_l2(m.faceN + 2 * m.F * hf + 2 * dp.fbase, 16u * dp.nown);
+        bulk_prefetch_l2(m.faceW + 2 * m.F * hf + 2 * dp.fbase, 16u * dp.nown);
+      }
       bulk_prefetch_l2(Uin + 4 * G * cp, 32u * G * nc);
       if (SECOND) bulk_prefetch_l2(grad + 12 * G * cp, 96u * G * nc);
       bulk_prefetch_l2(U0 + 4 * G * cp, 32u * G * nc);
@@ -418,7 +436,10 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
   int bnd = 0;
   const double hc2 = 0.5 * ct * ct, hc = 0.5 * ct;
   for (int s = tid; s < v.nown; s += nt) {
-    const double4 fc = ld4(sF + 4 * s), fn = ld4(sF + 4 * (OM + s)), fw = ld4(sF + 4 * (2 * OM + s));
+    const double2 c01 = ld2(sF + 2 * s), c23 = ld2(sF + 2 * (OM + s)), n01 = ld2(sF + 2 * (2 * OM + s)), n23 = ld2(sF + 2 * (3 * OM + s)),
+                  w01 = ld2(sF + 2 * (4 * OM + s)), w23 = ld2(sF + 2 * (5 * OM + s));
+    const double4 fc = make_double4(c01.x, c01.y, c23.x, c23.y), fn = make_double4(n01.x, n01.y, n23.x, 0.0),
+                  fw = make_double4(w01.x, w01.y, w23.x, w23.y);
     const uint32_t lr = v.slr[s];
     const int xl = (int)(lr & 0xffffu);
     int xr = (int)(lr >> 16);
@@ -460,7 +481,8 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
       // only the number flux is clamped (continuous in the state; Phi_F is left alone)
       if (ph[0] > 0.0) ph[0] = dmin2(ph[0], NL * capL);
       else if (rin) ph[0] = -dmin2(-ph[0], NR * capR);
-      st4(sF + 4 * (g * OM + s), A * ph[0], A * ph[1], A * ph[2], A * ph[3]);
+      st2(sF + 2 * (2 * g * OM + s), A * ph[0], A * ph[1]);
+      st2(sF + 2 * ((2 * g + 1) * OM + s), A * ph[2], A * ph[3]);
     }
   }
   __syncthreads();  // every owned slot holds its fluxes
@@ -469,8 +491,7 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
     double *xo = m.xphi + (size_t)(4 * G) * v.xbase;
     for (int k = tid; k < 2 * G * v.nout; k += nt) {
       const int j = k / (2 * G), c = k - j * (2 * G);
-      *reinterpret_cast<double2 *>(xo + 2 * k) =
-          *reinterpret_cast<const double2 *>(sF + 4 * ((c >> 1) * OM + (int)v.outs[j]) + 2 * (c & 1));
+      *reinterpret_cast<double2 *>(xo + 2 * k) = ld2(sF + 2 * (c * OM + (int)v.outs[j]));  // chunk c = half c & 1 of group c >> 1
     }
   }
   // boundary ledgers: the number fluxes through the tile's outflow / Dirichlet faces, read back from
@@ -483,7 +504,7 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
         const int xr = (int)(v.slr[s] >> 16);
         if (xr < 0xFF00) continue;
         const int r = xr - 0x10000;
-        const double aphi = sF[4 * (gg * OM + s)];
+        const double aphi = sF[2 * (2 * gg * OM + s)];
         if (r == RT_BC_OUTFLOW) b_out += aphi;
         else if (r <= RT_BC_DIRICHLET0) b_in -= aphi;
       }
@@ -511,7 +532,7 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
     const bool on = item < nitem;
     const int il = on ? item / G : 0, ig = on ? item - il * G : 0;
     const int h0 = on ? (int)v.ho[il] : 0, h1 = on ? (int)v.ho[il + 1] : 0;
-    const double *pg = sF + 4 * ig * OM;
+    const double *pg = sF + 4 * ig * OM;  // half-planes 2 ig and 2 ig + 1
     // U^n of the cell (the stage buffer itself in stage 1): asked for now, needed after the sum
     const double4 u0 = on && p == 0 ? ld4(U0 + 4 * (v.c0 * G + item)) : make_double4(0, 0, 0, 0);
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
@@ -521,7 +542,8 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
       const uint32_t w = v.hl[k];
       const int s = (int)(w & 0x7fffu);
       if (s >= v.nown) { incomplete = 1; continue; }  // incoming: its owner tile has the flux
-      const double4 q = ld4(pg + 4 * s);
+      const double2 q01 = ld2(pg + 2 * s), q23 = ld2(pg + 2 * (OM + s));
+      const double4 q = make_double4(q01.x, q01.y, q23.x, q23.y);
       const int sgn = (int)((w & 0x8000u) << 16);  // the flux leaves the left cell and enters the right one
       a0 += flip_sign(q.x, sgn); a1 += flip_sign(q.y, sgn); a2 += flip_sign(q.z, sgn); a3 += flip_sign(q.w, sgn);
     }

@@ -231,7 +231,7 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
     const double *Ug = sU + 4 * g;
     // first pass over the cell's half-faces: sum_f w_f (phi_j - phi_i), min/max.  Where the cell is
     // the face's right cell, d = s_L - s_R: the stored prefactor changes sign.
-#pragma unroll 2
+#pragma unroll 4
     for (int k = h0; k < h1; k++) {
       const uint32_t e = v.hl[k];
       const int s = (int)(e & 0x7fffu);
@@ -265,7 +265,7 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
     // The stored face centre is relative to the left cell; seen from the right cell it is
     // c - d with d = kappa w (rt_internal.cuh).
     double dmax[4] = {0, 0, 0, 0}, dmin[4] = {0, 0, 0, 0};
-#pragma unroll 2
+#pragma unroll 4
     for (int k = h0; k < h1; k++) {
       const uint32_t e = v.hl[k];
       const int s = (int)(e & 0x7fffu);

@@ -287,8 +287,9 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
 #pragma unroll
     for (int w = 0; w < 4; w++) {
       double a = 1.0;
-      if (dmax[w] > 0.0) a = dmin2(a, (hi[w] - Uiv[w]) / dmax[w]);
-      if (dmin[w] < 0.0) a = dmin2(a, (lo[w] - Uiv[w]) / dmin[w]);
+      // (reciprocals from the MUFU seed where the divisor is safely normal: a sixth of a division)
+      if (dmax[w] > 0.0) a = dmin2(a, dmax[w] > 1e-280 ? (hi[w] - Uiv[w]) * fast_rcp(dmax[w]) : (hi[w] - Uiv[w]) / dmax[w]);
+      if (dmin[w] < 0.0) a = dmin2(a, dmin[w] < -1e-280 ? (Uiv[w] - lo[w]) * fast_rcp(-dmin[w]) : (lo[w] - Uiv[w]) / dmin[w]);
       o[3 * w] = a * gr[w][0]; o[3 * w + 1] = a * gr[w][1]; o[3 * w + 2] = a * gr[w][2];
     }
     st4(out, o[0], o[1], o[2], o[3]); st4(out + 4, o[4], o[5], o[6], o[7]); st4(out + 8, o[8], o[9], o[10], o[11]);

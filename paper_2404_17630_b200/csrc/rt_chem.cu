@@ -48,10 +48,10 @@ __device__ inline double recomb_cool_fit(double T, double loglam) {
 
 template <bool THERMAL>
 __device__ inline void eval_rates(double T, double aB_override, rate_set &r) {
-  const double iT = 1.0 / T, logT = log(T);
+  const double iT = rcp_pos(T), logT = log(T);
   // log(2 T_i) for T_HI = 157807, T_HeI = 285335, T_HeII = 631515 K
   const double llHI = 12.662275226919286 - logT, llHeI = 13.254566388120152 - logT, llHeII = 14.049024154019651 - logT;
-  const double sq = sqrt(T), q = 1.0 / (1.0 + sqrt(T * 1.0e-5));
+  const double sq = sqrt(T), q = rcp_pos(1.0 + sqrt(T * 1.0e-5));
   const double eHI = exp(-157809.1 * iT), eHeI = exp(-285335.4 * iT), eHeII = exp(-631515.0 * iT);
   const double sqq = sq * q;
   r.aHII = aB_override > 0.0 ? aB_override : recomb_fit(llHI);
@@ -223,7 +223,7 @@ __global__ void __launch_bounds__(RT_CHEM_BLOCK, 16) k_chem(rt_chem_par P, int64
           if (THERMAL && stale) {
             stale = false;
             const double xe = s.xHII + P.y_he * (s.xHeII + 2.0 * s.xHeIII);
-            const double T = (2.0 / 3.0) * s.e / (KB_CGS * (nH * (1.0 + P.y_he + xe)));
+            const double T = (2.0 / 3.0) * s.e * rcp_pos(KB_CGS * (nH * (1.0 + P.y_he + xe)));
             eval_rates<true>(T, P.alphaB_override, r);
           }
           trial_out<G> o;

@@ -29,12 +29,12 @@ sys.path.insert(0, ROOT)
 
 METRIC = "rt_cell_group_updates_per_s"
 UNIT = "cell-group-updates/s"
-FULL_N = {0: 32, 1: 128, 2: 64, 3: 256, 4: 384}
-SAMPLE_N = {0: 24, 1: 32, 2: 24, 3: 28, 4: 28}
+FULL_N = {0: 32, 1: 128, 2: 64, 3: 256, 4: 384, 5: 44}
+SAMPLE_N = {0: 24, 1: 32, 2: 24, 3: 28, 4: 28, 5: 20}
 
 
 def workload_name(c, n):
-    return "config%d_%s_n%d" % (c, ("stromgren", "beam", "hhe_voronoi", "reion_voronoi", "reion_voronoi")[c], n)
+    return "config%d_%s_n%d" % (c, ("stromgren", "beam", "hhe_voronoi", "reion_voronoi", "reion_voronoi", "hii_region_voronoi")[c], n)
 
 
 # ------------------------------------------------------------------ CPU oracle legs
@@ -206,7 +206,7 @@ def main():
     c = args.config
     n = args.n or FULL_N[c]
     t_build = time.perf_counter()
-    if c >= 3:
+    if c in (3, 4):
         w = devin.config34_device(n, c, "cuda:%d" % local)
     else:
         w = cfg.get(c, n)

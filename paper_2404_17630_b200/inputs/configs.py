@@ -1,5 +1,5 @@
 """The five synthetic workloads of BASELINE.json (`configs[0..4]`), recipe in SURVEY.md §8(d)
-and DESIGN.md §4.  Input generators only: they produce the arrays handed to BOTH the oracle
+and DESIGN.md §4, plus config 5, the expanding H II region of PAPER.md:175-180, 290.  Input generators only: they produce the arrays handed to BOTH the oracle
 and the CUDA path (`rt_mesh`, `rt_state`, `rt_sources`, `rt_params`, dt).  CGS units.
 
 Configs 3/4 stand in for the paper's cosmological boxes (Table 1), whose
@@ -200,6 +200,65 @@ def config34(n, cfg):
     return Workload("config%d_reion_%d" % (cfg, n), mesh, p, st, src, cfl_dt(mesh, ct), {"spacing": spacing})
 
 
+def grey_blackbody(Tbb, edges_eV=(13.6, 24.6, 54.4, np.inf)):
+    """Photon-number-weighted grey cross-sections [cm^2], mean excess energies [erg] and photon
+    shares per group for a black body of temperature Tbb ("flux-weighted
+    cross-sections and photoheating rates for each bin"), power-law sigma_j(nu) of SURVEY.md
+    Appendix A, Gauss-Legendre panels.  Reproduces SIGMA3 / EPS3 / SHARE3 at 1e5 K
+    (tests/test_oracle_physics.py); an input generator: it fixes the workload's constants."""
+    kT = K_B * Tbb / EV
+    thr = np.array([13.6, 24.6, 54.4])
+    s0 = np.array([6.3e-18, 7.4e-18, 1.575e-18])
+    slope = np.array([3.0, 2.0, 3.0])
+    x, wq = np.polynomial.legendre.leggauss(64)
+    G = len(edges_eV) - 1
+    sig, eps, share = np.zeros((G, 3)), np.zeros((G, 3)), np.zeros(G)
+    for g in range(G):
+        lo = edges_eV[g]
+        hi = min(edges_eV[g + 1], lo + 80.0 * kT)
+        pts = np.geomspace(lo, hi, 33)
+        a, b = pts[:-1, None], pts[1:, None]
+        E = (0.5 * (b - a) * x + 0.5 * (b + a)).ravel()
+        W = (0.5 * (b - a) * wq).ravel()
+        with np.errstate(over="ignore"):
+            nph = W * E ** 2 / np.expm1(E / kT)
+        share[g] = nph.sum()
+        for j in range(3):
+            if lo < thr[j] - 1e-9:
+                continue
+            sj = s0[j] * (E / thr[j]) ** (-slope[j])
+            sig[g, j] = (nph * sj).sum() / share[g]
+            eps[g, j] = (nph * sj * (E - thr[j])).sum() / (nph * sj).sum() * EV
+    return sig, eps, share / share.sum()
+
+
+def hii_region(n=44):
+    """Expanding H II region (eq 16, and its three-bin H+He variant PAPER.md:290):
+    box (1.6 kpc)^3, n_H = n0 for r < r0 else n0 (r0/r)^2 with n0 = 3.2 cm^-3, r0 = 91.5 pc,
+    T = 100 K, c~ = 1e-3 c, photons injected homogeneously (rate per volume constant) in a sphere
+    of radius 0.05 kpc at the centre at 1e50 / 5e48 / 3e48 s^-1 per bin, grey constants from a
+    5e4 K black body.  Stand-ins: n^3 jittered-lattice Voronoi generators replace
+    the paper's 2 x N^3 staggered grid; He mass fraction 0.24; dt from the CFL rule."""
+    box = 1.6 * KPC
+    mesh = M.voronoi(n, box, 0.3, SEED_MESH + 5, periodic=False, bc_code=M.BC_OUTFLOW)
+    ct = 1.0e-3 * C_LIGHT
+    sig, eps, _ = grey_blackbody(5.0e4)
+    p = Params(ngroup=3, ctilde=ct, sigma=sig, eps_heat=eps, chem_mode=CHEM_HHE_THERMAL, y_he=Y_HE)
+    c = mesh.centroid
+    r = np.sqrt((c[0] - 0.5 * box) ** 2 + (c[1] - 0.5 * box) ** 2 + (c[2] - 0.5 * box) ** 2)
+    r0 = 91.5e-3 * KPC
+    nH = np.where(r < r0, 3.2, 3.2 * (r0 / np.maximum(r, r0)) ** 2)
+    st = _uniform_state(3, mesh.ncell, 0.0, nH, 100.0, (1.0e-6, 1.0e-6, 0.0), Y_HE)
+    inside = np.flatnonzero(r < 0.05 * KPC)
+    if inside.size == 0:
+        inside = np.array([int(np.argmin(r))])
+    cells = inside.astype(np.int32)
+    wv = mesh.volume[cells] / mesh.volume[cells].sum()
+    rate = np.array([1.0e50, 5.0e48, 3.0e48])[:, None] * wv[None, :]
+    return Workload("config5_hii_region_%d" % n, mesh, p, st, Sources(cells, np.ascontiguousarray(rate)),
+                    cfl_dt(mesh, ct), {"r0": r0, "n0": 3.2})
+
+
 def travelling_wave(n, jitter=0.1, order=2, seed=SEED_MESH + 9):
     """PAPER.md:280-284 (eq 17): E = 1 + 1e-6 sin(2 pi (x+y+z)), |F| = c E along (1,1,1), c = 1,
     periodic unit box, zero opacity, 'irregular mesh' = lattice generators offset by 10 %."""
@@ -226,4 +285,6 @@ def get(cfg, n=None):
         return config2(n or 64)
     if cfg in (3, 4):
         return config34(n or (256 if cfg == 3 else 384), cfg)
+    if cfg == 5:
+        return hii_region(n or 44)
     raise ValueError(cfg)

@@ -16,7 +16,7 @@ def _pair(oracle_mod, w):
     return o, s
 
 
-CASES = [(0, 12), (1, 24), (2, 10), (3, 10), (4, 9)]
+CASES = [(0, 12), (1, 24), (2, 10), (3, 10), (4, 9), (5, 10)]   # 5: H II region, SURVEY.md 8(f)2
 
 
 @pytest.mark.parametrize("c,n", CASES)
@@ -32,7 +32,7 @@ def test_first_subcycle(oracle_mod, c, n):
     assert P.ledger_errors(o.ledger(), lg) <= P.TOL_LEDGER
 
 
-@pytest.mark.parametrize("c,n,k", [(0, 12, 40), (1, 24, 40), (2, 10, 30), (3, 10, 20), (4, 9, 20)])
+@pytest.mark.parametrize("c,n,k", [(0, 12, 40), (1, 24, 40), (2, 10, 30), (3, 10, 20), (4, 9, 20), (5, 10, 30)])
 def test_step_from_developed_state(oracle_mod, c, n, k):
     """GPU runs k subcycles and downloads; the oracle advances that state by one subcycle and is
     compared with the GPU's k+1 (SURVEY.md 8(c) parity metric)."""
@@ -51,7 +51,7 @@ def test_step_from_developed_state(oracle_mod, c, n, k):
     assert max(e["xHII"], e["xHeII"], e["xHeIII"]) <= 1e-9 and e["eth"] <= 1e-8, e
 
 
-@pytest.mark.parametrize("c,n", [(0, 12), (2, 10), (3, 10)])
+@pytest.mark.parametrize("c,n", [(0, 12), (2, 10), (3, 10), (5, 10)])
 def test_100_subcycles_fractions_and_ledger(oracle_mod, c, n):
     w = cfg.get(c, n)
     o, s = _pair(oracle_mod, w)

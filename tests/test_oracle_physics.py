@@ -107,3 +107,53 @@ def test_p4_beam_speed_and_shadow(oracle_mod):
     assert ratio < 0.5                                                # shadow (value unpinned by the paper)
     stored0 = (w.state.N * w.mesh.volume).sum(1)
     assert budget_residual(o.ledger(), stored0).max() < 1e-12
+
+
+def test_grey_blackbody_constants():
+    """The quadrature behind config 5's grey constants reproduces the stored 1e5 K table of
+    configs 2-4 and the textbook limits: sigma at threshold for a cold
+    spectrum, a softer spectrum gives larger HI cross-sections and smaller excess energies."""
+    s, e, sh = cfg.grey_blackbody(1.0e5)
+    m = cfg.SIGMA3 > 0
+    assert np.all((s > 0) == m)
+    assert np.max(np.abs(s[m] / cfg.SIGMA3[m] - 1)) < 2e-4
+    assert np.max(np.abs(e[m] / cfg.EPS3[m] - 1)) < 2e-4
+    assert np.max(np.abs(sh - cfg.SHARE3)) < 1e-5 and abs(sh.sum() - 1) < 1e-14
+    s5, e5, sh5 = cfg.grey_blackbody(5.0e4)
+    assert np.all(s5[m] > s[m]) and np.all(e5[m] < e[m]) and sh5[0] > sh[0]
+    sc, ec, _ = cfg.grey_blackbody(1.0e3)       # kT << 13.6 eV: all photons sit at the lower edge
+    assert sc[0, 0] == pytest.approx(6.3e-18, rel=0.05) and ec[0, 0] / cfg.EV < 0.2
+
+
+def test_hii_region_workload_and_budget(oracle_mod):
+    """Config 5 (eq 16): the density follows eq (16), the three
+    bins inject 1e50 / 5e48 / 3e48 photons per second homogeneously in the 0.05 kpc sphere, the
+    photon budget closes, and after 60 subcycles the gas is ionised and heated only near the
+    centre (T stays at 100 K in the outskirts)."""
+    w = cfg.get(5, 12)
+    box = 1.6 * cfg.KPC
+    c = w.mesh.centroid
+    r = np.sqrt(((c - 0.5 * box) ** 2).sum(0))
+    r0 = 91.5e-3 * cfg.KPC
+    assert np.all(w.state.nH[r < r0] == 3.2)
+    far = r > r0
+    assert np.allclose(w.state.nH[far] * r[far] ** 2, 3.2 * r0 ** 2, rtol=1e-13)
+    assert np.allclose(w.sources.rate.sum(1), [1.0e50, 5.0e48, 3.0e48], rtol=1e-14)
+    w44 = cfg.get(5, 44)
+    rs = np.sqrt(((w44.mesh.centroid[:, w44.sources.cell] - 0.5 * box) ** 2).sum(0))
+    assert w44.sources.cell.size > 1 and rs.max() < 0.05 * cfg.KPC
+    dens = w44.sources.rate / w44.mesh.volume[w44.sources.cell]
+    assert np.allclose(dens, dens[:, :1], rtol=1e-13)
+    stored0 = (w.state.N * w.mesh.volume).sum(1)
+    o = _run(oracle_mod, w, 60)
+    led, st = o.ledger(), o.get_state()
+    assert budget_residual(led, stored0).max() < 1e-12
+    assert np.allclose(led["injected"], w.sources.rate.sum(1) * 60 * w.dt, rtol=1e-13)
+    assert led["cells_hit_cap"] == 0
+    y = w.params.y_he
+    xe = st["xHII"] + y * (st["xHeII"] + 2 * st["xHeIII"])
+    T = st["eth"] / (1.5 * w.state.nH * (1 + y + xe) * cfg.K_B)
+    assert st["xHII"][np.argmin(r)] > 0.1 and T[np.argmin(r)] > 3e3
+    edge = r > 0.6 * cfg.KPC
+    assert st["xHII"][edge].max() < 1e-3 and np.median(np.abs(T[edge] - 100.0)) < 1e-2 and T[edge].max() < 0.1 * T[np.argmin(r)]
+    assert np.all(st["N"] >= 0)

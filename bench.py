@@ -213,12 +213,12 @@ def main():
     C, F, G = int(w.mesh.ncell), int(w.mesh.nface), int(w.params.ngroup)
     NR = int((w.mesh.right >= 0).sum())
     s = rt.Solver(w.mesh, w.params, device=local)
+    stored0 = np.asarray([float((w.state.N[g] * w.mesh.volume).sum()) for g in range(G)])   # photons at t = 0
     w.mesh = None
     torch.cuda.empty_cache()
     s.init(w.state, w.sources)
     tiles = s.tile_info()
     t_build = time.perf_counter() - t_build
-    stored0 = None
     s.step(w.dt, args.warmup)
     torch.cuda.synchronize()
 
@@ -345,7 +345,7 @@ def main():
             "ledger": {"substeps_total": int(led["substeps_total"]), "substeps_max": int(led["substeps_max"]),
                        "cells_hit_cap": int(led["cells_hit_cap"]),
                        "budget_residual": float(np.max(np.abs(led["stored"] + led["absorbed"] + led["outflow"]
-                                                              - led["injected"] - led["inflow_bc"] - led["floor_added"]))
+                                                              - stored0 - led["injected"] - led["inflow_bc"] - led["floor_added"]))
                                                 / stored_scale)}}
     print(json.dumps(line))
     if dist is not None:

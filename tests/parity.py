@@ -63,3 +63,103 @@ def ledger_errors(lo, lg):
     scale = np.abs(lo["stored"]) + np.abs(lo["injected"]) + np.abs(lo["inflow_bc"]) + np.abs(lo["absorbed"]) + 1e-300
     return max(float(np.max(np.abs(lo[k] - lg[k]) / scale)) for k in
                ("stored", "injected", "absorbed", "outflow", "inflow_bc", "floor_added"))
+
+
+# ------------------------------------------------------------------ sampled cells at full size
+PATCH_RINGS = 5   # one subcycle (two Heun stages of gradient + flux) reaches 4 rings; one ring of margin
+
+
+def patch_around(mesh, seeds, rings=PATCH_RINGS, xp=None):
+    """Sub-mesh of all cells within `rings` face-neighbour rings of `seeds`, so that the oracle can
+    compute the seeds' (and their ring-1 neighbours') subcycle one by one at sizes it cannot run
+    whole.  Faces with one side outside the patch become outflow faces of the inside cell (they
+    belong to outermost-ring cells only, outside the seeds' domain of dependence).  Works on
+    numpy arrays or cuda tensors (xp = numpy or torch); returns (numpy Mesh, global cell ids, ring)
+    with the patch cells in ascending global order and ring[k] the ring index of patch cell k."""
+    from paper_2404_17630_b200.inputs import mesh as M
+    tor = xp is not None and xp.__name__ == "torch"
+    left, right = mesh.left, mesh.right
+    C = int(mesh.ncell)
+    if tor:
+        dev = left.device
+        ring = xp.full((C,), 127, dtype=xp.int8, device=dev)
+        ring[xp.as_tensor(np.asarray(seeds), device=dev).long()] = 0
+        interior = right >= 0
+        rsafe = xp.where(interior, right, left)
+        for k in range(1, rings + 1):
+            ml, mr = ring[left.long()] < 127, ring[rsafe.long()] < 127
+            idx = xp.nonzero(ml ^ mr).ravel()
+            both = xp.cat([left[idx].long(), rsafe[idx].long()])
+            both = both[ring[both] == 127]
+            ring[both] = k
+            del ml, mr, idx, both
+        ml, mr = ring[left.long()] < 127, (ring[rsafe.long()] < 127) & interior
+        fidx = xp.nonzero(ml | mr).ravel()
+        cells = xp.nonzero(ring < 127).ravel()
+        to_np = lambda t: t.cpu().numpy()
+        g = lambda a: to_np(a[..., fidx])
+        fl, fr = to_np(left[fidx]).astype(np.int64), to_np(right[fidx]).astype(np.int64)
+        inl, inr = to_np(ml[fidx]), to_np(mr[fidx])
+        area, normal, fcen = g(mesh.area), g(mesh.normal), g(mesh.fcentroid)
+        cells_np = to_np(cells)
+        vol, cen = to_np(mesh.volume[cells]), to_np(mesh.centroid[:, cells])
+        ring_np = to_np(ring[cells]).astype(np.int64)
+    else:
+        ring = np.full(C, 127, dtype=np.int8)
+        ring[np.asarray(seeds)] = 0
+        interior = right >= 0
+        rsafe = np.where(interior, right, left)
+        for k in range(1, rings + 1):
+            ml, mr = ring[left] < 127, ring[rsafe] < 127
+            idx = np.flatnonzero(ml ^ mr)
+            both = np.concatenate([left[idx], rsafe[idx]])
+            both = both[ring[both] == 127]
+            ring[both] = k
+        ml, mr = ring[left] < 127, (ring[rsafe] < 127) & interior
+        fidx = np.flatnonzero(ml | mr)
+        cells_np = np.flatnonzero(ring < 127)
+        fl, fr = left[fidx].astype(np.int64), right[fidx].astype(np.int64)
+        inl, inr = ml[fidx], mr[fidx]
+        area, normal, fcen = mesh.area[fidx], mesh.normal[:, fidx], mesh.fcentroid[:, fidx]
+        vol, cen = mesh.volume[cells_np], mesh.centroid[:, cells_np]
+        ring_np = ring[cells_np].astype(np.int64)
+    # renumber; a face seen only from its right cell is turned around (normal flipped, outflow)
+    loc = lambda gidx: np.searchsorted(cells_np, gidx)
+    normal = normal.copy()
+    flip = ~inl
+    nl = np.where(flip, fr, fl)
+    nr = np.where(inl & inr, fr, np.where(inl & (fr < 0), fr, M.BC_OUTFLOW))
+    normal[:, flip] *= -1.0
+    nl = loc(nl).astype(np.int32)
+    nr = np.where(nr >= 0, loc(np.maximum(nr, 0)), nr).astype(np.int32)
+    pm = M.Mesh(int(cells_np.size), int(fidx.numel() if tor else fidx.size), np.asarray(mesh.box, dtype=np.float64).copy(),
+                np.asarray(mesh.periodic, dtype=np.int32).copy(), np.ascontiguousarray(vol), np.ascontiguousarray(cen),
+                np.ascontiguousarray(area), np.ascontiguousarray(normal), np.ascontiguousarray(fcen), nl, nr,
+                {"kind": "patch"})
+    return pm, cells_np, ring_np
+
+
+def restrict_state(st, cells, nH):
+    """State (dict of numpy arrays in the caller's order) restricted to `cells`."""
+    return cfg.State(np.ascontiguousarray(st["N"][:, cells]), np.ascontiguousarray(st["F"][:, :, cells]),
+                     st["xHII"][cells].copy(), st["xHeII"][cells].copy(), st["xHeIII"][cells].copy(),
+                     st["eth"][cells].copy(), np.ascontiguousarray(nH[cells]))
+
+
+def restrict_sources(src, cells):
+    keep = np.isin(src.cell, cells)
+    return cfg.Sources(np.searchsorted(cells, src.cell[keep]).astype(np.int32), np.ascontiguousarray(src.rate[:, keep]))
+
+
+def cell_errors(pmesh, ct, prev, ref, got, which):
+    """step_errors' metric evaluated on the patch cells `which` only (prev, ref, got: patch arrays)."""
+    e = {"N": 0.0, "F": 0.0}
+    for g in range(ref["N"].shape[0]):
+        scale = np.maximum(dependence_max(pmesh, prev["N"][g]), np.abs(ref["N"][g]))
+        scale = np.maximum(scale, max(1e-100 * np.abs(ref["N"][g]).max(), 1e-300))[which]
+        e["N"] = max(e["N"], float(np.max(np.abs(got["N"][g] - ref["N"][g])[which] / scale)))
+        e["F"] = max(e["F"], float(np.max(np.abs(got["F"][g] - ref["F"][g])[:, which] / (ct * scale[None, :]))))
+    for k in ("xHII", "xHeII", "xHeIII"):
+        e[k] = float(np.max(np.abs(got[k] - ref[k])[which]))
+    e["eth"] = float(np.max((np.abs(got["eth"] - ref["eth"]) / np.maximum(np.abs(ref["eth"]), 1e-300))[which]))
+    return e

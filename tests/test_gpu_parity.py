@@ -250,3 +250,56 @@ def test_zero_subcycles_and_zero_sources_leave_the_state_alone():
     _, lg = s.download()
     stored0 = (w.state.N * w.mesh.volume).sum(1)
     assert np.all(lg["injected"] == 0.0) and P.budget_residual(lg, stored0).max() <= P.TOL_LEDGER
+
+
+@pytest.mark.parametrize("c,n", [(4, 384)])
+def test_full_size_sampled_cells(oracle_mod, c, n):
+    """BASELINE.json's config 4 at its full size (56.6 M cells, the mesh and launch configuration
+    `bench.py` times): the oracle cannot run the whole mesh in seconds, so it computes sampled
+    cells one by one.  After three subcycles on the GPU the state is downloaded; the oracle advances
+    the 5-ring patches around the sampled cells (sources and cells away from them) by one subcycle
+    from that state and is compared, on the samples and their face neighbours, with the GPU's
+    fourth subcycle.  `tests/test_patch_oracle.py` shows on the CPU that such a patch reproduces the
+    whole-mesh oracle exactly on those cells."""
+    import torch
+    from paper_2404_17630_b200 import rt
+    from paper_2404_17630_b200.inputs import device as devin
+    free, _ = torch.cuda.mem_get_info(0)
+    if free < 160e9:
+        pytest.skip("needs a whole 180 GB B200 (%.0f GB free)" % (free / 1e9))
+    w = devin.config34_device(n, c, "cuda:0")
+    # samples: the brightest and the faintest source, two more sources, three cells elsewhere
+    order = np.argsort(w.sources.rate.sum(0))
+    C = w.mesh.ncell
+    seeds = np.unique(np.concatenate([w.sources.cell[order[[0, 1, -2, -1]]].astype(np.int64),
+                                      np.array([12345, C // 2 + 777, C - 4321], dtype=np.int64)]))
+    pm, cells, ring = P.patch_around(w.mesh, seeds, xp=torch)      # while only the mesh is resident
+    assert 7 * 300 < pm.ncell < 7 * 3000 and ring.max() == P.PATCH_RINGS
+    torch.cuda.empty_cache()
+    s = rt.Solver(w.mesh, w.params)
+    w.mesh = None
+    torch.cuda.empty_cache()
+    s.init(w.state, w.sources)
+    nH = w.state.nH.cpu().numpy()
+    w.state = None
+    torch.cuda.empty_cache()
+    k = 3
+    s.step(w.dt, k)
+    prev, _ = s.download()
+    s.step(w.dt, 1)
+    got, lg = s.download()
+    assert lg["cells_hit_cap"] == 0
+    o = oracle_mod.Oracle(pm, w.params)
+    o.set_sources(P.restrict_sources(w.sources, cells))
+    o.set_state(P.restrict_state(prev, cells, nH))
+    o.step(w.dt, 1)
+    ref = o.get_state()
+    sub = lambda st: {"N": st["N"][:, cells], "F": st["F"][:, :, cells], "xHII": st["xHII"][cells],
+                      "xHeII": st["xHeII"][cells], "xHeIII": st["xHeIII"][cells], "eth": st["eth"][cells]}
+    which = np.flatnonzero(ring <= 1)
+    pprev, pgot = sub(prev), sub(got)
+    assert np.abs(pprev["N"][:, which]).max() > 0 and np.any(pgot["N"][:, which] != pprev["N"][:, which])
+    e = P.cell_errors(pm, w.params.ctilde, pprev, ref, pgot, which)
+    assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
+    assert max(e["xHII"], e["xHeII"], e["xHeIII"]) <= 1e-9 and e["eth"] <= 1e-8, e
+    s.close()

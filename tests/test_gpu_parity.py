@@ -32,7 +32,9 @@ def test_first_subcycle(oracle_mod, c, n):
     assert P.ledger_errors(o.ledger(), lg) <= P.TOL_LEDGER
 
 
-@pytest.mark.parametrize("c,n,k", [(0, 12, 40), (1, 24, 40), (2, 10, 30), (3, 10, 20), (4, 9, 20), (5, 10, 30)])
+# (the last three: configs 0, 1 and 2 at BASELINE.json's full size, every cell compared)
+@pytest.mark.parametrize("c,n,k", [(0, 12, 40), (1, 24, 40), (2, 10, 30), (3, 10, 20), (4, 9, 20), (5, 10, 30),
+                                   (0, 32, 80), (1, 128, 100), (2, 64, 30)])
 def test_step_from_developed_state(oracle_mod, c, n, k):
     """GPU runs k subcycles and downloads; the oracle advances that state by one subcycle and is
     compared with the GPU's k+1 (SURVEY.md 8(c) parity metric)."""
@@ -46,9 +48,44 @@ def test_step_from_developed_state(oracle_mod, c, n, k):
     got, _ = s.download()
     o = oracle_mod.Oracle(w.mesh, w.params); o.set_sources(w.sources); o.set_state(P.as_state(dev))
     o.step(w.dt, 1)
-    e = P.step_errors(w.mesh, w.params.ctilde, dev, o.get_state(), got)
+    # the full-size beam has a ten-decade edge two cells wide: there the scale is the subcycle's whole
+    # domain of dependence (tests/test_oracle_conditioning.py: the oracle's own response to 1-ulp
+    # noise is 5e-9 in the one-ring metric and 7e-16 in this one)
+    rings = P.DEPENDENCE_RINGS if (c, n) == (1, 128) else 1
+    e = P.step_errors(w.mesh, w.params.ctilde, dev, o.get_state(), got, rings=rings)
     assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
     assert max(e["xHII"], e["xHeII"], e["xHeIII"]) <= 1e-9 and e["eth"] <= 1e-8, e
+
+
+@pytest.mark.parametrize("k", [2, 30])
+def test_hii_region_full_size_outside_the_chaotic_cells(oracle_mod, k):
+    """Config 5 at the paper's size (44^3 generators).  In the few strongly irradiated
+    cells around the sources the oracle's own sub-stepping is chaotic (parity.chaotic_cells,
+    tests/test_oracle_conditioning.py): there both sides must agree at the integration-error level;
+    every cell outside those cells' domain of dependence is compared at the usual tolerances."""
+    from paper_2404_17630_b200 import rt
+    w = cfg.get(5, 44)
+    s = rt.Solver(w.mesh, w.params); s.init(w.state, w.sources)
+    s.step(w.dt, k)
+    dev, _ = s.download()
+    dev["nH"] = w.state.nH
+    s.step(w.dt, 1)
+    got, lg = s.download()
+    o = oracle_mod.Oracle(w.mesh, w.params); o.set_sources(w.sources); o.set_state(P.as_state(dev))
+    o.step(w.dt, 1)
+    ref = o.get_state()
+    bad = P.chaotic_cells(oracle_mod, w, dev)
+    reach = P.dependence_max(w.mesh, bad.astype(np.float64), rings=P.DEPENDENCE_RINGS) > 0
+    C = w.mesh.ncell
+    print("config 5 at 44^3, k = %d: %d chaotic cells, %d cells in their domain of dependence of %d" % (k, bad.sum(), reach.sum(), C))
+    assert bad.sum() <= 0.002 * C and reach.sum() <= 0.1 * C
+    e = P.cell_errors(w.mesh, w.params.ctilde, dev, ref, got, np.flatnonzero(~reach))
+    assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
+    assert max(e["xHII"], e["xHeII"], e["xHeIII"]) <= 1e-9 and e["eth"] <= 1e-8, e
+    for f in ("xHII", "xHeII", "xHeIII"):
+        assert np.max(np.abs(got[f] - ref[f])) <= 5e-3, f
+    assert np.max(np.abs(got["eth"] - ref["eth"]) / ref["eth"]) <= 2e-2
+    assert lg["cells_hit_cap"] == 0 and got["N"].min() >= 0.0
 
 
 @pytest.mark.parametrize("c,n", [(0, 12), (2, 10), (3, 10), (5, 10)])
@@ -252,10 +289,10 @@ def test_zero_subcycles_and_zero_sources_leave_the_state_alone():
     assert np.all(lg["injected"] == 0.0) and P.budget_residual(lg, stored0).max() <= P.TOL_LEDGER
 
 
-@pytest.mark.parametrize("c,n", [(4, 384)])
+@pytest.mark.parametrize("c,n", [(3, 256), (4, 384)])
 def test_full_size_sampled_cells(oracle_mod, c, n):
-    """BASELINE.json's config 4 at its full size (56.6 M cells, the mesh and launch configuration
-    `bench.py` times): the oracle cannot run the whole mesh in seconds, so it computes sampled
+    """BASELINE.json's configs 3 and 4 at their full sizes (16.8 M and 56.6 M cells; for config 4 the
+    mesh and launch configuration `bench.py` times): the oracle cannot run the whole mesh in seconds, so it computes sampled
     cells one by one.  After three subcycles on the GPU the state is downloaded; the oracle advances
     the 5-ring patches around the sampled cells (sources and cells away from them) by one subcycle
     from that state and is compared, on the samples and their face neighbours, with the GPU's
@@ -264,8 +301,11 @@ def test_full_size_sampled_cells(oracle_mod, c, n):
     import torch
     from paper_2404_17630_b200 import rt
     from paper_2404_17630_b200.inputs import device as devin
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info(0)
-    if free < 160e9:
+    if free < (160e9 if n == 384 else 60e9):
         pytest.skip("needs a whole 180 GB B200 (%.0f GB free)" % (free / 1e9))
     w = devin.config34_device(n, c, "cuda:0")
     # samples: the brightest and the faintest source, two more sources, three cells elsewhere
@@ -300,6 +340,10 @@ def test_full_size_sampled_cells(oracle_mod, c, n):
     pprev, pgot = sub(prev), sub(got)
     assert np.abs(pprev["N"][:, which]).max() > 0 and np.any(pgot["N"][:, which] != pprev["N"][:, which])
     e = P.cell_errors(pm, w.params.ctilde, pprev, ref, pgot, which)
+    print("full-size sampled parity: config %d, n = %d, %d patch cells, %d compared:" % (c, n, pm.ncell, which.size), e)
     assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
     assert max(e["xHII"], e["xHeII"], e["xHeIII"]) <= 1e-9 and e["eth"] <= 1e-8, e
     s.close()
+    del s, w
+    gc.collect()
+    torch.cuda.empty_cache()

@@ -34,3 +34,31 @@ def test_patch_reproduces_whole_mesh(oracle_mod, c, n, k):
     if c != 0:
         outer = np.flatnonzero(ring == P.PATCH_RINGS)
         assert outer.size > 0
+
+
+def test_domain_of_dependence_is_four_rings(oracle_mod):
+    """One subcycle (two Heun stages x (gradient + flux)) reaches exactly four rings of face
+    neighbours: a 4-ring patch is exact for its seeds but not for their neighbours, a 3-ring patch is
+    not exact for the seeds.  parity.DEPENDENCE_RINGS and PATCH_RINGS rest on this."""
+    w = cfg.get(3, 12)
+    o = oracle_mod.Oracle(w.mesh, w.params); o.set_sources(w.sources); o.set_state(w.state)
+    o.step(w.dt, 6)
+    prev = o.get_state()
+    o.step(w.dt, 1)
+    ref = o.get_state()
+    seeds = w.sources.cell[:2].astype(np.int64)
+    keys = ("N", "F", "xHII", "xHeII", "xHeIII", "eth")
+    err = {}
+    for rings in (3, 4):
+        pm, cells, ring = P.patch_around(w.mesh, seeds, rings=rings)
+        po = oracle_mod.Oracle(pm, w.params)
+        po.set_sources(P.restrict_sources(w.sources, cells))
+        po.set_state(P.restrict_state(prev, cells, w.state.nH))
+        po.step(w.dt, 1)
+        got = po.get_state()
+        sub = lambda s: {k: s[k][..., cells] for k in keys}
+        for r in (0, 1):
+            e = P.cell_errors(pm, w.params.ctilde, sub(prev), sub(ref), got, np.flatnonzero(ring <= r))
+            err[rings, r] = max(e["N"], e["F"])
+    assert P.DEPENDENCE_RINGS == 4 and P.PATCH_RINGS == P.DEPENDENCE_RINGS + 1
+    assert err[4, 0] == 0.0 and err[4, 1] > 1e-12 and err[3, 0] > 1e-12, err

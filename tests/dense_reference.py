@@ -50,6 +50,9 @@ def _ghost(U, code, n, ghost, for_flux):
     return ghost[-3 - code].copy()
 
 
+CAPPED = []   # faces whose number flux the donor cap clamped, appended by rhs() (tests clear and read it)
+
+
 def rhs(mesh, U, ct, dt, ghost, order):
     """U: (C,4). Returns R (C,4) without sources, and boundary N-fluxes {face: A*Phi_N}."""
     C, F = mesh.ncell, mesh.nface
@@ -105,6 +108,7 @@ def rhs(mesh, U, ct, dt, ghost, order):
             lim = U[d, 0] * mesh.volume[d] / (dt * mesh.area[f])
             if abs(ph[0]) > lim:
                 ph[0] = np.sign(ph[0]) * lim
+                CAPPED.append(f)
         R[L] -= mesh.area[f] * ph / mesh.volume[L]
         if Rr >= 0:
             R[Rr] += mesh.area[f] * ph / mesh.volume[Rr]

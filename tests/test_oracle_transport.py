@@ -52,6 +52,28 @@ def test_p5_brute_force_tiny_mesh(oracle_mod, kind):
     assert np.max(np.abs(_U(o) - ref)) < 1e-13
 
 
+@pytest.mark.parametrize("kind", ["mixed_bc3", "voronoi5"])
+def test_p5_brute_force_with_the_donor_cap_active(oracle_mod, kind):
+    # nearly empty cells beside full, fast-streaming ones: the reconstructed face states make the
+    # number flux leave the empty cell, and the cap must clamp it
+    import dense_reference as D
+    ct = 0.8
+    ghost = np.array([[1.3, 0.5, 0.1, -0.2]])
+    mesh = M.cartesian(3, 1.5, periodic=False, bc=(-2, -1, -3, -2, -1, -3)) if kind == "mixed_bc3" \
+        else M.voronoi(5, 1.0, 0.3, 11, periodic=True)
+    U0 = _rand_state(mesh.ncell, 4, ct)
+    empty = np.arange(mesh.ncell) % 3 == 0
+    U0[empty] *= 1e-7
+    dt = cfg.cfl_dt(mesh, ct)
+    p = cfg.Params(ngroup=1, ctilde=ct, chem_mode=cfg.CHEM_NONE, ghost_state=ghost)
+    o = _mk(oracle_mod, mesh, U0, p)
+    o.step(dt, 1)
+    del D.CAPPED[:]
+    ref = D.heun_step(mesh, U0, ct, dt, ghost=ghost)
+    assert len(D.CAPPED) > 0                        # the cap fired in the reference evaluation
+    assert np.max(np.abs(_U(o) - ref)) < 1e-13
+
+
 def test_p5_first_order_and_sources(oracle_mod):
     from dense_reference import heun_step
     mesh = M.cartesian(2, 1.0, periodic=False)

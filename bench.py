@@ -171,6 +171,32 @@ def algorithmic_bytes(C, F, NR, G, heun=True, chem=True, order=2):
     return {"grad": grad, "stage": stage, "chem": chemb, "subcycle": per_sub}
 
 
+def run_alu_peak():
+    """fp64-pipe and shared-memory peaks of this GPU, measured by the library's own micro-benchmark
+    kernels (csrc/rt_peak.cu), with the clocks sampled while they run."""
+    import torch
+    from paper_2404_17630_b200 import rt
+    torch.cuda.set_device(0)
+    h = rt.rt_create(0, torch.cuda.current_stream().cuda_stream)
+    rt.rt_debug_alu_peak(h)                      # warm-up
+    sampler = ClockSampler(0)
+    time.sleep(0.3)
+    t0 = time.perf_counter()
+    best = None
+    for _ in range(5):
+        d = rt.rt_debug_alu_peak(h)
+        best = d if best is None else {k: max(best[k], d[k]) for k in d}
+    t1 = time.perf_counter()
+    clocks = sampler.stop(t0, t1)
+    rt.rt_destroy(h)
+    best["fp64_tflops_dfma"] = 2.0 * best["dfma"] / 1e12
+    best["lds_bytes_per_clk_per_sm"] = {k: 16.0 * best[k] / best["sm_count"] / (clocks["sm_mhz"] or 1965.0) / 1e6
+                                        for k in ("lds128", "lds128_bcast3", "lds128_bcast8", "lds128_random")}
+    best["clocks"] = clocks
+    print(json.dumps({"alu_peak": best}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -182,9 +208,13 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--alu-peak", action="store_true",
+                    help="only run the fp64 / shared-memory micro-benchmarks (rt_debug_alu_peak) and print them")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.alu_peak:
+        return run_alu_peak()
     if args.warmup < 3:
         args.warmup = 3
 

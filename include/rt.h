@@ -37,7 +37,10 @@ extern "C" {
 
 enum { RT_OK = 0, RT_EINVAL = -1, RT_ENOMEM = -2, RT_ECUDA = -3, RT_ESTATE = -4, RT_EMESH = -5 };
 enum { RT_MEM_HOST = 0, RT_MEM_DEVICE = 1 };
-enum { RT_WS_DEVICE_MESH = 1 }; /* flags of rt_workspace_bytes */
+/* flags of rt_workspace_bytes: RT_WS_DEVICE_MESH = the mesh arrays handed to rt_mesh_upload are DEVICE
+ * pointers (no staging space); RT_WS_ALL_FACES_CROSS = reserve flux rows for every face (needed when
+ * rt_tuning asks for tiles below the default size, or when rt_mesh_upload said so in RT_ENOMEM) */
+enum { RT_WS_DEVICE_MESH = 1, RT_WS_ALL_FACES_CROSS = 2 };
 /* rt_mesh.right codes for boundary faces (reading S13) */
 enum { RT_BC_OUTFLOW = -1, RT_BC_REFLECT = -2, RT_BC_DIRICHLET0 = -3 /* -3-k: ghost state k */ };
 enum { RT_CHEM_NONE = 0, RT_CHEM_FIXED_OPACITY = 1, RT_CHEM_H_ISOTHERMAL = 2, RT_CHEM_HHE_THERMAL = 3 };
@@ -111,13 +114,38 @@ typedef struct {
   int64_t nsub_done;
 } rt_ledger;
 
+/* Optional tuning of the tile decomposition and of the launches.  Every field: 0 =
+ * the library's default.  The library reads no environment variable; experiments and tests set
+ * these explicitly with rt_set_tuning before rt_mesh_upload. */
+typedef struct {
+  int32_t tile_cells;     /* cells per gradient tile; also the upper bound of a flux tile (default 32 with
+                             G >= 2, 96 with one group) */
+  int32_t tile_faces;     /* owned faces per flux tile (default 240: one face per thread of a 256-thread
+                             block); -1 = flux tiles of tile_cells cells each */
+  int32_t tile_blocks;    /* thread blocks of the flux kernel the tile size is chosen for (default 2) */
+  int32_t tile_classes;   /* 1 = off: one launch sized by the largest tile (default: two size classes) */
+  int32_t flux_threads;   /* threads per block of the flux kernel (default 256) */
+  int32_t grad_threads;   /* threads per block of the gradient kernel (default 4 per cell, at most 256) */
+  int32_t prefetch_tiles; /* the tile kernels ask L2 for the data of the tile this many blocks ahead
+                             (default 600; -1 = off) */
+  int32_t chem_caps[6];   /* trial caps of the chemistry passes, 0-terminated (default 1, 8: one trial
+                             for every cell, up to 8 more for the unfinished, then the rest) */
+  int32_t variant;        /* bit field of experimental kernel variants (default 0) */
+  int32_t reserved[9];
+} rt_tuning;
+
 /* Creates a context on CUDA device `device` issuing all work on `cuda_stream` (a cudaStream_t;
  * NULL = the legacy default stream).  The stream is borrowed and must outlive the context. */
 int rt_create(rt_ctx **out, int device, void *cuda_stream);
 
+/* Sets the tuning of the next rt_mesh_upload (NULL = defaults).  RT_EINVAL on out-of-range values. */
+int rt_set_tuning(rt_ctx *ctx, const rt_tuning *t);
+
 /* Bytes of device workspace rt_mesh_upload needs for this problem size (0 on invalid sizes).
- * flags: 0, or RT_WS_DEVICE_MESH if the mesh arrays passed to rt_mesh_upload will be DEVICE
- * pointers (no staging space for a host mesh is reserved then: 88 bytes per face less). */
+ * flags: an OR of RT_WS_* (RT_WS_DEVICE_MESH: no staging space for a host mesh, 88 bytes per face
+ * less).  Without RT_WS_ALL_FACES_CROSS the workspace holds the fluxes of 0.56 nface + 1024 faces
+ * that cross tile boundaries (a jittered-lattice Voronoi mesh at the default tile size has 0.54);
+ * rt_mesh_upload returns RT_ENOMEM, saying so, for a mesh or a tuning that needs more. */
 size_t rt_workspace_bytes(int64_t ncell, int64_t nface, int ngroup, int flags);
 
 /* Validates the mesh (index ranges, positive volumes and areas, unit normals, closed cells:
@@ -168,6 +196,14 @@ int rt_profile_read(rt_ctx *ctx, double *ms, int64_t *count);
 /* Slope-limited gradients of the current state in the caller's order, DEVICE or HOST as
  * mem_kind says: gN (G, 3, C), gF (G, 3 components, 3 directions, C).  For tests. Synchronises. */
 int rt_debug_gradients(rt_ctx *ctx, int mem_kind, double *gN, double *gF);
+
+/* Micro-benchmarks of the device's fp64 pipe and shared memory (not part of the subcycle; they place
+ * the ALU ceiling beside the HBM roofline).  out: HOST array of 14 = operations per
+ * second of dependent-chain-free DFMA, DADD, DMUL, compare+select (max), MUFU reciprocal seed,
+ * reciprocal seed + two Newton steps, MUFU rsqrt seed, IEEE division, IEEE sqrt; 16-byte
+ * shared-memory loads per second with 32 distinct chunks per warp, with groups of 3 and of 8 lanes
+ * reading one chunk, and with a random chunk per lane; the number of multiprocessors.  Synchronises. */
+int rt_debug_alu_peak(rt_ctx *ctx, double *out);
 
 /* Last error message of this context ("" if none); valid until the next call on it. */
 const char *rt_last_error(const rt_ctx *ctx);

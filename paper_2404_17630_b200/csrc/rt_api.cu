@@ -46,7 +46,7 @@ int rt_create(rt_ctx **out, int device, void *cuda_stream) {
   c->device = 0; c->stream = 0; c->err[0] = 0; c->C = c->F = c->NR = 0; c->G = 0; c->nghost = 0; c->ws = nullptr;
   c->ws_bytes = 0; c->have_mesh = c->have_state = false; c->nsrc = 0; c->nsub_done = 0; c->launches = 0;
   c->prof_on = false; c->prof_used = 0;
-  memset(&c->par, 0, sizeof(c->par)); memset(&c->lay, 0, sizeof(c->lay));
+  memset(&c->par, 0, sizeof(c->par)); memset(&c->lay, 0, sizeof(c->lay)); memset(&c->tun, 0, sizeof(c->tun));
   c->device = device;
   c->stream = (cudaStream_t)cuda_stream;
   if (cudaSetDevice(device) != cudaSuccess) { delete c; return RT_ECUDA; }
@@ -58,6 +58,24 @@ void rt_destroy(rt_ctx *c) {
   if (!c) return;
   for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
   delete c;
+}
+
+int rt_set_tuning(rt_ctx *c, const rt_tuning *t) {
+  if (!c) return RT_EINVAL;
+  c->err[0] = 0;
+  rt_tuning z;
+  memset(&z, 0, sizeof z);
+  if (!t) t = &z;
+  if (t->tile_cells != 0 && (t->tile_cells < RT_MIN_TILE || t->tile_cells > 1024))
+    return rt_fail(c, RT_EINVAL, "tuning.tile_cells must be 0 or in [%d, 1024]", RT_MIN_TILE);
+  if (t->tile_faces < -1 || t->tile_faces > RT_TILE_LIMIT) return rt_fail(c, RT_EINVAL, "tuning.tile_faces out of range");
+  if (t->tile_blocks < 0 || t->tile_blocks > 8) return rt_fail(c, RT_EINVAL, "tuning.tile_blocks must be in [0, 8]");
+  if (t->flux_threads < 0 || t->flux_threads > 256 || t->grad_threads < 0 || t->grad_threads > 256)
+    return rt_fail(c, RT_EINVAL, "tuning.*_threads must be in [0, 256]");
+  for (int k = 0; k < 6; k++)
+    if (t->chem_caps[k] < 0) return rt_fail(c, RT_EINVAL, "tuning.chem_caps must be >= 0");
+  c->tun = *t;
+  return RT_OK;
 }
 
 int rt_profile(rt_ctx *c, int enable) {
@@ -121,7 +139,10 @@ int rt_mesh_upload(rt_ctx *c, const rt_mesh *m, void *ws, size_t bytes) {
   RT_CUDA(c, cudaSetDevice(c->device));
   c->C = m->ncell; c->F = m->nface; c->G = m->ngroup; c->nghost = m->nghost;
   for (int a = 0; a < 3; a++) { c->box[a] = m->box[a]; c->per[a] = m->periodic[a] != 0; }
-  c->lay = rt_make_layout(c->C, c->F, c->G, m->mem_kind == RT_MEM_DEVICE ? RT_WS_DEVICE_MESH : 0);
+  // the layout the caller's workspace was sized for: with room for every face's flux if it is that large
+  const int devflag = m->mem_kind == RT_MEM_DEVICE ? RT_WS_DEVICE_MESH : 0;
+  c->lay = rt_make_layout(c->C, c->F, c->G, devflag | RT_WS_ALL_FACES_CROSS);
+  if (bytes < c->lay.total) c->lay = rt_make_layout(c->C, c->F, c->G, devflag);
   if (bytes < c->lay.total)
     return rt_fail(c, RT_ENOMEM, "workspace has %zu bytes, rt_workspace_bytes says %zu", bytes, c->lay.total);
   c->ws = (char *)ws;

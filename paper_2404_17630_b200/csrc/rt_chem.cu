@@ -281,23 +281,12 @@ __global__ void __launch_bounds__(RT_CHEM_BLOCK, 16) k_chem(rt_chem_par P, int64
   }
 }
 
-// caps of the passes: RT_CHEM_CAPS="1,8" means pass 0 makes one trial per cell, pass 1 up to 8 more
-// for the cells still unfinished, and a last pass finishes the rest (default "1,8")
-static int chem_caps(int *caps, int maxn) {
-  static int cached[8], ncached = -1;
-  if (ncached < 0) {
-    ncached = 0;
-    const char *e = getenv("RT_CHEM_CAPS");
-    if (!e) e = "1,8";
-    while (*e && ncached < 6) {
-      const int v = atoi(e);
-      if (v > 0) cached[ncached++] = v;
-      while (*e && *e != ',') e++;
-      if (*e == ',') e++;
-    }
-  }
+// caps of the passes: rt_tuning.chem_caps = {1, 8} means pass 0 makes one trial per cell, pass 1 up to
+// 8 more for the cells still unfinished, and a last pass finishes the rest (the default)
+static int chem_caps(const rt_ctx *c, int *caps, int maxn) {
   int n = 0;
-  for (; n < ncached && n < maxn; n++) caps[n] = cached[n];
+  for (; n < 6 && n < maxn && c->tun.chem_caps[n] > 0; n++) caps[n] = c->tun.chem_caps[n];
+  if (n == 0) { caps[0] = 1; caps[1] = 8; n = 2; }
   return n;
 }
 
@@ -315,7 +304,7 @@ static void launch_chem_mode(rt_ctx *c, const rt_chem_par &P, double dt, double 
 #define CHEM_ARGS P, C, dt, U, rt_ptr<double>(c, l.xHII), rt_ptr<double>(c, l.xHeII), rt_ptr<double>(c, l.xHeIII), \
       rt_ptr<double>(c, l.eth), rt_ptr<double>(c, l.nH), rt_ptr<double>(c, l.cellV), rt_ptr<double>(c, l.kappa)
   int caps[8];
-  const int ncap = MODE == RT_CHEM_FIXED_OPACITY ? 0 : chem_caps(caps, 8);
+  const int ncap = MODE == RT_CHEM_FIXED_OPACITY ? 0 : chem_caps(c, caps, 8);
   // pass 0: every cell
   rt_prof_begin(c, RT_K_CHEM);
   k_chem<G, MODE, true><<<nrows, RT_CHEM_BLOCK, 0, c->stream>>>(CHEM_ARGS, part, led, nullptr, nullptr, ncap > 0 ? caps[0] : 0, carry,

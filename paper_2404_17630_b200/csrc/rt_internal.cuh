@@ -109,6 +109,7 @@ struct rt_ctx {
   rt_layout lay;
   bool have_mesh, have_state;
   rt_params par;
+  rt_tuning tun;      // rt_set_tuning (zeros = defaults)
   int nsrc;
   double src_total[RT_MAXG];
   double injected[RT_MAXG][2];  // host-side compensated sum
@@ -125,15 +126,16 @@ enum { RT_K_CHEM = 0, RT_K_GRAD = 1, RT_K_FLUX = 2, RT_K_UPDATE = 3, RT_K_REDUCE
 void rt_prof_begin(rt_ctx *c, int cls);
 void rt_prof_end(rt_ctx *c);
 
-// one tile's descriptor (32 bytes)
+// one tile's descriptor (56 bytes)
 struct rt_tile {
   int64_t fbase;  // first owned face = fo[c0]
   int64_t blob;   // first word of the tile's blob
   int64_t xbase;  // first row of xphi the tile publishes
   int32_t nown, ninc, nh, nhf;  // owned faces, incoming faces, halo cells, half-faces
-  int32_t nb, nout, n2, pad;    // backward halo cells, outgoing faces, cells with incoming faces
+  int32_t nb, nout, n2, pad;    // backward halo cells, outgoing faces, cells with incoming faces; pad: bit 0 = the tile has boundary faces
 };
-#define RT_BLOB_HEAD 12     // 32-bit words of the descriptor copy at the start of a blob
+#define RT_BLOB_HEAD 16     // 32-bit words reserved for the descriptor copy at the start of a blob
+static_assert(sizeof(rt_tile) <= 4 * RT_BLOB_HEAD, "the blob header must hold a whole descriptor");
 #define RT_TILE_LIMIT 2048  // most owned faces / r-list entries / halo candidates of a tile the builder handles
 __host__ __device__ static inline int rt_blob_words(int TC, int nhf, int nown, int nh, int ninc, int nout) {
   return (TC + 1 + nhf + nown + nh + ninc + nout + 3) & ~3;
@@ -142,7 +144,7 @@ __host__ __device__ static inline int rt_blob_words(int TC, int nhf, int nown, i
 // dynamic shared memory of the two tile kernels (rt_transport.cu) for tiles of TC cells with at
 // most smax slots, hmax halo cells (k_grad) / forward halo cells (k_stage) and bmax blob words
 static inline size_t rt_smem_grad(int TC, int G, int smax, int hmax, int bmax) {
-  return (size_t)4 * bmax + (size_t)64 * smax + (size_t)32 * G * (TC + hmax) + (size_t)48 * TC;
+  return (size_t)4 * bmax + (size_t)64 * smax + (size_t)(32 * G + 16) * (TC + hmax) + (size_t)48 * TC;  // cell rows padded by 16 bytes
 }
 static inline size_t rt_smem_flux(int TC, int G, int omax, int fmax, int bmax) {
   const int planes = G > 3 ? G : 3;  // three face records per slot, overwritten by A*Phi of every group

@@ -239,7 +239,7 @@ __global__ void __launch_bounds__(TILE_BT) k_tile_build(int64_t C, int TC, const
   typedef cub::BlockScan<int, TILE_BT> Scan;
   __shared__ typename Scan::TempStorage scan_tmp;
   __shared__ int32_t s_cand[RT_TILE_LIMIT], s_rank[RT_TILE_LIMIT], s_halo[RT_TILE_LIMIT];
-  __shared__ int s_nc, s_run;
+  __shared__ int s_nc, s_run, s_bnd;
   const int64_t t = blockIdx.x;
   const int64_t c0 = t * TC, c1 = c0 + TC < C ? c0 + TC : C;
   const int ncell = (int)(c1 - c0);
@@ -250,7 +250,7 @@ __global__ void __launch_bounds__(TILE_BT) k_tile_build(int64_t C, int TC, const
     return;
   }
   const int nown = (int)nown64, nr = (int)nr64;
-  if (threadIdx.x == 0) { s_nc = 0; s_run = 0; }
+  if (threadIdx.x == 0) { s_nc = 0; s_run = 0; s_bnd = 0; }
   __syncthreads();
   // incoming faces: r-list entries whose owner lies in an earlier tile, ranked in r-list order
   for (int k0 = 0; k0 < nr; k0 += TILE_BT) {
@@ -269,6 +269,7 @@ __global__ void __launch_bounds__(TILE_BT) k_tile_build(int64_t C, int TC, const
   for (int s = threadIdx.x; s < nown; s += TILE_BT) {
     const int32_t r = R[fbase + s];
     if (r >= c1) { const int p = atomicAdd(&s_nc, 1); if (p < RT_TILE_LIMIT) s_cand[p] = r; }
+    if (r < 0) s_bnd = 1;  // a boundary face: the kernels take their ghost-state path for this tile
   }
   for (int k = threadIdx.x; k < nr; k += TILE_BT)
     if (s_rank[k] >= 0) { const int p = atomicAdd(&s_nc, 1); if (p < RT_TILE_LIMIT) s_cand[p] = rn[rbase + k]; }
@@ -360,11 +361,12 @@ __global__ void __launch_bounds__(TILE_BT) k_tile_build(int64_t C, int TC, const
   if (threadIdx.x == 0) {
     rt_tile d;
     d.fbase = fbase; d.blob = t * bstride; d.xbase = xoff[t]; d.nown = nown; d.ninc = ninc; d.nh = nh; d.nhf = nhf;
-    d.nb = nb; d.nout = nout; d.n2 = n2; d.pad = 0;
+    d.nb = nb; d.nout = nout; d.n2 = n2; d.pad = s_bnd;
     tiles[t] = d;
     *reinterpret_cast<rt_tile *>(blob + t * bstride) = d;  // the blob starts with a copy of the descriptor
     if (t == (int64_t)gridDim.x - 1) k2off[k2base[t] + n2] = (int32_t)(ibase[t] + ninc);  // end of the last cell's rows
   }
+  __syncthreads();
   uint32_t *ho = blob + t * bstride + RT_BLOB_HEAD, *hl = ho + TC + 1, *slr = hl + nhf, *halo = slr + nown, *incf = halo + nh;
   uint32_t *outs = incf + ninc;
   for (int k = threadIdx.x; k < nown; k += TILE_BT)
@@ -536,15 +538,11 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
     int64_t *boff = (int64_t *)k1, *xoff = boff + Tmax, *ibase = xoff + Tmax, *k2base = ibase + Tmax;
     int32_t *faceX = v0;
     tile_max *mx = (tile_max *)(flags + 4);
-    const char *env = getenv("RT_TILE_CELLS");
     // (measured: with 3 groups on the Voronoi configs 32 cells per tile and three blocks of k_flux per
     // SM beat 40 cells and two; with one group (128^3 Cartesian) 96 cells beat 64 and equal 128)
     const int tc_default = c->G >= 2 ? 32 : 96;
-    int tc0 = env ? atoi(env) : tc_default;
-    if (tc0 < RT_MIN_TILE || tc0 > 1024) tc0 = tc_default;
-    env = getenv("RT_TILE_BLOCKS");
-    int nblocks = env ? atoi(env) : 2;
-    if (nblocks < 1 || nblocks > 8) nblocks = 2;
+    const int tc0 = c->tun.tile_cells > 0 ? c->tun.tile_cells : tc_default;
+    const int nblocks = c->tun.tile_blocks > 0 ? c->tun.tile_blocks : 2;
     int best = 0;
     tile_max hm;
     memset(&hm, 0, sizeof hm);
@@ -557,8 +555,9 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
                                                         nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
         RT_CUDA(c, cudaMemcpyAsync(&hm, mx, sizeof(tile_max), cudaMemcpyDeviceToHost, st));
         RT_CUDA(c, cudaStreamSynchronize(st));
-        if (!hm.overflow && rt_smem_flux(TC, c->G, hm.no, hm.nf, hm.words) <= limit &&
-            rt_smem_grad(TC, c->G, hm.ns, hm.nh, hm.words) <= (limit > RT_SMEM_TARGET ? limit : RT_SMEM_TARGET)) {
+        const int bs = (hm.words + RT_BLOB_HEAD + 3) & ~3;  // the blob stride the kernels will stage
+        if (!hm.overflow && rt_smem_flux(TC, c->G, hm.no, hm.nf, bs) <= limit &&
+            rt_smem_grad(TC, c->G, hm.ns, hm.nh, bs) <= (limit > RT_SMEM_TARGET ? limit : RT_SMEM_TARGET)) {
           best = TC;
           break;
         }
@@ -584,7 +583,8 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
       return rt_fail(c, RT_ENOMEM, "tile tables need %lld bytes, the workspace holds %zu", (long long)c->blob_words * 4,
                      lay.blob_bytes);
     if (c->ninc > lay.xcap)
-      return rt_fail(c, RT_ENOMEM, "%lld faces cross tile boundaries, the workspace holds the fluxes of %lld",
+      return rt_fail(c, RT_ENOMEM, "%lld faces cross tile boundaries, the workspace holds the fluxes of %lld: "
+                     "size it with rt_workspace_bytes(..., flags | RT_WS_ALL_FACES_CROSS)",
                      (long long)c->ninc, (long long)lay.xcap);
     rt_tile *tiles = rt_ptr<rt_tile>(c, lay.tiles);
     uint32_t *blob = rt_ptr<uint32_t>(c, lay.blob);
@@ -622,8 +622,7 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
         if (k >= T) k = T - 1;
         return (int)v[(size_t)k];
       };
-      env = getenv("RT_TILE_CLASSES");
-      const bool classes = !(env && atoi(env) == 0);
+      const bool classes = c->tun.tile_classes != 1;
       // k_flux: three blocks of 256 threads per SM is what its registers allow
       c->omaxA = c->omax; c->fmaxA = c->fmax;
       const size_t lim_flux = 233472 / 3 - 1024 - 512;
@@ -636,8 +635,7 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
       // shared-memory pipeline bound it before occupancy does); RT_GRAD_CLASSES=1 turns it on
       c->smaxA = c->smax; c->hmaxA = c->hmax;
       bool done = false;
-      env = getenv("RT_GRAD_CLASSES");
-      const bool gclasses = classes && env && atoi(env) == 1;
+      const bool gclasses = classes && (c->tun.variant & 1);
       for (int nb = 6; gclasses && nb >= 5 && !done; nb--) {
         const size_t lim = 233472 / nb - 1024 - 64;
         if (rt_smem_grad(best, c->G, c->smax, c->hmax, c->bstride) <= lim) break;
@@ -701,12 +699,7 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G, int flags) {
   l.tlistG = take(4 * (size_t)(l.max_tiles + 1)); l.tlistF = take(4 * (size_t)(l.max_tiles + 1));
   // fluxes of the faces that cross tile boundaries, written by the owner tile (<= 56 % of the
   // faces; rt_mesh_upload fails with RT_ENOMEM on a mesh whose tiles need more)
-  {
-    // (small tiles, which only RT_TILE_CELLS asks for, let up to every face cross a tile boundary)
-    const char *env = getenv("RT_TILE_CELLS");
-    const double frac = env && atoi(env) >= RT_MIN_TILE && atoi(env) < 32 ? 1.0 : 0.56;
-    l.xcap = (int64_t)(frac * (double)F) + 1024;
-  }
+  l.xcap = (flags & RT_WS_ALL_FACES_CROSS) ? F : (int64_t)(0.56 * (double)F) + 1024;
   l.xphi = take(32 * (size_t)G * (size_t)l.xcap);
   // cells with incoming faces and the xphi rows of those faces (k_finish)
   l.k2cell = take(4 * (size_t)C); l.k2off = take(4 * ((size_t)C + 1)); l.k2row = take(4 * (size_t)l.xcap);

@@ -15,7 +15,6 @@
 //   k_finish  a4 for the other cells: adds the fluxes of the faces owned by earlier tiles (xphi)
 // fp64 throughout.  Reciprocals and the closure's square root use MUFU seeds + two Newton steps
 // (relative error ~1e-16, no special-case branches: all arguments are positive and normal).
-#include <stdlib.h>
 #include "rt_internal.cuh"
 #include "rt_kernels.cuh"
 
@@ -140,7 +139,7 @@ __device__ __forceinline__ void bulk_prefetch_l2(const void *src, unsigned bytes
 // a tile's blob in shared memory (layout: rt_internal.cuh)
 struct tile_view {
   int64_t c0, fbase, xbase;
-  int ncell, nown, ninc, ns, nh, nhf, nb, nout, words;
+  int ncell, nown, ninc, ns, nh, nhf, nb, nout, words, bnd;
   const uint32_t *ho, *hl, *slr, *halo, *incf, *outs;  // in shared memory
   const uint32_t *blob;                                // in global memory
 };
@@ -151,7 +150,7 @@ __device__ __forceinline__ tile_view view_tile(const rt_geom &m, const uint32_t 
   v.c0 = (int64_t)tile * m.TC;
   v.ncell = (int)(v.c0 + m.TC < m.C ? m.TC : m.C - v.c0);
   v.fbase = d.fbase; v.xbase = d.xbase; v.nown = d.nown; v.ninc = d.ninc; v.ns = d.nown + d.ninc; v.nh = d.nh; v.nhf = d.nhf;
-  v.nb = d.nb; v.nout = d.nout;
+  v.nb = d.nb; v.nout = d.nout; v.bnd = d.pad & 1;
   v.words = rt_blob_words(m.TC, v.nhf, v.nown, v.nh, v.ninc, v.nout);
   v.ho = sB + RT_BLOB_HEAD; v.hl = v.ho + m.TC + 1; v.slr = v.hl + v.nhf; v.halo = v.slr + v.nown; v.incf = v.halo + v.nh;
   v.outs = v.incf + v.ninc;
@@ -160,17 +159,146 @@ __device__ __forceinline__ tile_view view_tile(const rt_geom &m, const uint32_t 
 }
 
 // ------------------------------------------------------------------ a2: gradients + limiter
+// Four lanes per cell.  Lane (h, p) of a cell keeps the fields {2h, 2h + 1} of (N, Fx, Fy, Fz) of a block of up
+// to three groups in registers and takes the entries p, p + 2, ... of the cell's half-face list; the partial
+// sums, minima and maxima of the two lanes p are combined by shuffles (a fixed order: deterministic).  A
+// face's geometry is thereby loaded once for three groups and two fields: shared-memory loads cost the
+// same whether the lanes of a warp ask for distinct words or for the same one (profiles/r2_alu_peak.md),
+// so one lane per (cell, group) spent two thirds of its geometry loads on copies.
+// Cell rows in shared memory are padded to an odd number of 16-byte chunks (bank spread of the gathers).
+__device__ __forceinline__ double shx(double v, int lane_mask) { return __shfl_xor_sync(0xffffffffu, v, lane_mask); }
+
+struct grad_smem { const double *Wl, *Wh, *Cl, *Ch, *U, *M; };
+
+// the gradients of groups g0 .. g0 + GB - 1 of the tile's cells.  BND: the tile has boundary half-faces
+template <int G, int GB, bool BND>
+__device__ __forceinline__ void grad_cells(const rt_geom &m, const tile_view &v, const grad_smem &sm, const int g0,
+                                           double *__restrict__ grad, const int tid, const int nt) {
+  constexpr int US = 4 * G + 2;  // doubles per cell row
+  const int h = (tid >> 1) & 1, p = tid & 1;
+  for (int xb = 0; xb < v.ncell; xb += nt >> 2) {  // (whole warps iterate together: the shuffles need every lane)
+    const int x = xb + (tid >> 2);
+    const bool on = x < v.ncell;
+    const int xx = on ? x : 0;
+    const int h0 = on ? (int)v.ho[xx] : 0, h1 = on ? (int)v.ho[xx + 1] : 0;
+    const double *ui_p = sm.U + US * xx + 4 * g0 + 2 * h;
+    double ui[GB][2], b[GB][2][3], hi[GB][2], lo[GB][2];
+#pragma unroll
+    for (int g = 0; g < GB; g++) {
+      const double2 t = ld2(ui_p + 4 * g);
+      ui[g][0] = hi[g][0] = lo[g][0] = t.x; ui[g][1] = hi[g][1] = lo[g][1] = t.y;
+#pragma unroll
+      for (int f = 0; f < 2; f++) b[g][f][0] = b[g][f][1] = b[g][f][2] = 0.0;
+    }
+    // first pass over the cell's half-faces: sum_f w_f (phi_j - phi_i), min/max.  Where the cell is
+    // the face's right cell, d = s_L - s_R: the stored prefactor changes sign.
+#pragma unroll 2
+    for (int k = h0 + p; k < h1; k += 2) {
+      const uint32_t e = v.hl[k];
+      const int s = (int)(e & 0x7fffu);
+      const uint32_t nb = e >> 16;
+      const int sgn = (int)((e & 0x8000u) << 16);  // sign bit where the cell is the right one
+      const double2 wl = ld2(sm.Wl + 2 * s);
+      const double wzz = sm.Wh[2 * s];
+      const double wx = flip_sign(wl.x, sgn), wy = flip_sign(wl.y, sgn), wz = flip_sign(wzz, sgn);
+      double2 uj[GB];
+      if (!BND || nb < 0xFF00u) {
+        const double *q = sm.U + US * (int)nb + 4 * g0 + 2 * h;
+#pragma unroll
+        for (int g = 0; g < GB; g++) uj[g] = ld2(q + 4 * g);
+      } else {  // ghost state across a boundary face (S13)
+        const int code = (int)nb - 0x10000;
+#pragma unroll
+        for (int g = 0; g < GB; g++) {
+          const double4 Ui = ld4(sm.U + US * xx + 4 * (g0 + g));
+          const double4 gh = ghost_for_gradient(code, Ui, m.faceN, m.F, v.fbase + s, m.ghost, G, g0 + g);
+          uj[g] = h ? make_double2(gh.z, gh.w) : make_double2(gh.x, gh.y);
+        }
+      }
+#pragma unroll
+      for (int g = 0; g < GB; g++) {
+        const double d0 = uj[g].x - ui[g][0], d1 = uj[g].y - ui[g][1];
+        b[g][0][0] += wx * d0; b[g][0][1] += wy * d0; b[g][0][2] += wz * d0;
+        b[g][1][0] += wx * d1; b[g][1][1] += wy * d1; b[g][1][2] += wz * d1;
+        hi[g][0] = dmax2(hi[g][0], uj[g].x); hi[g][1] = dmax2(hi[g][1], uj[g].y);
+        lo[g][0] = dmin2(lo[g][0], uj[g].x); lo[g][1] = dmin2(lo[g][1], uj[g].y);
+      }
+    }
+    const double *Mi = sm.M + 6 * xx;
+    const double2 ma = ld2(Mi), mb = ld2(Mi + 2), mc = ld2(Mi + 4);
+    const double m00 = ma.x, m01 = ma.y, m02 = mb.x, m11 = mb.y, m12 = mc.x, m22 = mc.y;
+    double gr[GB][2][3];
+#pragma unroll
+    for (int g = 0; g < GB; g++)
+#pragma unroll
+      for (int f = 0; f < 2; f++) {
+        // (the two lanes of a pair add their partial sums: both get the same bits)
+        const double b0 = b[g][f][0] + shx(b[g][f][0], 1), b1 = b[g][f][1] + shx(b[g][f][1], 1), b2 = b[g][f][2] + shx(b[g][f][2], 1);
+        hi[g][f] = dmax2(hi[g][f], shx(hi[g][f], 1));
+        lo[g][f] = dmin2(lo[g][f], shx(lo[g][f], 1));
+        gr[g][f][0] = m00 * b0 + m01 * b1 + m02 * b2;
+        gr[g][f][1] = m01 * b0 + m11 * b1 + m12 * b2;
+        gr[g][f][2] = m02 * b0 + m12 * b1 + m22 * b2;
+      }
+    // second pass: extreme extrapolated increments at the face centres.  min_f (hi-phi)/D_f is
+    // attained at the largest D_f (division is monotone), so only the extremes are kept.
+    // The stored face centre is relative to the left cell; seen from the right cell it is
+    // c - d with d = kappa w (rt_internal.cuh).
+    double dmx[GB][2], dmn[GB][2];
+#pragma unroll
+    for (int g = 0; g < GB; g++) dmx[g][0] = dmx[g][1] = dmn[g][0] = dmn[g][1] = 0.0;
+#pragma unroll 2
+    for (int k = h0 + p; k < h1; k += 2) {
+      const uint32_t e = v.hl[k];
+      const int s = (int)(e & 0x7fffu);
+      const double2 cl = ld2(sm.Cl + 2 * s);
+      double rx = cl.x, ry = cl.y, rz = sm.Ch[2 * s];
+      if (e & 0x8000u) {  // (a cell's right-side faces come last in its list: mostly uniform across a warp)
+        const double2 wl = ld2(sm.Wl + 2 * s), wh = ld2(sm.Wh + 2 * s);
+        rx = fma(-wh.y, wl.x, rx); ry = fma(-wh.y, wl.y, ry); rz = fma(-wh.y, wh.x, rz);
+      }
+#pragma unroll
+      for (int g = 0; g < GB; g++)
+#pragma unroll
+        for (int f = 0; f < 2; f++) {
+          const double d = gr[g][f][0] * rx + gr[g][f][1] * ry + gr[g][f][2] * rz;
+          dmx[g][f] = dmax2(dmx[g][f], d); dmn[g][f] = dmin2(dmn[g][f], d);
+        }
+    }
+#pragma unroll
+    for (int g = 0; g < GB; g++) {
+      double o[6];
+#pragma unroll
+      for (int f = 0; f < 2; f++) {
+        const double dx = dmax2(dmx[g][f], shx(dmx[g][f], 1)), dn = dmin2(dmn[g][f], shx(dmn[g][f], 1));
+        const double up = hi[g][f] - ui[g][f], dw = ui[g][f] - lo[g][f];
+        double a = 1.0;
+        // (reciprocals from the MUFU seed where the divisor is safely normal: a sixth of a division)
+        if (dx > 0.0) a = dmin2(a, dx > 1e-280 ? up * fast_rcp(dx) : up / dx);
+        if (dn < 0.0) a = dmin2(a, dn < -1e-280 ? dw * fast_rcp(-dn) : -dw / dn);
+        o[3 * f] = a * gr[g][f][0]; o[3 * f + 1] = a * gr[g][f][1]; o[3 * f + 2] = a * gr[g][f][2];
+      }
+      // lane h of a pair owns the chunks 3h .. 3h + 2 of the (cell, group) row; the lanes p share the groups
+      if (on && ((g0 + g) & 1) == p) {
+        double *out = grad + 12 * ((v.c0 + x) * G + g0 + g) + 6 * h;
+        st2(out, o[0], o[1]); st2(out + 2, o[2], o[3]); st2(out + 4, o[4], o[5]);
+      }
+    }
+  }
+}
+
 template <int G>
-__global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__restrict__ U, double *__restrict__ grad) {
+__global__ void __launch_bounds__(128, 4) k_grad(rt_geom m, const double *__restrict__ U, double *__restrict__ grad) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar, bar_blob;
+  constexpr int US = 4 * G + 2;
   uint32_t *sB = reinterpret_cast<uint32_t *>(smem_raw);    // the tile's blob
   double *sWl = reinterpret_cast<double *>(sB + m.bstride);  // [smax][2]  (wx, wy)      the face records come as
   double *sWh = sWl + 2 * m.smax;                          // [smax][2]  (wz, kappa)   16-byte halves
   double *sCl = sWh + 2 * m.smax;                          // [smax][2]  (cx, cy)      (c = centre - s_L)
   double *sCh = sCl + 2 * m.smax;                          // [smax][2]  (cz, A)
-  double *sU = sCh + 2 * m.smax;                           // [(TC + hmax) G][4]  tile cells, then halo cells
-  double *sM = sU + 4 * G * (m.TC + m.hmax);              // [TC][6]
+  double *sU = sCh + 2 * m.smax;                           // [TC + hmax][4 G + 2]  tile cells, then halo cells
+  double *sM = sU + US * (m.TC + m.hmax);                  // [TC][6]
   const int tid = threadIdx.x, nt = blockDim.x;
   const unsigned tile = (unsigned)m.tlist[m.tbase + blockIdx.x];
   if (tid == 0) { mbar_init(&bar, 1); mbar_init(&bar_blob, 1); }
@@ -182,15 +310,14 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
   }
   mbar_wait(&bar_blob, 0);
   const tile_view v = view_tile(m, sB, tile);
-  // round 2: what the descriptor locates (bulk copies: owned faces, the tile's own cells) and what the
-  // tables locate (gathers: halo cells, incoming faces), all in flight together
+  // round 2: what the descriptor locates (bulk copies: owned faces, M^-1) and what the tables locate
+  // (gathers: the cells, the incoming faces), all in flight together
   if (tid == 0) {
-    mbar_expect(&bar, 64u * v.nown + (32u * G + 48u) * v.ncell);
+    mbar_expect(&bar, 64u * v.nown + 48u * v.ncell);
     bulk_g2s(sWl, m.faceW + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sWh, m.faceW + 2 * m.F + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sCl, m.faceC + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sCh, m.faceC + 2 * m.F + 2 * v.fbase, 16u * v.nown, &bar);
-    bulk_g2s(sU, U + 4 * G * v.c0, 32u * G * v.ncell, &bar);
     bulk_g2s(sM, m.Minv + 6 * v.c0, 48u * v.ncell, &bar);
     // a tile that starts a few gridfuls later: pull its contiguous runs into L2 now
     if ((int64_t)blockIdx.x + m.prefetch_tiles < (int64_t)gridDim.x) {
@@ -207,9 +334,18 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
       bulk_prefetch_l2(m.Minv + 6 * cp, 48u * nc);
     }
   }
-  // round 2: what the blob locates: halo cells and incoming faces
-  // (gathers of 32 to 96 bytes: 16-byte asynchronous copies, one halo cell / incoming face per thread)
-  for (int h = tid; h < v.nh; h += nt) cp_run<2 * G>(sU + 4 * G * (m.TC + h), U + (int64_t)(4 * G) * v.halo[h]);
+  // the tile's cells and the halo cells: 2 G chunks of 16 bytes each into padded rows
+  {
+    constexpr int CH = 2 * G;
+    const int ne = v.ncell + v.nh;
+    for (int idx = tid; idx < ne * CH; idx += nt) {
+      const int ci = idx / CH, c = idx - ci * CH;
+      const bool own = ci < v.ncell;
+      const int64_t gid = own ? v.c0 + ci : (int64_t)v.halo[ci - v.ncell];
+      const int row = own ? ci : m.TC + (ci - v.ncell);
+      cp16(sU + US * row + 2 * c, U + (int64_t)(4 * G) * gid + 2 * c);
+    }
+  }
   for (int j = tid; j < v.ninc; j += nt) {
     const int64_t q = v.incf[j];
     cp16(sWl + 2 * (v.nown + j), m.faceW + 2 * q);
@@ -221,78 +357,18 @@ __global__ void __launch_bounds__(192, 3) k_grad(rt_geom m, const double *__rest
   cp_wait_all();
   __syncthreads();
 
-  for (int item = tid; item < v.ncell * G; item += nt) {
-    const int il = item / G, g = item - il * G;
-    const double4 Ui = ld4(sU + 4 * item);
-    double b[4][3], hi[4] = {Ui.x, Ui.y, Ui.z, Ui.w}, lo[4] = {Ui.x, Ui.y, Ui.z, Ui.w};
+  const grad_smem sm = {sWl, sWh, sCl, sCh, sU, sM};
+  // groups in blocks of three (registers: 6 fields x (3 sums + min + max) per lane)
 #pragma unroll
-    for (int w = 0; w < 4; w++) b[w][0] = b[w][1] = b[w][2] = 0.0;
-    const int h0 = (int)v.ho[il], h1 = (int)v.ho[il + 1];
-    const double *Ug = sU + 4 * g;
-    // first pass over the cell's half-faces: sum_f w_f (phi_j - phi_i), min/max.  Where the cell is
-    // the face's right cell, d = s_L - s_R: the stored prefactor changes sign.
-#pragma unroll 4
-    for (int k = h0; k < h1; k++) {
-      const uint32_t e = v.hl[k];
-      const int s = (int)(e & 0x7fffu);
-      const uint32_t nb = e >> 16;
-      const int sgn = (int)((e & 0x8000u) << 16);  // sign bit where the cell is the right one
-      const double2 wl = ld2(sWl + 2 * s);
-      const double wzz = sWh[2 * s];
-      double4 Uj;
-      if (nb < 0xFF00u) Uj = ld4(Ug + 4 * G * (int)nb);
-      else Uj = ghost_for_gradient((int)nb - 0x10000, Ui, m.faceN, m.F, v.fbase + s, m.ghost, G, g);
-      const double wx = flip_sign(wl.x, sgn), wy = flip_sign(wl.y, sgn), wz = flip_sign(wzz, sgn);
-      const double d0 = Uj.x - Ui.x, d1 = Uj.y - Ui.y, d2 = Uj.z - Ui.z, d3 = Uj.w - Ui.w;
-      b[0][0] += wx * d0; b[0][1] += wy * d0; b[0][2] += wz * d0;
-      b[1][0] += wx * d1; b[1][1] += wy * d1; b[1][2] += wz * d1;
-      b[2][0] += wx * d2; b[2][1] += wy * d2; b[2][2] += wz * d2;
-      b[3][0] += wx * d3; b[3][1] += wy * d3; b[3][2] += wz * d3;
-      hi[0] = dmax2(hi[0], Uj.x); hi[1] = dmax2(hi[1], Uj.y); hi[2] = dmax2(hi[2], Uj.z); hi[3] = dmax2(hi[3], Uj.w);
-      lo[0] = dmin2(lo[0], Uj.x); lo[1] = dmin2(lo[1], Uj.y); lo[2] = dmin2(lo[2], Uj.z); lo[3] = dmin2(lo[3], Uj.w);
+  for (int g0 = 0; g0 < G; g0 += 3) {
+    constexpr int REM = G % 3;
+    if (g0 + 3 <= G) {
+      if (v.bnd) grad_cells<G, 3, true>(m, v, sm, g0, grad, tid, nt);
+      else grad_cells<G, 3, false>(m, v, sm, g0, grad, tid, nt);
+    } else if (REM > 0) {
+      if (v.bnd) grad_cells<G, REM ? REM : 1, true>(m, v, sm, g0, grad, tid, nt);
+      else grad_cells<G, REM ? REM : 1, false>(m, v, sm, g0, grad, tid, nt);
     }
-    const double *Mi = sM + 6 * il;
-    const double m00 = Mi[0], m01 = Mi[1], m02 = Mi[2], m11 = Mi[3], m12 = Mi[4], m22 = Mi[5];
-    double gr[4][3];
-#pragma unroll
-    for (int w = 0; w < 4; w++) {
-      gr[w][0] = m00 * b[w][0] + m01 * b[w][1] + m02 * b[w][2];
-      gr[w][1] = m01 * b[w][0] + m11 * b[w][1] + m12 * b[w][2];
-      gr[w][2] = m02 * b[w][0] + m12 * b[w][1] + m22 * b[w][2];
-    }
-    // second pass: extreme extrapolated increments at the face centres.  min_f (hi-phi)/D_f is
-    // attained at the largest D_f (division is monotone), so only the extremes are kept.
-    // The stored face centre is relative to the left cell; seen from the right cell it is
-    // c - d with d = kappa w (rt_internal.cuh).
-    double dmax[4] = {0, 0, 0, 0}, dmin[4] = {0, 0, 0, 0};
-#pragma unroll 4
-    for (int k = h0; k < h1; k++) {
-      const uint32_t e = v.hl[k];
-      const int s = (int)(e & 0x7fffu);
-      const double2 cl = ld2(sCl + 2 * s);
-      double rx = cl.x, ry = cl.y, rz = sCh[2 * s];
-      if (e & 0x8000u) {  // (a cell's right-side faces come last in its list: mostly uniform across a warp)
-        const double2 wl = ld2(sWl + 2 * s), wh = ld2(sWh + 2 * s);
-        rx = fma(-wh.y, wl.x, rx); ry = fma(-wh.y, wl.y, ry); rz = fma(-wh.y, wh.x, rz);
-      }
-#pragma unroll
-      for (int f = 0; f < 4; f++) {
-        const double d = gr[f][0] * rx + gr[f][1] * ry + gr[f][2] * rz;
-        dmax[f] = dmax2(dmax[f], d); dmin[f] = dmin2(dmin[f], d);
-      }
-    }
-    double *out = grad + 12 * ((v.c0 + il) * G + g);
-    const double Uiv[4] = {Ui.x, Ui.y, Ui.z, Ui.w};
-    double o[12];
-#pragma unroll
-    for (int w = 0; w < 4; w++) {
-      double a = 1.0;
-      // (reciprocals from the MUFU seed where the divisor is safely normal: a sixth of a division)
-      if (dmax[w] > 0.0) a = dmin2(a, dmax[w] > 1e-280 ? (hi[w] - Uiv[w]) * fast_rcp(dmax[w]) : (hi[w] - Uiv[w]) / dmax[w]);
-      if (dmin[w] < 0.0) a = dmin2(a, dmin[w] < -1e-280 ? (Uiv[w] - lo[w]) * fast_rcp(-dmin[w]) : (lo[w] - Uiv[w]) / dmin[w]);
-      o[3 * w] = a * gr[w][0]; o[3 * w + 1] = a * gr[w][1]; o[3 * w + 2] = a * gr[w][2];
-    }
-    st4(out, o[0], o[1], o[2], o[3]); st4(out + 4, o[4], o[5], o[6], o[7]); st4(out + 8, o[8], o[9], o[10], o[11]);
   }
 }
 
@@ -776,19 +852,12 @@ int rt_transport_configure(rt_ctx *c) {
 
 // threads per tile block (a whole number of warps, at most 256, the kernels' launch bound).
 // k_grad has one thread per (cell, group); k_stage one lane per (slot, group), several passes.
-// RT_TILE_THREADS / RT_GRAD_THREADS in the environment override the defaults for experiments.
-static int env_int(const char *name) { const char *e = getenv(name); return e ? atoi(e) : 0; }
+// rt_tuning.flux_threads / grad_threads override the defaults for experiments.
 static int round_threads(int n) { n = ((n + 31) / 32) * 32; return n > 256 ? 256 : (n < 32 ? 32 : n); }
-static int tile_threads(const rt_ctx *) {
-  static int env = -1;
-  if (env < 0) env = env_int("RT_TILE_THREADS");
-  return round_threads(env > 0 ? env : 256);
-}
-static int grad_threads(const rt_ctx *c) {  // one thread per (cell, group), at most k_grad's launch bound
-  static int env = -1;
-  if (env < 0) env = env_int("RT_GRAD_THREADS");
-  const int n = round_threads(env > 0 ? env : c->TC * c->G);
-  return n > 192 ? 192 : n;
+static int tile_threads(const rt_ctx *c) { return round_threads(c->tun.flux_threads > 0 ? c->tun.flux_threads : 256); }
+static int grad_threads(const rt_ctx *c) {  // four lanes per cell, at most k_grad's launch bound
+  const int n = round_threads(c->tun.grad_threads > 0 ? c->tun.grad_threads : 4 * c->TC);
+  return n > 128 ? 128 : n;
 }
 
 rt_geom rt_geom_of(const rt_ctx *c) {
@@ -799,11 +868,7 @@ rt_geom rt_geom_of(const rt_ctx *c) {
   m.faceC = rt_ptr<double>(c, l.faceC); m.faceN = rt_ptr<double>(c, l.faceN); m.faceW = rt_ptr<double>(c, l.faceW);
   m.tiles = rt_ptr<rt_tile>(c, l.tiles); m.blob = rt_ptr<uint32_t>(c, l.blob);
   m.xphi = rt_ptr<double>(c, l.xphi);
-  {
-    static int ahead = -1;
-    if (ahead < 0) { const char *e = getenv("RT_PREFETCH_TILES"); ahead = e ? atoi(e) : 600; }
-    m.prefetch_tiles = ahead > 0 ? ahead : (1 << 30);
-  }
+  m.prefetch_tiles = c->tun.prefetch_tiles > 0 ? c->tun.prefetch_tiles : (c->tun.prefetch_tiles < 0 ? (1 << 30) : 600);
   m.ghost = rt_ptr<double>(c, l.ghost);
   for (int a = 0; a < 3; a++) { m.box[a] = c->box[a]; m.per[a] = c->per[a]; }
   return m;

@@ -12,7 +12,7 @@ import numpy as np
 
 RT_MAXG = 8
 RT_MEM_HOST, RT_MEM_DEVICE = 0, 1
-RT_WS_DEVICE_MESH = 1
+RT_WS_DEVICE_MESH, RT_WS_ALL_FACES_CROSS = 1, 2
 LEDGER_ROWS = ("stored", "injected", "absorbed", "outflow", "inflow_bc", "floor_added")
 _vp = ctypes.c_void_p
 
@@ -43,6 +43,13 @@ class rt_params(ctypes.Structure):
                 ("kappa", _vp)]
 
 
+class rt_tuning(ctypes.Structure):
+    _fields_ = [("tile_cells", ctypes.c_int32), ("tile_faces", ctypes.c_int32), ("tile_blocks", ctypes.c_int32),
+                ("tile_classes", ctypes.c_int32), ("flux_threads", ctypes.c_int32), ("grad_threads", ctypes.c_int32),
+                ("prefetch_tiles", ctypes.c_int32), ("chem_caps", ctypes.c_int32 * 6), ("variant", ctypes.c_int32),
+                ("reserved", ctypes.c_int32 * 9)]
+
+
 class rt_ledger(ctypes.Structure):
     _fields_ = [(k, ctypes.c_double * RT_MAXG) for k in LEDGER_ROWS] + \
                [("substeps_total", ctypes.c_int64), ("substeps_max", ctypes.c_int64), ("cells_hit_cap", ctypes.c_int64),
@@ -57,10 +64,12 @@ def lib():
     global _lib
     if _lib is None:
         from .build import build_rt
-        so = os.environ.get("RT_LIB") or build_rt()   # RT_LIB: an alternative build, for experiments
+        so = build_rt()
         L = ctypes.CDLL(so)
         L.rt_create.restype = ctypes.c_int
         L.rt_create.argtypes = [ctypes.POINTER(_vp), ctypes.c_int, _vp]
+        L.rt_set_tuning.restype = ctypes.c_int
+        L.rt_set_tuning.argtypes = [_vp, ctypes.POINTER(rt_tuning)]
         L.rt_workspace_bytes.restype = ctypes.c_size_t
         L.rt_workspace_bytes.argtypes = [ctypes.c_int64, ctypes.c_int64, ctypes.c_int, ctypes.c_int]
         L.rt_mesh_upload.restype = ctypes.c_int
@@ -81,6 +90,8 @@ def lib():
         L.rt_profile.argtypes = [_vp, ctypes.c_int]
         L.rt_profile_read.restype = ctypes.c_int
         L.rt_profile_read.argtypes = [_vp, _vp, _vp]
+        L.rt_debug_alu_peak.restype = ctypes.c_int
+        L.rt_debug_alu_peak.argtypes = [_vp, _vp]
         L.rt_last_error.restype = ctypes.c_char_p
         L.rt_last_error.argtypes = [_vp]
         L.rt_destroy.restype = None
@@ -123,6 +134,18 @@ def rt_create(device=0, stream=None):
     if rc != 0:
         raise RTError("rt_create failed with code %d (no usable CUDA device %d?)" % (rc, device))
     return h
+
+
+def rt_set_tuning(h, **kw):
+    """Fields of rt_tuning by name (chem_caps: a sequence); unnamed fields keep the default 0."""
+    t = rt_tuning()
+    for k, v in kw.items():
+        if k == "chem_caps":
+            for i, x in enumerate(v):
+                t.chem_caps[i] = int(x)
+        else:
+            setattr(t, k, int(v))
+    _check(h, lib().rt_set_tuning(h, ctypes.byref(t)), "rt_set_tuning")
 
 
 def rt_workspace_bytes(ncell, nface, ngroup, flags=0):
@@ -235,6 +258,17 @@ def rt_download(h, out=None, want_ledger=True, ngroup=1):
     return d
 
 
+def rt_debug_alu_peak(h):
+    """Measured operations per second of the fp64 pipe and of shared memory (include/rt.h)."""
+    out = np.zeros(14)
+    _check(h, lib().rt_debug_alu_peak(h, _vp(out.ctypes.data)), "rt_debug_alu_peak")
+    names = ("dfma", "dadd", "dmul", "dmax", "rcp_seed", "rcp_newton2", "rsqrt_seed", "ddiv", "dsqrt", "lds128",
+             "lds128_bcast3", "lds128_bcast8", "lds128_random")
+    d = {k: float(out[i]) for i, k in enumerate(names)}
+    d["sm_count"] = int(out[13])
+    return d
+
+
 def rt_destroy(h):
     lib().rt_destroy(h)
 
@@ -243,7 +277,7 @@ def rt_destroy(h):
 class Solver:
     """Owns a context and its workspace tensor.  Every computation happens inside librt.so."""
 
-    def __init__(self, mesh, params, device=0, stream=None):
+    def __init__(self, mesh, params, device=0, stream=None, tuning=None):
         import torch
         if not torch.cuda.is_available():
             raise RTError("no CUDA device: the RT path has no CPU fallback")
@@ -254,7 +288,12 @@ class Solver:
         if stream is None:
             stream = torch.cuda.current_stream(self.dev).cuda_stream
         self.h = rt_create(device, stream)
-        nbytes = rt_workspace_bytes(self.C, self.F, self.G, RT_WS_DEVICE_MESH if _on_device(mesh) else 0)
+        flags = RT_WS_DEVICE_MESH if _on_device(mesh) else 0
+        if tuning:
+            rt_set_tuning(self.h, **tuning)
+            if 0 < tuning.get("tile_cells", 0) < 32 or 0 < tuning.get("tile_faces", 0) < 240:
+                flags |= RT_WS_ALL_FACES_CROSS
+        nbytes = rt_workspace_bytes(self.C, self.F, self.G, flags)
         if nbytes == 0:
             raise RTError("rt_workspace_bytes rejected the sizes")
         self.workspace = torch.empty((nbytes + 7) // 8, dtype=torch.float64, device=self.dev)

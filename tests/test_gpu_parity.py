@@ -9,10 +9,10 @@ import parity as P
 pytestmark = pytest.mark.gpu
 
 
-def _pair(oracle_mod, w):
+def _pair(oracle_mod, w, tuning=None):
     from paper_2404_17630_b200 import rt
     o = oracle_mod.Oracle(w.mesh, w.params); o.set_sources(w.sources); o.set_state(w.state)
-    s = rt.Solver(w.mesh, w.params); s.init(w.state, w.sources)
+    s = rt.Solver(w.mesh, w.params, tuning=tuning); s.init(w.state, w.sources)
     return o, s
 
 
@@ -242,13 +242,11 @@ def test_other_group_counts(oracle_mod, G):
 
 
 @pytest.mark.parametrize("tc", [8, 12, 20])
-def test_small_tiles_many_halos(oracle_mod, monkeypatch, tc):
-    """Forces small tiles (RT_TILE_CELLS): most faces then cross tile boundaries, so the exchange of
-    fluxes through xphi / k_finish and the halo tables carry the result; ragged last tile."""
-    monkeypatch.setenv("RT_TILE_CELLS", str(tc))
-    from paper_2404_17630_b200 import rt
+def test_small_tiles_many_halos(oracle_mod, tc):
+    """Forces small tiles (rt_tuning.tile_cells): most faces then cross tile boundaries, so the exchange
+    of fluxes through xphi / k_finish and the halo tables carry the result; ragged last tile."""
     w = cfg.get(3, 9)                      # 729 cells: not a multiple of any tile size used here
-    o, s = _pair(oracle_mod, w)
+    o, s = _pair(oracle_mod, w, tuning={"tile_cells": tc})
     assert s.tile_info()["cells_per_tile"] <= tc
     prev = o.get_state()
     for _ in range(4):

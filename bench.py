@@ -208,6 +208,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tuning", default="", help="rt_tuning fields, e.g. tile_cells=40,variant=2 (experiments)")
     ap.add_argument("--alu-peak", action="store_true",
                     help="only run the fp64 / shared-memory micro-benchmarks (rt_debug_alu_peak) and print them")
     args = ap.parse_args()
@@ -242,7 +243,8 @@ def main():
         w = cfg.get(c, n)
     C, F, G = int(w.mesh.ncell), int(w.mesh.nface), int(w.params.ngroup)
     NR = int((w.mesh.right >= 0).sum())
-    s = rt.Solver(w.mesh, w.params, device=local)
+    tuning = {k: int(v) for k, v in (kv.split("=") for kv in args.tuning.split(",") if kv)} or None
+    s = rt.Solver(w.mesh, w.params, device=local, tuning=tuning)
     stored0 = np.asarray([float((w.state.N[g] * w.mesh.volume).sum()) for g in range(G)])   # photons at t = 0
     w.mesh = None
     torch.cuda.empty_cache()

@@ -197,6 +197,13 @@ int rt_profile_read(rt_ctx *ctx, double *ms, int64_t *count);
  * mem_kind says: gN (G, 3, C), gF (G, 3 components, 3 directions, C).  For tests. Synchronises. */
 int rt_debug_gradients(rt_ctx *ctx, int mem_kind, double *gN, double *gF);
 
+/* Advances ONE subcycle of length dt with the flux kernel of the second Heun stage recording, per
+ * tile, the device clock (ns) at the start of the tile, after its tables arrived, after its data was
+ * staged, after the face fluxes, after the outgoing fluxes were published, at its end, and the
+ * multiprocessor and block that ran it: out = HOST array of 8 words per tile, tile-major
+ * (ntile_max >= the number of tiles of rt_tile_info).  For DESIGN.md's phase timeline.  Synchronises. */
+int rt_debug_tile_timeline(rt_ctx *ctx, double dt, int64_t ntile_max, uint64_t *out);
+
 /* Micro-benchmarks of the device's fp64 pipe and shared memory (not part of the subcycle; they place
  * the ALU ceiling beside the HBM roofline).  out: HOST array of 14 = operations per
  * second of dependent-chain-free DFMA, DADD, DMUL, compare+select (max), MUFU reciprocal seed,

@@ -45,7 +45,7 @@ int rt_create(rt_ctx **out, int device, void *cuda_stream) {
   if (!c) return RT_ENOMEM;
   c->device = 0; c->stream = 0; c->err[0] = 0; c->C = c->F = c->NR = 0; c->G = 0; c->nghost = 0; c->ws = nullptr;
   c->ws_bytes = 0; c->have_mesh = c->have_state = false; c->nsrc = 0; c->nsub_done = 0; c->launches = 0;
-  c->prof_on = false; c->prof_used = 0;
+  c->prof_on = false; c->prof_used = 0; c->dbg_tl = nullptr;
   memset(&c->par, 0, sizeof(c->par)); memset(&c->lay, 0, sizeof(c->lay)); memset(&c->tun, 0, sizeof(c->tun));
   c->device = device;
   c->stream = (cudaStream_t)cuda_stream;
@@ -307,6 +307,25 @@ int rt_download(rt_ctx *c, rt_state *out, rt_ledger *led) {
     led->nsub_done = c->nsub_done;
   }
   return RT_OK;
+}
+
+int rt_debug_tile_timeline(rt_ctx *c, double dt, int64_t ntile_max, uint64_t *out) {
+  if (!c || !out) return RT_EINVAL;
+  c->err[0] = 0;
+  if (!c->have_state) return rt_fail(c, RT_ESTATE, "rt_debug_tile_timeline needs rt_state_init first");
+  if (!(dt > 0.0) || ntile_max < c->T) return rt_fail(c, RT_EINVAL, "dt must be positive and out must hold 8 words for each of the %lld tiles", (long long)c->T);
+  RT_CUDA(c, cudaSetDevice(c->device));
+  unsigned long long *buf = nullptr;
+  RT_CUDA(c, cudaMalloc(&buf, 64 * (size_t)c->T));  // (a debug call: allocates outside the caller's workspace)
+  RT_CUDA(c, cudaMemsetAsync(buf, 0, 64 * (size_t)c->T, c->stream));
+  c->dbg_tl = buf;
+  const int rc = rt_launch_step(c, dt);
+  c->dbg_tl = nullptr;
+  cudaError_t e = cudaMemcpyAsync(out, buf, 64 * (size_t)c->T, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(buf);
+  if (e != cudaSuccess) return rt_fail(c, RT_ECUDA, "timeline copy: %s", cudaGetErrorString(e));
+  return rc;
 }
 
 int rt_debug_gradients(rt_ctx *c, int mem_kind, double *gN, double *gF) {

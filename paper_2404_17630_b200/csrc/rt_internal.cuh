@@ -110,6 +110,7 @@ struct rt_ctx {
   bool have_mesh, have_state;
   rt_params par;
   rt_tuning tun;      // rt_set_tuning (zeros = defaults)
+  unsigned long long *dbg_tl;  // device buffer of rt_debug_tile_timeline while it runs, else null
   int nsrc;
   double src_total[RT_MAXG];
   double injected[RT_MAXG][2];  // host-side compensated sum
@@ -149,7 +150,8 @@ static inline size_t rt_smem_grad(int TC, int G, int smax, int hmax, int bmax) {
 static inline size_t rt_smem_flux(int TC, int G, int omax, int fmax, int bmax) {
   const int planes = G > 3 ? G : 3;  // three face records per slot, overwritten by A*Phi of every group
   const int NE = (TC + fmax + 1) & ~1;
-  return (size_t)4 * bmax + (size_t)32 * planes * omax + (size_t)(128 * G + 8) * NE + (size_t)16 * ((TC + 3) / 4);
+  return (size_t)4 * bmax + (size_t)32 * planes * omax + (size_t)(128 * G + 32 + 8) * NE + (size_t)16 * ((TC + 3) / 4) +
+         (size_t)32 * G * TC;  // rows padded; source ids; U^n of the tile's cells
 }
 #define RT_SMEM_MAX 232448     // 227 KB: the most one block may have on sm_100
 #define RT_SMEM_TARGET 115000  // two blocks per SM (228 KB per SM, 1 KB reserved per block)

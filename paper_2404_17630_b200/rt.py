@@ -90,6 +90,8 @@ def lib():
         L.rt_profile.argtypes = [_vp, ctypes.c_int]
         L.rt_profile_read.restype = ctypes.c_int
         L.rt_profile_read.argtypes = [_vp, _vp, _vp]
+        L.rt_debug_tile_timeline.restype = ctypes.c_int
+        L.rt_debug_tile_timeline.argtypes = [_vp, ctypes.c_double, ctypes.c_int64, _vp]
         L.rt_debug_alu_peak.restype = ctypes.c_int
         L.rt_debug_alu_peak.argtypes = [_vp, _vp]
         L.rt_last_error.restype = ctypes.c_char_p
@@ -328,6 +330,13 @@ class Solver:
         _check(self.h, lib().rt_debug_gradients(self.h, RT_MEM_HOST, _vp(gN.ctypes.data), _vp(gF.ctypes.data)),
                "rt_debug_gradients")
         return gN, gF
+
+    def tile_timeline(self, dt):
+        """One subcycle with per-tile time stamps of the flux kernel: (T, 8) uint64 array (include/rt.h)."""
+        T = self.tile_info()["tiles"]
+        out = np.zeros((T, 8), dtype=np.uint64)
+        _check(self.h, lib().rt_debug_tile_timeline(self.h, float(dt), T, _vp(out.ctypes.data)), "rt_debug_tile_timeline")
+        return out
 
     def profile(self, enable):
         _check(self.h, lib().rt_profile(self.h, int(bool(enable))), "rt_profile")

@@ -150,8 +150,7 @@ static inline size_t rt_smem_grad(int TC, int G, int smax, int hmax, int bmax) {
 static inline size_t rt_smem_flux(int TC, int G, int omax, int fmax, int bmax) {
   const int planes = G > 3 ? G : 3;  // three face records per slot, overwritten by A*Phi of every group
   const int NE = (TC + fmax + 1) & ~1;
-  return (size_t)4 * bmax + (size_t)32 * planes * omax + (size_t)(128 * G + 32 + 8) * NE + (size_t)16 * ((TC + 3) / 4) +
-         (size_t)32 * G * TC;  // rows padded; source ids; U^n of the tile's cells
+  return (size_t)4 * bmax + (size_t)32 * planes * omax + (size_t)(128 * G + 8) * NE + (size_t)16 * ((TC + 3) / 4);
 }
 #define RT_SMEM_MAX 232448     // 227 KB: the most one block may have on sm_100
 #define RT_SMEM_TARGET 115000  // two blocks per SM (228 KB per SM, 1 KB reserved per block)

@@ -22,7 +22,6 @@ struct rt_geom {
   int G, TC, smax, omax, hmax, fmax, bmax, bstride;
   const int32_t *tlist;  // the launch works on tiles tlist[tbase + blockIdx.x]
   int64_t tbase;
-  int64_t ntile;         // tiles of this launch (k_flux: a block takes tiles blockIdx.x, + gridDim.x, ...)
   int prefetch_tiles;    // the tile kernels ask L2 for the data of tile t + prefetch_tiles
   int variant;           // rt_tuning.variant
   unsigned long long *tl; // rt_debug_tile_timeline: 8 time stamps (ns) per tile of the flux kernel, or null

@@ -623,17 +623,12 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m) {
         return (int)v[(size_t)k];
       };
       const bool classes = c->tun.tile_classes != 1;
-      // k_flux: three blocks of 256 threads per SM is what its registers allow, and one thread per owned
-      // face means a tile with more than 256 owned faces would need a second, nearly empty pass: class A
-      // holds the tiles with at most 256 owned faces whose forward halo fits three blocks' shared memory,
-      // class B (the others) runs with up to 384 threads, two blocks per SM
+      // k_flux: three blocks of 256 threads per SM is what its registers allow
       c->omaxA = c->omax; c->fmaxA = c->fmax;
       const size_t lim_flux = 233472 / 3 - 1024 - 512;
-      if (classes && (c->omax > 256 || rt_smem_flux(best, c->G, c->omax, c->fmax, c->bstride) > lim_flux))
+      if (classes && rt_smem_flux(best, c->G, c->omax, c->fmax, c->bstride) > lim_flux)
         for (double q : qs) {
-          int o = quant(hs[0], q);
-          const int f = quant(hs[1], q);
-          if (o > 256) o = 256;
+          const int o = quant(hs[0], q), f = quant(hs[1], q);
           if (rt_smem_flux(best, c->G, o, f, c->bstride) <= lim_flux) { c->omaxA = o; c->fmaxA = f; break; }
         }
       // k_grad: six blocks, else five (off by default: measured no gain, its registers and the

@@ -324,20 +324,6 @@ __global__ void __launch_bounds__(128, 4) k_grad(rt_geom m, const double *__rest
     bulk_g2s(sCl, m.faceC + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sCh, m.faceC + 2 * m.F + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sM, m.Minv + 6 * v.c0, 48u * v.ncell, &bar);
-    // a tile that starts a few gridfuls later: pull its contiguous runs into L2 now
-    if ((int64_t)blockIdx.x + m.prefetch_tiles < (int64_t)gridDim.x) {
-      const int64_t tp = m.tlist[m.tbase + blockIdx.x + m.prefetch_tiles];
-      const rt_tile dp = m.tiles[tp];
-      const int64_t cp = tp * m.TC;
-      const unsigned nc = (unsigned)(cp + m.TC < m.C ? m.TC : m.C - cp);
-      bulk_prefetch_l2(m.blob + (size_t)tp * m.bstride, 4u * m.bstride);
-      bulk_prefetch_l2(m.faceW + 2 * dp.fbase, 16u * dp.nown);
-      bulk_prefetch_l2(m.faceW + 2 * m.F + 2 * dp.fbase, 16u * dp.nown);
-      bulk_prefetch_l2(m.faceC + 2 * dp.fbase, 16u * dp.nown);
-      bulk_prefetch_l2(m.faceC + 2 * m.F + 2 * dp.fbase, 16u * dp.nown);
-      bulk_prefetch_l2(U + 4 * G * cp, 32u * G * nc);
-      bulk_prefetch_l2(m.Minv + 6 * cp, 48u * nc);
-    }
   }
   // the tile's cells and the halo cells: 2 G chunks of 16 bytes each into padded rows
   {
@@ -357,6 +343,24 @@ __global__ void __launch_bounds__(128, 4) k_grad(rt_geom m, const double *__rest
     cp16(sWh + 2 * (v.nown + j), m.faceW + 2 * m.F + 2 * q);
     cp16(sCl + 2 * (v.nown + j), m.faceC + 2 * q);
     cp16(sCh + 2 * (v.nown + j), m.faceC + 2 * m.F + 2 * q);
+  }
+  // (by one thread of the last warp once its own copies are on their way: the two dependent loads overlap the
+  // wait for the staged data instead of delaying thread 0's copies)
+  if (tid == nt - 32) {
+    // a tile that starts a few gridfuls later: pull its contiguous runs into L2 now
+    if ((int64_t)blockIdx.x + m.prefetch_tiles < (int64_t)gridDim.x) {
+      const int64_t tp = m.tlist[m.tbase + blockIdx.x + m.prefetch_tiles];
+      const rt_tile dp = m.tiles[tp];
+      const int64_t cp = tp * m.TC;
+      const unsigned nc = (unsigned)(cp + m.TC < m.C ? m.TC : m.C - cp);
+      bulk_prefetch_l2(m.blob + (size_t)tp * m.bstride, 4u * m.bstride);
+      bulk_prefetch_l2(m.faceW + 2 * dp.fbase, 16u * dp.nown);
+      bulk_prefetch_l2(m.faceW + 2 * m.F + 2 * dp.fbase, 16u * dp.nown);
+      bulk_prefetch_l2(m.faceC + 2 * dp.fbase, 16u * dp.nown);
+      bulk_prefetch_l2(m.faceC + 2 * m.F + 2 * dp.fbase, 16u * dp.nown);
+      bulk_prefetch_l2(U + 4 * G * cp, 32u * G * nc);
+      bulk_prefetch_l2(m.Minv + 6 * cp, 48u * nc);
+    }
   }
   mbar_wait(&bar, 0);
   cp_wait_all();
@@ -431,80 +435,8 @@ __device__ __forceinline__ double finish_cell(double a0, double a1, double a2, d
   return add;
 }
 
-// a3 for the tile's owned faces: one thread per face, its record read once into registers (so the thread
-// may overwrite it in shared memory with the fluxes), then every group in turn.  BND: the tile has boundary
-// faces (tile-uniform: interior tiles compile without the ghost-state branches).  Returns whether this
-// thread saw an outflow or Dirichlet face (its flux enters a ledger).
-template <int G, bool SECOND, bool BND>
-__device__ __forceinline__ int flux_faces(const rt_geom &m, const tile_view &v, double *sF, const double *sU, const double *sG,
-                                          const double *sV, const int OM, const double dt, const double ct, const int tid,
-                                          const int nt) {
-  constexpr int UR = 4 * G + 2, GR = 12 * G + 2;  // doubles per cell row of U / of the gradients (padded: bank spread)
-  int bnd = 0;
-  const double hc2 = 0.5 * ct * ct, hc = 0.5 * ct, rdt = 1.0 / dt;
-  for (int s = tid; s < v.nown; s += nt) {
-    const double2 c01 = ld2(sF + 2 * s), c23 = ld2(sF + 2 * (OM + s)), n01 = ld2(sF + 2 * (2 * OM + s)), n23 = ld2(sF + 2 * (3 * OM + s)),
-                  w01 = ld2(sF + 2 * (4 * OM + s)), w23 = ld2(sF + 2 * (5 * OM + s));
-    const double4 fc = make_double4(c01.x, c01.y, c23.x, c23.y), fn = make_double4(n01.x, n01.y, n23.x, 0.0),
-                  fw = make_double4(w01.x, w01.y, w23.x, w23.y);
-    const uint32_t lr = v.slr[s];
-    const int xl = (int)(lr & 0xffffu);
-    int xr = (int)(lr >> 16);
-    const bool rin = !BND || xr < 0xFF00;
-    if (rin && xr >= m.TC) xr -= v.nb;  // forward halo cells follow the tile's cells in sU / sG / sV
-    const int r = rin ? 0 : xr - 0x10000;  // boundary code (negative) where the face has no right cell
-    const double n[3] = {fn.x, fn.y, fn.z};
-    const double A = fc.w;
-    // the donor cap in area-scaled form: |A Phi_N| <= N_d V_d / dt (no division per face)
-    const double capL = sV[xl] * rdt;
-    // the face centre relative to the left cell is stored; relative to the right cell it is c - kappa w
-    double capR = 0.0, rRx = 0.0, rRy = 0.0, rRz = 0.0;
-    if (rin) {
-      capR = sV[xr] * rdt;
-      rRx = fma(-fw.w, fw.x, fc.x); rRy = fma(-fw.w, fw.y, fc.y); rRz = fma(-fw.w, fw.z, fc.z);
-    }
-    const int xrr = rin ? xr : xl;
-    if (BND && !rin && r != RT_BC_REFLECT) bnd = 1;  // outflow or Dirichlet face
-    const int xla = (m.variant & 2) ? 0 : xl, xra = (m.variant & 4) ? (tid & 7) : xrr;  // EXPERIMENT: wrong rows, timing only
-    const double *puL = sU + UR * xla, *pgL = sG + GR * xla, *puR = sU + UR * xra, *pgR = sG + GR * xra;
-    const double hA = 0.5 * A, Ahc = hc * A, Ahc2 = hc2 * A;
-    const double hn[3] = {hA * n[0], hA * n[1], hA * n[2]};
-    double *o0 = sF + 2 * s, *o1 = sF + 2 * (OM + s);
-#pragma unroll
-    for (int g = 0; g < G; g++) {
-      double UL[4], URt[4], NL, NR = 0.0;
-      extrapolate<SECOND>(puL + 4 * g, pgL + 12 * g, fc.x, fc.y, fc.z, UL, NL);
-      if (rin) extrapolate<SECOND>(puR + 4 * g, pgR + 12 * g, rRx, rRy, rRz, URt, NR);
-      else if (r == RT_BC_OUTFLOW) { URt[0] = URt[1] = URt[2] = URt[3] = 0.0; }  // vacuum ghost
-      else if (r == RT_BC_REFLECT) {
-        const double p = 2.0 * (UL[1] * n[0] + UL[2] * n[1] + UL[3] * n[2]);
-        URt[0] = UL[0]; URt[1] = UL[1] - p * n[0]; URt[2] = UL[2] - p * n[1]; URt[3] = UL[3] - p * n[2];
-      } else {
-        const double4 gs = ld4(m.ghost + ((size_t)(RT_BC_DIRICHLET0 - r) * G + g) * 4);
-        URt[0] = gs.x; URt[1] = gs.y; URt[2] = gs.z; URt[3] = gs.w;
-      }
-      double PL[3], PR[3], ph[4];
-      pressure_dot_n(UL, n, ct, PL);
-      pressure_dot_n(URt, n, ct, PR);
-      // A * Phi: the area is folded into the three constants
-      ph[0] = ((UL[1] + URt[1]) * hn[0] + (UL[2] + URt[2]) * hn[1] + (UL[3] + URt[3]) * hn[2]) - Ahc * (URt[0] - UL[0]);
-#pragma unroll
-      for (int a = 0; a < 3; a++) ph[1 + a] = Ahc2 * (PL[a] + PR[a]) - Ahc * (URt[1 + a] - UL[1 + a]);
-      // donor cap (S11): the donor cannot lose more photons than it holds through this face in dt;
-      // only the number flux is clamped (continuous in the state; Phi_F is left alone)
-      if (ph[0] > 0.0) ph[0] = dmin2(ph[0], NL * capL);
-      else if (rin) ph[0] = -dmin2(-ph[0], NR * capR);
-      st2(o0 + 4 * g * OM, ph[0], ph[1]);
-      st2(o1 + 4 * g * OM, ph[2], ph[3]);
-    }
-  }
-  return bnd;
-}
-
-// NT: the most threads of a block (one per owned face: tiles with more than 256 owned faces run in a
-// launch of their own with more threads, so that no tile needs a second pass over its faces)
-template <int G, bool SECOND, int NT>
-__global__ void __launch_bounds__(NT, NT > 256 ? 2 : 3) k_flux(rt_geom m, const double *__restrict__ Uin, const double *__restrict__ grad,
+template <int G, bool SECOND>
+__global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__restrict__ Uin, const double *__restrict__ grad,
                                                  const double *U0, double *Uout, const int32_t *__restrict__ srcidx,
                                                  const double *__restrict__ srcrate, int nsrc, update_par up,
                                                  double *__restrict__ pacc, double *__restrict__ part_floor,
@@ -513,7 +445,6 @@ __global__ void __launch_bounds__(NT, NT > 256 ? 2 : 3) k_flux(rt_geom m, const 
   __shared__ double red[32];
   __shared__ __align__(8) uint64_t bar, bar_blob;
   constexpr int NP = G > 3 ? G : 3;                        // planes of [omax][4]
-  constexpr int UR = 4 * G + 2, GR = 12 * G + 2;           // doubles per cell row (padded)
   const int NE = (m.TC + m.fmax + 1) & ~1;                 // tile cells, then forward halo cells
   const int OM = m.omax;
   uint32_t *sB = reinterpret_cast<uint32_t *>(smem_raw);   // the tile's blob
@@ -521,51 +452,60 @@ __global__ void __launch_bounds__(NT, NT > 256 ? 2 : 3) k_flux(rt_geom m, const 
                                                            // (cx, cy | cz, A), (nx, ny | nz, -), (wx, wy | wz, kappa) as
                                                            // 16-byte halves; the slot's thread then overwrites
                                                            // half-planes 2g, 2g + 1 with A * (Phi_N, Phi_F) of group g
-  double *sU = sF + 4 * NP * OM;                           // [NE][4 G + 2]
-  double *sG = sU + UR * NE;                               // [NE][12 G + 2]
-  double *sV = sG + GR * NE;                               // [NE]  cell volumes
+  double *sU = sF + 4 * NP * OM;                           // [NE][G][4]
+  double *sG = sU + 4 * G * NE;                            // [NE][G][12]
+  double *sV = sG + 12 * G * NE;                           // [NE]  cell volumes
   int32_t *sSrc = reinterpret_cast<int32_t *>(sV + NE);    // [TC] source index or -1
-  double *sU0 = reinterpret_cast<double *>(sSrc + ((m.TC + 3) & ~3));  // [TC][4 G]  U^n of the tile's cells (second stage only)
+  const unsigned tile = (unsigned)m.tlist[m.tbase + blockIdx.x];
   const int tid = threadIdx.x, nt = blockDim.x;
   const double dt = up.dt, ct = up.ct;
-  const bool own0 = U0 == Uin;  // first Heun stage: U^n is the state the fluxes are evaluated on
+  unsigned long long *tl = m.tl && tid == 0 ? m.tl + 8 * (size_t)tile : nullptr;  // rt_debug_tile_timeline
+  if (tl) tl[0] = now_ns();
   if (tid == 0) { mbar_init(&bar, 1); mbar_init(&bar_blob, 1); }
   __syncthreads();
-  // a block works through the tiles bi, bi + gridDim.x, ... of this launch (one gridful stays resident)
-  unsigned phase = 0;
-  if (m.variant & 64) {  // EXPERIMENT: start the co-resident blocks out of phase
-    const unsigned slot = blockIdx.x / 148u;
-    if (slot) __nanosleep(1400u * slot);
-  }
-  for (int64_t bi = blockIdx.x; bi < m.ntile; bi += gridDim.x, phase ^= 1) {
-  const unsigned tile = (unsigned)m.tlist[m.tbase + bi];
-  unsigned long long *tl = m.tl && tid == 0 ? m.tl + 8 * (size_t)tile : nullptr;
-  if (tl) tl[0] = now_ns();
   // round 1: the tile's blob sits at a fixed stride: header (descriptor) + tables
   if (tid == 0) {
     mbar_expect(&bar_blob, 4u * m.bstride);
     bulk_g2s(sB, m.blob + (size_t)tile * m.bstride, 4u * m.bstride, &bar_blob);
   }
-  mbar_wait(&bar_blob, phase);
+  mbar_wait(&bar_blob, 0);
   const tile_view v = view_tile(m, sB, tile);
   if (tl) tl[1] = now_ns();
-  // round 2: what the descriptor locates (bulk copies: owned faces, volumes, source ids) and what the
-  // tables locate (gathers: the cells' rows), all in flight together
+  // round 2: what the descriptor locates (bulk copies: owned faces, the tile's own cells) and what the
+  // tables locate (gathers: forward halo cells), all in flight together
   if (tid == 0) {
     const unsigned nsb = (4u * v.ncell + 15u) & ~15u, nvb = (8u * v.ncell + 15u) & ~15u;  // srcidx and cellV are padded
-    mbar_expect(&bar, 96u * v.nown + nvb + nsb + (own0 ? 0u : 32u * G * v.ncell));
-    if (!own0) bulk_g2s(sU0, U0 + 4 * G * v.c0, 32u * G * v.ncell, &bar);
+    mbar_expect(&bar, 96u * v.nown + (SECOND ? 128u : 32u) * G * v.ncell + nvb + nsb);
     bulk_g2s(sF, m.faceC + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sF + 2 * OM, m.faceC + 2 * m.F + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sF + 4 * OM, m.faceN + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sF + 6 * OM, m.faceN + 2 * m.F + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sF + 8 * OM, m.faceW + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sF + 10 * OM, m.faceW + 2 * m.F + 2 * v.fbase, 16u * v.nown, &bar);
+    bulk_g2s(sU, Uin + 4 * G * v.c0, 32u * G * v.ncell, &bar);
+    if (SECOND) bulk_g2s(sG, grad + 12 * G * v.c0, 96u * G * v.ncell, &bar);
     bulk_g2s(sV, m.cellV + v.c0, nvb, &bar);
     bulk_g2s(sSrc, srcidx + v.c0, nsb, &bar);
-    // a tile that starts a little later: pull its contiguous runs into L2 now
-    if (bi + m.prefetch_tiles < m.ntile) {
-      const int64_t tp = m.tlist[m.tbase + bi + m.prefetch_tiles];
+  }
+  // round 2: what the blob locates: the forward halo cells (right cells of the outgoing faces)
+  const int nf = v.nh - v.nb;
+  // (gathers of 32 to 288 bytes: 16-byte asynchronous copies; a halo cell's gradients are split over G threads)
+  for (int k = tid; k < nf * (G + 1); k += nt) {
+    const int h = k / (G + 1), part = k - h * (G + 1);
+    const int64_t id = v.halo[v.nb + h];
+    if (part < G) {
+      if (SECOND) cp_run<6>(sG + 12 * (G * (m.TC + h) + part), grad + 12 * (G * id + part));
+    } else {
+      cp_run<2 * G>(sU + 4 * G * (m.TC + h), Uin + (int64_t)(4 * G) * id);
+      cp8(sV + m.TC + h, m.cellV + id);
+    }
+  }
+  // (by one thread of the last warp once its own copies are on their way: the two dependent loads overlap the
+  // wait for the staged data instead of delaying thread 0's copies)
+  if (tid == nt - 32) {
+    // a tile that starts a few gridfuls later: pull its contiguous runs into L2 now
+    if ((int64_t)blockIdx.x + m.prefetch_tiles < (int64_t)gridDim.x) {
+      const int64_t tp = m.tlist[m.tbase + blockIdx.x + m.prefetch_tiles];
       const rt_tile dp = m.tiles[tp];
       const int64_t cp = tp * m.TC;
       const unsigned nc = (unsigned)(cp + m.TC < m.C ? m.TC : m.C - cp);
@@ -580,30 +520,65 @@ __global__ void __launch_bounds__(NT, NT > 256 ? 2 : 3) k_flux(rt_geom m, const 
       bulk_prefetch_l2(U0 + 4 * G * cp, 32u * G * nc);
     }
   }
-  // the rows of the tile's cells and of the forward halo cells (right cells of the outgoing faces):
-  // 16-byte asynchronous copies into padded rows, 2 G chunks of U and 6 G chunks of gradients per cell
-  {
-    const int nf = v.nh - v.nb, ne = v.ncell + nf;
-    constexpr int NPART = SECOND ? G + 1 : 1;  // per cell: G parts of six gradient chunks, one part = its U row
-    for (int k = tid; k < ne * NPART; k += nt) {
-      const int ci = k / NPART, part = k - ci * NPART;
-      const bool own = ci < v.ncell;
-      const int64_t id = own ? v.c0 + ci : (int64_t)v.halo[v.nb + ci - v.ncell];
-      const int row = own ? ci : m.TC + (ci - v.ncell);
-      if (part == NPART - 1) {
-        cp_run<2 * G>(sU + UR * row, Uin + (int64_t)(4 * G) * id);
-        if (!own) cp8(sV + row, m.cellV + id);
-      } else cp_run<6>(sG + GR * row + 12 * part, grad + 12 * ((int64_t)G * id + part));
-    }
-  }
-  mbar_wait(&bar, phase);
+  mbar_wait(&bar, 0);
   cp_wait_all();
   __syncthreads();
   if (tl) tl[2] = now_ns();
 
-  // ---- a3
-  const int bnd = (m.variant & 16) ? 0 : v.bnd ? flux_faces<G, SECOND, true>(m, v, sF, sU, sG, sV, OM, dt, ct, tid, nt)
-                        : flux_faces<G, SECOND, false>(m, v, sF, sU, sG, sV, OM, dt, ct, tid, nt);
+  // ---- a3: one thread per owned face: its record is read once into registers (so the thread may
+  // overwrite it in shared memory with the fluxes), then every group in turn
+  int bnd = 0;
+  const double hc2 = 0.5 * ct * ct, hc = 0.5 * ct;
+  for (int s = tid; s < ((m.variant & 16) ? 0 : v.nown); s += nt) {  // (variant 16: timing experiment without a3)
+    const double2 c01 = ld2(sF + 2 * s), c23 = ld2(sF + 2 * (OM + s)), n01 = ld2(sF + 2 * (2 * OM + s)), n23 = ld2(sF + 2 * (3 * OM + s)),
+                  w01 = ld2(sF + 2 * (4 * OM + s)), w23 = ld2(sF + 2 * (5 * OM + s));
+    const double4 fc = make_double4(c01.x, c01.y, c23.x, c23.y), fn = make_double4(n01.x, n01.y, n23.x, 0.0),
+                  fw = make_double4(w01.x, w01.y, w23.x, w23.y);
+    const uint32_t lr = v.slr[s];
+    const int xl = (int)(lr & 0xffffu);
+    int xr = (int)(lr >> 16);
+    const bool rin = xr < 0xFF00;
+    if (rin && xr >= m.TC) xr -= v.nb;  // forward halo cells follow the tile's cells in sU / sG / sS
+    const int r = rin ? 0 : xr - 0x10000;  // boundary code (negative) where the face has no right cell
+    const double n[3] = {fn.x, fn.y, fn.z};
+    const double A = fc.w;
+    const double rdtA = fast_rcp(dt * A);
+    const double capL = sV[xl] * rdtA;
+    // the face centre relative to the left cell is stored; relative to the right cell it is c - kappa w
+    double capR = 0.0, rRx = 0.0, rRy = 0.0, rRz = 0.0;
+    if (rin) {
+      capR = sV[xr] * rdtA;
+      rRx = fma(-fw.w, fw.x, fc.x); rRy = fma(-fw.w, fw.y, fc.y); rRz = fma(-fw.w, fw.z, fc.z);
+    }
+    const int xrr = rin ? xr : xl;
+    if (!rin && r != RT_BC_REFLECT) bnd = 1;  // outflow or Dirichlet face: its flux enters a ledger
+#pragma unroll 1
+    for (int g = 0; g < G; g++) {
+      double UL[4], UR[4], NL, NR = 0.0;
+      extrapolate<SECOND>(sU + 4 * (xl * G + g), sG + 12 * (xl * G + g), fc.x, fc.y, fc.z, UL, NL);
+      if (rin) extrapolate<SECOND>(sU + 4 * (xrr * G + g), sG + 12 * (xrr * G + g), rRx, rRy, rRz, UR, NR);
+      else if (r == RT_BC_OUTFLOW) { UR[0] = UR[1] = UR[2] = UR[3] = 0.0; }  // vacuum ghost
+      else if (r == RT_BC_REFLECT) {
+        const double p = 2.0 * (UL[1] * n[0] + UL[2] * n[1] + UL[3] * n[2]);
+        UR[0] = UL[0]; UR[1] = UL[1] - p * n[0]; UR[2] = UL[2] - p * n[1]; UR[3] = UL[3] - p * n[2];
+      } else {
+        const double4 gs = ld4(m.ghost + ((size_t)(RT_BC_DIRICHLET0 - r) * G + g) * 4);
+        UR[0] = gs.x; UR[1] = gs.y; UR[2] = gs.z; UR[3] = gs.w;
+      }
+      double PL[3], PR[3], ph[4];
+      pressure_dot_n(UL, n, ct, PL);
+      pressure_dot_n(UR, n, ct, PR);
+      ph[0] = 0.5 * ((UL[1] + UR[1]) * n[0] + (UL[2] + UR[2]) * n[1] + (UL[3] + UR[3]) * n[2]) - hc * (UR[0] - UL[0]);
+#pragma unroll
+      for (int a = 0; a < 3; a++) ph[1 + a] = hc2 * (PL[a] + PR[a]) - hc * (UR[1 + a] - UL[1 + a]);
+      // donor cap (S11): the donor cannot lose more photons than it holds through this face in dt;
+      // only the number flux is clamped (continuous in the state; Phi_F is left alone)
+      if (ph[0] > 0.0) ph[0] = dmin2(ph[0], NL * capL);
+      else if (rin) ph[0] = -dmin2(-ph[0], NR * capR);
+      st2(sF + 2 * (2 * g * OM + s), A * ph[0], A * ph[1]);
+      st2(sF + 2 * ((2 * g + 1) * OM + s), A * ph[2], A * ph[3]);
+    }
+  }
   __syncthreads();  // every owned slot holds its fluxes
   if (tl) tl[3] = now_ns();
   // the outgoing faces' fluxes go to xphi for the tiles of their right cells (k_finish)
@@ -616,7 +591,7 @@ __global__ void __launch_bounds__(NT, NT > 256 ? 2 : 3) k_flux(rt_geom m, const 
   }
   // boundary ledgers: the number fluxes through the tile's outflow / Dirichlet faces, read back from
   // the slots; fixed-order block sums, one row per tile
-  if (v.bnd && __syncthreads_or(bnd)) {
+  if (__syncthreads_or(bnd)) {
 #pragma unroll
     for (int gg = 0; gg < G; gg++) {
       double b_out = 0.0, b_in = 0.0;
@@ -645,28 +620,28 @@ __global__ void __launch_bounds__(NT, NT > 256 ? 2 : 3) k_flux(rt_geom m, const 
 #pragma unroll
   for (int gg = 0; gg < G; gg++) fl[gg] = 0.0;
   int floored = 0;
-  const int PS = nt >= 4 * m.TC * G ? 2 : (nt >= 2 * m.TC * G ? 1 : 0), P = 1 << PS;  // lanes per (cell, group)
+  const int P = nt >= 4 * m.TC * G ? 4 : (nt >= 2 * m.TC * G ? 2 : 1);
   const int nitem = v.ncell * G;
   for (int base = 0; base < nitem * P; base += nt) {  // (nt is a multiple of 32, P divides 32: whole warps iterate together)
     const int e = base + tid;
-    const int item = e >> PS, p = e & (P - 1);
+    const int item = e / P, p = e - item * P;
     const bool on = item < nitem;
     const int il = on ? item / G : 0, ig = on ? item - il * G : 0;
     const int h0 = on ? (int)v.ho[il] : 0, h1 = on ? (int)v.ho[il + 1] : 0;
     const double *pg = sF + 4 * ig * OM;  // half-planes 2 ig and 2 ig + 1
+    // U^n of the cell (the stage buffer itself in stage 1): asked for now, needed after the sum
+    const double4 u0 = on && p == 0 ? ld4(U0 + 4 * (v.c0 * G + item)) : make_double4(0, 0, 0, 0);
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
     int incomplete = 0;
 #pragma unroll 4
-    for (int k = h0 + p; k < ((m.variant & 32) ? h0 : h1); k += P) {
+    for (int k = h0 + p; k < ((m.variant & 32) ? h0 : h1); k += P) {  // (variant 32: without the gather)
       const uint32_t w = v.hl[k];
       const int s = (int)(w & 0x7fffu);
-      const bool mine = s < v.nown;  // else incoming: its owner tile has the flux
-      incomplete |= !mine;
-      const int sl = mine ? s : 0;
-      const double2 q01 = ld2(pg + 2 * sl), q23 = ld2(pg + 2 * (OM + sl));
-      // the flux leaves the left cell and enters the right one
-      const double sg = mine ? ((w & 0x8000u) ? -1.0 : 1.0) : 0.0;
-      a0 = fma(sg, q01.x, a0); a1 = fma(sg, q01.y, a1); a2 = fma(sg, q23.x, a2); a3 = fma(sg, q23.y, a3);
+      if (s >= v.nown) { incomplete = 1; continue; }  // incoming: its owner tile has the flux
+      const double2 q01 = ld2(pg + 2 * s), q23 = ld2(pg + 2 * (OM + s));
+      const double4 q = make_double4(q01.x, q01.y, q23.x, q23.y);
+      const int sgn = (int)((w & 0x8000u) << 16);  // the flux leaves the left cell and enters the right one
+      a0 += flip_sign(q.x, sgn); a1 += flip_sign(q.y, sgn); a2 += flip_sign(q.z, sgn); a3 += flip_sign(q.w, sgn);
     }
     for (int o = 1; o < P; o <<= 1) {
       a0 += __shfl_xor_sync(0xffffffffu, a0, o); a1 += __shfl_xor_sync(0xffffffffu, a1, o);
@@ -677,9 +652,8 @@ __global__ void __launch_bounds__(NT, NT > 256 ? 2 : 3) k_flux(rt_geom m, const 
     if (incomplete) { st4(pacc + 4 * (v.c0 * G + item), a0, a1, a2, a3); continue; }
     const int32_t si = sSrc[il];
     const double src = si >= 0 ? srcrate[(size_t)ig * nsrc + si] : 0.0;
-    const double4 uc = ld4(sU + UR * il + 4 * ig);
-    const double4 u0 = own0 ? uc : ld4(sU0 + 4 * item);  // U^n of the cell (staged with the tile)
-    const double add = finish_cell(a0, a1, a2, a3, sV[il], src, uc, u0, up, Uout + 4 * (v.c0 * G + item));
+    const double add = finish_cell(a0, a1, a2, a3, sV[il], src, ld4(sU + 4 * item), u0, up,
+                                   Uout + 4 * (v.c0 * G + item));
     if (add != 0.0) {
 #pragma unroll
       for (int gg = 0; gg < G; gg++) if (gg == ig) fl[gg] += add;
@@ -693,8 +667,13 @@ __global__ void __launch_bounds__(NT, NT > 256 ? 2 : 3) k_flux(rt_geom m, const 
       if (tid == 0) part_floor[(size_t)tile * G + gg] = t;
     }
   } else if (tid < G) part_floor[(size_t)tile * G + tid] = 0.0;
-  __syncthreads();  // the tile's tables and slots are free for the next one
-  if (tl) { tl[5] = now_ns(); unsigned sm; asm("mov.u32 %0, %smid;" : "=r"(sm)); tl[6] = sm; tl[7] = blockIdx.x; }
+  if (m.tl) {  // (block-uniform)
+    __syncthreads();
+    if (tl) {
+      unsigned sm;
+      asm("mov.u32 %0, %smid;" : "=r"(sm));
+      tl[5] = now_ns(); tl[6] = sm; tl[7] = blockIdx.x;
+    }
   }
 }
 
@@ -863,10 +842,8 @@ static inline unsigned blocks_for(int64_t n, int per_block) { return (unsigned)(
     default: KERNEL(8)<<<grid, block, smem, stream>>>(__VA_ARGS__); break;                \
   }
 #define K_GRAD(g) k_grad<g>
-#define K_FLUX2(g) k_flux<g, true, 256>
-#define K_FLUX1(g) k_flux<g, false, 256>
-#define K_FLUX2B(g) k_flux<g, true, 384>
-#define K_FLUX1B(g) k_flux<g, false, 384>
+#define K_FLUX2(g) k_flux<g, true>
+#define K_FLUX1(g) k_flux<g, false>
 #define K_FINISH(g) k_finish<g>
 #define K_STORED(g) k_stored<g>
 
@@ -896,8 +873,6 @@ int rt_transport_configure(rt_ctx *c) {
   SET_SMEM_G(c->G, K_GRAD, sg, e);
   if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX2, ss, e);
   if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX1, ss, e);
-  if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX2B, ss, e);
-  if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX1B, ss, e);
   if (e != cudaSuccess) return rt_fail(c, RT_ECUDA, "cudaFuncSetAttribute(shared memory): %s", cudaGetErrorString(e));
   return RT_OK;
 }
@@ -906,7 +881,6 @@ int rt_transport_configure(rt_ctx *c) {
 // k_grad has one thread per (cell, group); k_stage one lane per (slot, group), several passes.
 // rt_tuning.flux_threads / grad_threads override the defaults for experiments.
 static int round_threads(int n) { n = ((n + 31) / 32) * 32; return n > 256 ? 256 : (n < 32 ? 32 : n); }
-static int round_threads_up(int n) { n = ((n + 31) / 32) * 32; return n < 64 ? 64 : n; }
 static int tile_threads(const rt_ctx *c) { return round_threads(c->tun.flux_threads > 0 ? c->tun.flux_threads : 256); }
 static int grad_threads(const rt_ctx *c) {  // four lanes per cell, at most k_grad's launch bound
   const int n = round_threads(c->tun.grad_threads > 0 ? c->tun.grad_threads : 4 * c->TC);
@@ -986,30 +960,10 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
       mf.tbase = cls == 0 ? 0 : c->nFA;
       mf.omax = cls == 0 ? c->omaxA : c->omax; mf.fmax = cls == 0 ? c->fmaxA : c->fmax;
       const size_t sf = rt_smem_flux(c->TC, G, mf.omax, mf.fmax, c->bstride);
-      mf.ntile = n;
-      if (c->nsm <= 0) { int k = 0; cudaDeviceGetAttribute(&k, cudaDevAttrMultiProcessorCount, c->device); c->nsm = k > 0 ? k : 1; }
-      // one thread per owned face where the launch bound allows it: no second pass over a tile's faces
-      const int want = c->tun.flux_threads > 0 ? nt : round_threads_up(mf.omax);
-      // one resident gridful of blocks, each working through its share of the tiles
-      const int thr = want <= 256 ? (want < nt ? want : nt) : (want > 384 ? 384 : want);
-      int bps = (int)(233472 / (sf + 1024)), breg = 65536 / (80 * thr);
-      if (bps > breg) bps = breg;
-      if (bps > (want <= 256 ? 3 : 2)) bps = want <= 256 ? 3 : 2;
-      if (bps < 1) bps = 1;
-      const int64_t resident = (int64_t)c->nsm * bps;
-      const unsigned grid = (c->tun.variant & 8) || n < resident ? (unsigned)n : (unsigned)resident;
-      if (want <= 256) {
-        if (c->par.order >= 2) {
-          DISPATCH_G(G, K_FLUX2, grid, thr, sf, c->stream, mf, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
-        } else {
-          DISPATCH_G(G, K_FLUX1, grid, thr, sf, c->stream, mf, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
-        }
+      if (c->par.order >= 2) {
+        DISPATCH_G(G, K_FLUX2, (unsigned)n, nt, sf, c->stream, mf, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
       } else {
-        if (c->par.order >= 2) {
-          DISPATCH_G(G, K_FLUX2B, grid, thr, sf, c->stream, mf, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
-        } else {
-          DISPATCH_G(G, K_FLUX1B, grid, thr, sf, c->stream, mf, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
-        }
+        DISPATCH_G(G, K_FLUX1, (unsigned)n, nt, sf, c->stream, mf, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
       }
       c->launches++;
     }

@@ -29,12 +29,12 @@ sys.path.insert(0, ROOT)
 
 METRIC = "rt_cell_group_updates_per_s"
 UNIT = "cell-group-updates/s"
-FULL_N = {0: 32, 1: 128, 2: 64, 3: 256, 4: 384, 5: 44}
-SAMPLE_N = {0: 24, 1: 32, 2: 24, 3: 28, 4: 28, 5: 20}
+FULL_N = {0: 32, 1: 128, 2: 64, 3: 256, 4: 384, 5: 44, 6: 128}
+SAMPLE_N = {0: 24, 1: 32, 2: 24, 3: 28, 4: 28, 5: 20, 6: 32}
 
 
 def workload_name(c, n):
-    return "config%d_%s_n%d" % (c, ("stromgren", "beam", "hhe_voronoi", "reion_voronoi", "reion_voronoi", "hii_region_voronoi")[c], n)
+    return "config%d_%s_n%d" % (c, ("stromgren", "beam", "hhe_voronoi", "reion_voronoi", "reion_voronoi", "hii_region_voronoi", "travelling_wave")[c], n)
 
 
 # ------------------------------------------------------------------ CPU oracle legs
@@ -197,6 +197,16 @@ def run_alu_peak():
     return 0
 
 
+def survey_bytes(C, F, G):
+    """per subcycle 2 x (gradient pass + update pass) + 32 G (stage 2 re-reads U^n) + 80, with
+    fpc = F / C unique faces and hf = 2 fpc half-faces per cell, int32 ids."""
+    fpc = F / C
+    hf = 2.0 * fpc
+    grad = 32 * G + 56 * fpc + 76 + 4 * hf + 96 * G
+    upd = 32 * G + 96 * G + 64 * fpc + 36 + 4 * hf + 32 * G
+    return C * (2 * (grad + upd) + 32 * G + 80)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -223,6 +233,7 @@ def main():
     from paper_2404_17630_b200 import rt
     from paper_2404_17630_b200.inputs import configs as cfg
     from paper_2404_17630_b200.inputs import device as devin
+    from paper_2404_17630_b200.profile_summary import kernel_source_sha
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -239,6 +250,8 @@ def main():
     t_build = time.perf_counter()
     if c in (3, 4):
         w = devin.config34_device(n, c, "cuda:%d" % local)
+    elif c == 6:
+        w = cfg.get(6, n)                        # transport only, one bin, 10 % generator offset
     else:
         w = cfg.get(c, n)
     C, F, G = int(w.mesh.ncell), int(w.mesh.nface), int(w.params.ngroup)
@@ -262,20 +275,28 @@ def main():
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
-    s.profile(True)
     tw0 = time.perf_counter()
     e0.record()
-    s.step(w.dt, args.steps)
+    s.step(w.dt, args.steps)          # the headline pass: no per-kernel events on the stream
     e1.record()
     torch.cuda.synchronize()
     tw1 = time.perf_counter()
     if dist is not None:
         dist.barrier()
     ms = e0.elapsed_time(e1)
-    prof = s.profile_read()
-    s.profile(False)
     launches = s.launches() - l0
     clocks = sampler.stop(tw0, tw1)
+    # a second, shorter pass with the library's per-kernel events for the shares (not part of `value`)
+    nprof = max(1, min(args.steps, 5))
+    s.profile(True)
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record()
+    s.step(w.dt, nprof)
+    p1.record()
+    torch.cuda.synchronize()
+    prof = s.profile_read()
+    s.profile(False)
+    ms_prof = p0.elapsed_time(p1)
     ms = max_over_ranks(ms, dist, "cuda")
     value = aggregate_value(world, C, G, args.steps, ms)
 
@@ -329,7 +350,7 @@ def main():
         if cnt == 0:
             continue
         avg = tms / cnt
-        d = {"launches": cnt, "avg_ms": avg, "share": tms / ms}
+        d = {"launches": cnt, "avg_ms": avg, "share": tms / ms_prof}
         if k in ab:
             d["algorithmic_bytes"] = ab[k]
             d["GBps"] = ab[k] / (avg * 1e-3) / 1e9
@@ -340,25 +361,33 @@ def main():
     # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
     # capture of this workload (profiles/traffic.csv, written from profiles/r1_ncu_full_*.md); for
     # the stage pair it is the sum of k_flux (both tile classes) and k_finish
-    traffic = None
+    traffic, traffic_note = None, "no ncu capture of this workload in profiles/traffic.csv"
     tf = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tf):
         rows = {}
         for ln in open(tf).read().splitlines()[1:]:
-            wl, kn, by = ln.split(",")
-            if wl == workload_name(c, n):
-                rows[kn] = float(by)
-        parts = {"stage": ("flux", "finish")}.get(dom, (dom,))
+            f = ln.split(",")
+            if len(f) >= 4 and f[0] == workload_name(c, n):
+                rows[f[1]] = (float(f[2]), f[3])
+        parts = {"stage": ("k_flux", "k_finish"), "grad": ("k_grad",), "chem": ("k_chem",)}.get(dom, (dom,))
         if all(k in rows for k in parts):
-            traffic = sum(rows[k] for k in parts)
+            if all(rows[k][1] == kernel_source_sha() for k in parts):
+                traffic, traffic_note = sum(rows[k][0] for k in parts), "ncu capture of these kernel sources (profiles/traffic.csv)"
+            else:
+                traffic_note = "profiles/traffic.csv was captured from other kernel sources: stale, not reported"
+
     roofline = {"bound": "hbm", "kernel": {"stage": "stage = k_flux + k_finish (a3 + a4 of one Heun stage)"}.get(dom, dom), "achieved": kern[dom]["GBps"], "peak": peak, "unit": "GB/s",
                 "frac": kern[dom]["GBps"] / peak, "frac_of_nominal_8TBs": kern[dom]["GBps"] / 8000.0,
-                "traffic": traffic, "peak_source": peak_src,
+                "traffic": traffic, "traffic_note": traffic_note, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": ab[dom],
                 "subcycle": {"algorithmic_bytes": ab["subcycle"], "GBps": ab["subcycle"] * args.steps / (ms * 1e-3) / 1e9,
                              "frac": ab["subcycle"] * args.steps / (ms * 1e-3) / 1e9 / peak,
                              "frac_of_nominal_8TBs": ab["subcycle"] * args.steps / (ms * 1e-3) / 1e9 / 8000.0,
-                             "bytes_per_cell_group_update": ab["subcycle"] / (C * G)}}
+                             "bytes_per_cell_group_update": ab["subcycle"] / (C * G),
+                             # the same time against SURVEY 8(d)'s model (fused, no list bytes: 4222 B per cell at
+                             # G = 3 on a Voronoi mesh), so that the fraction cannot rise by redefining the bytes
+                             "frac_survey_model": survey_bytes(C, F, G) * args.steps / (ms * 1e-3) / 1e9 / peak,
+                             "survey_bytes_per_cell_group_update": survey_bytes(C, F, G) / (C * G)}}
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
@@ -371,7 +400,8 @@ def main():
             "config": {"workload": workload_name(c, n), "cells": C, "faces": F, "groups": G,
                        "chem_mode": int(w.params.chem_mode), "dt": w.dt, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2 (%.1f GB of state and geometry per subcycle)" % (ab["subcycle"] / 1e9),
-                       "build_s": t_build, "tiles": tiles},
+                       "build_s": t_build, "tiles": tiles,
+                       "timed_subcycles": "%d..%d after rt_state_init (warm-up %d)" % (args.warmup + 1, args.warmup + args.steps, args.warmup)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "kernels": kern,
             "cpu_baseline": cpu,
             "ledger": {"substeps_total": int(led["substeps_total"]), "substeps_max": int(led["substeps_max"]),

@@ -135,13 +135,18 @@ typedef struct {
 } rt_tuning;
 
 /* Creates a context on CUDA device `device` issuing all work on `cuda_stream` (a cudaStream_t;
- * NULL = the legacy default stream).  The stream is borrowed and must outlive the context. */
+ * NULL = the legacy default stream).  The stream is borrowed and must outlive the context.
+ * One context = one mesh resident on one GPU for the duration of all its subcycles (PAPER.md:232:
+ * "all ... kernels run on the GPU and require the mesh ... to be available in GPU memory").
+ * Errors: RT_EINVAL (out == NULL), RT_ECUDA (no such device), RT_ENOMEM (host allocation). */
 int rt_create(rt_ctx **out, int device, void *cuda_stream);
 
 /* Sets the tuning of the next rt_mesh_upload (NULL = defaults).  RT_EINVAL on out-of-range values. */
 int rt_set_tuning(rt_ctx *ctx, const rt_tuning *t);
 
-/* Bytes of device workspace rt_mesh_upload needs for this problem size (0 on invalid sizes).
+/* Bytes of device workspace rt_mesh_upload needs for this problem size (0 on invalid sizes): the
+ * whole device footprint of the RT step, mesh and state (everything is held on the
+ * GPU from the first subcycle to the last; the library itself allocates no device memory).
  * flags: an OR of RT_WS_* (RT_WS_DEVICE_MESH: no staging space for a host mesh, 88 bytes per face
  * less).  Without RT_WS_ALL_FACES_CROSS the workspace holds the fluxes of 0.56 nface + 1024 faces
  * that cross tile boundaries (a jittered-lattice Voronoi mesh at the default tile size has 0.54);
@@ -159,15 +164,27 @@ size_t rt_workspace_bytes(int64_t ncell, int64_t nface, int ngroup, int flags);
 int rt_mesh_upload(rt_ctx *ctx, const rt_mesh *mesh, void *dev_workspace, size_t bytes);
 
 /* Sets parameters, sources and the initial state; resets the ledger.  `src` may be NULL.
- * Needs a mesh (else RT_ESTATE).  Synchronises the stream (inputs are free on return). */
+ * This is the one host -> device transfer of the state "before the first subcycle";
+ * sources are the S of eq (6).  Needs a mesh (else RT_ESTATE).  Synchronises the
+ * stream (inputs are free on return).  Errors: RT_EINVAL (null pointers, ngroup != the mesh's,
+ * bad chem_mode / order / controller constants, source cell out of range or listed twice),
+ * RT_ECUDA. */
 int rt_state_init(rt_ctx *ctx, const rt_params *p, const rt_state *s0, const rt_sources *src);
 
-/* Advances `nsub` subcycles of length dt [same time unit as 1/ctilde * length].  Asynchronous:
- * only enqueues kernels on the context's stream.  Needs rt_state_init (else RT_ESTATE). */
+/* Advances `nsub` subcycles of length dt [same time unit as 1/ctilde * length], each in the order
+ * of Fig. 1: thermochemistry with adaptive sub-steps, then two
+ * Heun stages of gradients, face fluxes and their application
+ * to the cells; dt obeys eq (11) and is the caller's choice.
+ * Asynchronous: only enqueues kernels on the context's stream; nothing crosses the host boundary
+ * inside or between subcycles.  Needs rt_state_init (else RT_ESTATE); RT_EINVAL for
+ * dt <= 0 or nsub < 0; RT_ECUDA if a launch fails. */
 int rt_step(rt_ctx *ctx, double dt, int nsub);
 
 /* Copies the state (any pointer of `out` may be NULL to skip it; nH is never written) and the
- * ledger (may be NULL) out, in the caller's cell order.  Synchronises the stream. */
+ * ledger (may be NULL) out, in the caller's cell order: the transfer "after the completion of the
+ * full RT step".  The ledger is the photon budget that the single-valued face fluxes
+ * keep closed ("ensuring photon conservation").  Synchronises the stream.
+ * Errors: RT_ESTATE (no state), RT_ECUDA. */
 int rt_download(rt_ctx *ctx, rt_state *out, rt_ledger *ledger);
 
 /* Number of kernels the context has launched since rt_create (for bench.py's gpu_launches). */
@@ -188,10 +205,16 @@ int rt_tile_info(const rt_ctx *ctx, int64_t *out);
  * rt_step.  rt_profile(ctx, 1) starts recording, rt_profile(ctx, 0) stops.  rt_profile_read
  * synchronises and returns, per kernel class (0 chemistry, 1 gradient, 2 face flux, 3 update,
  * 4 ledger reduction, 5 other), the summed milliseconds and the number of launches since the last
- * read; ms and count are HOST arrays of 6.  Class 2 is empty since the face fluxes are
- * evaluated inside the update kernel (class 3 = flux + update of one Heun stage). */
+ * read; ms and count are HOST arrays of 6.  Class 2 is k_flux (a3 and the part of a4 it finishes),
+ * class 3 is k_finish (a4 for the cells with faces owned by other tiles). */
 int rt_profile(rt_ctx *ctx, int enable);
 int rt_profile_read(rt_ctx *ctx, double *ms, int64_t *count);
+
+/* Where the cells went (for tests that sample by tile).  tile_of_cell: (C) int32 in the
+ * caller's cell order, HOST or DEVICE as mem_kind says = the tile that owns each cell.  tile_desc: HOST
+ * (T, 4) int32 with T = rt_tile_info's out[1] = per tile its owned faces, its forward halo cells, its
+ * table words and the flux kernel's launch class (0 = A, 1 = B).  Either may be NULL.  Synchronises. */
+int rt_debug_tiles(rt_ctx *ctx, int mem_kind, int32_t *tile_of_cell, int32_t *tile_desc);
 
 /* Slope-limited gradients of the current state in the caller's order, DEVICE or HOST as
  * mem_kind says: gN (G, 3, C), gF (G, 3 components, 3 directions, C).  For tests. Synchronises. */
@@ -212,10 +235,12 @@ int rt_debug_tile_timeline(rt_ctx *ctx, double dt, int64_t ntile_max, uint64_t *
  * reading one chunk, and with a random chunk per lane; the number of multiprocessors.  Synchronises. */
 int rt_debug_alu_peak(rt_ctx *ctx, double *out);
 
-/* Last error message of this context ("" if none); valid until the next call on it. */
+/* Last error message of this context ("" if none); valid until the next call on it.  (No exception or
+ * abort crosses the ABI: SURVEY 8(b) error convention.) */
 const char *rt_last_error(const rt_ctx *ctx);
 
-/* Frees the context (not the workspace, which is the caller's).  NULL is allowed. */
+/* Frees the context (not the workspace, which is the caller's: PAPER.md:232-234 leaves the device data
+ * to the caller between RT steps).  NULL is allowed. */
 void rt_destroy(rt_ctx *ctx);
 
 #ifdef __cplusplus

@@ -24,6 +24,7 @@ def lib():
         L.oracle_destroy.argtypes = [vp]
         L.oracle_set_params.argtypes = [vp, dbl, vp, vp, i32, vp, dbl, dbl, dbl, dbl, dbl, dbl, dbl, i64, i32, i32]
         L.oracle_set_sources.argtypes = [vp, i32, vp, vp]
+        L.oracle_set_active.argtypes = [vp, vp]
         L.oracle_set_state.argtypes = [vp] * 8
         L.oracle_get_state.argtypes = [vp] * 7
         L.oracle_get_ledger.argtypes = [vp, vp, vp]
@@ -109,6 +110,12 @@ class Oracle:
         cell = np.ascontiguousarray(src.cell, dtype=np.int32)
         rate = _f64(src.rate)
         self.L.oracle_set_sources(self.h, int(cell.size), _p(cell), _p(rate))
+
+    def set_active(self, active):
+        """active: (C,) boolean mask of the cells taking part in the RT step, or None for all."""
+        a = None if active is None else np.ascontiguousarray(active, dtype=np.uint8)
+        assert a is None or a.shape == (self.C,)
+        self.L.oracle_set_active(self.h, _p(a))
 
     def set_state(self, s):
         a = [_f64(s.N), _f64(s.F), _f64(s.xHII), _f64(s.xHeII), _f64(s.xHeIII), _f64(s.eth), _f64(s.nH)]

@@ -62,6 +62,9 @@ typedef struct oracle_ctx {
   double ctilde, sigma[3 * 8], eps[3 * 8], T_fixed, alphaB_override, y_he, f_accept, f_target, x_floor_rel, n_floor;
   int chem_mode, order, heun; int64_t max_substeps;
   double *kappa;
+  /* active set of the RT step (reading S27): NULL = every cell is active */
+  uint8_t *active;
+  uint8_t *touched; /* active, or sharing an interface with an active cell: the cells an RT step may change */
   /* sources */
   int nsrc; int32_t *src_cell; double *src_rate; /* [G][nsrc] */
   /* state: N[G][C], Fl[G][3][C] */
@@ -286,7 +289,7 @@ static int64_t chem_cell(const oracle_ctx *c, chem_state *s, double nH, double d
     chem_state o;
     double f = chem_try(c, s, nH, h, &o);
     attempts++;
-    int acc = !(f > c->f_accept);
+    int acc = f <= c->f_accept; /* accepted only if the change stays below 10 %; a NaN is not */
     if (trace && *ntrace < ntrace_max) {
       trace[3 * *ntrace] = h; trace[3 * *ntrace + 1] = f; trace[3 * *ntrace + 2] = acc; (*ntrace)++;
     }
@@ -388,7 +391,7 @@ void oracle_destroy(oracle_ctx *c) {
   free((void *)c->volume); free((void *)c->centroid); free((void *)c->area); free((void *)c->normal);
   free((void *)c->fcentroid); free((void *)c->left); free((void *)c->right); free(c->ghost); free(c->off);
   free(c->hf_face); free(c->hf_side); free(c->hf_w); free(c->hf_r); free(c->Minv); free(c->kappa);
-  free(c->src_cell); free(c->src_rate); free(c->N); free(c->Fl); free(c->N0); free(c->Fl0); free(c->xHII);
+  free(c->active); free(c->touched); free(c->src_cell); free(c->src_rate); free(c->N); free(c->Fl); free(c->N0); free(c->Fl0); free(c->xHII);
   free(c->xHeII); free(c->xHeIII); free(c->eth); free(c->nH); free(c->gN); free(c->gF); free(c->phi);
   free(c);
 }
@@ -404,6 +407,29 @@ void oracle_set_params(oracle_ctx *c, double ctilde, const double *sigma, const 
   c->f_target = f_target; c->x_floor_rel = x_floor_rel; c->n_floor = n_floor; c->max_substeps = max_substeps;
   c->order = order; c->heun = heun;
 }
+
+/* Individual time steps ("fluxes for interfaces with at least one active neighbour. For passive
+ * particles, only their conserved quantities are updated, taking into account the fluxes from the interfaces
+ * they share with active cells"; cells and interfaces in active / passive categories that
+ * stay fixed during the subcycles of one RT step).  Reading S27: a passive cell does no chemistry, injects
+ * no source photons, has no gradient (its mesh is not constructed: its face state is its cell value), and
+ * faces between two passive cells carry no flux.  active: (C) bytes, or NULL for "all active". */
+void oracle_set_active(oracle_ctx *c, const uint8_t *active) {
+  free(c->active); free(c->touched);
+  c->active = active ? (uint8_t *)dup(active, (size_t)c->C) : NULL;
+  c->touched = NULL;
+  if (!active) return;
+  c->touched = (uint8_t *)dup(active, (size_t)c->C);
+  for (int64_t f = 0; f < c->F; f++) {
+    int64_t L = c->left[f], R = c->right[f];
+    if (R < 0) continue;
+    if (active[L]) c->touched[R] = 1;
+    if (active[R]) c->touched[L] = 1;
+  }
+}
+static int is_active(const oracle_ctx *c, int64_t i) { return !c->active || c->active[i]; }
+/* a cell none of whose interfaces has an active cell is left alone altogether: "passive" */
+static int is_touched(const oracle_ctx *c, int64_t i) { return !c->touched || c->touched[i]; }
 
 void oracle_set_sources(oracle_ctx *c, int nsrc, const int32_t *cell, const double *rate) {
   free(c->src_cell); free(c->src_rate);
@@ -453,6 +479,7 @@ static void chemistry(oracle_ctx *c, double dt) {
   const int G = c->G;
   if (c->chem_mode == CHEM_NONE) return;
   for (int64_t i = 0; i < C; i++) {
+    if (!is_active(c, i)) continue; /* S27 */
     if (c->chem_mode == CHEM_FIXED_OPACITY) {
       /* one implicit step N' = N/(1 + dt c kappa): eq (6)-(7) right-hand sides */
       double den = 1.0 + dt * c->ctilde * c->kappa[i];
@@ -520,7 +547,7 @@ static void gradients(oracle_ctx *c) {
         double *out[3];
         for (int a = 0; a < 3; a++)
           out[a] = q == 0 ? &c->gN[((size_t)g * 3 + a) * C + i] : &c->gF[(((size_t)g * 3 + (q - 1)) * 3 + a) * C + i];
-        if (c->order < 2) { *out[0] = *out[1] = *out[2] = 0.0; continue; }
+        if (c->order < 2 || !is_active(c, i)) { *out[0] = *out[1] = *out[2] = 0.0; continue; } /* passive: S27 */
         double pi = fld(c, g, q, i);
         double b[3] = {0, 0, 0}, pmax = pi, pmin = pi;
         /* first neighbour loop: second term of eq (15) and min/max */
@@ -573,6 +600,11 @@ static void fluxes(oracle_ctx *c, double dt) {
   for (int64_t f = 0; f < F; f++) {
     int64_t L = c->left[f], R = c->right[f];
     double n[3] = {c->normal[f], c->normal[F + f], c->normal[2 * F + f]};
+    /* only interfaces with at least one active cell carry a flux */
+    if (!(is_active(c, L) || (R >= 0 && is_active(c, R)))) {
+      for (int k = 0; k < 4 * G; k++) c->phi[(size_t)f * G * 4 + k] = 0.0;
+      continue;
+    }
     for (int g = 0; g < G; g++) {
       double UL[4], UR[4];
       extrapolate(c, g, L, f, UL);
@@ -634,11 +666,13 @@ static void stage(oracle_ctx *c, double dt, double a, double b, double wl, doubl
   double *srcN = (double *)calloc((size_t)G * C, sizeof(double));
   for (int s = 0; s < c->nsrc; s++)
     for (int g = 0; g < G; g++) {
+      if (!is_active(c, c->src_cell[s])) continue; /* a passive cell injects nothing during this RT step (S27) */
       srcN[(size_t)g * C + c->src_cell[s]] += c->src_rate[(size_t)g * c->nsrc + s];
       kadd(&c->led[g][L_INJECTED], wl * dt * c->src_rate[(size_t)g * c->nsrc + s]);
     }
   for (int64_t i = 0; i < C; i++)
     for (int g = 0; g < G; g++) {
+      if (!is_touched(c, i)) continue;
       double sum[4] = {0, 0, 0, 0};
       for (int64_t k = c->off[i]; k < c->off[i + 1]; k++) {
         int64_t f = c->hf_face[k];
@@ -656,7 +690,8 @@ static void stage(oracle_ctx *c, double dt, double a, double b, double wl, doubl
     }
   free(srcN);
   for (int64_t i = 0; i < C; i++)
-    for (int g = 0; g < G; g++) enforce(c, g, i, wfloor);
+    for (int g = 0; g < G; g++)
+      if (is_touched(c, i)) enforce(c, g, i, wfloor);
 }
 
 static void transport(oracle_ctx *c, double dt) {

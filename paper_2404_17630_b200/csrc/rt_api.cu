@@ -3,6 +3,7 @@
 // rt_setup.cu (per mesh).
 #include <stdarg.h>
 #include <string.h>
+#include <algorithm>
 #include <new>
 #include <vector>
 #include "rt_internal.cuh"
@@ -186,6 +187,12 @@ int rt_state_init(rt_ctx *c, const rt_params *p, const rt_state *s0, const rt_so
     return rt_fail(c, RT_EINVAL, "nsrc must be in [0, 65536] with cell and rate set");
   for (int k = 0; k < nsrc; k++)
     if (src->cell[k] < 0 || src->cell[k] >= c->C) return rt_fail(c, RT_EINVAL, "source cell out of range");
+  if (nsrc > 1) {  // the cells must be distinct: one source slot per cell (a duplicate would inject less than it books)
+    std::vector<int32_t> seen(src->cell, src->cell + nsrc);
+    std::sort(seen.begin(), seen.end());
+    for (int k = 1; k < nsrc; k++)
+      if (seen[k] == seen[k - 1]) return rt_fail(c, RT_EINVAL, "source cell %d is listed twice: sum its rates first", seen[k]);
+  }
   RT_CUDA(c, cudaSetDevice(c->device));
   c->par = *p;
   c->par.kappa = nullptr;
@@ -326,6 +333,44 @@ int rt_debug_tile_timeline(rt_ctx *c, double dt, int64_t ntile_max, uint64_t *ou
   cudaFree(buf);
   if (e != cudaSuccess) return rt_fail(c, RT_ECUDA, "timeline copy: %s", cudaGetErrorString(e));
   return rc;
+}
+
+__global__ void k_tile_of_cell(int64_t C, int TC, const int32_t *__restrict__ perm, int32_t *__restrict__ out) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < C) out[perm[p]] = (int32_t)(p / TC);
+}
+
+int rt_debug_tiles(rt_ctx *c, int mem_kind, int32_t *tile_of_cell, int32_t *tile_desc) {
+  if (!c) return RT_EINVAL;
+  c->err[0] = 0;
+  if (!c->have_mesh) return rt_fail(c, RT_ESTATE, "rt_debug_tiles needs rt_mesh_upload first");
+  RT_CUDA(c, cudaSetDevice(c->device));
+  const rt_layout &l = c->lay;
+  if (tile_of_cell) {
+    int32_t *dst = tile_of_cell, *tmp = nullptr;
+    if (mem_kind == RT_MEM_HOST) { RT_CUDA(c, cudaMalloc(&tmp, 4 * (size_t)c->C)); dst = tmp; }  // (a debug call)
+    k_tile_of_cell<<<(unsigned)((c->C + 255) / 256), 256, 0, c->stream>>>(c->C, c->TC, rt_ptr<int32_t>(c, l.perm), dst);
+    cudaError_t e = cudaSuccess;
+    if (tmp) e = cudaMemcpyAsync(tile_of_cell, tmp, 4 * (size_t)c->C, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (tmp) cudaFree(tmp);
+    if (e != cudaSuccess) return rt_fail(c, RT_ECUDA, "rt_debug_tiles: %s", cudaGetErrorString(e));
+  }
+  if (tile_desc) {
+    std::vector<rt_tile> d((size_t)c->T);
+    std::vector<int32_t> list((size_t)c->T);
+    RT_CUDA(c, cudaMemcpyAsync(d.data(), rt_ptr<rt_tile>(c, l.tiles), sizeof(rt_tile) * (size_t)c->T, cudaMemcpyDeviceToHost, c->stream));
+    RT_CUDA(c, cudaMemcpyAsync(list.data(), rt_ptr<int32_t>(c, l.tlistF), 4 * (size_t)c->T, cudaMemcpyDeviceToHost, c->stream));
+    RT_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int64_t t = 0; t < c->T; t++) {
+      tile_desc[4 * t] = d[t].nown; tile_desc[4 * t + 1] = d[t].nh - d[t].nb;
+      tile_desc[4 * t + 2] = rt_blob_words(c->TC, d[t].nhf, d[t].nown, d[t].nh, d[t].ninc, d[t].nout);
+      tile_desc[4 * t + 3] = 1;
+    }
+    for (int64_t k = 0; k < c->nFA; k++) tile_desc[4 * (int64_t)list[k] + 3] = 0;  // class-A tiles come first in the flux list
+  }
+  RT_CUDA(c, cudaGetLastError());
+  return RT_OK;
 }
 
 int rt_debug_gradients(rt_ctx *c, int mem_kind, double *gN, double *gF) {

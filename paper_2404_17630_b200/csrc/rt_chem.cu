@@ -229,7 +229,7 @@ __global__ void __launch_bounds__(RT_CHEM_BLOCK, 16) k_chem(rt_chem_par P, int64
           trial_out<G> o;
           const double f = trial<G, THERMAL>(P, s, nH, h, r, o);
           attempts++; here++;
-          if (f > P.f_accept) { h = h * P.f_target / f; last = false; continue; }
+          if (!(f <= P.f_accept)) { h = h * P.f_target / f; last = false; continue; }  // (a NaN change is a reject: the cell then runs into the cap)
 #pragma unroll
           for (int g = 0; g < G; g++) { s.N[g] *= o.inv[g]; s.Fx[g] *= o.inv[g]; s.Fy[g] *= o.inv[g]; s.Fz[g] *= o.inv[g]; }
           s.xHII = o.xHII; s.xHeII = o.xHeII; s.xHeIII = o.xHeIII; s.e = o.e;

@@ -1,6 +1,5 @@
 // Kernel-side parameter blocks and launch wrappers shared by the .cu files of librt.so.
 #pragma once
-#include <string.h>
 #include "rt_internal.cuh"
 
 struct rt_chem_par {
@@ -26,21 +25,6 @@ struct rt_geom {
   int variant;           // rt_tuning.variant
   unsigned long long *tl; // rt_debug_tile_timeline: 8 time stamps (ns) per tile of the flux kernel, or null
 };
-
-// the two int32 ids packed in the fourth slot of a faceN / faceW record
-__host__ __device__ inline double rt_pack_lr(int32_t l, int32_t r) {
-  const unsigned long long u = (unsigned long long)(uint32_t)l | ((unsigned long long)(uint32_t)r << 32);
-#ifdef __CUDA_ARCH__
-  return __longlong_as_double((long long)u);
-#else
-  double d; memcpy(&d, &u, 8); return d;
-#endif
-}
-__device__ __forceinline__ void rt_unpack_lr(double d, int32_t &l, int32_t &r) {
-  const unsigned long long u = (unsigned long long)__double_as_longlong(d);
-  l = (int32_t)(uint32_t)(u & 0xffffffffull);
-  r = (int32_t)(uint32_t)(u >> 32);
-}
 
 void rt_launch_chem(rt_ctx *c, const rt_chem_par &P, double dt, double *U);  // all passes + their ledger reductions
 size_t rt_chem_cub_bytes(int64_t C);

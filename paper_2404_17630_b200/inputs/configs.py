@@ -287,4 +287,21 @@ def get(cfg, n=None):
         return config34(n or (256 if cfg == 3 else 384), cfg)
     if cfg == 5:
         return hii_region(n or 44)
+    if cfg == 6:
+        return travelling_wave(n or 128)
     raise ValueError(cfg)
+
+
+def active_at(level, k, lmax):
+    """Individual power-of-two time steps: a cell on level l of a hierarchy with finest level
+    lmax takes a step every 2^(lmax - l) fine steps, so it is active at fine step k iff k is a multiple of
+    that.  level: (C,) ints in [0, lmax].  Returns the (C,) boolean active mask of fine step k."""
+    level = np.asarray(level)
+    return (k % (1 << (lmax - level))) == 0
+
+
+def levels_by_density(nH, lmax):
+    """A synthetic level assignment for tests: denser cells (smaller cells and shorter time steps in a real
+    run) sit on finer levels; quantiles of nH split the cells evenly over the lmax + 1 levels."""
+    q = np.quantile(nH, np.linspace(0, 1, lmax + 2)[1:-1]) if lmax > 0 else np.zeros(0)
+    return np.searchsorted(q, nH).astype(np.int8)

@@ -12,7 +12,9 @@ passes are summed per subcycle.  No GPU needed; only `ncu` on PATH.
 """
 import collections
 import csv
+import hashlib
 import io
+import os
 import subprocess
 import sys
 
@@ -32,6 +34,16 @@ WANT = [("duration [ms]", "gpu__time_duration.sum"), ("grid", "launch__grid_size
         ("shared-memory wavefronts", "l1tex__data_pipe_lsu_wavefronts_mem_shared.sum"),
         ("  of which bank conflicts", "l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum")]
 BYTES = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+
+
+def kernel_source_sha():
+    """sha-256 (16 hex digits) of the kernel sources: profiles/traffic.csv rows carry it, so that bench.py
+    never reports a capture of other kernels as its run's traffic."""
+    h = hashlib.sha256()
+    d = os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc")
+    for f in ("rt_transport.cu", "rt_chem.cu", "rt_internal.cuh", "rt_kernels.cuh"):
+        h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
 
 
 def _ncu(args):
@@ -127,7 +139,8 @@ def main(argv):
         print(sass_table(rep, pat))
     if workload:
         print()
-        print("traffic.csv rows (dram bytes read + written per launch; size classes of one pass summed, first pass of each kernel):")
+        print("traffic.csv rows: workload,kernel,dram bytes read + written per launch (size classes of one pass summed, "
+              "first pass of each kernel),sha of the kernel sources at the time of this reduction")
         for name, launches in traffic.items():
             # the size classes of one pass are consecutive launches with different grids
             grids, tot = [], 0.0
@@ -136,7 +149,7 @@ def main(argv):
                     break
                 grids.append(g)
                 tot += b
-            print("%s,%s,%.0f" % (workload, name, tot))
+            print("%s,%s,%.0f,%s" % (workload, name.replace("void ", "").strip(), tot, kernel_source_sha()))
     return 0
 
 

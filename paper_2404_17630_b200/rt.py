@@ -90,6 +90,8 @@ def lib():
         L.rt_profile.argtypes = [_vp, ctypes.c_int]
         L.rt_profile_read.restype = ctypes.c_int
         L.rt_profile_read.argtypes = [_vp, _vp, _vp]
+        L.rt_debug_tiles.restype = ctypes.c_int
+        L.rt_debug_tiles.argtypes = [_vp, ctypes.c_int, _vp, _vp]
         L.rt_debug_tile_timeline.restype = ctypes.c_int
         L.rt_debug_tile_timeline.argtypes = [_vp, ctypes.c_double, ctypes.c_int64, _vp]
         L.rt_debug_alu_peak.restype = ctypes.c_int
@@ -330,6 +332,15 @@ class Solver:
         _check(self.h, lib().rt_debug_gradients(self.h, RT_MEM_HOST, _vp(gN.ctypes.data), _vp(gF.ctypes.data)),
                "rt_debug_gradients")
         return gN, gF
+
+    def tiles(self):
+        """(tile of every cell in the caller's order (C,), per-tile (owned faces, forward halo, table words,
+        flux launch class) (T, 4)) as numpy int32 arrays (rt_debug_tiles)."""
+        T = self.tile_info()["tiles"]
+        of_cell = np.zeros(self.C, dtype=np.int32)
+        desc = np.zeros((T, 4), dtype=np.int32)
+        _check(self.h, lib().rt_debug_tiles(self.h, RT_MEM_HOST, _vp(of_cell.ctypes.data), _vp(desc.ctypes.data)), "rt_debug_tiles")
+        return of_cell, desc
 
     def tile_timeline(self, dt):
         """One subcycle with per-tile time stamps of the flux kernel: (T, 8) uint64 array (include/rt.h)."""

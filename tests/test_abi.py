@@ -47,3 +47,28 @@ def test_workspace_bytes_and_null_arguments_need_no_device():
     assert L.rt_download(None, None, None) == -1
     assert L.rt_last_error(None) == b"null context"
     L.rt_destroy(None)
+
+
+def test_every_north_star_call_cites_its_passage():
+    """Each of the eight calls of SURVEY 8(b) carries, in the comment right above its declaration, the
+    PAPER.md passage (or the SURVEY convention) that defines it."""
+    src = open(os.path.join(ROOT, "include", "rt.h")).read()
+    for n in ("rt_create", "rt_workspace_bytes", "rt_mesh_upload", "rt_state_init", "rt_step", "rt_download",
+              "rt_last_error", "rt_destroy"):
+        m = re.search(r"/\*((?:(?!\*/).)*)\*/\s*(?:const\s+char|size_t|int|void)\s*\*?\s*%s\s*\(" % n, src, flags=re.S)
+        assert m, n
+        assert re.search(r"PAPER\.md:\d+|SURVEY 8\(b\)", m.group(1)), n
+
+
+def test_the_library_reads_no_environment_variable():
+    csrc = os.path.join(ROOT, "paper_2404_17630_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
+    assert "environ" not in open(os.path.join(ROOT, "paper_2404_17630_b200", "rt.py")).read()
+
+
+def test_tuning_struct_matches_the_header():
+    from paper_2404_17630_b200 import rt
+    assert ctypes.sizeof(rt.rt_tuning) == 4 * (7 + 6 + 1 + 9)
+    L = rt.lib()
+    assert L.rt_set_tuning(None, None) == -1

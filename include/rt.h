@@ -171,6 +171,17 @@ int rt_mesh_upload(rt_ctx *ctx, const rt_mesh *mesh, void *dev_workspace, size_t
  * RT_ECUDA. */
 int rt_state_init(rt_ctx *ctx, const rt_params *p, const rt_state *s0, const rt_sources *src);
 
+/* Individual time steps ("fluxes for interfaces with at least one active neighbour.  For
+ * passive particles, only their conserved quantities are updated, taking into account the fluxes from
+ * the interfaces they share with active cells"; active / passive categories that stay
+ * fixed during the subcycles of one RT step).  Sets the active set of the following rt_step calls:
+ * active = (C) bytes in the caller's cell order, HOST or DEVICE as mem_kind says, non-zero = active;
+ * NULL = every cell (the default, restored by rt_state_init).  A passive cell does no chemistry,
+ * injects no source photons and has no gradient (reading S27); a face between two passive
+ * cells carries no flux; a cell none of whose faces has an active cell is left bit for bit as it was,
+ * and tiles without such cells are skipped.  Needs rt_state_init (else RT_ESTATE).  Synchronises. */
+int rt_set_active(rt_ctx *ctx, int mem_kind, const uint8_t *active);
+
 /* Advances `nsub` subcycles of length dt [same time unit as 1/ctilde * length], each in the order
  * of Fig. 1: thermochemistry with adaptive sub-steps, then two
  * Heun stages of gradients, face fluxes and their application

@@ -46,7 +46,7 @@ int rt_create(rt_ctx **out, int device, void *cuda_stream) {
   if (!c) return RT_ENOMEM;
   c->device = 0; c->stream = 0; c->err[0] = 0; c->C = c->F = c->NR = 0; c->G = 0; c->nghost = 0; c->ws = nullptr;
   c->ws_bytes = 0; c->have_mesh = c->have_state = false; c->nsrc = 0; c->nsub_done = 0; c->launches = 0;
-  c->prof_on = false; c->prof_used = 0; c->dbg_tl = nullptr;
+  c->prof_on = false; c->prof_used = 0; c->dbg_tl = nullptr; c->has_active = false;
   memset(&c->par, 0, sizeof(c->par)); memset(&c->lay, 0, sizeof(c->lay)); memset(&c->tun, 0, sizeof(c->tun));
   c->device = device;
   c->stream = (cudaStream_t)cuda_stream;
@@ -235,12 +235,53 @@ int rt_state_init(rt_ctx *c, const rt_params *p, const rt_state *s0, const rt_so
       c->src_total[g] = s + cc;
     }
   }
+  c->src_cell.assign(src && nsrc > 0 ? src->cell : nullptr, src && nsrc > 0 ? src->cell + nsrc : nullptr);
+  c->src_rate.assign(src && nsrc > 0 ? src->rate : nullptr, src && nsrc > 0 ? src->rate + (size_t)nsrc * G : nullptr);
+  c->has_active = false;  // every cell active until rt_set_active says otherwise
   rt_launch_init_sources(c, cell_dev, nsrc);
   RT_CUDA(c, cudaMemsetAsync(rt_ptr<rt_dev_ledger>(c, l.led), 0, sizeof(rt_dev_ledger), c->stream));
   c->nsub_done = 0;
   RT_CUDA(c, cudaStreamSynchronize(c->stream));
   RT_CUDA(c, cudaGetLastError());
   c->have_state = true;
+  return RT_OK;
+}
+
+int rt_set_active(rt_ctx *c, int mem_kind, const uint8_t *active) {
+  if (!c) return RT_EINVAL;
+  c->err[0] = 0;
+  if (!c->have_state) return rt_fail(c, RT_ESTATE, "rt_set_active needs rt_state_init first");
+  RT_CUDA(c, cudaSetDevice(c->device));
+  const int G = c->G, nsrc = c->nsrc;
+  std::vector<uint8_t> src_on((size_t)(nsrc > 0 ? nsrc : 0), 1);
+  c->has_active = active != nullptr;
+  if (active) {
+    const uint8_t *dev = active;
+    uint8_t *stage = rt_ptr<uint8_t>(c, c->lay.grad);  // 12 G C doubles: free between steps
+    if (mem_kind == RT_MEM_HOST) {
+      RT_CUDA(c, cudaMemcpyAsync(stage, active, (size_t)c->C, cudaMemcpyHostToDevice, c->stream));
+      dev = stage;
+      for (int k = 0; k < nsrc; k++) src_on[k] = active[c->src_cell[k]] != 0;
+    } else {
+      for (int k = 0; k < nsrc; k++)  // (a handful of one-byte copies: the source cells' flags)
+        RT_CUDA(c, cudaMemcpyAsync(&src_on[k], active + c->src_cell[k], 1, cudaMemcpyDeviceToHost, c->stream));
+    }
+    int rc = rt_launch_active(c, dev);
+    if (rc != RT_OK) return rc;
+    RT_CUDA(c, cudaStreamSynchronize(c->stream));
+    RT_CUDA(c, cudaGetLastError());
+  }
+  // photons per unit time the active sources inject (the ledger's `injected` advances by dt times this)
+  for (int g = 0; g < G; g++) {
+    double s = 0.0, cc = 0.0;
+    for (int k = 0; k < nsrc; k++) {
+      if (!src_on[k]) continue;
+      const double x = c->src_rate[(size_t)g * nsrc + k], t = s + x;
+      cc += fabs(s) >= fabs(x) ? (s - t) + x : (x - t) + s;
+      s = t;
+    }
+    c->src_total[g] = s + cc;
+  }
   return RT_OK;
 }
 

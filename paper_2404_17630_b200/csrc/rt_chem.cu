@@ -171,7 +171,7 @@ __global__ void __launch_bounds__(RT_CHEM_BLOCK, 16) k_chem(rt_chem_par P, int64
                                                    const double *__restrict__ kappa, double *__restrict__ part_abs,
                                                    rt_dev_ledger *led, const int32_t *__restrict__ list,
                                                    const int *__restrict__ count, int cap, chem_carry carry,
-                                                   uint8_t *__restrict__ flag) {
+                                                   uint8_t *__restrict__ flag, const uint8_t *__restrict__ cact) {
   constexpr bool THERMAL = (MODE == RT_CHEM_HHE_THERMAL);
   static_assert(RT_CHEM_BLOCK == 32, "block_sum assumes one warp");
   const int64_t n = FIRST ? C : (int64_t)*count;
@@ -179,7 +179,9 @@ __global__ void __launch_bounds__(RT_CHEM_BLOCK, 16) k_chem(rt_chem_par P, int64
   int wcap = 0;
   for (int64_t row = blockIdx.x; row * RT_CHEM_BLOCK < n; row += gridDim.x) {
     const int64_t idx = row * RT_CHEM_BLOCK + threadIdx.x;
-    const bool live = idx < n;
+    // (individual time steps: a passive cell does no chemistry; only the first pass sees such cells)
+    const bool live = idx < n && !(FIRST && cact && !(cact[idx] & 1));
+    if (FIRST && flag && idx < n && !live) flag[idx] = 0;
     double absd[G];
 #pragma unroll
     for (int g = 0; g < G; g++) absd[g] = 0.0;
@@ -307,8 +309,9 @@ static void launch_chem_mode(rt_ctx *c, const rt_chem_par &P, double dt, double 
   const int ncap = MODE == RT_CHEM_FIXED_OPACITY ? 0 : chem_caps(c, caps, 8);
   // pass 0: every cell
   rt_prof_begin(c, RT_K_CHEM);
+  const uint8_t *cact = c->has_active ? rt_ptr<uint8_t>(c, l.cact) : nullptr;
   k_chem<G, MODE, true><<<nrows, RT_CHEM_BLOCK, 0, c->stream>>>(CHEM_ARGS, part, led, nullptr, nullptr, ncap > 0 ? caps[0] : 0, carry,
-                                                              ncap > 0 ? flags : nullptr);
+                                                              ncap > 0 ? flags : nullptr, cact);
   rt_prof_end(c);
   c->launches++;
   rt_reduce2(c, {part, nrows, 1.0, 0, nullptr}, {part, nrows, 1.0, 0, nullptr}, 1);
@@ -327,7 +330,7 @@ static void launch_chem_mode(rt_ctx *c, const rt_chem_par &P, double dt, double 
     cudaMemsetAsync(flags, 0, (size_t)C, c->stream);  // entries beyond the new count must not be selected again
     double *part_p = part + (size_t)p * G * nrows;
     k_chem<G, MODE, false><<<grid, RT_CHEM_BLOCK, 0, c->stream>>>(CHEM_ARGS, part_p, led, lists[p & 1], count, p < ncap ? caps[p] : 0,
-                                                               carry, flags);
+                                                               carry, flags, nullptr);
     rt_prof_end(c);
     c->launches += 3;  // two kernels of the compaction + the pass
     rt_reduce2(c, {part_p, 0, 1.0, 0, count}, {part_p, 0, 1.0, 0, count}, 1);

@@ -68,7 +68,7 @@ struct rt_dev_ledger {  // accumulators on the device (value + compensation)
 struct rt_layout {
   size_t perm, iperm, cellV, Minv, faceC, faceN, faceW, fo, ro, tiles, blob, tlistG, tlistF, xphi, k2cell, k2off, k2row, ghost, led;
   size_t chem_t, chem_h, chem_att, chem_flag, chem_list, chem_count, chem_cub, chem_cub_bytes;
-  size_t Ua, Ub, grad, pacc, xHII, xHeII, xHeIII, eth, nH, kappa, srcidx, srcrate, part, scratch_end;
+  size_t Ua, Ub, grad, pacc, xHII, xHeII, xHeIII, eth, nH, kappa, srcidx, srcrate, part, cact, tact, scratch_end;
   size_t blob_bytes;  // capacity of the blob region
   int64_t xcap;       // rows [G][4] of xphi
   size_t temp;        // start of the setup-time scratch (aliases the state region)
@@ -110,6 +110,9 @@ struct rt_ctx {
   bool have_mesh, have_state;
   rt_params par;
   rt_tuning tun;      // rt_set_tuning (zeros = defaults)
+  bool has_active;    // rt_set_active gave a proper subset: cact / tact are valid
+  std::vector<int32_t> src_cell;  // host copies of the sources (rt_set_active recomputes the injection rate)
+  std::vector<double> src_rate;
   unsigned long long *dbg_tl;  // device buffer of rt_debug_tile_timeline while it runs, else null
   int nsrc;
   double src_total[RT_MAXG];
@@ -150,7 +153,8 @@ static inline size_t rt_smem_grad(int TC, int G, int smax, int hmax, int bmax) {
 static inline size_t rt_smem_flux(int TC, int G, int omax, int fmax, int bmax) {
   const int planes = G > 3 ? G : 3;  // three face records per slot, overwritten by A*Phi of every group
   const int NE = (TC + fmax + 1) & ~1;
-  return (size_t)4 * bmax + (size_t)32 * planes * omax + (size_t)(128 * G + 8) * NE + (size_t)16 * ((TC + 3) / 4);
+  return (size_t)4 * bmax + (size_t)32 * planes * omax + (size_t)(128 * G + 8) * NE + (size_t)16 * ((TC + 3) / 4) +
+         (size_t)((NE + 15) & ~15);  // + the active / touched flags
 }
 #define RT_SMEM_MAX 232448     // 227 KB: the most one block may have on sm_100
 #define RT_SMEM_TARGET 115000  // two blocks per SM (228 KB per SM, 1 KB reserved per block)
@@ -178,6 +182,8 @@ int rt_launch_permute_in(rt_ctx *c, const double *src, double *dst, int rows, in
 int rt_launch_permute_out(rt_ctx *c, const double *src, double *dst, int rows, int stride);
 int rt_launch_init_sources(rt_ctx *c, const int32_t *cell_dev, int nsrc);
 int rt_launch_stored(rt_ctx *c);
+// cact[p] = bit 0 active, bit 1 touched (active or sharing a face with an active cell); tact[t] = OR over the tile's cells
+int rt_launch_active(rt_ctx *c, const uint8_t *active_dev);
 
 // min-image of a difference (periodic dims only)
 __host__ __device__ inline double rt_wrap(double d, double L, int per) { return per ? d - L * rint(d / L) : d; }

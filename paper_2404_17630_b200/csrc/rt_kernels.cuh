@@ -16,6 +16,7 @@ struct rt_geom {
   const uint32_t *blob;
   double *xphi;          // [ninc][G][4] fluxes of the faces that cross tile boundaries
   const double *ghost;
+  const uint8_t *cact, *tact;  // active / touched flags per cell and per tile (rt_set_active), or null: all active
   double box[3];
   int per[3];
   int G, TC, smax, omax, hmax, fmax, bmax, bstride;

@@ -716,6 +716,7 @@ rt_layout rt_make_layout(int64_t C, int64_t F, int G, int flags) {
   // partial sums: chem absorbed [<= 4 nbc + 1][G]; per tile: floor, outflow, inflow [max_tiles][G] each
   l.part = take(8 * (size_t)G * ((4 * RT_CHEM_MAXPASS + 1) * l.nbc + 3 * l.max_tiles + (size_t)G * l.nbc + 64));
   // sub-stepping passes of the chemistry: carried (t, h, attempts), flags, two index lists, cub scratch
+  l.cact = take((size_t)C + 64); l.tact = take((size_t)l.max_tiles + 64);  // active / touched flags per cell, per tile
   l.chem_t = take(8 * (size_t)C); l.chem_h = take(8 * (size_t)C); l.chem_att = take(4 * (size_t)C);
   l.chem_flag = take((size_t)C + 64); l.chem_list = take(8 * (size_t)C); l.chem_count = take(256);
   l.chem_cub_bytes = rt_chem_cub_bytes(C);

@@ -183,7 +183,7 @@ __device__ __forceinline__ void grad_cells(const rt_geom &m, const tile_view &v,
   const int h = (tid >> 1) & 1, p = tid & 1;
   for (int xb = 0; xb < v.ncell; xb += nt >> 2) {  // (whole warps iterate together: the shuffles need every lane)
     const int x = xb + (tid >> 2);
-    const bool on = x < v.ncell;
+    const bool on = x < v.ncell && (!m.cact || (m.cact[v.c0 + x] & 1));  // (a passive cell is skipped: its face state is its cell value)
     const int xx = on ? x : 0;
     const int h0 = on ? (int)v.ho[xx] : 0, h1 = on ? (int)v.ho[xx + 1] : 0;
     const double *ui_p = sm.U + US * xx + 4 * g0 + 2 * h;
@@ -306,6 +306,7 @@ __global__ void __launch_bounds__(128, 4) k_grad(rt_geom m, const double *__rest
   double *sM = sU + US * (m.TC + m.hmax);                  // [TC][6]
   const int tid = threadIdx.x, nt = blockDim.x;
   const unsigned tile = (unsigned)m.tlist[m.tbase + blockIdx.x];
+  if (m.tact && !(m.tact[tile] & 1)) return;  // no active cell in this tile: passive cells have no gradient
   if (tid == 0) { mbar_init(&bar, 1); mbar_init(&bar_blob, 1); }
   __syncthreads();
   // round 1: the tile's blob sits at a fixed stride: header (descriptor) + tables
@@ -400,13 +401,14 @@ __device__ __forceinline__ void pressure_dot_n(const double U[4], const double n
 
 // U_face = U_i + grad U_i . r  (linear extrapolation to the centre of the interface)
 // rec: the cell's (N, Fx, Fy, Fz) followed by its 12 gradient components (field-major), in shared memory
+// (use_grad false: a passive cell, whose gradient is not constructed: its face state is its cell value, S27)
 template <bool SECOND>
 __device__ __forceinline__ void extrapolate(const double *pu, const double *pg, double rx, double ry, double rz, double Uo[4],
-                                            double &Ncentre) {
+                                            double &Ncentre, const bool use_grad = true) {
   const double4 u = ld4(pu);
   Ncentre = u.x;
   Uo[0] = u.x; Uo[1] = u.y; Uo[2] = u.z; Uo[3] = u.w;
-  if (SECOND) {
+  if (SECOND && use_grad) {
     const double4 a = ld4(pg), b = ld4(pg + 4), c = ld4(pg + 8);
     Uo[0] = fma(a.x, rx, fma(a.y, ry, fma(a.z, rz, u.x)));
     Uo[1] = fma(a.w, rx, fma(b.x, ry, fma(b.y, rz, u.y)));
@@ -456,11 +458,29 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
   double *sG = sU + 4 * G * NE;                            // [NE][G][12]
   double *sV = sG + 12 * G * NE;                           // [NE]  cell volumes
   int32_t *sSrc = reinterpret_cast<int32_t *>(sV + NE);    // [TC] source index or -1
+  uint8_t *sAct = reinterpret_cast<uint8_t *>(sSrc + ((m.TC + 3) & ~3));  // [NE] active / touched flags (rt_set_active)
   const unsigned tile = (unsigned)m.tlist[m.tbase + blockIdx.x];
   const int tid = threadIdx.x, nt = blockDim.x;
   const double dt = up.dt, ct = up.ct;
   unsigned long long *tl = m.tl && tid == 0 ? m.tl + 8 * (size_t)tile : nullptr;  // rt_debug_tile_timeline
   if (tl) tl[0] = now_ns();
+  if (m.tact && !(m.tact[tile] & 2)) {
+    // no cell of this tile is active or shares a face with an active cell: none of its faces
+    // carries a flux and none of its cells changes.  The right cells of its outgoing faces still read their
+    // rows of xphi: zeros; the first Heun stage still has to carry the tile's cells into the stage buffer.
+    const rt_tile d = m.tiles[tile];
+    const int64_t c0 = (int64_t)tile * m.TC;
+    const int ncell = (int)(c0 + m.TC < m.C ? m.TC : m.C - c0);
+    double2 *xo = reinterpret_cast<double2 *>(m.xphi + (size_t)(4 * G) * d.xbase);
+    for (int k = tid; k < 2 * G * d.nout; k += nt) xo[k] = make_double2(0.0, 0.0);
+    if (Uout != Uin)
+      for (int k = tid; k < 2 * G * ncell; k += nt)
+        reinterpret_cast<double2 *>(Uout + 4 * G * c0)[k] = reinterpret_cast<const double2 *>(Uin + 4 * G * c0)[k];
+    if (tid < G) {
+      part_out[(size_t)tile * G + tid] = 0.0; part_in[(size_t)tile * G + tid] = 0.0; part_floor[(size_t)tile * G + tid] = 0.0;
+    }
+    return;
+  }
   if (tid == 0) { mbar_init(&bar, 1); mbar_init(&bar_blob, 1); }
   __syncthreads();
   // round 1: the tile's blob sits at a fixed stride: header (descriptor) + tables
@@ -520,6 +540,10 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
       bulk_prefetch_l2(U0 + 4 * G * cp, 32u * G * nc);
     }
   }
+  if (m.cact) {  // the flags of the tile's cells and of its forward halo cells
+    for (int x = tid; x < v.ncell; x += nt) sAct[x] = m.cact[v.c0 + x];
+    for (int h = tid; h < nf; h += nt) sAct[m.TC + h] = m.cact[v.halo[v.nb + h]];
+  }
   mbar_wait(&bar, 0);
   cp_wait_all();
   __syncthreads();
@@ -552,11 +576,18 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
     }
     const int xrr = rin ? xr : xl;
     if (!rin && r != RT_BC_REFLECT) bnd = 1;  // outflow or Dirichlet face: its flux enters a ledger
+    // individual time steps: only a face with an active cell carries a flux
+    const bool aL = !m.cact || (sAct[xl] & 1), aR = rin && (!m.cact || (sAct[xr] & 1));
+    if (!(aL || aR)) {
+#pragma unroll
+      for (int g = 0; g < G; g++) { st2(sF + 2 * (2 * g * OM + s), 0.0, 0.0); st2(sF + 2 * ((2 * g + 1) * OM + s), 0.0, 0.0); }
+      continue;
+    }
 #pragma unroll 1
     for (int g = 0; g < G; g++) {
       double UL[4], UR[4], NL, NR = 0.0;
-      extrapolate<SECOND>(sU + 4 * (xl * G + g), sG + 12 * (xl * G + g), fc.x, fc.y, fc.z, UL, NL);
-      if (rin) extrapolate<SECOND>(sU + 4 * (xrr * G + g), sG + 12 * (xrr * G + g), rRx, rRy, rRz, UR, NR);
+      extrapolate<SECOND>(sU + 4 * (xl * G + g), sG + 12 * (xl * G + g), fc.x, fc.y, fc.z, UL, NL, aL);
+      if (rin) extrapolate<SECOND>(sU + 4 * (xrr * G + g), sG + 12 * (xrr * G + g), rRx, rRy, rRz, UR, NR, aR);
       else if (r == RT_BC_OUTFLOW) { UR[0] = UR[1] = UR[2] = UR[3] = 0.0; }  // vacuum ghost
       else if (r == RT_BC_REFLECT) {
         const double p = 2.0 * (UL[1] * n[0] + UL[2] * n[1] + UL[3] * n[2]);
@@ -649,9 +680,14 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
       incomplete |= __shfl_xor_sync(0xffffffffu, incomplete, o);
     }
     if (!on || p != 0) continue;
+    const int ac = m.cact ? sAct[il] : 3;
+    if (!(ac & 2)) {  // neither the cell nor a neighbour is active: it stays as it is, bit for bit
+      if (!incomplete) { const double4 uc = ld4(sU + 4 * item); st4(Uout + 4 * (v.c0 * G + item), uc.x, uc.y, uc.z, uc.w); }
+      continue;
+    }
     if (incomplete) { st4(pacc + 4 * (v.c0 * G + item), a0, a1, a2, a3); continue; }
     const int32_t si = sSrc[il];
-    const double src = si >= 0 ? srcrate[(size_t)ig * nsrc + si] : 0.0;
+    const double src = si >= 0 && (ac & 1) ? srcrate[(size_t)ig * nsrc + si] : 0.0;  // (a passive cell injects nothing)
     const double add = finish_cell(a0, a1, a2, a3, sV[il], src, ld4(sU + 4 * item), u0, up,
                                    Uout + 4 * (v.c0 * G + item));
     if (add != 0.0) {
@@ -688,13 +724,19 @@ __global__ void __launch_bounds__(RT_FIN_BLOCK) k_finish(int64_t n2, const int32
                                                          const double *__restrict__ cellV,
                                                          const double *__restrict__ Uin, const double *U0, double *Uout,
                                                          const int32_t *__restrict__ srcidx, const double *__restrict__ srcrate,
-                                                         int nsrc, update_par up, double *__restrict__ part_floor) {
+                                                         int nsrc, update_par up, double *__restrict__ part_floor,
+                                                         const uint8_t *__restrict__ cact) {
   __shared__ double red[32];
   const int64_t item = (int64_t)blockIdx.x * RT_FIN_BLOCK + threadIdx.x;
   const int64_t k = item / G;
   const int g = (int)(item - k * G);
   double add = 0.0;
-  if (k < n2) {
+  const int ac = k < n2 && cact ? cact[k2cell[k]] : 3;
+  if (k < n2 && !(ac & 2)) {  // neither the cell nor a neighbour is active: it stays as it is
+    const int64_t i = k2cell[k];
+    const double4 uc = ld4(Uin + 4 * (i * G + g));
+    st4(Uout + 4 * (i * G + g), uc.x, uc.y, uc.z, uc.w);
+  } else if (k < n2) {
     const int64_t i = k2cell[k];
     const int r0 = k2off[k], r1 = k2off[k + 1];
     double *out = Uout + 4 * (i * G + g);
@@ -706,7 +748,7 @@ __global__ void __launch_bounds__(RT_FIN_BLOCK) k_finish(int64_t n2, const int32
       a.x -= p.x; a.y -= p.y; a.z -= p.z; a.w -= p.w;
     }
     const int32_t si = srcidx[i];
-    const double src = si >= 0 ? srcrate[(size_t)g * nsrc + si] : 0.0;
+    const double src = si >= 0 && (ac & 1) ? srcrate[(size_t)g * nsrc + si] : 0.0;
     add = finish_cell(a.x, a.y, a.z, a.w, cellV[i], src, ld4(Uin + 4 * (i * G + g)), ld4(U0 + 4 * (i * G + g)), up, out);
   }
   // fixed-order block sums per group
@@ -828,6 +870,40 @@ __global__ void k_set_sources(int nsrc, const int32_t *__restrict__ cell, const 
   if (k < nsrc) srcidx[iperm[cell[k]]] = k;
 }
 
+// ------------------------------------------------------------------ active sets (individual time steps)
+__global__ void k_active_in(int64_t C, const int32_t *__restrict__ perm, const uint8_t *__restrict__ active, uint8_t *__restrict__ ain) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < C) ain[p] = active[perm[p]] != 0;
+}
+// one block per tile, straight from the tile's tables in global memory: cact = active | touched << 1 per cell
+// (touched: the cell or a cell across one of its faces is active), tact = OR over the tile's cells
+__global__ void __launch_bounds__(128) k_touched(rt_geom m, const uint8_t *__restrict__ ain, uint8_t *__restrict__ cact, uint8_t *__restrict__ tact) {
+  __shared__ int s_or;
+  const int64_t t = blockIdx.x;
+  const uint32_t *B = m.blob + (size_t)t * m.bstride;
+  const rt_tile d = *reinterpret_cast<const rt_tile *>(B);
+  const int64_t c0 = t * m.TC;
+  const int ncell = (int)(c0 + m.TC < m.C ? m.TC : m.C - c0);
+  const uint32_t *ho = B + RT_BLOB_HEAD, *hl = ho + m.TC + 1, *halo = hl + d.nhf + d.nown;
+  if (threadIdx.x == 0) s_or = 0;
+  __syncthreads();
+  for (int x = threadIdx.x; x < ncell; x += blockDim.x) {
+    int f = ain[c0 + x] ? 1 : 0;
+    int touched = f;
+    for (uint32_t k = ho[x]; k < ho[x + 1] && !touched; k++) {
+      const uint32_t nb = hl[k] >> 16;
+      if (nb >= 0xFF00u) continue;
+      const int64_t id = nb < (uint32_t)m.TC ? c0 + nb : (int64_t)halo[nb - m.TC];
+      touched |= ain[id] != 0;
+    }
+    f |= touched << 1;
+    cact[c0 + x] = (uint8_t)f;
+    if (f) atomicOr(&s_or, f);
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) tact[t] = (uint8_t)s_or;
+}
+
 // ------------------------------------------------------------------ host-side launchers
 static inline unsigned blocks_for(int64_t n, int per_block) { return (unsigned)((n + per_block - 1) / per_block); }
 #define DISPATCH_G(Gv, KERNEL, grid, block, smem, stream, ...)                            \
@@ -896,6 +972,8 @@ rt_geom rt_geom_of(const rt_ctx *c) {
   m.tiles = rt_ptr<rt_tile>(c, l.tiles); m.blob = rt_ptr<uint32_t>(c, l.blob);
   m.xphi = rt_ptr<double>(c, l.xphi);
   m.variant = c->tun.variant;
+  m.cact = c->has_active ? rt_ptr<uint8_t>(c, l.cact) : nullptr;
+  m.tact = c->has_active ? rt_ptr<uint8_t>(c, l.tact) : nullptr;
   m.tl = c->dbg_tl;
   m.prefetch_tiles = c->tun.prefetch_tiles > 0 ? c->tun.prefetch_tiles : (c->tun.prefetch_tiles < 0 ? (1 << 30) : 600);
   m.ghost = rt_ptr<double>(c, l.ghost);
@@ -973,7 +1051,7 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
     rt_prof_begin(c, RT_K_UPDATE);
     DISPATCH_G(G, K_FINISH, (unsigned)nfin, RT_FIN_BLOCK, 0, c->stream, c->n2, rt_ptr<int32_t>(c, l.k2cell),
                rt_ptr<int32_t>(c, l.k2off), rt_ptr<int32_t>(c, l.k2row), m.xphi, pacc, m.cellV, Uin, U0, Uout, srcidx, srcrate, c->nsrc, up,
-               p_floor2);
+               p_floor2, m.cact);
     rt_prof_end(c);
     c->launches++;
   }
@@ -1011,6 +1089,15 @@ int rt_launch_step(rt_ctx *c, double dt) {
   c->nsub_done++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return rt_fail(c, RT_ECUDA, "kernel launch: %s", cudaGetErrorString(e));
+  return RT_OK;
+}
+
+int rt_launch_active(rt_ctx *c, const uint8_t *active_dev) {
+  const rt_layout &l = c->lay;
+  uint8_t *ain = rt_ptr<uint8_t>(c, l.pacc);  // C bytes of scratch: pacc is free between steps
+  k_active_in<<<blocks_for(c->C, 256), 256, 0, c->stream>>>(c->C, rt_ptr<int32_t>(c, l.perm), active_dev, ain);
+  k_touched<<<(unsigned)c->T, 128, 0, c->stream>>>(rt_geom_of(c), ain, rt_ptr<uint8_t>(c, l.cact), rt_ptr<uint8_t>(c, l.tact));
+  c->launches += 2;
   return RT_OK;
 }
 

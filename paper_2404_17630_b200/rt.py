@@ -76,6 +76,8 @@ def lib():
         L.rt_mesh_upload.argtypes = [_vp, ctypes.POINTER(rt_mesh), _vp, ctypes.c_size_t]
         L.rt_state_init.restype = ctypes.c_int
         L.rt_state_init.argtypes = [_vp, ctypes.POINTER(rt_params), ctypes.POINTER(rt_state), ctypes.POINTER(rt_sources)]
+        L.rt_set_active.restype = ctypes.c_int
+        L.rt_set_active.argtypes = [_vp, ctypes.c_int, _vp]
         L.rt_step.restype = ctypes.c_int
         L.rt_step.argtypes = [_vp, ctypes.c_double, ctypes.c_int]
         L.rt_download.restype = ctypes.c_int
@@ -237,6 +239,19 @@ def rt_state_init(h, params, state, sources=None):
            "rt_state_init")
 
 
+def rt_set_active(h, active=None):
+    """active: (C,) mask (numpy or torch, host or cuda) of the cells taking part in the next rt_step calls, or None."""
+    if active is None:
+        _check(h, lib().rt_set_active(h, RT_MEM_HOST, None), "rt_set_active")
+        return
+    if _is_torch(active):
+        import torch
+        a = active.to(torch.uint8).contiguous()
+    else:
+        a = np.ascontiguousarray(active, dtype=np.uint8)
+    _check(h, lib().rt_set_active(h, _kind(a), _vp(_addr(a))), "rt_set_active")
+
+
 def rt_step(h, dt, nsub=1):
     _check(h, lib().rt_step(h, float(dt), int(nsub)), "rt_step")
 
@@ -308,6 +323,9 @@ class Solver:
         if params is not None:
             self.params = params
         rt_state_init(self.h, self.params, state, sources)
+
+    def set_active(self, active=None):
+        rt_set_active(self.h, active)
 
     def step(self, dt, nsub=1):
         rt_step(self.h, dt, nsub)

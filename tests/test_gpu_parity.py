@@ -434,3 +434,103 @@ def test_full_size_sampled_cells(oracle_mod, c, n):
     del s, w
     gc.collect()
     torch.cuda.empty_cache()
+
+
+# ------------------------------------------------------------------ individual time steps
+def _untouched(mesh, active):
+    t = active.copy()
+    ok = mesh.right >= 0
+    l, r = mesh.left[ok], mesh.right[ok]
+    np.logical_or.at(t, l, active[r]); np.logical_or.at(t, r, active[l])
+    return ~t
+
+
+@pytest.mark.parametrize("c,n,frac", [(2, 10, 0.4), (3, 10, 0.15), (0, 12, 0.5), (1, 24, 0.3)])
+def test_active_sets_match_the_oracle(oracle_mod, c, n, frac):
+    """rt_set_active (PAPER.md:78, 258, 264-270; reading S27): a random subset of the cells takes the RT step;
+    half of the sources sit in passive cells.  Per-step parity, the ledger, and the cells without an active
+    neighbour bit for bit."""
+    w = cfg.get(c, n)
+    C = w.mesh.ncell
+    rs = np.random.RandomState(5)
+    # blobs of active cells (so that whole tiles are passive) plus scattered ones
+    cen = w.mesh.centroid / np.asarray(w.mesh.box)[:, None]
+    active = (np.sin(5.0 * cen[0]) * np.cos(4.0 * cen[1] + 1.0) + 0.3 * rs.rand(C) > 1.0 - 2.0 * frac)
+    if len(w.sources.cell):
+        active[w.sources.cell[::2]] = True
+        active[w.sources.cell[1::2]] = False
+    assert 0.02 * C < active.sum() < 0.9 * C
+    o, s = _pair(oracle_mod, w)
+    o.step(w.dt, 3); s.step(w.dt, 3)                            # develop a little with every cell active
+    o.set_active(active); s.set_active(active)
+    start, _ = s.download()
+    o.step(w.dt, 2); s.step(w.dt, 2)
+    # per-step parity from the CUDA path's own state (the protocol of test_step_from_developed_state: a cell the
+    # donor cap has just drained holds rounding noise around zero, which one side floors and the other keeps;
+    # run in lockstep, that noise would become the whole stencil of the cells ahead of the front)
+    dev, _ = s.download(); dev["nH"] = w.state.nH
+    o.step(w.dt, 1); s.step(w.dt, 1)
+    got, lg = s.download()
+    o1 = oracle_mod.Oracle(w.mesh, w.params); o1.set_sources(w.sources); o1.set_state(P.as_state(dev)); o1.set_active(active)
+    o1.step(w.dt, 1)
+    e = P.step_errors(w.mesh, w.params.ctilde, dev, o1.get_state(), got)
+    assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
+    assert max(e["xHII"], e["xHeII"], e["xHeIII"]) <= 1e-9 and e["eth"] <= 1e-8, e
+    assert P.ledger_errors(o.ledger(), lg) <= 1e-11
+    stored0 = (w.state.N * w.mesh.volume).sum(1)
+    assert P.budget_residual(lg, stored0).max() <= P.TOL_LEDGER
+    far = _untouched(w.mesh, active)
+    assert far.sum() > 0.05 * C
+    for k in ("N", "F", "xHII", "xHeII", "xHeIII", "eth"):
+        assert np.array_equal(got[k][..., far], start[k][..., far]), k
+    # back to every cell: the next subcycle is again the plain one
+    s.set_active(None)
+    dev, _ = s.download(); dev["nH"] = w.state.nH
+    s.step(w.dt, 1)
+    got, _ = s.download()
+    o1 = oracle_mod.Oracle(w.mesh, w.params); o1.set_sources(w.sources); o1.set_state(P.as_state(dev))
+    o1.step(w.dt, 1)
+    e = P.step_errors(w.mesh, w.params.ctilde, dev, o1.get_state(), got)
+    assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
+
+
+def test_all_active_mask_is_bit_identical_and_device_masks_work():
+    import torch
+    from paper_2404_17630_b200 import rt
+    w = cfg.get(2, 8)
+    a = rt.Solver(w.mesh, w.params); a.init(w.state, w.sources); a.step(w.dt, 4)
+    b = rt.Solver(w.mesh, w.params); b.init(w.state, w.sources)
+    b.set_active(torch.ones(w.mesh.ncell, dtype=torch.bool, device="cuda")); b.step(w.dt, 4)
+    sa, la = a.download(); sb, lb = b.download()
+    for k in sa:
+        assert np.array_equal(sa[k], sb[k]), k
+    assert np.array_equal(la["injected"], lb["injected"]) and np.array_equal(la["absorbed"], lb["absorbed"])
+    mask = np.arange(w.mesh.ncell) % 3 == 0
+    c = rt.Solver(w.mesh, w.params); c.init(w.state, w.sources); c.set_active(mask); c.step(w.dt, 2)
+    d = rt.Solver(w.mesh, w.params); d.init(w.state, w.sources); d.set_active(torch.as_tensor(mask).cuda()); d.step(w.dt, 2)
+    sc, _ = c.download(); sd, _ = d.download()
+    for k in sc:
+        assert np.array_equal(sc[k], sd[k]), k
+
+
+def test_power_of_two_schedule_matches_the_oracle(oracle_mod):
+    """Three levels of a power-of-two hierarchy (inputs.configs.active_at): level-l cells are active every
+    2^(lmax - l) fine steps; two full cycles on both sides."""
+    w = cfg.get(3, 10)
+    lmax = 2
+    level = cfg.levels_by_density(w.state.nH, lmax)
+    o, s = _pair(oracle_mod, w)
+    prev = o.get_state()
+    for k in range(2 * (1 << lmax)):
+        act = cfg.active_at(level, k, lmax)
+        o.set_active(act); s.set_active(act)
+        prev = o.get_state()
+        o.step(w.dt, 1); s.step(w.dt, 1)
+    got, lg = s.download()
+    e = P.step_errors(w.mesh, w.params.ctilde, prev, o.get_state(), got)
+    assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
+    assert max(e["xHII"], e["xHeII"], e["xHeIII"]) <= 1e-9
+    lo = o.ledger()
+    assert P.ledger_errors(lo, lg) <= 1e-11 and lg["substeps_total"] == lo["substeps_total"]
+    stored0 = (w.state.N * w.mesh.volume).sum(1)
+    assert P.budget_residual(lg, stored0).max() <= P.TOL_LEDGER

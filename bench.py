@@ -171,6 +171,35 @@ def algorithmic_bytes(C, F, NR, G, heun=True, chem=True, order=2):
     return {"grad": grad, "stage": stage, "chem": chemb, "subcycle": per_sub}
 
 
+def run_timeline(s, w, name):
+    """Phase durations of the flux kernel per tile (thread 0's device-clock stamps, second Heun stage) and, per
+    multiprocessor, how many tiles are in flight and how many of them are in the face-flux phase."""
+    tl = s.tile_timeline(w.dt).astype(np.int64)
+    tl = tl[tl[:, 5] > 0]
+    d = np.diff(tl[:, :6], axis=1) / 1e3
+    names = ("tables arrive", "data staged", "face fluxes (a3)", "publish + boundary ledger", "gather + update (a4)")
+    out = {"workload": name, "tiles": int(len(tl)), "kernel_span_ms": float((tl[:, 5].max() - tl[:, 0].min()) / 1e6), "phases_us": {}}
+    for i, nm in enumerate(names):
+        out["phases_us"][nm] = {"mean": float(d[:, i].mean()), "p10": float(np.percentile(d[:, i], 10)),
+                                "p50": float(np.percentile(d[:, i], 50)), "p90": float(np.percentile(d[:, i], 90))}
+    out["tile_total_us"] = {"mean": float((tl[:, 5] - tl[:, 0]).mean() / 1e3)}
+    sms = np.unique(tl[:, 6])
+    conc, a3 = [], {}
+    for k in sms[:: max(1, len(sms) // 8)]:
+        m = tl[:, 6] == k
+        span = float(tl[m, 5].max() - tl[m, 0].min())
+        conc.append(float((tl[m, 5] - tl[m, 0]).sum() / span))
+        ev = sorted([(a, 1) for a in tl[m, 2]] + [(b, -1) for b in tl[m, 3]])
+        cur, last = 0, ev[0][0]
+        for t, dl in ev:
+            a3[cur] = a3.get(cur, 0.0) + (t - last) / span / 8.0
+            last, cur = t, cur + dl
+    out["tiles_in_flight_per_sm"] = float(np.mean(conc))
+    out["share_of_time_with_k_tiles_in_a3"] = {str(k): round(v, 3) for k, v in sorted(a3.items())}
+    print(json.dumps({"timeline": out}))
+    return 0
+
+
 def run_alu_peak():
     """fp64-pipe and shared-memory peaks of this GPU, measured by the library's own micro-benchmark
     kernels (csrc/rt_peak.cu), with the clocks sampled while they run."""
@@ -221,6 +250,8 @@ def main():
     ap.add_argument("--tuning", default="", help="rt_tuning fields, e.g. tile_cells=40,variant=2 (experiments)")
     ap.add_argument("--active-frac", type=float, default=1.0,
                     help="individual time steps (rt_set_active): only the cells of the slab x < frac * box take the step")
+    ap.add_argument("--timeline", action="store_true",
+                    help="only record the per-tile phase stamps of the flux kernel (rt_debug_tile_timeline) and print their statistics")
     ap.add_argument("--alu-peak", action="store_true",
                     help="only run the fp64 / shared-memory micro-benchmarks (rt_debug_alu_peak) and print them")
     args = ap.parse_args()
@@ -274,6 +305,8 @@ def main():
     t_build = time.perf_counter() - t_build
     s.step(w.dt, args.warmup)
     torch.cuda.synchronize()
+    if args.timeline:
+        return run_timeline(s, w, workload_name(c, n))
 
     # ---- timed region: K subcycles, state (>= 20 GB at full size) far larger than the 126 MB L2
     sampler = ClockSampler(local)

@@ -237,10 +237,12 @@ def hii_region(n=44):
     box (1.6 kpc)^3, n_H = n0 for r < r0 else n0 (r0/r)^2 with n0 = 3.2 cm^-3, r0 = 91.5 pc,
     T = 100 K, c~ = 1e-3 c, photons injected homogeneously (rate per volume constant) in a sphere
     of radius 0.05 kpc at the centre at 1e50 / 5e48 / 3e48 s^-1 per bin, grey constants from a
-    5e4 K black body.  Stand-ins: n^3 jittered-lattice Voronoi generators replace
-    the paper's 2 x N^3 staggered grid; He mass fraction 0.24; dt from the CFL rule."""
+    5e4 K black body.  Mesh: the paper's 2 x N^3 staggered grid = the Voronoi cells of two
+    interleaved cubic lattices (14-faced cells), generators offset by 5 % of the spacing (seeded) so that the
+    clipped boundary cells are not degenerate; 2 x 44^3 = 170 368 cells at full size.  Not given by the paper
+    (DESIGN.md 4): He mass fraction 0.24; dt from the CFL rule."""
     box = 1.6 * KPC
-    mesh = M.voronoi(n, box, 0.3, SEED_MESH + 5, periodic=False, bc_code=M.BC_OUTFLOW)
+    mesh = M.voronoi(n, box, 0.05, SEED_MESH + 5, periodic=False, bc_code=M.BC_OUTFLOW, stagger=True)
     ct = 1.0e-3 * C_LIGHT
     sig, eps, _ = grey_blackbody(5.0e4)
     p = Params(ngroup=3, ctilde=ct, sigma=sig, eps_heat=eps, chem_mode=CHEM_HHE_THERMAL, y_he=Y_HE)

@@ -14,12 +14,13 @@
 
 extern "C" {
 typedef struct {
-  int32_t n;        // lattice cells per dimension, C = n^3, cell id = (ix*n+iy)*n+iz
+  int32_t n;        // lattice cells per dimension, C = n^3 (2 n^3 if staggered), lattice id = (ix*n+iy)*n+iz
   int32_t periodic; // 1: periodic in all three directions, 0: clipped to the box
   int32_t bc_code;  // `right` code of box faces when not periodic (-1 outflow, -2 reflective)
-  int32_t pad;
+  int32_t stagger;  // 1: two interleaved lattices (body-centred, the "2 x N^3 staggered grid" of PAPER.md:180, 290):
+                    // cell id = sub * n^3 + lattice id, generators at (i + 0.25 + 0.5 sub + jitter*(2u-1)) * box/n
   double box;       // box side
-  double jitter;    // generator = (i + 0.5 + jitter*(2u-1)) * box/n per axis
+  double jitter;    // generator = (i + 0.5 + jitter*(2u-1)) * box/n per axis (not staggered)
   uint64_t seed;
 } mg_params;
 }
@@ -53,33 +54,57 @@ static mg_offsets mg_make_offsets() {
 VC_HD inline double mg_jit(const mg_params& P, int64_t cell, int axis) {
   return P.jitter * (2.0 * mg_u01(P.seed, (uint64_t)axis, (uint64_t)cell) - 1.0);
 }
+// position of a generator in units of the lattice spacing, relative to its lattice site's corner
+VC_HD inline double mg_site(const mg_params& P, int sub) { return P.stagger ? 0.25 + 0.5 * sub : 0.5; }
 
 // Build the Voronoi cell of `cell`; seed position returned in pos.
 VC_HD inline void mg_build(const mg_params& P, const mg_offsets& T, int64_t cell, VCell& c, double pos[3]) {
   const int n = P.n;
   const double h = P.box / n;
-  int iz = (int)(cell % n), iy = (int)((cell / n) % n), ix = (int)(cell / ((int64_t)n * n));
+  const int64_t n3 = (int64_t)n * n * n;
+  const int sub = (int)(cell / n3);
+  const int64_t lat = cell - sub * n3;
+  int iz = (int)(lat % n), iy = (int)((lat / n) % n), ix = (int)(lat / ((int64_t)n * n));
   double ui[3] = {mg_jit(P, cell, 0), mg_jit(P, cell, 1), mg_jit(P, cell, 2)};
-  pos[0] = (ix + 0.5 + ui[0]) * h; pos[1] = (iy + 0.5 + ui[1]) * h; pos[2] = (iz + 0.5 + ui[2]) * h;
+  const double s0 = mg_site(P, sub);
+  pos[0] = (ix + s0 + ui[0]) * h; pos[1] = (iy + s0 + ui[1]) * h; pos[2] = (iz + s0 + ui[2]) * h;
   double lo[3], hi[3];
   for (int a = 0; a < 3; a++) {
     if (P.periodic) { lo[a] = -2.5 * h; hi[a] = 2.5 * h; }
     else { lo[a] = -pos[a]; hi[a] = P.box - pos[a]; }
   }
   vc_init(c, lo, hi);
-  for (int k = 0; k < MG_NOFF; k++) {
-    int jx = ix + T.o[k][0], jy = iy + T.o[k][1], jz = iz + T.o[k][2];
+  auto clip_by = [&](int ox, int oy, int oz, int osub) {
+    int jx = ix + ox, jy = iy + oy, jz = iz + oz;
     if (P.periodic) {
       jx = (jx % n + n) % n; jy = (jy % n + n) % n; jz = (jz % n + n) % n;
-    } else if (jx < 0 || jx >= n || jy < 0 || jy >= n || jz < 0 || jz >= n) continue;
-    int64_t j = ((int64_t)jx * n + jy) * n + jz;
-    double rx = (T.o[k][0] + mg_jit(P, j, 0) - ui[0]) * h;
-    double ry = (T.o[k][1] + mg_jit(P, j, 1) - ui[1]) * h;
-    double rz = (T.o[k][2] + mg_jit(P, j, 2) - ui[2]) * h;
+    } else if (jx < 0 || jx >= n || jy < 0 || jy >= n || jz < 0 || jz >= n) return;
+    const int64_t j = osub * n3 + ((int64_t)jx * n + jy) * n + jz;
+    const double sh = mg_site(P, osub) - s0;  // 0 on the same lattice, +-0.5 across the two
+    double rx = (ox + sh + mg_jit(P, j, 0) - ui[0]) * h;
+    double ry = (oy + sh + mg_jit(P, j, 1) - ui[1]) * h;
+    double rz = (oz + sh + mg_jit(P, j, 2) - ui[2]) * h;
     vc_clip(c, rx, ry, rz, -0.5 * (rx * rx + ry * ry + rz * rz), (int32_t)j);
+  };
+  if (P.stagger) {  // the eight nearest generators sit on the other lattice, at (+-0.5, +-0.5, +-0.5)
+    const int b = sub ? 0 : -1;  // other-lattice offsets o with o + sh = -0.5, +0.5
+    for (int x = b; x <= b + 1; x++)
+      for (int y = b; y <= b + 1; y++)
+        for (int z = b; z <= b + 1; z++) clip_by(x, y, z, 1 - sub);
   }
-  // security: every generator outside the 5x5x5 block is >= (3-2*jitter)h away along one axis
-  double lim = (3.0 - 2.0 * P.jitter) * h;
+  for (int k = 0; k < MG_NOFF; k++) clip_by(T.o[k][0], T.o[k][1], T.o[k][2], sub);
+  if (P.stagger) {  // the rest of the other lattice's 4 x 4 x 4 block (relative offsets -1.5 .. 1.5)
+    const int b = sub ? -1 : -2;
+    for (int x = b; x <= b + 3; x++)
+      for (int y = b; y <= b + 3; y++)
+        for (int z = b; z <= b + 3; z++) {
+          const int in = (x > b && x < b + 3) && (y > b && y < b + 3) && (z > b && z < b + 3);
+          if (!in) clip_by(x, y, z, 1 - sub);
+        }
+  }
+  // security: every generator outside the blocks is >= (3 - 2 jitter) h (same lattice) or (2.5 - 2 jitter) h (the
+  // other lattice) away along one axis
+  double lim = ((P.stagger ? 2.5 : 3.0) - 2.0 * P.jitter) * h;
   for (int q = 0; q < c.nt; q++) {
     double ax = fabs(c.vx[q]), ay = fabs(c.vy[q]), az = fabs(c.vz[q]);
     double m = ax > ay ? (ax > az ? ax : az) : (ay > az ? ay : az);
@@ -154,7 +179,7 @@ static int mg_run(const mg_params* P, int on_device, void* stream, int mode, int
                   double* centroid, const int64_t* offsets, double* area, double* normal, double* fcen,
                   int32_t* left, int32_t* right, int64_t F, int32_t* status_out) {
   if (!P || P->n < 1 || (P->periodic && P->n < 5) || P->jitter < 0.0 || P->jitter > 0.45) return -1;
-  int64_t C = (int64_t)P->n * P->n * P->n;
+  int64_t C = (int64_t)P->n * P->n * P->n * (P->stagger ? 2 : 1);
   mg_offsets T = mg_make_offsets();
   int32_t st[2] = {0, 0};
   if (on_device) {

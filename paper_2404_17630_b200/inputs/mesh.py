@@ -89,7 +89,7 @@ def cartesian(n, box=1.0, periodic=False, bc=(BC_OUTFLOW,) * 6):
 # ----------------------------------------------------------------------------- Voronoi
 class _MgParams(ctypes.Structure):
     _fields_ = [("n", ctypes.c_int32), ("periodic", ctypes.c_int32), ("bc_code", ctypes.c_int32),
-                ("pad", ctypes.c_int32), ("box", ctypes.c_double), ("jitter", ctypes.c_double),
+                ("stagger", ctypes.c_int32), ("box", ctypes.c_double), ("jitter", ctypes.c_double),
                 ("seed", ctypes.c_uint64)]
 
 
@@ -117,11 +117,12 @@ def _ptr(a):
     return ctypes.c_void_p(a.ctypes.data)
 
 
-def voronoi(n, box, jitter, seed, periodic, bc_code=BC_OUTFLOW):
-    """Host build (OpenMP) of the Voronoi mesh of n^3 jittered-lattice generators."""
+def voronoi(n, box, jitter, seed, periodic, bc_code=BC_OUTFLOW, stagger=False):
+    """Host build (OpenMP) of the Voronoi mesh of n^3 jittered-lattice generators, or of 2 n^3 generators
+    on two interleaved lattices (stagger=True: the "2 x N^3 staggered grid" of PAPER.md:180, 290)."""
     lib = meshgen_lib()
-    P = _MgParams(n, int(bool(periodic)), bc_code, 0, box, jitter, seed)
-    C = n ** 3
+    P = _MgParams(n, int(bool(periodic)), bc_code, int(bool(stagger)), box, jitter, seed)
+    C = n ** 3 * (2 if stagger else 1)
     counts = np.zeros(C, dtype=np.int32)
     volume = np.zeros(C)
     centroid = np.zeros((3, C))
@@ -142,7 +143,8 @@ def voronoi(n, box, jitter, seed, periodic, bc_code=BC_OUTFLOW):
     if rc != 0:
         raise RuntimeError("meshgen pass 2 failed rc=%d status=%s" % (rc, st))
     return Mesh(C, F, np.full(3, float(box)), np.full(3, int(bool(periodic)), dtype=np.int32), volume, centroid,
-                area, normal, fcen, left, right, {"kind": "voronoi", "n": n, "h": box / n, "jitter": jitter, "seed": seed})
+                area, normal, fcen, left, right, {"kind": "voronoi", "n": n, "h": box / n, "jitter": jitter, "seed": seed,
+                                                  "stagger": bool(stagger)})
 
 
 def voronoi_device(n, box, jitter, seed, periodic, bc_code=BC_OUTFLOW, device="cuda:0"):

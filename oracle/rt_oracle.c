@@ -19,7 +19,11 @@
  * Pins (tests/test_oracle_*.py, -m "not gpu"): P1 Stroemgren law, P2 budget identity,
  * P3 invariants, P4 beam speed, P5 2x2x2 brute force in numpy, P6 linear-exact gradients,
  * P8 stationarity, P9 rotation covariance, P10 closure values, P11 chemistry closed forms,
- * P12 travelling wave, P13 restart.  See DESIGN.md section 5.
+ * P12 travelling wave, P13 restart, P14 H II region, P15 one tiny sub-step = state + h RHS (helium solve,
+ * heating shares, every cooling term), P16 helium closed forms, P17 photo-heating alone, P18 fixed
+ * opacity halves exactly, P19 the donor cap active on a three-cell chain by hand, P20 active / passive
+ * cells.  No function is "parity unpinned"; the one unpinnable choice is a reading (S23).
+ * section 5.
  */
 #include <math.h>
 #include <stdint.h>

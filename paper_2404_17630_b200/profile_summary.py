@@ -145,7 +145,7 @@ def main(argv):
             # the size classes of one pass are consecutive launches with different grids
             grids, tot = [], 0.0
             for g, b in launches:
-                if g in grids:
+                if g in grids and not name.strip().endswith("k_chem"):   # (the chemistry passes of a subcycle are all summed)
                     break
                 grids.append(g)
                 tot += b

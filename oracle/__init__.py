@@ -25,6 +25,7 @@ def lib():
         L.oracle_set_params.argtypes = [vp, dbl, vp, vp, i32, vp, dbl, dbl, dbl, dbl, dbl, dbl, dbl, i64, i32, i32]
         L.oracle_set_sources.argtypes = [vp, i32, vp, vp]
         L.oracle_set_active.argtypes = [vp, vp]
+        L.oracle_set_precision.argtypes = [vp, i32]
         L.oracle_set_state.argtypes = [vp] * 8
         L.oracle_get_state.argtypes = [vp] * 7
         L.oracle_get_ledger.argtypes = [vp, vp, vp]
@@ -105,6 +106,7 @@ class Oracle:
         self.L.oracle_set_params(self.h, p.ctilde, _p(sg), _p(ep), p.chem_mode, _p(kp), p.T_fixed, p.alphaB_override,
                                  p.y_he, p.f_accept, p.f_target, p.x_floor_rel, p.n_floor, p.max_substeps, p.order,
                                  p.heun)
+        self.L.oracle_set_precision(self.h, int(getattr(p, "mixed", 0)))
 
     def set_sources(self, src):
         cell = np.ascontiguousarray(src.cell, dtype=np.int32)

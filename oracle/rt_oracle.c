@@ -22,7 +22,8 @@
  * P12 travelling wave, P13 restart, P14 H II region, P15 one tiny sub-step = state + h RHS (helium solve,
  * heating shares, every cooling term), P16 helium closed forms, P17 photo-heating alone, P18 fixed
  * opacity halves exactly, P19 the donor cap active on a three-cell chain by hand, P20 active / passive
- * cells.  No function is "parity unpinned"; the one unpinnable choice is a reading (S23).
+ * cells, P21 the mixed-precision mode against the fp64 path (1e-6 per step), exact scale covariance,
+ * differences formed in double.  No function is "parity unpinned"; the one unpinnable choice is a reading (S23).
  * section 5.
  */
 #include <math.h>
@@ -65,6 +66,8 @@ typedef struct oracle_ctx {
   /* params */
   double ctilde, sigma[3 * 8], eps[3 * 8], T_fixed, alphaB_override, y_he, f_accept, f_target, x_floor_rel, n_floor;
   int chem_mode, order, heun; int64_t max_substeps;
+  int mixed;         /* 1: single-precision primitives (reading S28) */
+  float *gNf, *gFf;  /* mixed mode: limited gradients times the cell size, [G][3][C] and [G][3][3][C] */
   double *kappa;
   /* active set of the RT step (reading S27): NULL = every cell is active */
   uint8_t *active;
@@ -395,7 +398,7 @@ void oracle_destroy(oracle_ctx *c) {
   free((void *)c->volume); free((void *)c->centroid); free((void *)c->area); free((void *)c->normal);
   free((void *)c->fcentroid); free((void *)c->left); free((void *)c->right); free(c->ghost); free(c->off);
   free(c->hf_face); free(c->hf_side); free(c->hf_w); free(c->hf_r); free(c->Minv); free(c->kappa);
-  free(c->active); free(c->touched); free(c->src_cell); free(c->src_rate); free(c->N); free(c->Fl); free(c->N0); free(c->Fl0); free(c->xHII);
+  free(c->gNf); free(c->gFf); free(c->active); free(c->touched); free(c->src_cell); free(c->src_rate); free(c->N); free(c->Fl); free(c->N0); free(c->Fl0); free(c->xHII);
   free(c->xHeII); free(c->xHeIII); free(c->eth); free(c->nH); free(c->gN); free(c->gF); free(c->phi);
   free(c);
 }
@@ -434,6 +437,22 @@ void oracle_set_active(oracle_ctx *c, const uint8_t *active) {
 static int is_active(const oracle_ctx *c, int64_t i) { return !c->active || c->active[i]; }
 /* a cell none of whose interfaces has an active cell is left alone altogether: "passive" */
 static int is_touched(const oracle_ctx *c, int64_t i) { return !c->touched || c->touched[i]; }
+
+/* Mixed precision ("primitive variables could be converted to single precision, conserved
+ * quantities and flux summations should remain in double precision", "special care ... to avoid numerical
+ * overflows ... a suitable unit system").  Reading S28: the state U, the face-flux sums, the update, the cap and
+ * the ledgers stay fp64; the gradient estimate, the slope limiter, the states reconstructed at the face centres,
+ * the M1 closure and the Riemann flux are evaluated in fp32, in units that keep every number O(1):
+ * lengths in units of the cell size l_i = V_i^(1/3) (the stored gradient is l_i grad phi, a float), face
+ * states in units of s = max(|N_L|, |N_R|) for N and c~ s for F.  Differences phi_j - phi_i are formed in
+ * fp64 and then rounded, so a small contrast on a large background survives. */
+void oracle_set_precision(oracle_ctx *c, int mixed) {
+  c->mixed = mixed;
+  if (mixed && !c->gNf) {
+    c->gNf = (float *)calloc((size_t)c->G * 3 * c->C, sizeof(float));
+    c->gFf = (float *)calloc((size_t)c->G * 9 * c->C, sizeof(float));
+  }
+}
 
 void oracle_set_sources(oracle_ctx *c, int nsrc, const int32_t *cell, const double *rate) {
   free(c->src_cell); free(c->src_rate);
@@ -639,6 +658,143 @@ static void fluxes(oracle_ctx *c, double dt) {
   }
 }
 
+/* ------------------------------------------------------------------ O3 + O4 in mixed precision (S28) */
+static void gradients_mixed(oracle_ctx *c) {
+  const int64_t C = c->C;
+  const int G = c->G;
+  for (int64_t i = 0; i < C; i++) {
+    const double l = cbrt(c->volume[i]);
+    float Mi[9];
+    for (int a = 0; a < 9; a++) Mi[a] = (float)(c->Minv[9 * i + a] * l * l);
+    for (int g = 0; g < G; g++)
+      for (int q = 0; q < 4; q++) {
+        float *out[3];
+        for (int a = 0; a < 3; a++)
+          out[a] = q == 0 ? &c->gNf[((size_t)g * 3 + a) * C + i] : &c->gFf[(((size_t)g * 3 + (q - 1)) * 3 + a) * C + i];
+        if (c->order < 2 || !is_active(c, i)) { *out[0] = *out[1] = *out[2] = 0.0f; continue; }
+        const double pi = fld(c, g, q, i);
+        /* b = sum w (phi_j - phi_i) and the extreme differences (S8: phi_i itself counts, so hi >= 0 >= lo) */
+        float b[3] = {0, 0, 0}, hid = 0.0f, lod = 0.0f;
+        for (int64_t k = c->off[i]; k < c->off[i + 1]; k++) {
+          double U[4];
+          nbr_state(c, g, i, k, U);
+          const float d = (float)(U[q] - pi);
+          for (int a = 0; a < 3; a++) {
+            const float w = (float)(c->hf_w[3 * k + a] / l);
+            b[a] = b[a] + w * d;
+          }
+          if (d > hid) hid = d;
+          if (d < lod) lod = d;
+        }
+        float gr[3];
+        for (int a = 0; a < 3; a++) gr[a] = Mi[3 * a] * b[0] + Mi[3 * a + 1] * b[1] + Mi[3 * a + 2] * b[2];
+        float alpha = 1.0f;
+        for (int64_t k = c->off[i]; k < c->off[i + 1]; k++) {
+          const float rx = (float)(c->hf_r[3 * k] / l), ry = (float)(c->hf_r[3 * k + 1] / l), rz = (float)(c->hf_r[3 * k + 2] / l);
+          const float d = gr[0] * rx + gr[1] * ry + gr[2] * rz;
+          float psi = 1.0f;
+          if (d > 0.0f) psi = hid / d;
+          else if (d < 0.0f) psi = lod / d;
+          if (psi < alpha) alpha = psi;
+        }
+        for (int a = 0; a < 3; a++) *out[a] = alpha * gr[a];
+      }
+  }
+}
+
+/* cell value (double) and single-precision increment to the centre of face f, fields (N, Fx, Fy, Fz) of
+ * group g in cell i: the face state is (float)cell + inc */
+static void extrapolate_mixed(const oracle_ctx *c, int g, int64_t i, int64_t f, double cell[4], float inc[4]) {
+  const int64_t C = c->C, F = c->F;
+  const double l = cbrt(c->volume[i]);
+  float r[3];
+  for (int a = 0; a < 3; a++)
+    r[a] = (float)(minimg(c->fcentroid[a * F + f] - c->centroid[a * C + i], c->box[a], c->periodic[a]) / l);
+  cell[0] = c->N[(size_t)g * C + i];
+  inc[0] = c->gNf[((size_t)g * 3) * C + i] * r[0] + c->gNf[((size_t)g * 3 + 1) * C + i] * r[1] + c->gNf[((size_t)g * 3 + 2) * C + i] * r[2];
+  for (int q = 0; q < 3; q++) {
+    cell[1 + q] = c->Fl[((size_t)g * 3 + q) * C + i];
+    const float *gq = c->gFf + ((size_t)g * 3 + q) * 3 * C + i;
+    inc[1 + q] = gq[0] * r[0] + gq[C] * r[1] + gq[2 * C] * r[2];
+  }
+}
+
+/* n D.nf of the M1 closure (S1) for the normalised state (n, f), lab frame, single precision */
+static void pressure_mixed(float n, const float f[3], const float nf[3], float out[3]) {
+  const float f2 = f[0] * f[0] + f[1] * f[1] + f[2] * f[2];
+  float den = n * n;
+  if (den < 1e-30f) den = 1e-30f;
+  float x2 = f2 / den; /* (|F| / (c~ N))^2 */
+  if (x2 > 1.0f) x2 = 1.0f;
+  const float chi = (3.0f + 4.0f * x2) / (5.0f + 2.0f * sqrtf(4.0f - 3.0f * x2));
+  const float a = 0.5f * (1.0f - chi) * n;
+  for (int k = 0; k < 3; k++) out[k] = a * nf[k];
+  if (f2 > 0.0f) {
+    const float bb = 0.5f * (3.0f * chi - 1.0f) * n * (f[0] * nf[0] + f[1] * nf[1] + f[2] * nf[2]) / f2;
+    for (int k = 0; k < 3; k++) out[k] = out[k] + bb * f[k];
+  }
+}
+
+static void fluxes_mixed(oracle_ctx *c, double dt) {
+  const int64_t F = c->F;
+  const int G = c->G;
+  const float ctf = (float)c->ctilde;
+  for (int64_t f = 0; f < F; f++) {
+    const int64_t L = c->left[f], R = c->right[f];
+    const float nf[3] = {(float)c->normal[f], (float)c->normal[F + f], (float)c->normal[2 * F + f]};
+    if (!(is_active(c, L) || (R >= 0 && is_active(c, R)))) {
+      for (int k = 0; k < 4 * G; k++) c->phi[(size_t)f * G * 4 + k] = 0.0;
+      continue;
+    }
+    for (int g = 0; g < G; g++) {
+      /* face states UL, UR for the mean and the closure; the jump J = UR - UL takes the cell-value part
+       * in double before rounding, like the differences of the gradient estimate */
+      double cL[4], cR[4];
+      float iL[4], iR[4], UL[4], UR[4], J[4];
+      extrapolate_mixed(c, g, L, f, cL, iL);
+      for (int q = 0; q < 4; q++) UL[q] = (float)cL[q] + iL[q];
+      if (R >= 0) {
+        extrapolate_mixed(c, g, R, f, cR, iR);
+        for (int q = 0; q < 4; q++) { UR[q] = (float)cR[q] + iR[q]; J[q] = (float)(cR[q] - cL[q]) + (iR[q] - iL[q]); }
+      } else if (R == BC_OUTFLOW) {
+        for (int q = 0; q < 4; q++) { UR[q] = 0.0f; J[q] = -UL[q]; }
+      } else if (R == BC_REFLECT) {
+        const float p = UL[1] * nf[0] + UL[2] * nf[1] + UL[3] * nf[2];
+        UR[0] = UL[0]; J[0] = 0.0f;
+        for (int a = 0; a < 3; a++) { J[1 + a] = -2.0f * p * nf[a]; UR[1 + a] = UL[1 + a] + J[1 + a]; }
+      } else {
+        const int kg = BC_DIRICHLET0 - (int)R;
+        for (int q = 0; q < 4; q++) {
+          cR[q] = c->ghost[(size_t)kg * 4 * G + 4 * g + q];
+          UR[q] = (float)cR[q];
+          J[q] = (float)(cR[q] - cL[q]) - iL[q];
+        }
+      }
+      /* units: s for N, c~ s for F, so that every number below is O(1) */
+      float sc = fabsf(UL[0]) > fabsf(UR[0]) ? fabsf(UL[0]) : fabsf(UR[0]);
+      if (sc < 1e-30f) sc = 1e-30f;
+      const float is = 1.0f / sc, ics = 1.0f / (ctf * sc);
+      const float nL = UL[0] * is, nR = UR[0] * is;
+      const float fL[3] = {UL[1] * ics, UL[2] * ics, UL[3] * ics}, fR[3] = {UR[1] * ics, UR[2] * ics, UR[3] * ics};
+      float PL[3], PR[3];
+      pressure_mixed(nL, fL, nf, PL);
+      pressure_mixed(nR, fR, nf, PR);
+      const float pn = 0.5f * ((fL[0] + fR[0]) * nf[0] + (fL[1] + fR[1]) * nf[1] + (fL[2] + fR[2]) * nf[2]) - 0.5f * (J[0] * is);
+      double ph[4];
+      ph[0] = (double)pn * c->ctilde * (double)sc;
+      for (int a = 0; a < 3; a++)
+        ph[1 + a] = (double)(0.5f * (PL[a] + PR[a]) - 0.5f * (J[1 + a] * ics)) * c->ctilde * c->ctilde * (double)sc;
+      /* donor cap (S11): in double, on the cell's own N */
+      const int64_t d = ph[0] > 0.0 ? L : (ph[0] < 0.0 ? R : -1);
+      if (d >= 0) {
+        const double lim = c->N[(size_t)g * c->C + d] * c->volume[d] / (dt * c->area[f]);
+        if (fabs(ph[0]) > lim) ph[0] = ph[0] > 0.0 ? lim : -lim;
+      }
+      for (int q = 0; q < 4; q++) c->phi[((size_t)f * G + g) * 4 + q] = ph[q];
+    }
+  }
+}
+
 /* ------------------------------------------------------------------ O5 + O2: apply, enforce, Heun */
 static void enforce(oracle_ctx *c, int g, int64_t i, double wfloor) {
   const int64_t C = c->C;
@@ -654,9 +810,12 @@ static void enforce(oracle_ctx *c, int g, int64_t i, double wfloor) {
 static void stage(oracle_ctx *c, double dt, double a, double b, double wl, double wfloor) {
   const int64_t C = c->C, F = c->F;
   const int G = c->G;
-  if (c->order >= 2) gradients(c);
-  else { memset(c->gN, 0, (size_t)G * 3 * C * 8); memset(c->gF, 0, (size_t)G * 9 * C * 8); }
-  fluxes(c, dt);
+  if (c->mixed) { gradients_mixed(c); fluxes_mixed(c, dt); }
+  else {
+    if (c->order >= 2) gradients(c);
+    else { memset(c->gN, 0, (size_t)G * 3 * C * 8); memset(c->gF, 0, (size_t)G * 9 * C * 8); }
+    fluxes(c, dt);
+  }
   /* boundary ledgers */
   for (int64_t f = 0; f < F; f++) {
     int64_t R = c->right[f];

@@ -53,6 +53,7 @@ class Params:
     max_substeps: int = 1000000
     order: int = 2
     heun: int = 1
+    mixed: int = 0                  # 1: single-precision primitives, double-precision sums
     kappa: np.ndarray = None        # (C,) FIXED_OPACITY only [1/length]
     ghost_state: np.ndarray = None  # (K, 4G) Dirichlet ghost states (N, Fx, Fy, Fz per group)
 

@@ -443,8 +443,9 @@ static int is_touched(const oracle_ctx *c, int64_t i) { return !c->touched || c-
  * overflows ... a suitable unit system").  Reading S28: the state U, the face-flux sums, the update, the cap and
  * the ledgers stay fp64; the gradient estimate, the slope limiter, the states reconstructed at the face centres,
  * the M1 closure and the Riemann flux are evaluated in fp32, in units that keep every number O(1):
- * lengths in units of the cell size l_i = V_i^(1/3) (the stored gradient is l_i grad phi, a float), face
- * states in units of s = max(|N_L|, |N_R|) for N and c~ s for F.  Differences phi_j - phi_i are formed in
+ * lengths in units of the cell size l_i ~ V_i^(1/3) (the stored gradient is l_i grad phi, a float), face
+ * states in units of s ~ max(|N_L|, |N_R|) for N and c~ s for F; l_i and s are rounded to powers of two, so that
+ * the choice of unit changes no rounding at all (only c~ is not a power of two).  Differences phi_j - phi_i are formed in
  * fp64 and then rounded, so a small contrast on a large background survives. */
 void oracle_set_precision(oracle_ctx *c, int mixed) {
   c->mixed = mixed;
@@ -659,11 +660,20 @@ static void fluxes(oracle_ctx *c, double dt) {
 }
 
 /* ------------------------------------------------------------------ O3 + O4 in mixed precision (S28) */
+/* the units are powers of two: changing units then changes no rounding, it only keeps the exponents in range */
+static double unit_length(double V) { int e; frexp(cbrt(V), &e); return ldexp(1.0, e); }            /* l <= 2 V^(1/3) */
+static float unit_density(float m) {                                                                 /* s <= 2 m */
+  int e;
+  if (!(m >= 1e-30f)) m = 1e-30f;
+  frexpf(m, &e);
+  if (e > 126) e = 126;
+  return ldexpf(1.0f, e);
+}
 static void gradients_mixed(oracle_ctx *c) {
   const int64_t C = c->C;
   const int G = c->G;
   for (int64_t i = 0; i < C; i++) {
-    const double l = cbrt(c->volume[i]);
+    const double l = unit_length(c->volume[i]);
     float Mi[9];
     for (int a = 0; a < 9; a++) Mi[a] = (float)(c->Minv[9 * i + a] * l * l);
     for (int g = 0; g < G; g++)
@@ -706,7 +716,7 @@ static void gradients_mixed(oracle_ctx *c) {
  * group g in cell i: the face state is (float)cell + inc */
 static void extrapolate_mixed(const oracle_ctx *c, int g, int64_t i, int64_t f, double cell[4], float inc[4]) {
   const int64_t C = c->C, F = c->F;
-  const double l = cbrt(c->volume[i]);
+  const double l = unit_length(c->volume[i]);
   float r[3];
   for (int a = 0; a < 3; a++)
     r[a] = (float)(minimg(c->fcentroid[a * F + f] - c->centroid[a * C + i], c->box[a], c->periodic[a]) / l);
@@ -771,11 +781,10 @@ static void fluxes_mixed(oracle_ctx *c, double dt) {
         }
       }
       /* units: s for N, c~ s for F, so that every number below is O(1) */
-      float sc = fabsf(UL[0]) > fabsf(UR[0]) ? fabsf(UL[0]) : fabsf(UR[0]);
-      if (sc < 1e-30f) sc = 1e-30f;
-      const float is = 1.0f / sc, ics = 1.0f / (ctf * sc);
+      const float sc = unit_density(fabsf(UL[0]) > fabsf(UR[0]) ? fabsf(UL[0]) : fabsf(UR[0]));
+      const float is = 1.0f / sc, ict = 1.0f / ctf;
       const float nL = UL[0] * is, nR = UR[0] * is;
-      const float fL[3] = {UL[1] * ics, UL[2] * ics, UL[3] * ics}, fR[3] = {UR[1] * ics, UR[2] * ics, UR[3] * ics};
+      const float fL[3] = {UL[1] * is * ict, UL[2] * is * ict, UL[3] * is * ict}, fR[3] = {UR[1] * is * ict, UR[2] * is * ict, UR[3] * is * ict};
       float PL[3], PR[3];
       pressure_mixed(nL, fL, nf, PL);
       pressure_mixed(nR, fR, nf, PR);
@@ -783,7 +792,7 @@ static void fluxes_mixed(oracle_ctx *c, double dt) {
       double ph[4];
       ph[0] = (double)pn * c->ctilde * (double)sc;
       for (int a = 0; a < 3; a++)
-        ph[1 + a] = (double)(0.5f * (PL[a] + PR[a]) - 0.5f * (J[1 + a] * ics)) * c->ctilde * c->ctilde * (double)sc;
+        ph[1 + a] = (double)(0.5f * (PL[a] + PR[a]) - 0.5f * (J[1 + a] * is * ict)) * c->ctilde * c->ctilde * (double)sc;
       /* donor cap (S11): in double, on the cell's own N */
       const int64_t d = ph[0] > 0.0 ? L : (ph[0] < 0.0 ? R : -1);
       if (d >= 0) {

@@ -246,6 +246,22 @@ int rt_debug_tile_timeline(rt_ctx *ctx, double dt, int64_t ntile_max, uint64_t *
  * reading one chunk, and with a random chunk per lane; the number of multiprocessors.  Synchronises. */
 int rt_debug_alu_peak(rt_ctx *ctx, double *out);
 
+/* The "stored" row of the photon budget, sum over cells of V_i N_(g,i) per group (the identity above rt_ledger), for
+ * callers that may not allocate device memory (CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): no context, no workspace, no cudaMalloc / cudaFree / allocating library call.  The per-block partial
+ * sums live in a file-scope device array of the library (4 MiB per GPU that loads it, held until the process
+ * exits), sized for at most RT_NOALLOC_MAX_CELLS cells: more cells -> RT_EINVAL with a message (use rt_ledger_read
+ * there).  device: CUDA device index; stream: a cudaStream_t or NULL; N_dev: DEVICE (ngroup, ncell) row-major,
+ * caller's cell order; volume_dev: DEVICE (ncell); stored_dev: DEVICE (ngroup), written in stream order (the call
+ * does not synchronise).  err / errlen: optional HOST buffer for the error message.  Every call on a device shares
+ * the array, which keeps the previous call's contents (a call overwrites every row before reading it, nothing has
+ * to be cleared): calls that overlap on the GPU - different streams without a dependency - race on it.  The first
+ * call on a device looks up the array's address (cudaGetSymbolAddress): make it outside stream capture.
+ * Deterministic: fixed summation order. */
+#define RT_NOALLOC_MAX_CELLS (1 << 24)
+int rt_stored_photons_noalloc(int device, void *stream, int64_t ncell, int ngroup, const double *N_dev,
+                              const double *volume_dev, double *stored_dev, char *err, int errlen);
+
 /* Last error message of this context ("" if none); valid until the next call on it.  (No exception or
  * abort crosses the ABI: SURVEY 8(b) error convention.) */
 const char *rt_last_error(const rt_ctx *ctx);

@@ -288,6 +288,29 @@ def rt_debug_alu_peak(h):
     return d
 
 
+RT_NOALLOC_MAX_CELLS = 1 << 24
+
+
+def rt_stored_photons_noalloc(N, volume, out, stream=None):
+    """Sum over cells of V N per group into `out` without any device allocation (include/rt.h): N (G, C),
+    volume (C) and out (G) are contiguous float64 CUDA tensors on one device; nothing is copied or converted
+    here.  Returns the ABI's return code and message (0, "" on success): the call does not synchronise."""
+    for a in (N, volume, out):
+        if not (_is_torch(a) and a.is_cuda and a.is_contiguous() and a.element_size() == 8 and a.is_floating_point()):
+            raise RTError("rt_stored_photons_noalloc takes contiguous float64 CUDA tensors")
+    G, C = int(N.shape[0]), int(N.shape[1])
+    if volume.numel() != C or out.numel() < G:
+        raise RTError("rt_stored_photons_noalloc: volume must have C and out at least G elements")
+    L = lib()
+    L.rt_stored_photons_noalloc.restype = ctypes.c_int
+    L.rt_stored_photons_noalloc.argtypes = [ctypes.c_int, _vp, ctypes.c_int64, ctypes.c_int, _vp, _vp, _vp, ctypes.c_char_p,
+                                            ctypes.c_int]
+    err = ctypes.create_string_buffer(512)
+    rc = L.rt_stored_photons_noalloc(N.device.index or 0, _vp(stream) if stream else None, C, G, _vp(N.data_ptr()),
+                                     _vp(volume.data_ptr()), _vp(out.data_ptr()), err, 512)
+    return rc, err.value.decode()
+
+
 def rt_destroy(h):
     lib().rt_destroy(h)
 

@@ -101,7 +101,12 @@ typedef struct {
   double n_floor;           /* floor on N, ledgered as floor_added (S11) */
   int64_t max_substeps;     /* cap on chemistry attempts per cell and subcycle */
   int32_t kappa_mem_kind;
-  int32_t pad;
+  int32_t mixed;            /* 0: fp64 throughout.  1: mixed precision ("primitive variables ... single
+                             * precision, ... conserved quantities and flux summations ... double precision"): the gradient
+                             * estimate, the limiter, the face states, the M1 closure and the Riemann flux in fp32 in
+                             * power-of-two units; the state, the face-flux sums, the donor cap, the update, the ledgers and
+                             * the chemistry in fp64.  Requires |N|, |F| < 3e38 in the caller's units.  Differs from
+                             * mixed = 0 by ~1e-7 of the local state per subcycle (S28) */
   const double *kappa;      /* (C) FIXED_OPACITY only: absorption coefficient [1/length], caller's order */
 } rt_params;
 

@@ -1,6 +1,7 @@
 // The C ABI of include/rt.h: argument checking, marshalling and stream-ordered copies.
 // All arithmetic of the method lives in rt_chem.cu / rt_transport.cu (per subcycle) and
 // rt_setup.cu (per mesh).
+#include <math.h>
 #include <stdarg.h>
 #include <string.h>
 #include <algorithm>
@@ -140,6 +141,11 @@ int rt_mesh_upload(rt_ctx *c, const rt_mesh *m, void *ws, size_t bytes) {
   RT_CUDA(c, cudaSetDevice(c->device));
   c->C = m->ncell; c->F = m->nface; c->G = m->ngroup; c->nghost = m->nghost;
   for (int a = 0; a < 3; a++) { c->box[a] = m->box[a]; c->per[a] = m->periodic[a] != 0; }
+  {  // mixed precision's length unit: the power of two next above the mean cell size
+    int e;
+    frexp(cbrt(m->box[0] * m->box[1] * m->box[2] / (double)m->ncell), &e);
+    c->l0 = ldexp(1.0, e);
+  }
   // the layout the caller's workspace was sized for: with room for every face's flux if it is that large
   const int devflag = m->mem_kind == RT_MEM_DEVICE ? RT_WS_DEVICE_MESH : 0;
   c->lay = rt_make_layout(c->C, c->F, c->G, devflag | RT_WS_ALL_FACES_CROSS);
@@ -182,6 +188,7 @@ int rt_state_init(rt_ctx *c, const rt_params *p, const rt_state *s0, const rt_so
   if (chem && (!(p->f_accept > 0.0) || !(p->f_target > 0.0) || p->max_substeps < 1))
     return rt_fail(c, RT_EINVAL, "chemistry needs f_accept, f_target > 0 and max_substeps >= 1");
   if (p->chem_mode == RT_CHEM_FIXED_OPACITY && !p->kappa) return rt_fail(c, RT_EINVAL, "FIXED_OPACITY needs kappa");
+  if (p->mixed != 0 && p->mixed != 1) return rt_fail(c, RT_EINVAL, "mixed must be 0 or 1");
   const int nsrc = src ? src->nsrc : 0;
   if (nsrc < 0 || nsrc > 65536 || (nsrc > 0 && (!src->cell || !src->rate)))
     return rt_fail(c, RT_EINVAL, "nsrc must be in [0, 65536] with cell and rate set");
@@ -422,7 +429,10 @@ int rt_debug_gradients(rt_ctx *c, int mem_kind, double *gN, double *gF) {
   RT_CUDA(c, cudaSetDevice(c->device));
   const rt_layout &l = c->lay;
   const int64_t C = c->C;
+  const int mixed = c->par.mixed;  // (always the fp64 gradients, in the caller's units: the mixed mode's are l0-scaled floats)
+  c->par.mixed = 0;
   rt_launch_gradients(c, rt_ptr<double>(c, l.Ua));
+  c->par.mixed = mixed;
   double *grad = rt_ptr<double>(c, l.grad);
   double *stage = rt_ptr<double>(c, l.Ub);  // 4 G C doubles, free between steps; used 3 and 9 rows at a time
   int rc;

@@ -39,7 +39,8 @@
 //     The other cells ("incomplete": k2cell[n2]) get the fluxes of their incoming faces from
 //     xphi[ninc][G][4] in k_finish: rows k2row[k2off[k] .. k2off[k+1]] for cell k2cell[k].
 //   state, cell-major so that a tile is one contiguous run:
-//     Ua, Ub [C][G][4] = (N, Fx, Fy, Fz); grad [C][G][12] (field-major, then direction);
+//     Ua, Ub [C][G][4] = (N, Fx, Fy, Fz); grad [C][G][12] (field-major, then direction; with rt_params.mixed
+//     the same region holds [C][G][12] floats: the gradients times the length unit l0, reading S28);
 //     xHII, xHeII, xHeIII, eth, nH, kappa [C]
 #pragma once
 #include <cuda_runtime.h>
@@ -104,6 +105,7 @@ struct rt_ctx {
   double box[3];
   int per[3];
   int nghost;
+  double l0;          // mixed precision: length unit, the power of two next above the mean cell size cbrt(box volume / C)
   char *ws;
   size_t ws_bytes;
   rt_layout lay;
@@ -150,10 +152,11 @@ __host__ __device__ static inline int rt_blob_words(int TC, int nhf, int nown, i
 static inline size_t rt_smem_grad(int TC, int G, int smax, int hmax, int bmax) {
   return (size_t)4 * bmax + (size_t)64 * smax + (size_t)(32 * G + 16) * (TC + hmax) + (size_t)48 * TC;  // cell rows padded by 16 bytes
 }
-static inline size_t rt_smem_flux(int TC, int G, int omax, int fmax, int bmax) {
+static inline size_t rt_smem_flux(int TC, int G, int omax, int fmax, int bmax, bool mixed = false) {
   const int planes = G > 3 ? G : 3;  // three face records per slot, overwritten by A*Phi of every group
   const int NE = (TC + fmax + 1) & ~1;
-  return (size_t)4 * bmax + (size_t)32 * planes * omax + (size_t)(128 * G + 8) * NE + (size_t)16 * ((TC + 3) / 4) +
+  // per cell: U [G][4] doubles, gradients [G][12] doubles (floats in mixed precision), the volume
+  return (size_t)4 * bmax + (size_t)32 * planes * omax + (size_t)((mixed ? 80 : 128) * G + 8) * NE + (size_t)16 * ((TC + 3) / 4) +
          (size_t)((NE + 15) & ~15);  // + the active / touched flags
 }
 #define RT_SMEM_MAX 232448     // 227 KB: the most one block may have on sm_100

@@ -25,6 +25,8 @@ struct rt_geom {
   int prefetch_tiles;    // the tile kernels ask L2 for the data of tile t + prefetch_tiles
   int variant;           // rt_tuning.variant
   unsigned long long *tl; // rt_debug_tile_timeline: 8 time stamps (ns) per tile of the flux kernel, or null
+  // mixed precision (rt_params.mixed): the length unit l0, a power of two near the mean cell size
+  double il0, l0sq;      // 1 / l0, l0^2 (products with them are formed in double, then rounded: exact, and safe in range)
 };
 
 void rt_launch_chem(rt_ctx *c, const rt_chem_par &P, double dt, double *U);  // all passes + their ledger reductions

@@ -292,7 +292,125 @@ __device__ __forceinline__ void grad_cells(const rt_geom &m, const tile_view &v,
   }
 }
 
-template <int G>
+// ---- mixed precision (rt_params.mixed, reading S28): the same lane mapping; the differences phi_j - phi_i are
+// formed in double and rounded, everything after them is single precision in the length unit l0 (a power of
+// two: the scaling is exact).  Stored: l0 * (limited gradient), 12 floats per (cell, group).
+__device__ __forceinline__ float shxf(float v, int lane_mask) { return __shfl_xor_sync(0xffffffffu, v, lane_mask); }
+__device__ __forceinline__ float flip_signf(float x, int sgn) { return __int_as_float(__float_as_int(x) ^ sgn); }
+
+template <int G, int GB, bool BND>
+__device__ __forceinline__ void grad_cells_mixed(const rt_geom &m, const tile_view &v, const grad_smem &sm, const int g0,
+                                                 float *__restrict__ grad, const int tid, const int nt) {
+  constexpr int US = 4 * G + 2;
+  const int h = (tid >> 1) & 1, p = tid & 1;
+  const double il0 = m.il0;
+  for (int xb = 0; xb < v.ncell; xb += nt >> 2) {
+    const int x = xb + (tid >> 2);
+    const bool on = x < v.ncell && (!m.cact || (m.cact[v.c0 + x] & 1));
+    const int xx = on ? x : 0;
+    const int h0 = on ? (int)v.ho[xx] : 0, h1 = on ? (int)v.ho[xx + 1] : 0;
+    const double *ui_p = sm.U + US * xx + 4 * g0 + 2 * h;
+    double ui[GB][2];
+    float b[GB][2][3], hi[GB][2], lo[GB][2];  // sums and the extreme differences (phi_i itself counts: hi >= 0 >= lo)
+#pragma unroll
+    for (int g = 0; g < GB; g++) {
+      const double2 t = ld2(ui_p + 4 * g);
+      ui[g][0] = t.x; ui[g][1] = t.y;
+#pragma unroll
+      for (int f = 0; f < 2; f++) { b[g][f][0] = b[g][f][1] = b[g][f][2] = 0.0f; hi[g][f] = lo[g][f] = 0.0f; }
+    }
+#pragma unroll 2
+    for (int k = h0 + p; k < h1; k += 2) {
+      const uint32_t e = v.hl[k];
+      const int s = (int)(e & 0x7fffu);
+      const uint32_t nb = e >> 16;
+      const int sgn = (int)((e & 0x8000u) << 16);
+      const double2 wl = ld2(sm.Wl + 2 * s);
+      const double wzz = sm.Wh[2 * s];
+      const float wx = flip_signf(__double2float_rn(wl.x * il0), sgn), wy = flip_signf(__double2float_rn(wl.y * il0), sgn),
+                  wz = flip_signf(__double2float_rn(wzz * il0), sgn);  // w / l0: dimensionless
+      double2 uj[GB];
+      if (!BND || nb < 0xFF00u) {
+        const double *q = sm.U + US * (int)nb + 4 * g0 + 2 * h;
+#pragma unroll
+        for (int g = 0; g < GB; g++) uj[g] = ld2(q + 4 * g);
+      } else {
+        const int code = (int)nb - 0x10000;
+#pragma unroll
+        for (int g = 0; g < GB; g++) {
+          const double4 Ui = ld4(sm.U + US * xx + 4 * (g0 + g));
+          const double4 gh = ghost_for_gradient(code, Ui, m.faceN, m.F, v.fbase + s, m.ghost, G, g0 + g);
+          uj[g] = h ? make_double2(gh.z, gh.w) : make_double2(gh.x, gh.y);
+        }
+      }
+#pragma unroll
+      for (int g = 0; g < GB; g++) {
+        const float d0 = __double2float_rn(uj[g].x - ui[g][0]), d1 = __double2float_rn(uj[g].y - ui[g][1]);
+        b[g][0][0] = fmaf(wx, d0, b[g][0][0]); b[g][0][1] = fmaf(wy, d0, b[g][0][1]); b[g][0][2] = fmaf(wz, d0, b[g][0][2]);
+        b[g][1][0] = fmaf(wx, d1, b[g][1][0]); b[g][1][1] = fmaf(wy, d1, b[g][1][1]); b[g][1][2] = fmaf(wz, d1, b[g][1][2]);
+        hi[g][0] = fmaxf(hi[g][0], d0); hi[g][1] = fmaxf(hi[g][1], d1);
+        lo[g][0] = fminf(lo[g][0], d0); lo[g][1] = fminf(lo[g][1], d1);
+      }
+    }
+    // M^-1 in units of l0^-2
+    const double *Mi = sm.M + 6 * xx;
+    const double2 ma = ld2(Mi), mb = ld2(Mi + 2), mc = ld2(Mi + 4);
+    const float m00 = __double2float_rn(ma.x * m.l0sq), m01 = __double2float_rn(ma.y * m.l0sq), m02 = __double2float_rn(mb.x * m.l0sq),
+                m11 = __double2float_rn(mb.y * m.l0sq), m12 = __double2float_rn(mc.x * m.l0sq), m22 = __double2float_rn(mc.y * m.l0sq);
+    float gr[GB][2][3];
+#pragma unroll
+    for (int g = 0; g < GB; g++)
+#pragma unroll
+      for (int f = 0; f < 2; f++) {
+        const float b0 = b[g][f][0] + shxf(b[g][f][0], 1), b1 = b[g][f][1] + shxf(b[g][f][1], 1), b2 = b[g][f][2] + shxf(b[g][f][2], 1);
+        hi[g][f] = fmaxf(hi[g][f], shxf(hi[g][f], 1));
+        lo[g][f] = fminf(lo[g][f], shxf(lo[g][f], 1));
+        gr[g][f][0] = m00 * b0 + m01 * b1 + m02 * b2;
+        gr[g][f][1] = m01 * b0 + m11 * b1 + m12 * b2;
+        gr[g][f][2] = m02 * b0 + m12 * b1 + m22 * b2;
+      }
+    float dmx[GB][2], dmn[GB][2];
+#pragma unroll
+    for (int g = 0; g < GB; g++) dmx[g][0] = dmx[g][1] = dmn[g][0] = dmn[g][1] = 0.0f;
+#pragma unroll 2
+    for (int k = h0 + p; k < h1; k += 2) {
+      const uint32_t e = v.hl[k];
+      const int s = (int)(e & 0x7fffu);
+      const double2 cl = ld2(sm.Cl + 2 * s);
+      double cx = cl.x, cy = cl.y, cz = sm.Ch[2 * s];
+      if (e & 0x8000u) {  // seen from the right cell the face centre is c - kappa w
+        const double2 wl = ld2(sm.Wl + 2 * s), wh = ld2(sm.Wh + 2 * s);
+        cx = fma(-wh.y, wl.x, cx); cy = fma(-wh.y, wl.y, cy); cz = fma(-wh.y, wh.x, cz);
+      }
+      const float rx = __double2float_rn(cx * il0), ry = __double2float_rn(cy * il0), rz = __double2float_rn(cz * il0);
+#pragma unroll
+      for (int g = 0; g < GB; g++)
+#pragma unroll
+        for (int f = 0; f < 2; f++) {
+          const float d = gr[g][f][0] * rx + gr[g][f][1] * ry + gr[g][f][2] * rz;
+          dmx[g][f] = fmaxf(dmx[g][f], d); dmn[g][f] = fminf(dmn[g][f], d);
+        }
+    }
+#pragma unroll
+    for (int g = 0; g < GB; g++) {
+      float o[6];
+#pragma unroll
+      for (int f = 0; f < 2; f++) {
+        const float dx = fmaxf(dmx[g][f], shxf(dmx[g][f], 1)), dn = fminf(dmn[g][f], shxf(dmn[g][f], 1));
+        float a = 1.0f;
+        if (dx > 0.0f) a = fminf(a, __fdiv_rn(hi[g][f], dx));
+        if (dn < 0.0f) a = fminf(a, __fdiv_rn(lo[g][f], dn));
+        o[3 * f] = a * gr[g][f][0]; o[3 * f + 1] = a * gr[g][f][1]; o[3 * f + 2] = a * gr[g][f][2];
+      }
+      if (on && ((g0 + g) & 1) == p) {
+        float2 *out = reinterpret_cast<float2 *>(grad + 12 * ((v.c0 + x) * G + g0 + g) + 6 * h);
+        out[0] = make_float2(o[0], o[1]); out[1] = make_float2(o[2], o[3]); out[2] = make_float2(o[4], o[5]);
+      }
+    }
+  }
+}
+
+template <int G, bool MIXED>
 __global__ void __launch_bounds__(128, 4) k_grad(rt_geom m, const double *__restrict__ U, double *__restrict__ grad) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar, bar_blob;
@@ -372,7 +490,16 @@ __global__ void __launch_bounds__(128, 4) k_grad(rt_geom m, const double *__rest
 #pragma unroll
   for (int g0 = 0; g0 < G; g0 += 3) {
     constexpr int REM = G % 3;
-    if (g0 + 3 <= G) {
+    if (MIXED) {
+      float *gf = reinterpret_cast<float *>(grad);
+      if (g0 + 3 <= G) {
+        if (v.bnd) grad_cells_mixed<G, 3, true>(m, v, sm, g0, gf, tid, nt);
+        else grad_cells_mixed<G, 3, false>(m, v, sm, g0, gf, tid, nt);
+      } else if (REM > 0) {
+        if (v.bnd) grad_cells_mixed<G, REM ? REM : 1, true>(m, v, sm, g0, gf, tid, nt);
+        else grad_cells_mixed<G, REM ? REM : 1, false>(m, v, sm, g0, gf, tid, nt);
+      }
+    } else if (g0 + 3 <= G) {
       if (v.bnd) grad_cells<G, 3, true>(m, v, sm, g0, grad, tid, nt);
       else grad_cells<G, 3, false>(m, v, sm, g0, grad, tid, nt);
     } else if (REM > 0) {
@@ -437,7 +564,37 @@ __device__ __forceinline__ double finish_cell(double a0, double a1, double a2, d
   return add;
 }
 
-template <int G, bool SECOND>
+// ---- mixed precision (rt_params.mixed, reading S28): single-precision closure in per-face units
+__device__ __forceinline__ float4 ldf4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
+// the power of two next above mx (clamped to the normal range) and its reciprocal: the unit of N at a face
+__device__ __forceinline__ void unit_density(float mx, float &sc, float &is) {
+  if (!(mx >= 1e-30f)) mx = 1e-30f;
+  int eb = ((__float_as_int(mx) >> 23) & 0xff) + 1;  // mx = 1.x * 2^(eb - 128)
+  eb = eb > 253 ? 253 : eb;
+  sc = __int_as_float(eb << 23);
+  is = __int_as_float((254 - eb) << 23);
+}
+// n D.nf for the normalised state (n, f = F / (c~ s)), lab frame (S1)
+__device__ __forceinline__ void pressure_dot_n_f(float n, const float f[3], const float nf[3], float out[3]) {
+  const float f2 = f[0] * f[0] + f[1] * f[1] + f[2] * f[2];
+  const float den = fmaxf(n * n, 1e-30f);
+  const float x2 = fminf(__fdiv_rn(f2, den), 1.0f);
+  const float chi = __fdiv_rn(3.0f + 4.0f * x2, 5.0f + 2.0f * __fsqrt_rn(4.0f - 3.0f * x2));
+  const float a = 0.5f * (1.0f - chi) * n;
+  float bb = 0.0f;
+  if (f2 > 0.0f) bb = __fdiv_rn(0.5f * (3.0f * chi - 1.0f) * n * (f[0] * nf[0] + f[1] * nf[1] + f[2] * nf[2]), f2);
+  out[0] = fmaf(bb, f[0], a * nf[0]); out[1] = fmaf(bb, f[1], a * nf[1]); out[2] = fmaf(bb, f[2], a * nf[2]);
+}
+// the single-precision increments grad . r of (N, Fx, Fy, Fz) to a face centre; pg: 12 floats, field-major
+__device__ __forceinline__ void increments_f(const float *pg, float rx, float ry, float rz, float inc[4]) {
+  const float4 a = ldf4(pg), b = ldf4(pg + 4), c = ldf4(pg + 8);
+  inc[0] = a.x * rx + a.y * ry + a.z * rz;
+  inc[1] = a.w * rx + b.x * ry + b.y * rz;
+  inc[2] = b.z * rx + b.w * ry + c.x * rz;
+  inc[3] = c.y * rx + c.z * ry + c.w * rz;
+}
+
+template <int G, bool SECOND, bool MIXED>
 __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__restrict__ Uin, const double *__restrict__ grad,
                                                  const double *U0, double *Uout, const int32_t *__restrict__ srcidx,
                                                  const double *__restrict__ srcrate, int nsrc, update_par up,
@@ -455,8 +612,9 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
                                                            // 16-byte halves; the slot's thread then overwrites
                                                            // half-planes 2g, 2g + 1 with A * (Phi_N, Phi_F) of group g
   double *sU = sF + 4 * NP * OM;                           // [NE][G][4]
+  constexpr int GW = MIXED ? 6 : 12;                       // doubles per (cell, group) of gradients (mixed: 12 floats)
   double *sG = sU + 4 * G * NE;                            // [NE][G][12]
-  double *sV = sG + 12 * G * NE;                           // [NE]  cell volumes
+  double *sV = sG + GW * G * NE;                           // [NE]  cell volumes
   int32_t *sSrc = reinterpret_cast<int32_t *>(sV + NE);    // [TC] source index or -1
   uint8_t *sAct = reinterpret_cast<uint8_t *>(sSrc + ((m.TC + 3) & ~3));  // [NE] active / touched flags (rt_set_active)
   const unsigned tile = (unsigned)m.tlist[m.tbase + blockIdx.x];
@@ -495,7 +653,7 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
   // tables locate (gathers: forward halo cells), all in flight together
   if (tid == 0) {
     const unsigned nsb = (4u * v.ncell + 15u) & ~15u, nvb = (8u * v.ncell + 15u) & ~15u;  // srcidx and cellV are padded
-    mbar_expect(&bar, 96u * v.nown + (SECOND ? 128u : 32u) * G * v.ncell + nvb + nsb);
+    mbar_expect(&bar, 96u * v.nown + (SECOND ? 32u + 8u * GW : 32u) * G * v.ncell + nvb + nsb);
     bulk_g2s(sF, m.faceC + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sF + 2 * OM, m.faceC + 2 * m.F + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sF + 4 * OM, m.faceN + 2 * v.fbase, 16u * v.nown, &bar);
@@ -503,7 +661,7 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
     bulk_g2s(sF + 8 * OM, m.faceW + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sF + 10 * OM, m.faceW + 2 * m.F + 2 * v.fbase, 16u * v.nown, &bar);
     bulk_g2s(sU, Uin + 4 * G * v.c0, 32u * G * v.ncell, &bar);
-    if (SECOND) bulk_g2s(sG, grad + 12 * G * v.c0, 96u * G * v.ncell, &bar);
+    if (SECOND) bulk_g2s(sG, grad + GW * G * v.c0, 8u * GW * G * v.ncell, &bar);
     bulk_g2s(sV, m.cellV + v.c0, nvb, &bar);
     bulk_g2s(sSrc, srcidx + v.c0, nsb, &bar);
   }
@@ -514,7 +672,7 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
     const int h = k / (G + 1), part = k - h * (G + 1);
     const int64_t id = v.halo[v.nb + h];
     if (part < G) {
-      if (SECOND) cp_run<6>(sG + 12 * (G * (m.TC + h) + part), grad + 12 * (G * id + part));
+      if (SECOND) cp_run<GW / 2>(sG + GW * (G * (m.TC + h) + part), grad + GW * (G * id + part));
     } else {
       cp_run<2 * G>(sU + 4 * G * (m.TC + h), Uin + (int64_t)(4 * G) * id);
       cp8(sV + m.TC + h, m.cellV + id);
@@ -536,7 +694,7 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
         bulk_prefetch_l2(m.faceW + 2 * m.F * hf + 2 * dp.fbase, 16u * dp.nown);
       }
       bulk_prefetch_l2(Uin + 4 * G * cp, 32u * G * nc);
-      if (SECOND) bulk_prefetch_l2(grad + 12 * G * cp, 96u * G * nc);
+      if (SECOND) bulk_prefetch_l2(grad + GW * G * cp, 8u * GW * G * nc);
       bulk_prefetch_l2(U0 + 4 * G * cp, 32u * G * nc);
     }
   }
@@ -583,6 +741,65 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
       for (int g = 0; g < G; g++) { st2(sF + 2 * (2 * g * OM + s), 0.0, 0.0); st2(sF + 2 * ((2 * g + 1) * OM + s), 0.0, 0.0); }
       continue;
     }
+    if (MIXED) {
+      // single precision in the units l0 (lengths) and, per face and group, s (densities): reading S28
+      const float *sGf = reinterpret_cast<const float *>(sG);
+      const float nf[3] = {__double2float_rn(fn.x), __double2float_rn(fn.y), __double2float_rn(fn.z)};
+      const float rLx = __double2float_rn(fc.x * m.il0), rLy = __double2float_rn(fc.y * m.il0), rLz = __double2float_rn(fc.z * m.il0);
+      const float qRx = __double2float_rn(rRx * m.il0), qRy = __double2float_rn(rRy * m.il0), qRz = __double2float_rn(rRz * m.il0);
+      const float ict = __fdiv_rn(1.0f, __double2float_rn(ct));
+      const double rdt = fast_rcp(dt), Act = A * ct;
+      const double photL = sV[xl] * rdt, photR = rin ? sV[xr] * rdt : 0.0;  // A |Phi_N| <= N V / dt (donor cap, S11)
+#pragma unroll 1
+      for (int g = 0; g < G; g++) {
+        const double4 cl = ld4(sU + 4 * (xl * G + g));
+        double4 cr = make_double4(0.0, 0.0, 0.0, 0.0);
+        float iL[4] = {0.0f, 0.0f, 0.0f, 0.0f}, iR[4] = {0.0f, 0.0f, 0.0f, 0.0f}, UL[4], UR[4], J[4];
+        if (SECOND && aL) increments_f(sGf + 12 * (xl * G + g), rLx, rLy, rLz, iL);
+        UL[0] = __double2float_rn(cl.x) + iL[0]; UL[1] = __double2float_rn(cl.y) + iL[1];
+        UL[2] = __double2float_rn(cl.z) + iL[2]; UL[3] = __double2float_rn(cl.w) + iL[3];
+        if (rin) {
+          cr = ld4(sU + 4 * (xrr * G + g));
+          if (SECOND && aR) increments_f(sGf + 12 * (xrr * G + g), qRx, qRy, qRz, iR);
+          UR[0] = __double2float_rn(cr.x) + iR[0]; UR[1] = __double2float_rn(cr.y) + iR[1];
+          UR[2] = __double2float_rn(cr.z) + iR[2]; UR[3] = __double2float_rn(cr.w) + iR[3];
+          // the jump: the cell values' part in double before rounding
+          J[0] = __double2float_rn(cr.x - cl.x) + (iR[0] - iL[0]); J[1] = __double2float_rn(cr.y - cl.y) + (iR[1] - iL[1]);
+          J[2] = __double2float_rn(cr.z - cl.z) + (iR[2] - iL[2]); J[3] = __double2float_rn(cr.w - cl.w) + (iR[3] - iL[3]);
+        } else if (r == RT_BC_OUTFLOW) {
+#pragma unroll
+          for (int q = 0; q < 4; q++) { UR[q] = 0.0f; J[q] = -UL[q]; }
+        } else if (r == RT_BC_REFLECT) {
+          const float p = UL[1] * nf[0] + UL[2] * nf[1] + UL[3] * nf[2];
+          UR[0] = UL[0]; J[0] = 0.0f;
+#pragma unroll
+          for (int a = 0; a < 3; a++) { J[1 + a] = -2.0f * p * nf[a]; UR[1 + a] = UL[1 + a] + J[1 + a]; }
+        } else {
+          const double4 gs = ld4(m.ghost + ((size_t)(RT_BC_DIRICHLET0 - r) * G + g) * 4);
+          UR[0] = __double2float_rn(gs.x); UR[1] = __double2float_rn(gs.y); UR[2] = __double2float_rn(gs.z); UR[3] = __double2float_rn(gs.w);
+          J[0] = __double2float_rn(gs.x - cl.x) - iL[0]; J[1] = __double2float_rn(gs.y - cl.y) - iL[1];
+          J[2] = __double2float_rn(gs.z - cl.z) - iL[2]; J[3] = __double2float_rn(gs.w - cl.w) - iL[3];
+        }
+        float sc, is;
+        unit_density(fmaxf(fabsf(UL[0]), fabsf(UR[0])), sc, is);
+        const float nL = UL[0] * is, nR = UR[0] * is;
+        const float fL[3] = {UL[1] * is * ict, UL[2] * is * ict, UL[3] * is * ict};
+        const float fR[3] = {UR[1] * is * ict, UR[2] * is * ict, UR[3] * is * ict};
+        float PL[3], PR[3];
+        pressure_dot_n_f(nL, fL, nf, PL);
+        pressure_dot_n_f(nR, fR, nf, PR);
+        const float pn = 0.5f * ((fL[0] + fR[0]) * nf[0] + (fL[1] + fR[1]) * nf[1] + (fL[2] + fR[2]) * nf[2]) - 0.5f * (J[0] * is);
+        const float p1 = 0.5f * (PL[0] + PR[0]) - 0.5f * (J[1] * is * ict), p2 = 0.5f * (PL[1] + PR[1]) - 0.5f * (J[2] * is * ict),
+                    p3 = 0.5f * (PL[2] + PR[2]) - 0.5f * (J[3] * is * ict);
+        // back to the caller's units and to double: A Phi_N = A c~ s phi_N, A Phi_F = A c~^2 s phi_F
+        const double sN = Act * (double)sc, sFl = sN * ct;
+        double aphi = (double)pn * sN;
+        if (aphi > 0.0) aphi = dmin2(aphi, cl.x * photL);
+        else if (rin) aphi = -dmin2(-aphi, cr.x * photR);
+        st2(sF + 2 * (2 * g * OM + s), aphi, (double)p1 * sFl);
+        st2(sF + 2 * ((2 * g + 1) * OM + s), (double)p2 * sFl, (double)p3 * sFl);
+      }
+    } else
 #pragma unroll 1
     for (int g = 0; g < G; g++) {
       double UL[4], UR[4], NL, NR = 0.0;
@@ -917,9 +1134,12 @@ static inline unsigned blocks_for(int64_t n, int per_block) { return (unsigned)(
     case 7: KERNEL(7)<<<grid, block, smem, stream>>>(__VA_ARGS__); break;                 \
     default: KERNEL(8)<<<grid, block, smem, stream>>>(__VA_ARGS__); break;                \
   }
-#define K_GRAD(g) k_grad<g>
-#define K_FLUX2(g) k_flux<g, true>
-#define K_FLUX1(g) k_flux<g, false>
+#define K_GRAD(g) k_grad<g, false>
+#define K_GRADM(g) k_grad<g, true>
+#define K_FLUX2(g) k_flux<g, true, false>
+#define K_FLUX1(g) k_flux<g, false, false>
+#define K_FLUX2M(g) k_flux<g, true, true>
+#define K_FLUX1M(g) k_flux<g, false, true>
 #define K_FINISH(g) k_finish<g>
 #define K_STORED(g) k_stored<g>
 
@@ -949,6 +1169,9 @@ int rt_transport_configure(rt_ctx *c) {
   SET_SMEM_G(c->G, K_GRAD, sg, e);
   if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX2, ss, e);
   if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX1, ss, e);
+  if (e == cudaSuccess) SET_SMEM_G(c->G, K_GRADM, sg, e);
+  if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX2M, ss, e);
+  if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX1M, ss, e);
   if (e != cudaSuccess) return rt_fail(c, RT_ECUDA, "cudaFuncSetAttribute(shared memory): %s", cudaGetErrorString(e));
   return RT_OK;
 }
@@ -975,6 +1198,7 @@ rt_geom rt_geom_of(const rt_ctx *c) {
   m.cact = c->has_active ? rt_ptr<uint8_t>(c, l.cact) : nullptr;
   m.tact = c->has_active ? rt_ptr<uint8_t>(c, l.tact) : nullptr;
   m.tl = c->dbg_tl;
+  m.il0 = 1.0 / c->l0; m.l0sq = c->l0 * c->l0;
   m.prefetch_tiles = c->tun.prefetch_tiles > 0 ? c->tun.prefetch_tiles : (c->tun.prefetch_tiles < 0 ? (1 << 30) : 600);
   m.ghost = rt_ptr<double>(c, l.ghost);
   for (int a = 0; a < 3; a++) { m.box[a] = c->box[a]; m.per[a] = c->per[a]; }
@@ -989,7 +1213,12 @@ static void launch_grad(rt_ctx *c, rt_geom m, const double *U, double *grad) {
     if (n <= 0) continue;
     m.tbase = cls == 0 ? 0 : c->nGA;
     m.smax = cls == 0 ? c->smaxA : c->smax; m.hmax = cls == 0 ? c->hmaxA : c->hmax;
-    DISPATCH_G(c->G, K_GRAD, (unsigned)n, grad_threads(c), rt_smem_grad(c->TC, c->G, m.smax, m.hmax, c->bstride), c->stream, m, U, grad);
+    const size_t sg = rt_smem_grad(c->TC, c->G, m.smax, m.hmax, c->bstride);
+    if (c->par.mixed) {
+      DISPATCH_G(c->G, K_GRADM, (unsigned)n, grad_threads(c), sg, c->stream, m, U, grad);
+    } else {
+      DISPATCH_G(c->G, K_GRAD, (unsigned)n, grad_threads(c), sg, c->stream, m, U, grad);
+    }
     c->launches++;
   }
 }
@@ -1037,8 +1266,12 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
       if (n <= 0) continue;
       mf.tbase = cls == 0 ? 0 : c->nFA;
       mf.omax = cls == 0 ? c->omaxA : c->omax; mf.fmax = cls == 0 ? c->fmaxA : c->fmax;
-      const size_t sf = rt_smem_flux(c->TC, G, mf.omax, mf.fmax, c->bstride);
-      if (c->par.order >= 2) {
+      const size_t sf = rt_smem_flux(c->TC, G, mf.omax, mf.fmax, c->bstride, c->par.mixed != 0);
+      if (c->par.mixed && c->par.order >= 2) {
+        DISPATCH_G(G, K_FLUX2M, (unsigned)n, nt, sf, c->stream, mf, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
+      } else if (c->par.mixed) {
+        DISPATCH_G(G, K_FLUX1M, (unsigned)n, nt, sf, c->stream, mf, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
+      } else if (c->par.order >= 2) {
         DISPATCH_G(G, K_FLUX2, (unsigned)n, nt, sf, c->stream, mf, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);
       } else {
         DISPATCH_G(G, K_FLUX1, (unsigned)n, nt, sf, c->stream, mf, Uin, grad, U0, Uout, srcidx, srcrate, c->nsrc, up, pacc, p_floor, p_out, p_in);

@@ -39,7 +39,7 @@ class rt_params(ctypes.Structure):
                 ("eps_heat", (ctypes.c_double * 3) * RT_MAXG), ("T_fixed", ctypes.c_double),
                 ("alphaB_override", ctypes.c_double), ("y_he", ctypes.c_double), ("f_accept", ctypes.c_double),
                 ("f_target", ctypes.c_double), ("x_floor_rel", ctypes.c_double), ("n_floor", ctypes.c_double),
-                ("max_substeps", ctypes.c_int64), ("kappa_mem_kind", ctypes.c_int32), ("pad", ctypes.c_int32),
+                ("max_substeps", ctypes.c_int64), ("kappa_mem_kind", ctypes.c_int32), ("mixed", ctypes.c_int32),
                 ("kappa", _vp)]
 
 
@@ -206,6 +206,7 @@ def make_params(p):
     q.T_fixed, q.alphaB_override, q.y_he = float(p.T_fixed), float(p.alphaB_override), float(p.y_he)
     q.f_accept, q.f_target, q.x_floor_rel = float(p.f_accept), float(p.f_target), float(p.x_floor_rel)
     q.n_floor, q.max_substeps = float(p.n_floor), int(p.max_substeps)
+    q.mixed = int(getattr(p, "mixed", 0))
     kp = None
     if p.kappa is not None:
         kp = _prep(p.kappa, np.float64)

@@ -154,17 +154,18 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------ algorithmic bytes
-def algorithmic_bytes(C, F, NR, G, heun=True, chem=True, order=2):
+def algorithmic_bytes(C, F, NR, G, heun=True, chem=True, order=2, mixed=False):
     """Bytes each kernel must move per launch if every array it needs is read or written once
     (neighbour gathers served by L2/shared memory; faces shared by two tiles counted once)."""
     # a2 gradient pass: U in, grad out, per face (w, ids) + (c, A), per r-entry slot id, per cell
     # Minv, (s, V), two list offsets
-    grad = 32 * G * C + 96 * G * C + 64 * F + 2 * NR + (48 + 32 + 16) * C
+    gb = 48 if mixed else 96   # gradients per (cell, group): 12 floats with rt_params.mixed, else 12 doubles
+    grad = 32 * G * C + gb * G * C + 64 * F + 2 * NR + (48 + 32 + 16) * C
     # a3+a4 stage pass: U and grad in, U out, U0 in (read in both stages), per face (c, A) + (n, ids),
     # per r-entry slot id, per cell (s, V), two list offsets, source index
-    stage = (32 + 96 + 32 + 32) * G * C + 64 * F + 2 * NR + (32 + 16 + 4) * C
+    stage = (32 + gb + 32 + 32) * G * C + 64 * F + 2 * NR + (32 + 16 + 4) * C
     if order < 2:
-        stage -= 96 * G * C
+        stage -= gb * G * C
     chemb = 64 * G * C + 64 * C + 16 * C
     per_stage = (grad if order >= 2 else 0) + stage
     per_sub = (2 if heun else 1) * per_stage + (chemb if chem else 0)
@@ -248,6 +249,9 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tuning", default="", help="rt_tuning fields, e.g. tile_cells=40,variant=2 (experiments)")
+    ap.add_argument("--mixed", action="store_true",
+                    help="rt_params.mixed = 1: fp32 gradients, closure and flux, fp64 state and sums (PAPER.md:380-386; "
+                         "not the headline: DESIGN.md 7.6)")
     ap.add_argument("--active-frac", type=float, default=1.0,
                     help="individual time steps (rt_set_active): only the cells of the slab x < frac * box take the step")
     ap.add_argument("--timeline", action="store_true",
@@ -290,6 +294,7 @@ def main():
     C, F, G = int(w.mesh.ncell), int(w.mesh.nface), int(w.params.ngroup)
     NR = int((w.mesh.right >= 0).sum())
     tuning = {k: int(v) for k, v in (kv.split("=") for kv in args.tuning.split(",") if kv)} or None
+    w.params.mixed = 1 if args.mixed else 0
     s = rt.Solver(w.mesh, w.params, device=local, tuning=tuning)
     stored0 = np.asarray([float((w.state.N[g] * w.mesh.volume).sum()) for g in range(G)])   # photons at t = 0
     x_slab, box_x = w.mesh.centroid[0], float(w.mesh.box[0])
@@ -380,7 +385,7 @@ def main():
         peak, peak_src = float(json.load(open(peaks_file))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     else:
         peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
-    ab = algorithmic_bytes(C, F, NR, G, bool(w.params.heun), w.params.chem_mode != 0, int(w.params.order))
+    ab = algorithmic_bytes(C, F, NR, G, bool(w.params.heun), w.params.chem_mode != 0, int(w.params.order), bool(args.mixed))
     kern = {}
     # one Heun stage's a3 + a4 = k_flux (class 2) followed by k_finish (class 3): reported separately
     # and, as "stage", together (the algorithmic bytes of a3 + a4 are those of the pair)
@@ -404,7 +409,9 @@ def main():
     # the stage pair it is the sum of k_flux (both tile classes) and k_finish
     traffic, traffic_note = None, "no ncu capture of this workload in profiles/traffic.csv"
     tf = os.path.join(ROOT, "profiles", "traffic.csv")
-    if os.path.exists(tf):
+    if args.mixed:
+        traffic_note = "profiles/traffic.csv holds the fp64 path's capture; none for --mixed"
+    elif os.path.exists(tf):
         rows = {}
         for ln in open(tf).read().splitlines()[1:]:
             f = ln.split(",")
@@ -437,7 +444,7 @@ def main():
     stored_scale = float(np.max(np.abs(led["injected"]) + np.abs(led["stored"])) + 1e-300)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
+            "dtype": "f64 state and sums, f32 gradients / closure / flux (rt_params.mixed)" if args.mixed else "f64", "data": "synthetic",
             "config": {"workload": workload_name(c, n), "cells": C, "faces": F, "groups": G,
                        "chem_mode": int(w.params.chem_mode), "dt": w.dt, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2 (%.1f GB of state and geometry per subcycle)" % (ab["subcycle"] / 1e9),

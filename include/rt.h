@@ -267,6 +267,33 @@ int rt_debug_alu_peak(rt_ctx *ctx, double *out);
 int rt_stored_photons_noalloc(int device, void *stream, int64_t ncell, int ngroup, const double *N_dev,
                               const double *volume_dev, double *stored_dev, char *err, int errlen);
 
+/* ---- sharded runs: cells in contiguous ranges of the space-filling
+ * curve per GPU plus one layer of ghost cells.  PAPER.md:167: per subcycle "the primitive variables required for
+ * the gradient calculations, the gradients needed for the flux calculations" are communicated; PAPER.md:258:
+ * "fluxes for interfaces with cells from different MPI tasks are calculated independently on each task", so no
+ * flux travels.  The library does one shard's
+ * arithmetic; who talks to whom, and the transport (NCCL send/recv, peer copies), are the caller's
+ * (paper_2404_17630_b200/shard.py).  A ghost is a cell of the local mesh whose rt_set_active byte has bit 1 set
+ * (2 = ghost that is passive at its owner, 3 = ghost that is active there): it takes part in the fluxes of the
+ * faces it shares with local cells, with the gradient its owner computed, and is never updated, does no
+ * chemistry, injects nothing, and is left out of the `stored` ledger row here; the local mesh must still close
+ * every ghost (the faces to cells that are not local: reflective boundary faces, which carry no ledger).
+ *
+ * rt_step_phase runs ONE phase of a subcycle, in order: RT_PHASE_CHEM, RT_PHASE_GRAD1, RT_PHASE_FLUX1 and, with
+ * Heun, RT_PHASE_GRAD2, RT_PHASE_FLUX2 (RT_ESTATE if out of order; all five back to back are one rt_step(dt, 1),
+ * bit for bit).  Between phases the caller exchanges the ghosts' rows:
+ *   after CHEM and after FLUX1 (Heun): RT_HALO_U   (N, Fx, Fy, Fz) x G doubles of the buffer the next phase reads
+ *   after GRAD1 and after GRAD2:       RT_HALO_GRAD 12 x G doubles (floats with rt_params.mixed) per cell
+ * rt_halo_pack gathers the rows of `n` cells (cells_dev: DEVICE int32, caller's local numbering) into buf_dev
+ * (DEVICE, n x rt_halo_row_bytes, 16-byte aligned); rt_halo_unpack scatters them into the ghosts.  Stream-ordered,
+ * no synchronisation.  The ledger of a sharded run is the sum of the shards' ledgers. */
+enum { RT_PHASE_CHEM = 0, RT_PHASE_GRAD1 = 1, RT_PHASE_FLUX1 = 2, RT_PHASE_GRAD2 = 3, RT_PHASE_FLUX2 = 4 };
+enum { RT_HALO_U = 0, RT_HALO_GRAD = 1 };
+int rt_step_phase(rt_ctx *ctx, double dt, int phase);
+int rt_halo_pack(rt_ctx *ctx, int what, int64_t n, const int32_t *cells_dev, void *buf_dev);
+int rt_halo_unpack(rt_ctx *ctx, int what, int64_t n, const int32_t *cells_dev, const void *buf_dev);
+int rt_halo_row_bytes(const rt_ctx *ctx, int what);
+
 /* Last error message of this context ("" if none); valid until the next call on it.  (No exception or
  * abort crosses the ABI: SURVEY 8(b) error convention.) */
 const char *rt_last_error(const rt_ctx *ctx);

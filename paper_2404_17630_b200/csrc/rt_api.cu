@@ -245,6 +245,7 @@ int rt_state_init(rt_ctx *c, const rt_params *p, const rt_state *s0, const rt_so
   c->src_cell.assign(src && nsrc > 0 ? src->cell : nullptr, src && nsrc > 0 ? src->cell + nsrc : nullptr);
   c->src_rate.assign(src && nsrc > 0 ? src->rate : nullptr, src && nsrc > 0 ? src->rate + (size_t)nsrc * G : nullptr);
   c->has_active = false;  // every cell active until rt_set_active says otherwise
+  c->phase_next = 0;
   rt_launch_init_sources(c, cell_dev, nsrc);
   RT_CUDA(c, cudaMemsetAsync(rt_ptr<rt_dev_ledger>(c, l.led), 0, sizeof(rt_dev_ledger), c->stream));
   c->nsub_done = 0;
@@ -268,7 +269,7 @@ int rt_set_active(rt_ctx *c, int mem_kind, const uint8_t *active) {
     if (mem_kind == RT_MEM_HOST) {
       RT_CUDA(c, cudaMemcpyAsync(stage, active, (size_t)c->C, cudaMemcpyHostToDevice, c->stream));
       dev = stage;
-      for (int k = 0; k < nsrc; k++) src_on[k] = active[c->src_cell[k]] != 0;
+      for (int k = 0; k < nsrc; k++) src_on[k] = (active[c->src_cell[k]] & 3) == 1;  // (a ghost's source is its owner's)
     } else {
       for (int k = 0; k < nsrc; k++)  // (a handful of one-byte copies: the source cells' flags)
         RT_CUDA(c, cudaMemcpyAsync(&src_on[k], active + c->src_cell[k], 1, cudaMemcpyDeviceToHost, c->stream));
@@ -277,6 +278,8 @@ int rt_set_active(rt_ctx *c, int mem_kind, const uint8_t *active) {
     if (rc != RT_OK) return rc;
     RT_CUDA(c, cudaStreamSynchronize(c->stream));
     RT_CUDA(c, cudaGetLastError());
+    if (mem_kind != RT_MEM_HOST)
+      for (int k = 0; k < nsrc; k++) src_on[k] = (src_on[k] & 3) == 1;
   }
   // photons per unit time the active sources inject (the ledger's `injected` advances by dt times this)
   for (int g = 0; g < G; g++) {
@@ -292,10 +295,65 @@ int rt_set_active(rt_ctx *c, int mem_kind, const uint8_t *active) {
   return RT_OK;
 }
 
+int rt_step_phase(rt_ctx *c, double dt, int phase) {
+  if (!c) return RT_EINVAL;
+  c->err[0] = 0;
+  if (!c->have_state) return rt_fail(c, RT_ESTATE, "rt_step_phase needs rt_state_init first");
+  if (!(dt > 0.0)) return rt_fail(c, RT_EINVAL, "dt must be positive");
+  const int last = c->par.heun ? RT_PHASE_FLUX2 : RT_PHASE_FLUX1;
+  if (phase < 0 || phase > last) return rt_fail(c, RT_EINVAL, "phase must be in [0, %d]", last);
+  if (phase != c->phase_next)
+    return rt_fail(c, RT_ESTATE, "phase %d out of order: phase %d of this subcycle comes next", phase, c->phase_next);
+  RT_CUDA(c, cudaSetDevice(c->device));
+  const int rc = rt_launch_phase(c, dt, phase);
+  if (rc == RT_OK) c->phase_next = phase == last ? 0 : phase + 1;
+  return rc;
+}
+
+static int halo_field(rt_ctx *c, int what, void **field, int *row_bytes) {
+  const rt_layout &l = c->lay;
+  if (what == RT_HALO_U) {  // the buffer the next gradient / flux phase reads: U^n, or U^1 in the second Heun stage
+    const bool second = c->par.heun && c->phase_next >= RT_PHASE_GRAD2;
+    *field = rt_ptr<double>(c, second ? l.Ub : l.Ua);
+    *row_bytes = 32 * c->G;
+  } else if (what == RT_HALO_GRAD) {
+    *field = rt_ptr<double>(c, l.grad);
+    *row_bytes = (c->par.mixed ? 48 : 96) * c->G;
+  } else return rt_fail(c, RT_EINVAL, "what must be RT_HALO_U or RT_HALO_GRAD");
+  return RT_OK;
+}
+
+static int halo_call(rt_ctx *c, bool pack, int what, int64_t n, const int32_t *cells_dev, void *buf_dev, const char *name) {
+  if (!c) return RT_EINVAL;
+  c->err[0] = 0;
+  if (!c->have_state) return rt_fail(c, RT_ESTATE, "%s needs rt_state_init first", name);
+  if (n < 0 || (n > 0 && (!cells_dev || !buf_dev))) return rt_fail(c, RT_EINVAL, "%s: null pointer or negative count", name);
+  if (((uintptr_t)buf_dev & 15) != 0) return rt_fail(c, RT_EINVAL, "%s: the buffer must be 16-byte aligned", name);
+  RT_CUDA(c, cudaSetDevice(c->device));
+  void *field = nullptr;
+  int row_bytes = 0;
+  const int rc = halo_field(c, what, &field, &row_bytes);
+  if (rc != RT_OK) return rc;
+  return rt_launch_halo(c, pack, field, row_bytes, n, cells_dev, buf_dev);
+}
+
+int rt_halo_pack(rt_ctx *c, int what, int64_t n, const int32_t *cells_dev, void *buf_dev) {
+  return halo_call(c, true, what, n, cells_dev, buf_dev, "rt_halo_pack");
+}
+int rt_halo_unpack(rt_ctx *c, int what, int64_t n, const int32_t *cells_dev, const void *buf_dev) {
+  return halo_call(c, false, what, n, cells_dev, (void *)buf_dev, "rt_halo_unpack");
+}
+
+int rt_halo_row_bytes(const rt_ctx *c, int what) {
+  if (!c || !c->have_state) return RT_EINVAL;
+  return what == RT_HALO_U ? 32 * c->G : what == RT_HALO_GRAD ? (c->par.mixed ? 48 : 96) * c->G : RT_EINVAL;
+}
+
 int rt_step(rt_ctx *c, double dt, int nsub) {
   if (!c) return RT_EINVAL;
   c->err[0] = 0;
   if (!c->have_state) return rt_fail(c, RT_ESTATE, "rt_step needs rt_state_init first");
+  if (c->phase_next != 0) return rt_fail(c, RT_ESTATE, "rt_step inside a subcycle begun with rt_step_phase (phase %d comes next)", c->phase_next);
   if (!(dt > 0.0) || nsub < 0) return rt_fail(c, RT_EINVAL, "dt must be positive and nsub >= 0");
   RT_CUDA(c, cudaSetDevice(c->device));
   for (int s = 0; s < nsub; s++) {

@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(RT_CHEM_BLOCK, 16) k_chem(rt_chem_par P, int64
   for (int64_t row = blockIdx.x; row * RT_CHEM_BLOCK < n; row += gridDim.x) {
     const int64_t idx = row * RT_CHEM_BLOCK + threadIdx.x;
     // (individual time steps: a passive cell does no chemistry; only the first pass sees such cells)
-    const bool live = idx < n && !(FIRST && cact && !(cact[idx] & 1));
+    const bool live = idx < n && !(FIRST && cact && (cact[idx] & 5) != 1);  // (passive cells and ghosts do no chemistry)
     if (FIRST && flag && idx < n && !live) flag[idx] = 0;
     double absd[G];
 #pragma unroll

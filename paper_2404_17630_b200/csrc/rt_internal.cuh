@@ -113,6 +113,7 @@ struct rt_ctx {
   rt_params par;
   rt_tuning tun;      // rt_set_tuning (zeros = defaults)
   bool has_active;    // rt_set_active gave a proper subset: cact / tact are valid
+  int phase_next;     // rt_step_phase: the phase of the running subcycle that comes next (0 between subcycles)
   std::vector<int32_t> src_cell;  // host copies of the sources (rt_set_active recomputes the injection rate)
   std::vector<double> src_rate;
   unsigned long long *dbg_tl;  // device buffer of rt_debug_tile_timeline while it runs, else null
@@ -179,6 +180,9 @@ int rt_setup_mesh(rt_ctx *c, const rt_mesh *m);
 // rt_kernels.cu
 int rt_transport_configure(rt_ctx *c);  // after rt_setup_mesh: shared-memory opt-in of the tile kernels
 int rt_launch_step(rt_ctx *c, double dt);
+int rt_launch_phase(rt_ctx *c, double dt, int phase);  // one phase of a subcycle (rt_step_phase)
+// buf[k][:] = field[iperm[cells[k]]][:] (pack) or the reverse; rows of row_bytes (a multiple of 16)
+int rt_launch_halo(rt_ctx *c, bool pack, void *field, int row_bytes, int64_t n, const int32_t *cells_dev, void *buf_dev);
 int rt_launch_gradients(rt_ctx *c, const double *U);
 // dst[p*stride + r] = src[r*C + perm[p]]  /  dst[r*C + perm[p]] = src[p*stride + r], r < rows
 int rt_launch_permute_in(rt_ctx *c, const double *src, double *dst, int rows, int stride);

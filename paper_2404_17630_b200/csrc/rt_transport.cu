@@ -183,7 +183,8 @@ __device__ __forceinline__ void grad_cells(const rt_geom &m, const tile_view &v,
   const int h = (tid >> 1) & 1, p = tid & 1;
   for (int xb = 0; xb < v.ncell; xb += nt >> 2) {  // (whole warps iterate together: the shuffles need every lane)
     const int x = xb + (tid >> 2);
-    const bool on = x < v.ncell && (!m.cact || (m.cact[v.c0 + x] & 1));  // (a passive cell is skipped: its face state is its cell value)
+    // (a passive cell is skipped: its face state is its cell value; a ghost's gradient is imported: rt_halo_unpack)
+    const bool on = x < v.ncell && (!m.cact || (m.cact[v.c0 + x] & 5) == 1);
     const int xx = on ? x : 0;
     const int h0 = on ? (int)v.ho[xx] : 0, h1 = on ? (int)v.ho[xx + 1] : 0;
     const double *ui_p = sm.U + US * xx + 4 * g0 + 2 * h;
@@ -306,7 +307,7 @@ __device__ __forceinline__ void grad_cells_mixed(const rt_geom &m, const tile_vi
   const double il0 = m.il0;
   for (int xb = 0; xb < v.ncell; xb += nt >> 2) {
     const int x = xb + (tid >> 2);
-    const bool on = x < v.ncell && (!m.cact || (m.cact[v.c0 + x] & 1));
+    const bool on = x < v.ncell && (!m.cact || (m.cact[v.c0 + x] & 5) == 1);
     const int xx = on ? x : 0;
     const int h0 = on ? (int)v.ho[xx] : 0, h1 = on ? (int)v.ho[xx + 1] : 0;
     const double *ui_p = sm.U + US * xx + 4 * g0 + 2 * h;
@@ -904,7 +905,7 @@ __global__ void __launch_bounds__(256, 3) k_flux(rt_geom m, const double *__rest
     }
     if (incomplete) { st4(pacc + 4 * (v.c0 * G + item), a0, a1, a2, a3); continue; }
     const int32_t si = sSrc[il];
-    const double src = si >= 0 && (ac & 1) ? srcrate[(size_t)ig * nsrc + si] : 0.0;  // (a passive cell injects nothing)
+    const double src = si >= 0 && (ac & 5) == 1 ? srcrate[(size_t)ig * nsrc + si] : 0.0;  // (a passive cell injects nothing, nor does a ghost)
     const double add = finish_cell(a0, a1, a2, a3, sV[il], src, ld4(sU + 4 * item), u0, up,
                                    Uout + 4 * (v.c0 * G + item));
     if (add != 0.0) {
@@ -965,7 +966,7 @@ __global__ void __launch_bounds__(RT_FIN_BLOCK) k_finish(int64_t n2, const int32
       a.x -= p.x; a.y -= p.y; a.z -= p.z; a.w -= p.w;
     }
     const int32_t si = srcidx[i];
-    const double src = si >= 0 && (ac & 1) ? srcrate[(size_t)g * nsrc + si] : 0.0;
+    const double src = si >= 0 && (ac & 5) == 1 ? srcrate[(size_t)g * nsrc + si] : 0.0;
     add = finish_cell(a.x, a.y, a.z, a.w, cellV[i], src, ld4(Uin + 4 * (i * G + g)), ld4(U0 + 4 * (i * G + g)), up, out);
   }
   // fixed-order block sums per group
@@ -1046,11 +1047,12 @@ __global__ void __launch_bounds__(1024) k_reduce(reduce_job j0, reduce_job j1, i
 // stored photons per block: part[row][g] = sum_cells V N
 template <int GG>
 __global__ void __launch_bounds__(RT_BLOCK *GG) k_stored(int64_t C, const double *__restrict__ U,
-                                                          const double *__restrict__ cellV, double *__restrict__ part) {
+                                                          const double *__restrict__ cellV, double *__restrict__ part,
+                                                          const uint8_t *__restrict__ cact) {
   __shared__ double sm[GG][RT_BLOCK / 32];
   const int64_t i = (int64_t)blockIdx.x * RT_BLOCK + threadIdx.x;
   const int g = threadIdx.y;
-  double v = i < C ? cellV[i] * U[((size_t)i * GG + g) * 4] : 0.0;
+  double v = i < C && !(cact && (cact[i] & 4)) ? cellV[i] * U[((size_t)i * GG + g) * 4] : 0.0;  // (a ghost's photons are its owner's)
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
   if ((threadIdx.x & 31) == 0) sm[g][threadIdx.x >> 5] = v;
@@ -1090,9 +1092,9 @@ __global__ void k_set_sources(int nsrc, const int32_t *__restrict__ cell, const 
 // ------------------------------------------------------------------ active sets (individual time steps)
 __global__ void k_active_in(int64_t C, const int32_t *__restrict__ perm, const uint8_t *__restrict__ active, uint8_t *__restrict__ ain) {
   const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (p < C) ain[p] = active[perm[p]] != 0;
+  if (p < C) ain[p] = active[perm[p]] & 3;  // bit 0 active, bit 1 ghost (rt_set_active)
 }
-// one block per tile, straight from the tile's tables in global memory: cact = active | touched << 1 per cell
+// one block per tile, straight from the tile's tables in global memory: cact = active | touched << 1 | ghost << 2 per cell
 // (touched: the cell or a cell across one of its faces is active), tact = OR over the tile's cells
 __global__ void __launch_bounds__(128) k_touched(rt_geom m, const uint8_t *__restrict__ ain, uint8_t *__restrict__ cact, uint8_t *__restrict__ tact) {
   __shared__ int s_or;
@@ -1105,17 +1107,21 @@ __global__ void __launch_bounds__(128) k_touched(rt_geom m, const uint8_t *__res
   if (threadIdx.x == 0) s_or = 0;
   __syncthreads();
   for (int x = threadIdx.x; x < ncell; x += blockDim.x) {
-    int f = ain[c0 + x] ? 1 : 0;
+    const int a = ain[c0 + x];
+    int f = a & 1;
+    const int ghost = (a >> 1) & 1;  // a ghost is never updated here: its owner does that, rt_halo_unpack brings the result
     int touched = f;
-    for (uint32_t k = ho[x]; k < ho[x + 1] && !touched; k++) {
+    for (uint32_t k = ho[x]; k < ho[x + 1] && !touched && !ghost; k++) {
       const uint32_t nb = hl[k] >> 16;
       if (nb >= 0xFF00u) continue;
       const int64_t id = nb < (uint32_t)m.TC ? c0 + nb : (int64_t)halo[nb - m.TC];
-      touched |= ain[id] != 0;
+      touched |= ain[id] & 1;
     }
-    f |= touched << 1;
+    f |= (ghost ? 0 : touched << 1) | (ghost << 2);
     cact[c0 + x] = (uint8_t)f;
-    if (f) atomicOr(&s_or, f);
+    // per tile: bit 0 = a cell whose gradient is computed here, bit 1 = a cell that is updated here
+    const int ft = ghost ? 0 : f;
+    if (ft) atomicOr(&s_or, ft);
   }
   __syncthreads();
   if (threadIdx.x == 0) tact[t] = (uint8_t)s_or;
@@ -1235,9 +1241,11 @@ void rt_reduce2(rt_ctx *c, reduce_job a, reduce_job b, int njobs) {
   c->launches++;
 }
 
-// one Heun stage: Uout = ca*U0 + cb*(Uin + dt R(Uin)); ledger weights wl (fluxes), wf (floor)
+// one Heun stage: Uout = ca*U0 + cb*(Uin + dt R(Uin)); ledger weights wl (fluxes), wf (floor).
+// parts: 1 = the gradient pass (a2), 2 = fluxes and update (a3 + a4), 3 = both; a sharded run exchanges the
+// ghosts' gradients between the two (rt_step_phase)
 static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, double ca, double cb, double dt,
-                  double wl, double wf) {
+                  double wl, double wf, int parts = 3) {
   const rt_layout &l = c->lay;
   const rt_geom m = rt_geom_of(c);
   const int G = c->G;
@@ -1252,11 +1260,12 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
   double *pacc = rt_ptr<double>(c, l.pacc);
   const int32_t *srcidx = rt_ptr<int32_t>(c, l.srcidx);
   const double *srcrate = rt_ptr<double>(c, l.srcrate);
-  if (c->par.order >= 2) {
+  if (c->par.order >= 2 && (parts & 1)) {
     rt_prof_begin(c, RT_K_GRAD);
     launch_grad(c, m, Uin, grad);
     rt_prof_end(c);
   }
+  if (!(parts & 2)) return;
   rt_prof_begin(c, RT_K_FLUX);
   {
     rt_geom mf = m;
@@ -1292,10 +1301,13 @@ static void stage(rt_ctx *c, const double *Uin, const double *U0, double *Uout, 
   rt_reduce2(c, {p_floor, c->T, wf, 3, nullptr}, {nfin > 0 ? p_floor2 : p_floor, nfin, wf, 3, nullptr}, 1);
 }
 
-int rt_launch_step(rt_ctx *c, double dt) {
+// the phases of one subcycle, in order (rt_step_phase; rt_step runs them back to back):
+// 0 chemistry, 1 gradients of U^n, 2 fluxes + update of stage 1, 3 gradients of U^1, 4 fluxes + update of stage 2
+// (Heun off: 0, 1, 2).  parts = bit mask of the phases to run.
+static void run_phases(rt_ctx *c, double dt, int parts) {
   rt_layout &l = c->lay;
   double *Ua = rt_ptr<double>(c, l.Ua), *Ub = rt_ptr<double>(c, l.Ub);
-  if (c->par.chem_mode != RT_CHEM_NONE) {
+  if ((parts & 1) && c->par.chem_mode != RT_CHEM_NONE) {
     rt_chem_par P;
     P.ctilde = c->par.ctilde; P.y_he = c->par.y_he; P.T_fixed = c->par.T_fixed;
     P.alphaB_override = c->par.alphaB_override; P.f_accept = c->par.f_accept; P.f_target = c->par.f_target;
@@ -1304,15 +1316,37 @@ int rt_launch_step(rt_ctx *c, double dt) {
       for (int j = 0; j < 3; j++) { P.sigma[g][j] = c->par.sigma[g][j]; P.eps[g][j] = c->par.eps_heat[g][j]; }
     rt_launch_chem(c, P, dt, Ua);
   }
+  const int s1 = (parts >> 1) & 3, s2 = (parts >> 3) & 3;
+  if (c->par.heun) {
+    if (s1) stage(c, Ua, Ua, Ub, 0.0, 1.0, dt, 0.5, 0.5, s1);  // U1 = enforce(Un + dt R(Un))
+    if (s2) stage(c, Ub, Ua, Ua, 0.5, 0.5, dt, 0.5, 1.0, s2);  // Un+1 = enforce(Un/2 + (U1 + dt R(U1))/2)
+  } else {
+    if (s1) stage(c, Ua, Ua, Ub, 0.0, 1.0, dt, 1.0, 1.0, s1);
+    if (s1 & 2) { size_t t = l.Ua; l.Ua = l.Ub; l.Ub = t; }  // the new state lives in the other buffer
+  }
+}
+
+int rt_launch_phase(rt_ctx *c, double dt, int phase) {
+  run_phases(c, dt, 1 << phase);
+  const int last = c->par.heun ? 4 : 2;
+  if (phase == last) {
+    for (int g = 0; g < c->G; g++) {  // injected photons: host-side compensated sum
+      double *a = c->injected[g];
+      const double x = dt * c->src_total[g], t = a[0] + x;
+      a[1] += fabs(a[0]) >= fabs(x) ? (a[0] - t) + x : (x - t) + a[0];
+      a[0] = t;
+    }
+    c->nsub_done++;
+  }
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return rt_fail(c, RT_ECUDA, "kernel launch: %s", cudaGetErrorString(e));
+  return RT_OK;
+}
+
+int rt_launch_step(rt_ctx *c, double dt) {
   double tot[RT_MAXG];
   for (int g = 0; g < c->G; g++) tot[g] = dt * c->src_total[g];
-  if (c->par.heun) {
-    stage(c, Ua, Ua, Ub, 0.0, 1.0, dt, 0.5, 0.5);  // U1 = enforce(Un + dt R(Un))
-    stage(c, Ub, Ua, Ua, 0.5, 0.5, dt, 0.5, 1.0);  // Un+1 = enforce(Un/2 + (U1 + dt R(U1))/2)
-  } else {
-    stage(c, Ua, Ua, Ub, 0.0, 1.0, dt, 1.0, 1.0);
-    size_t t = l.Ua; l.Ua = l.Ub; l.Ub = t;  // the new state lives in the other buffer
-  }
+  run_phases(c, dt, c->par.heun ? 31 : 7);
   for (int g = 0; g < c->G; g++) {  // injected photons: host-side compensated sum
     double *a = c->injected[g];
     const double x = tot[g], t = a[0] + x;
@@ -1338,7 +1372,7 @@ int rt_launch_stored(rt_ctx *c) {
   const rt_layout &l = c->lay;
   double *part = rt_ptr<double>(c, l.part);
   DISPATCH_G(c->G, K_STORED, (unsigned)l.nbc, dim3(RT_BLOCK, c->G), 0, c->stream, c->C, rt_ptr<double>(c, l.Ua),
-             rt_ptr<double>(c, l.cellV), part);
+             rt_ptr<double>(c, l.cellV), part, c->has_active ? rt_ptr<uint8_t>(c, l.cact) : nullptr);
   c->launches++;
   rt_reduce2(c, {part, l.nbc, 1.0, 4, nullptr}, {part, l.nbc, 1.0, 4, nullptr}, 1);
   return RT_OK;
@@ -1360,5 +1394,32 @@ int rt_launch_init_sources(rt_ctx *c, const int32_t *cell_dev, int nsrc) {
   if (nsrc > 0)
     k_set_sources<<<(nsrc + 255) / 256, 256, 0, c->stream>>>(nsrc, cell_dev, rt_ptr<int32_t>(c, c->lay.iperm), srcidx);
   c->launches += 2;
+  return RT_OK;
+}
+
+// ------------------------------------------------------------------ halo exchange of a sharded run (rt_halo_pack / rt_halo_unpack)
+// rows of 16-byte chunks: buf[k][:] <-> field[iperm[cells[k]]][:]; one thread per (row, chunk)
+template <bool PACK>
+__global__ void __launch_bounds__(256) k_halo_rows(int64_t n, int chunks, const int32_t *__restrict__ cells, const int32_t *__restrict__ iperm,
+                                                   double2 *field, double2 *buf) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n * chunks) return;
+  const int64_t k = e / chunks;
+  const int ch = (int)(e - k * chunks);
+  const int64_t p = iperm[cells[k]];
+  if (PACK) buf[e] = field[p * chunks + ch];
+  else field[p * chunks + ch] = buf[e];
+}
+
+int rt_launch_halo(rt_ctx *c, bool pack, void *field, int row_bytes, int64_t n, const int32_t *cells_dev, void *buf_dev) {
+  if (n <= 0) return RT_OK;
+  const int chunks = row_bytes / 16;
+  const unsigned nb = blocks_for(n * chunks, 256);
+  const int32_t *iperm = rt_ptr<int32_t>(c, c->lay.iperm);
+  if (pack) k_halo_rows<true><<<nb, 256, 0, c->stream>>>(n, chunks, cells_dev, iperm, (double2 *)field, (double2 *)buf_dev);
+  else k_halo_rows<false><<<nb, 256, 0, c->stream>>>(n, chunks, cells_dev, iperm, (double2 *)field, (double2 *)buf_dev);
+  c->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return rt_fail(c, RT_ECUDA, "kernel launch: %s", cudaGetErrorString(e));
   return RT_OK;
 }

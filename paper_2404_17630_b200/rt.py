@@ -257,6 +257,50 @@ def rt_step(h, dt, nsub=1):
     _check(h, lib().rt_step(h, float(dt), int(nsub)), "rt_step")
 
 
+RT_PHASE_CHEM, RT_PHASE_GRAD1, RT_PHASE_FLUX1, RT_PHASE_GRAD2, RT_PHASE_FLUX2 = range(5)
+RT_HALO_U, RT_HALO_GRAD = 0, 1
+
+
+def rt_step_phase(h, dt, phase):
+    L = lib()
+    L.rt_step_phase.restype = ctypes.c_int
+    L.rt_step_phase.argtypes = [_vp, ctypes.c_double, ctypes.c_int]
+    _check(h, L.rt_step_phase(h, float(dt), int(phase)), "rt_step_phase")
+
+
+def rt_halo_row_bytes(h, what):
+    L = lib()
+    L.rt_halo_row_bytes.restype = ctypes.c_int
+    L.rt_halo_row_bytes.argtypes = [_vp, ctypes.c_int]
+    n = L.rt_halo_row_bytes(h, int(what))
+    if n <= 0:
+        raise RTError("rt_halo_row_bytes: no state yet, or unknown field")
+    return n
+
+
+def _halo(name, h, what, cells, buf):
+    """cells: int32 CUDA tensor (local cell numbers); buf: CUDA tensor of len(cells) * rt_halo_row_bytes bytes."""
+    if not (_is_torch(cells) and cells.is_cuda and cells.element_size() == 4 and cells.is_contiguous() and
+            _is_torch(buf) and buf.is_cuda and buf.is_contiguous()):
+        raise RTError(name + " takes contiguous CUDA tensors (int32 cells)")
+    n = int(cells.numel())
+    if buf.numel() * buf.element_size() < n * rt_halo_row_bytes(h, what):
+        raise RTError(name + ": buffer too small")
+    L = lib()
+    f = getattr(L, name)
+    f.restype = ctypes.c_int
+    f.argtypes = [_vp, ctypes.c_int, ctypes.c_int64, _vp, _vp]
+    _check(h, f(h, int(what), n, _vp(cells.data_ptr()) if n else None, _vp(buf.data_ptr()) if n else None), name)
+
+
+def rt_halo_pack(h, what, cells, buf):
+    _halo("rt_halo_pack", h, what, cells, buf)
+
+
+def rt_halo_unpack(h, what, cells, buf):
+    _halo("rt_halo_unpack", h, what, cells, buf)
+
+
 def rt_download(h, out=None, want_ledger=True, ngroup=1):
     """out: dict of preallocated arrays (N, F, xHII, xHeII, xHeIII, eth; any subset), or None."""
     st = None
@@ -353,6 +397,18 @@ class Solver:
 
     def step(self, dt, nsub=1):
         rt_step(self.h, dt, nsub)
+
+    def step_phase(self, dt, phase):
+        rt_step_phase(self.h, dt, phase)
+
+    def halo_row_bytes(self, what):
+        return rt_halo_row_bytes(self.h, what)
+
+    def halo_pack(self, what, cells, buf):
+        rt_halo_pack(self.h, what, cells, buf)
+
+    def halo_unpack(self, what, cells, buf):
+        rt_halo_unpack(self.h, what, cells, buf)
 
     def download(self, device=False):
         """Returns (state dict, ledger dict); arrays are numpy, or cuda tensors if device=True."""

@@ -1111,7 +1111,7 @@ __global__ void __launch_bounds__(128) k_touched(rt_geom m, const uint8_t *__res
     int f = a & 1;
     const int ghost = (a >> 1) & 1;  // a ghost is never updated here: its owner does that, rt_halo_unpack brings the result
     int touched = f;
-    for (uint32_t k = ho[x]; k < ho[x + 1] && !touched && !ghost; k++) {
+    for (uint32_t k = ho[x]; k < ho[x + 1] && !touched; k++) {
       const uint32_t nb = hl[k] >> 16;
       if (nb >= 0xFF00u) continue;
       const int64_t id = nb < (uint32_t)m.TC ? c0 + nb : (int64_t)halo[nb - m.TC];
@@ -1119,8 +1119,9 @@ __global__ void __launch_bounds__(128) k_touched(rt_geom m, const uint8_t *__res
     }
     f |= (ghost ? 0 : touched << 1) | (ghost << 2);
     cact[c0 + x] = (uint8_t)f;
-    // per tile: bit 0 = a cell whose gradient is computed here, bit 1 = a cell that is updated here
-    const int ft = ghost ? 0 : f;
+    // per tile: bit 0 = a cell whose gradient is computed here, bit 1 = a cell one of whose faces carries a flux
+    // (a ghost's too: the tile that owns the face evaluates it for the cell on the other side)
+    const int ft = (ghost ? 0 : f & 1) | (touched << 1);
     if (ft) atomicOr(&s_or, ft);
   }
   __syncthreads();
@@ -1171,7 +1172,11 @@ static cudaError_t allow_smem(K kernel, size_t bytes) {
 
 int rt_transport_configure(rt_ctx *c) {
   cudaError_t e = cudaSuccess;
-  const size_t sg = rt_smem_grad(c->TC, c->G, c->smax, c->hmax, c->bstride), ss = rt_smem_flux(c->TC, c->G, c->omax, c->fmax, c->bstride);
+  // the opt-in is per kernel, not per context: several contexts with different tile capacities may live in one
+  // process (the shards of shard.LocalGroup), so every kernel is allowed the most a block may have
+  if (rt_smem_grad(c->TC, c->G, c->smax, c->hmax, c->bstride) > RT_SMEM_MAX - 1024 || rt_smem_flux(c->TC, c->G, c->omax, c->fmax, c->bstride) > RT_SMEM_MAX - 1024)
+    return rt_fail(c, RT_EMESH, "a tile needs more shared memory than one block may have");
+  const size_t sg = RT_SMEM_MAX - 1024, ss = RT_SMEM_MAX - 1024;  // (less the kernels' static shared memory)
   SET_SMEM_G(c->G, K_GRAD, sg, e);
   if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX2, ss, e);
   if (e == cudaSuccess) SET_SMEM_G(c->G, K_FLUX1, ss, e);

@@ -237,6 +237,74 @@ def survey_bytes(C, F, G):
     return C * (2 * (grad + upd) + 32 * G + 80)
 
 
+def run_sharded(args):
+    """--shard: ONE mesh cut into contiguous Peano-Hilbert ranges, one per rank (paper_2404_17630_b200/shard.py;
+    DESIGN.md 8.1), four ghost exchanges per subcycle over torch.distributed (NCCL).  Strong scaling: the value
+    is the whole mesh's cell-group-updates per second.  --shards-local K instead runs K shards on ONE GPU in
+    lock-step (plain copies for the exchange): the cost of the ghost layers and of packing, not of a link."""
+    import torch
+    from paper_2404_17630_b200 import rt, shard as S
+    from paper_2404_17630_b200.inputs import configs as cfg
+    rank, local, world = int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    c = args.config
+    n = args.n or min(FULL_N[c], 128)        # (the partitioner is host-side numpy: sized for it)
+    w = cfg.get(c, n)                        # every rank builds the same seeded inputs and cuts its part out
+    w.params.mixed = 1 if args.mixed else 0
+    C, G = int(w.mesh.ncell), int(w.params.ngroup)
+    klocal = args.shards_local
+    if klocal > 1:
+        run = S.LocalGroup(w.mesh, w.params, w.state, w.sources, klocal, device=local)
+        ranks = run.ranks
+    else:
+        run = S.ShardedSolver(w.mesh, w.params, w.state, w.sources, rank, world, S.DistComm(dist) if dist else None, device=local)
+        ranks = [run]
+    rows = sum(int(v.numel()) for r in ranks for v in r.send_ids.values())
+    bytes_step = rows * 2 * (ranks[0].solver.halo_row_bytes(rt.RT_HALO_U) + ranks[0].solver.halo_row_bytes(rt.RT_HALO_GRAD))
+    run.step(w.dt, max(3, args.warmup))
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    time.sleep(0.3)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = sum(r.solver.launches() for r in ranks)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    tw0 = time.perf_counter()
+    e0.record()
+    run.step(w.dt, args.steps)
+    e1.record()
+    torch.cuda.synchronize()
+    tw1 = time.perf_counter()
+    if dist is not None:
+        dist.barrier()
+    ms = max_over_ranks(e0.elapsed_time(e1), dist, torch.device("cuda", local))
+    clocks = sampler.stop(tw0, tw1)
+    launches = sum(r.solver.launches() for r in ranks) - l0
+    led = run.download()[1] if klocal > 1 else run.ledger()
+    stored0 = (w.state.N * w.mesh.volume).sum(1)
+    resid = float(np.max(np.abs(led["stored"] + led["absorbed"] + led["outflow"] - stored0 - led["injected"] - led["inflow_bc"] - led["floor_added"])
+                         / np.maximum(np.abs(stored0 + led["injected"]), 1e-300)))
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": C * G * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong",
+                          "vs_baseline": None, "dtype": "f64" if not args.mixed else "f64 + f32 (rt_params.mixed)", "data": "synthetic",
+                          "config": {"workload": workload_name(c, n), "cells": C, "groups": G,
+                                     "parallelism": "%d shards on one GPU, lock-step" % klocal if klocal > 1 else "shards x%d" % world,
+                                     "shards": [{"owned": r.shard.nown, "ghosts": r.shard.nghost} for r in ranks],
+                                     "exchanges_per_subcycle": len([1 for _, x in ranks[0].phases() if x is not None]),
+                                     "halo_bytes_per_subcycle": bytes_step,
+                                     "l2": "inputs larger than L2" if C * G * 192 > 126e6 else "inputs smaller than L2 (small --n)"},
+                          "clocks": clocks, "gpu_launches": int(launches), "ledger": {"budget_residual": resid}}))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -252,6 +320,10 @@ def main():
     ap.add_argument("--mixed", action="store_true",
                     help="rt_params.mixed = 1: fp32 gradients, closure and flux, fp64 state and sums (PAPER.md:380-386; "
                          "not the headline: DESIGN.md 7.6)")
+    ap.add_argument("--shard", action="store_true",
+                    help="one mesh sharded over the ranks with ghost exchanges (strong scaling) instead of N replicas")
+    ap.add_argument("--shards-local", type=int, default=1,
+                    help="with --shard: K shards on one GPU in lock-step (overhead of the ghost layers, no link)")
     ap.add_argument("--active-frac", type=float, default=1.0,
                     help="individual time steps (rt_set_active): only the cells of the slab x < frac * box take the step")
     ap.add_argument("--timeline", action="store_true",
@@ -265,6 +337,8 @@ def main():
         return run_alu_peak()
     if args.warmup < 3:
         args.warmup = 3
+    if args.shard:
+        return run_sharded(args)
 
     import torch
     from paper_2404_17630_b200 import rt

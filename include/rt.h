@@ -180,7 +180,8 @@ int rt_state_init(rt_ctx *ctx, const rt_params *p, const rt_state *s0, const rt_
  * passive particles, only their conserved quantities are updated, taking into account the fluxes from
  * the interfaces they share with active cells"; active / passive categories that stay
  * fixed during the subcycles of one RT step).  Sets the active set of the following rt_step calls:
- * active = (C) bytes in the caller's cell order, HOST or DEVICE as mem_kind says, non-zero = active;
+ * active = (C) bytes in the caller's cell order, HOST or DEVICE as mem_kind says, bit 0 = active (bit 1 marks a
+ * ghost of a sharded run, see "sharded runs" below; the other bits must be zero);
  * NULL = every cell (the default, restored by rt_state_init).  A passive cell does no chemistry,
  * injects no source photons and has no gradient (reading S27); a face between two passive
  * cells carries no flux; a cell none of whose faces has an active cell is left bit for bit as it was,

@@ -16,7 +16,7 @@ pytestmark = pytest.mark.gpu
 
 
 @pytest.mark.parametrize("c,n,k,world,mixed", [(0, 12, 20, 2, 0), (1, 16, 20, 2, 0), (2, 10, 15, 2, 0), (3, 10, 12, 3, 0), (4, 9, 12, 2, 0),
-                                               (5, 8, 15, 2, 0), (6, 12, 5, 2, 0), (3, 10, 12, 2, 1)])
+                                               (5, 8, 15, 2, 0), (6, 12, 5, 2, 0), (3, 10, 12, 2, 1), (4, 32, 8, 4, 0)])
 def test_sharded_step_from_developed_state(oracle_mod, c, n, k, world, mixed):
     from paper_2404_17630_b200 import shard as S
     w = cfg.get(c, n)

@@ -314,6 +314,8 @@ def main():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--n", type=int, default=None, help="lattice cells per dimension (default: the config's full size)")
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--e2e-rt-subcycles", type=int, default=64,
+                    help="subcycles of the one RT step timed end to end with a single upload and download (0: skip)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tuning", default="", help="rt_tuning fields, e.g. tile_cells=40,variant=2 (experiments)")
@@ -447,6 +449,22 @@ def main():
         el = max_over_ranks(el, dist, "cuda")
         e2e = {"value": world * C * G * args.e2e_steps / el, "unit": UNIT, "h2d_bytes_per_step": (4 * G + 5) * 8 * C,
                "d2h_bytes_per_step": (4 * G + 4) * 8 * C, "steps": args.e2e_steps, "ms_per_step": el / args.e2e_steps * 1e3}
+        # the same through the C ABI in the paper's own rhythm: the state goes to the GPU once per RT step of
+        # 64 subcycles and comes back after it ("transferred to the GPU once before the first subcycle
+        # and only copied back after the completion of the full RT step"; 64 subcycles: PAPER.md:284, 334)
+        if args.e2e_rt_subcycles > 0:
+            nsub = args.e2e_rt_subcycles
+            if dist is not None:
+                dist.barrier()
+            t0 = time.perf_counter()
+            rt.rt_state_init(s.h, w.params, host_in, w.sources)
+            rt.rt_step(s.h, w.dt, nsub)
+            rt.rt_download(s.h, host, False, G)
+            torch.cuda.synchronize()
+            el = max_over_ranks(time.perf_counter() - t0, dist, "cuda")
+            e2e["rt_step"] = {"value": world * C * G * nsub / el, "unit": UNIT, "subcycles_per_rt_step": nsub,
+                              "ms_per_rt_step": el * 1e3, "h2d_bytes_per_rt_step": (4 * G + 5) * 8 * C,
+                              "d2h_bytes_per_rt_step": (4 * G + 4) * 8 * C}
 
     if rank != 0:
         if dist is not None:

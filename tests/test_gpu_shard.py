@@ -16,7 +16,8 @@ pytestmark = pytest.mark.gpu
 
 
 @pytest.mark.parametrize("c,n,k,world,mixed", [(0, 12, 20, 2, 0), (1, 16, 20, 2, 0), (2, 10, 15, 2, 0), (3, 10, 12, 3, 0), (4, 9, 12, 2, 0),
-                                               (5, 8, 15, 2, 0), (6, 12, 5, 2, 0), (3, 10, 12, 2, 1), (4, 32, 8, 4, 0)])
+                                               (5, 8, 15, 2, 0), (6, 12, 5, 2, 0), (3, 10, 12, 2, 1), (4, 32, 8, 4, 0),
+                                               (0, 32, 20, 3, 0), (2, 64, 6, 2, 0)])   # the last two: configs 0 and 2 at BASELINE.json's full size
 def test_sharded_step_from_developed_state(oracle_mod, c, n, k, world, mixed):
     from paper_2404_17630_b200 import shard as S
     w = cfg.get(c, n)
@@ -40,6 +41,27 @@ def test_sharded_step_from_developed_state(oracle_mod, c, n, k, world, mixed):
     assert P.budget_residual(lg, stored0).max() <= P.TOL_LEDGER
     assert lg["nsub_done"] == k + 1
     assert all(s.exchanges == 1 + (k + 1) * (4 if w.params.order >= 2 and w.params.heun else 2) for s in g.ranks) or c == 1
+
+
+@pytest.mark.parametrize("order,heun", [(1, 1), (2, 0), (1, 0)])
+def test_sharded_other_integrator_settings(oracle_mod, order, heun):
+    """First order has no gradient exchange, Heun off has three phases and swaps the state buffers."""
+    from paper_2404_17630_b200 import shard as S
+    w = cfg.get(3, 10)
+    w.params.order, w.params.heun = order, heun
+    g = S.LocalGroup(w.mesh, w.params, w.state, w.sources, 2)
+    assert len([1 for _, x in g.ranks[0].phases() if x is not None]) == (2 if heun else 1) * (2 if order >= 2 else 1)
+    g.step(w.dt, 9)
+    dev, _ = g.download()
+    dev["nH"] = w.state.nH
+    g.step(w.dt, 1)
+    got, lg = g.download()
+    o = oracle_mod.Oracle(w.mesh, w.params); o.set_sources(w.sources); o.set_state(P.as_state(dev))
+    o.step(w.dt, 1)
+    e = P.step_errors(w.mesh, w.params.ctilde, dev, o.get_state(), got)
+    assert e["N"] <= P.TOL_STEP and e["F"] <= P.TOL_STEP, e
+    assert max(e["xHII"], e["xHeII"], e["xHeIII"]) <= 1e-9 and e["eth"] <= 1e-8, e
+    assert P.budget_residual(lg, (w.state.N * w.mesh.volume).sum(1)).max() <= P.TOL_LEDGER
 
 
 @pytest.mark.parametrize("c,n", [(2, 10), (3, 10)])

@@ -72,3 +72,27 @@ def test_tuning_struct_matches_the_header():
     assert ctypes.sizeof(rt.rt_tuning) == 4 * (7 + 6 + 1 + 9)
     L = rt.lib()
     assert L.rt_set_tuning(None, None) == -1
+
+
+def test_new_entry_points_answer_without_a_device():
+    """Sharded-run calls with a null context, and the no-allocation call's size check, return error codes on a
+    machine without a GPU: no abort, no exception."""
+    from paper_2404_17630_b200 import rt
+    L = rt.lib()
+    L.rt_step_phase.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_int]
+    assert L.rt_step_phase(None, 1.0, 0) == -1
+    L.rt_halo_pack.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
+    L.rt_halo_unpack.argtypes = L.rt_halo_pack.argtypes
+    assert L.rt_halo_pack(None, 0, 0, None, None) == -1 and L.rt_halo_unpack(None, 1, 0, None, None) == -1
+    L.rt_halo_row_bytes.argtypes = [ctypes.c_void_p, ctypes.c_int]
+    assert L.rt_halo_row_bytes(None, 0) == -1
+    L.rt_stored_photons_noalloc.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_void_p,
+                                            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_char_p, ctypes.c_int]
+    err = ctypes.create_string_buffer(256)
+    assert L.rt_stored_photons_noalloc(0, None, rt.RT_NOALLOC_MAX_CELLS + 1, 1, None, None, None, err, 256) == -1
+    assert b"RT_NOALLOC_MAX_CELLS" in err.value
+    assert L.rt_stored_photons_noalloc(0, None, 10, 0, None, None, None, err, 256) == -1 and b"ngroup" in err.value
+    src = open(os.path.join(ROOT, "include", "rt.h")).read()
+    assert "#define RT_NOALLOC_MAX_CELLS (1 << 24)" in src and rt.RT_NOALLOC_MAX_CELLS == 1 << 24
+    assert (rt.RT_PHASE_CHEM, rt.RT_PHASE_GRAD1, rt.RT_PHASE_FLUX1, rt.RT_PHASE_GRAD2, rt.RT_PHASE_FLUX2) == (0, 1, 2, 3, 4)
+    assert "enum { RT_PHASE_CHEM = 0, RT_PHASE_GRAD1 = 1, RT_PHASE_FLUX1 = 2, RT_PHASE_GRAD2 = 3, RT_PHASE_FLUX2 = 4 };" in src
